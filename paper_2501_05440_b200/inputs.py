@@ -1,0 +1,467 @@
+"""Seeded synthetic problem generators (BASELINE.json configs C1..C5 and the pin problems).
+
+This module serves BOTH the CPU oracle (``oracle/``) and the CUDA library: it only builds
+plain NumPy arrays that describe a problem (surfaces, cells, lattice, cross sections,
+source, tally edges).  It holds none of the transport method's arithmetic: no RNG stream,
+no distance/collision sampling, no cumulative tables, no tallies.  It imports neither side.
+
+A *problem* is a dict of NumPy arrays / scalars ("problem dict"):
+
+geometry (SURVEY.md 8b/8c rules 11-16; "constructive solid geometry ... surface tracking")
+  surf_type  i32[ns]    0 PLANE_X, 1 PLANE_Y, 2 PLANE_Z, 3 PLANE(a,b,c,d), 4 CYL_X, 5 CYL_Y,
+                        6 CYL_Z, 7 SPHERE
+  surf_param f64[ns,4]  PLANE_X/Y/Z: (p,-,-,-); PLANE: (a,b,c,d) with a x+b y+c z = d;
+                        CYL_Z: (x0,y0,r,-) (CYL_X: (y0,z0,r), CYL_Y: (x0,z0,r)); SPHERE: (x0,y0,z0,r)
+  surf_bc    i32[ns]    0 TRANSMIT, 1 REFLECT, 2 VACUUM
+  cell_surf_off i32[nc+1], cell_surf_id i32[], cell_surf_sense i32[] (+1: f>0, -1: f<0)
+  cell_fill_type i32[nc] 0 material, 1 lattice;  cell_fill i32[nc] material id (or 0 for the lattice)
+  cell_bin   i32[nc]    spatial tally bin of the cell (added to the lattice element's bin)
+  univ_cell_off i32[nu+1]  cells are sorted by universe; universe 0 is the root
+  lat        None | dict(x0,y0,px,py,nx,ny, univ i32[ny,nx], bin i32[ny,nx])
+  n_bins     number of spatial tally bins
+physics
+  mode 'mg': G, n_mat, mg_sig_t/mg_sig_c/mg_sig_f/mg_nu/mg_chi f64[nm,G], mg_S f64[nm,G,G] (row = from)
+  mode 'ce': grid f64[n], nuc_A f64[nn], nuc_el/nuc_c/nuc_f f64[nn,n] (barns),
+             mat_nuc_off i32[nm+1], mat_nuc_id i32[], mat_nuc_dens f64[] (1/(b cm)),
+             nu0, nu1 (nu = nu0 + nu1*E[MeV]), watt_a [MeV], watt_b [1/MeV],
+             t_edges f64[nt+1] (s), e_edges f64[ne+1] (eV)
+source
+  src_lo, src_hi f64[3]; src_iso (1/0); src_dir f64[3]; src_group_pdf f64[G] | src_E (eV); src_t (s)
+run
+  run: dict(kind 'eigen'|'fixed', n_particles, n_inactive, n_active, seed)
+"""
+from __future__ import annotations
+
+import numpy as np
+
+PLANE_X, PLANE_Y, PLANE_Z, PLANE, CYL_X, CYL_Y, CYL_Z, SPHERE = range(8)
+TRANSMIT, REFLECT, VACUUM = range(3)
+
+
+# --------------------------------------------------------------------------- geometry builders
+class _Geom:
+    """Accumulates surfaces and cells; universe 0 (root) must be added first."""
+
+    def __init__(self):
+        self.st, self.sp, self.sb = [], [], []
+        self.cells = []  # (universe, [(surf, sense)], fill_type, fill, bin)
+
+    def surf(self, typ, params, bc=TRANSMIT):
+        p = list(params) + [0.0] * (4 - len(params))
+        self.st.append(typ)
+        self.sp.append(p)
+        self.sb.append(bc)
+        return len(self.st) - 1
+
+    def cell(self, univ, region, fill, bin_=0, lattice=False):
+        self.cells.append((univ, list(region), 1 if lattice else 0, fill, bin_))
+
+    def finish(self, lat=None, n_bins=1):
+        cells = sorted(enumerate(self.cells), key=lambda t: (t[1][0], t[0]))
+        nu = max(c[1][0] for c in cells) + 1
+        off, sid, sse, ft, fl, cb = [0], [], [], [], [], []
+        uoff = [0] * (nu + 1)
+        for _, (u, region, ftype, fill, b) in cells:
+            uoff[u + 1] += 1
+            for s, sense in region:
+                sid.append(s)
+                sse.append(sense)
+            off.append(len(sid))
+            ft.append(ftype)
+            fl.append(fill)
+            cb.append(b)
+        uoff = np.cumsum(uoff)
+        return dict(
+            surf_type=np.array(self.st, np.int32),
+            surf_param=np.array(self.sp, np.float64).reshape(-1, 4),
+            surf_bc=np.array(self.sb, np.int32),
+            cell_surf_off=np.array(off, np.int32),
+            cell_surf_id=np.array(sid, np.int32),
+            cell_surf_sense=np.array(sse, np.int32),
+            cell_fill_type=np.array(ft, np.int32),
+            cell_fill=np.array(fl, np.int32),
+            cell_bin=np.array(cb, np.int32),
+            univ_cell_off=uoff.astype(np.int32),
+            lat=lat,
+            n_bins=int(n_bins),
+        )
+
+
+def geom_box(lo, hi, bc=REFLECT, material=0):
+    """Rectangular box [lo,hi] bounded by six axis planes, one cell."""
+    g = _Geom()
+    bcs = bc if isinstance(bc, (list, tuple)) else [bc] * 6
+    reg = []
+    for ax, typ in enumerate((PLANE_X, PLANE_Y, PLANE_Z)):
+        s0 = g.surf(typ, [lo[ax]], bcs[2 * ax])
+        s1 = g.surf(typ, [hi[ax]], bcs[2 * ax + 1])
+        reg += [(s0, +1), (s1, -1)]
+    g.cell(0, reg, material)
+    return g.finish()
+
+
+def geom_infinite(material=0):
+    """All space, one cell without surfaces."""
+    g = _Geom()
+    g.cell(0, [], material)
+    return g.finish()
+
+
+def geom_slab(L, material=0):
+    """Slab 0<x<L, vacuum on both faces, infinite in y,z."""
+    g = _Geom()
+    s0 = g.surf(PLANE_X, [0.0], VACUUM)
+    s1 = g.surf(PLANE_X, [L], VACUUM)
+    g.cell(0, [(s0, +1), (s1, -1)], material)
+    return g.finish()
+
+
+def geom_sphere(r, bc=VACUUM, material=0):
+    g = _Geom()
+    s = g.surf(SPHERE, [0.0, 0.0, 0.0, r], bc)
+    g.cell(0, [(s, -1)], material)
+    return g.finish()
+
+
+def geom_pincell(pitch=1.26, r=0.54, fuel=0, mod=1):
+    """C3: fuel cylinder (CYL_Z) centred in a reflecting square; infinite in z (rule 15)."""
+    g = _Geom()
+    h = 0.5 * pitch
+    xm = g.surf(PLANE_X, [-h], REFLECT)
+    xp = g.surf(PLANE_X, [h], REFLECT)
+    ym = g.surf(PLANE_Y, [-h], REFLECT)
+    yp = g.surf(PLANE_Y, [h], REFLECT)
+    cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
+    g.cell(0, [(cy, -1)], fuel, bin_=0)
+    g.cell(0, [(xm, +1), (xp, -1), (ym, +1), (yp, -1), (cy, +1)], mod, bin_=1)
+    return g.finish(n_bins=2)
+
+
+def tube_positions():
+    """25 moderator-filled tube positions of a 17x17 assembly: our own 8-fold-symmetric
+    choice (a regular 5x5 sub-grid, spacing 3) -- NOT any published benchmark's pin map."""
+    return [(8 + i, 8 + j) for i in (-6, -3, 0, 3, 6) for j in (-6, -3, 0, 3, 6)]
+
+
+def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_reflect=False):
+    """C4: one (n_asm*n_pin+n_refl)^2 lattice; elements [0,n_asm*n_pin)^2
+    are fuelled assemblies, the rest moderator 'reflector' elements.  x=0,y=0 REFLECT,
+    outer faces VACUUM.  Materials: 0,1,2 fuel variants; 3,4 alternate fuel; 5 tube fill; 6 moderator.
+    Universes: 1..5 fuel pins (material u-1), 6 tube pin, 7 moderator-only."""
+    g = _Geom()
+    nfuel = n_asm * n_pin
+    n = nfuel + n_refl
+    side = n * pitch
+    outer = REFLECT if all_reflect else VACUUM
+    x0 = g.surf(PLANE_X, [0.0], REFLECT)
+    x1 = g.surf(PLANE_X, [side], outer)
+    y0 = g.surf(PLANE_Y, [0.0], REFLECT)
+    y1 = g.surf(PLANE_Y, [side], outer)
+    cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
+    g.cell(0, [(x0, +1), (x1, -1), (y0, +1), (y1, -1)], 0, lattice=True)
+    for u in range(1, 7):
+        g.cell(u, [(cy, -1)], u - 1)
+        g.cell(u, [(cy, +1)], 6)
+    g.cell(7, [], 6)
+    univ = np.full((n, n), 7, np.int32)
+    bins = np.full((n, n), nfuel * nfuel, np.int32)
+    tubes = set(tube_positions()) if n_pin == 17 else set()
+    for iy in range(nfuel):
+        for ix in range(nfuel):
+            ax, ay = ix // n_pin, iy // n_pin
+            px, py = ix % n_pin, iy % n_pin
+            edge = min(px, py, n_pin - 1 - px, n_pin - 1 - py)  # Chebyshev distance from assembly edge
+            if (px, py) in tubes:
+                u = 6
+            elif (ax + ay) % 2 == 0:
+                u = 1 if edge < 2 else (2 if edge < 5 else 3)
+            else:
+                u = 4 if edge < 3 else 5
+            univ[iy, ix] = u
+            bins[iy, ix] = iy * nfuel + ix
+    lat = dict(x0=0.0, y0=0.0, px=float(pitch), py=float(pitch), nx=n, ny=n, univ=univ, bin=bins)
+    return g.finish(lat=lat, n_bins=nfuel * nfuel + 1)
+
+
+# --------------------------------------------------------------------------- MG materials
+def mg_kinf(sig_t, S, nusf, chi):
+    """Input-design helper (used to scale Sigma_f to a target k); tests re-derive k independently."""
+    A = np.diag(sig_t) - S.T
+    return float(nusf @ np.linalg.solve(A, chi))
+
+
+def mg_fuel(rng, G=7, k_target=1.2, thermal_boost=1.0):
+    """SURVEY.md 8d C2 recipe: Sigma_t~U(0.2,1.5), c~U(0.6,0.95), downscatter + 2 upscatter terms,
+    nu~U(2.4,2.9), Sigma_f scaled so the infinite-medium k equals k_target, chi in groups 0-2."""
+    while True:
+        sig_t = rng.uniform(0.2, 1.5, G)
+        c = rng.uniform(0.6, 0.95, G)
+        sig_s = c * sig_t
+        S = np.zeros((G, G))
+        for g in range(G):
+            for gp in range(g, G):
+                S[g, gp] = np.exp(-0.9 * (gp - g)) * rng.uniform(0.5, 1.5)
+        if G >= 3:
+            S[G - 1, G - 2] = 0.05 * rng.uniform(0.5, 1.5)
+            S[G - 2, G - 3] = 0.02 * rng.uniform(0.5, 1.5)
+        S *= (sig_s / S.sum(axis=1))[:, None]
+        nu = rng.uniform(2.4, 2.9, G)
+        ramp = np.linspace(0.3, 1.0, G) if G > 1 else np.ones(1)
+        f = rng.uniform(0.2, 0.5, G) * ramp
+        if thermal_boost != 1.0 and G >= 2:
+            f[-2:] *= thermal_boost
+        chi = np.zeros(G)
+        w = np.array([3.0, 2.0, 0.2])[: min(3, G)]
+        chi[: len(w)] = rng.uniform(0.5, 1.0, len(w)) * w
+        chi /= chi.sum()
+        rem = sig_t - S.sum(axis=1)
+        k1 = mg_kinf(sig_t, S, nu * f * rem, chi)
+        s = k_target / k1
+        if s * f.max() <= 0.95:
+            break
+    sig_f = s * f * rem
+    sig_c = sig_t - S.sum(axis=1) - sig_f
+    return dict(sig_t=sig_t, sig_c=sig_c, sig_f=sig_f, nu=nu, chi=chi, S=S)
+
+
+def mg_moderator(rng, G=7):
+    """SURVEY.md 8d C3 recipe: Sigma_t~U(0.5,3), c~U(0.97,0.998), strong downscatter, no fission."""
+    sig_t = rng.uniform(0.5, 3.0, G)
+    c = rng.uniform(0.97, 0.998, G)
+    S = np.zeros((G, G))
+    for g in range(G):
+        for gp in range(g, G):
+            S[g, gp] = np.exp(-0.4 * (gp - g)) * rng.uniform(0.5, 1.5) * (1.0 if gp > g else 0.6)
+    if G >= 3:
+        S[G - 1, G - 2] = 0.05 * rng.uniform(0.5, 1.5)
+        S[G - 2, G - 3] = 0.02 * rng.uniform(0.5, 1.5)
+    S *= (c * sig_t / S.sum(axis=1))[:, None]
+    z = np.zeros(G)
+    return dict(sig_t=sig_t, sig_c=sig_t - S.sum(axis=1), sig_f=z.copy(), nu=z.copy(), chi=z.copy(), S=S)
+
+
+def _mg_pack(mats):
+    G = len(mats[0]["sig_t"])
+    out = dict(mode="mg", G=G, n_mat=len(mats))
+    for k in ("sig_t", "sig_c", "sig_f", "nu", "chi"):
+        out["mg_" + k] = np.ascontiguousarray(np.stack([m[k] for m in mats]), np.float64)
+    out["mg_S"] = np.ascontiguousarray(np.stack([m["S"] for m in mats]), np.float64)
+    return out
+
+
+def _src(lo, hi, G=None, pdf=None, iso=True, direction=(0.0, 0.0, 1.0), E=None, t=0.0):
+    d = dict(src_lo=np.array(lo, np.float64), src_hi=np.array(hi, np.float64), src_iso=int(iso),
+             src_dir=np.array(direction, np.float64), src_t=float(t))
+    if G is not None:
+        d["src_group_pdf"] = np.array(pdf if pdf is not None else [1.0] + [0.0] * (G - 1), np.float64)
+    if E is not None:
+        d["src_E"] = float(E)
+    return d
+
+
+def one_group_material(sig_t=1.0, sig_s=0.7, sig_f=0.15, nu=2.6):
+    return dict(sig_t=np.array([sig_t]), sig_c=np.array([sig_t - sig_s - sig_f]), sig_f=np.array([sig_f]),
+                nu=np.array([nu]), chi=np.array([1.0]), S=np.array([[sig_s]]))
+
+
+# --------------------------------------------------------------------------- the five configs
+def config1(n_particles=10_000, n_inactive=5, n_active=15, seed=1):
+    """C1: 1-group infinite medium, unit reflecting cube; Sigma_t 1.0, Sigma_s 0.7, nuSigma_f 0.39
+    (split nu=2.6, Sigma_f=0.15, Sigma_c=0.15) -> k_inf = 1.3."""
+    P = geom_box([0, 0, 0], [1, 1, 1], REFLECT)
+    P.update(_mg_pack([one_group_material()]))
+    P.update(_src([0, 0, 0], [1, 1, 1], G=1))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "C1"
+    return P
+
+
+def config2(n_particles=100_000, n_inactive=10, n_active=40, seed=1, mat_seed=2, G=7):
+    """C2: 7-group infinite medium (reflecting unit cube), synthetic fuel from seed 2, k_inf = 1.2."""
+    rng = np.random.default_rng(mat_seed)
+    m = mg_fuel(rng, G, 1.2)
+    P = geom_box([0, 0, 0], [1, 1, 1], REFLECT)
+    P.update(_mg_pack([m]))
+    P.update(_src([0, 0, 0], [1, 1, 1], G=G, pdf=m["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "C2"
+    return P
+
+
+def config3(n_particles=1_000_000, n_inactive=20, n_active=80, seed=1, same_material=False, G=7):
+    """C3: 2-D pin cell, fuel = C2 material, moderator from seed 3.  same_material=True fills the
+    moderator with the fuel (pin: flux fraction -> area fraction, k -> C2 closed form)."""
+    fuel = mg_fuel(np.random.default_rng(2), G, 1.2)
+    mod = fuel if same_material else mg_moderator(np.random.default_rng(3), G)
+    P = geom_pincell()
+    P.update(_mg_pack([fuel, mod]))
+    P.update(_src([-0.63, -0.63, 0], [0.63, 0.63, 0], G=G, pdf=fuel["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "C3"
+    return P
+
+
+def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform=False,
+            n_asm=2, n_pin=17, n_refl=17, G=7):
+    """C4: 2-D quarter core stand-in for the paper's C5G7 workload: 7 synthetic
+    materials from seed 4.  uniform=True: all materials identical + all faces reflecting (pin)."""
+    rng = np.random.default_rng(4)
+    mats = [mg_fuel(rng, G, kt) for kt in (1.05, 1.15, 1.25)]
+    mats += [mg_fuel(rng, G, kt, thermal_boost=1.5) for kt in (1.10, 1.20)]
+    mats += [mg_moderator(rng, G), mg_moderator(rng, G)]
+    if uniform:
+        mats = [mg_fuel(np.random.default_rng(2), G, 1.2)] * 7
+    P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform)
+    P.update(_mg_pack(mats))
+    side = n_asm * n_pin * 1.26
+    P.update(_src([0, 0, 0], [side, side, 0], G=G, pdf=mats[0]["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "C4"
+    return P
+
+
+# --------------------------------------------------------------------------- CE data
+def ce_nuclides(seed=5, n_grid=50_000, jitter=False, n_res=200):
+    """SURVEY.md 8d C5 recipe: five synthetic nuclides on a log-spaced union grid (eV), flat
+    potential + 1/v + (heavy only) single-level Breit-Wigner resonances, Lorentzian, no interference."""
+    rng = np.random.default_rng(seed)
+    lg = np.linspace(np.log(1e-5), np.log(2e7), n_grid)
+    if jitter:
+        step = lg[1] - lg[0]
+        lg[1:-1] += rng.uniform(-0.4, 0.4, n_grid - 2) * step
+    E = np.exp(lg)
+    E[0], E[-1] = 1e-5, 2e7
+    inv_v = np.sqrt(0.0253 / E)
+
+    def resonances(lo_pk, hi_pk):
+        E0 = np.exp(rng.uniform(np.log(1.0), np.log(1e4), n_res))
+        gam = E0 * np.exp(rng.uniform(np.log(3e-3), np.log(1e-2), n_res))
+        pk = np.exp(rng.uniform(np.log(lo_pk), np.log(hi_pk), n_res)) / np.sqrt(E0)
+        pk *= np.sqrt(1.0)  # peaks in barns at E0 (x E0^-1/2 as the recipe states)
+        out = np.zeros_like(E)
+        for e0, gm, p in zip(E0, gam, pk):
+            out += p / (1.0 + ((E - e0) / (0.5 * gm)) ** 2)
+        return out
+
+    nn = 5
+    A = np.array([235.0, 238.0, 16.0, 1.0, 10.0])
+    el = np.zeros((nn, n_grid))
+    ca = np.zeros((nn, n_grid))
+    fi = np.zeros((nn, n_grid))
+    r_fis = resonances(20.0, 500.0)
+    r_fer = resonances(10.0, 400.0)
+    # fissile
+    el[0] = 11.5 + 0.05 * r_fis
+    ca[0] = 100.0 * inv_v + 0.40 * r_fis
+    fi[0] = 580.0 * inv_v + 1.2 + 0.55 * r_fis
+    # fertile
+    ramp = np.clip((E - 0.8e6) / (1.5e6 - 0.8e6), 0.0, 1.0)
+    el[1] = 9.0 + 0.10 * r_fer
+    ca[1] = 2.7 * inv_v + 0.90 * r_fer
+    fi[1] = 0.5 * ramp
+    # oxygen-like
+    el[2] = 3.8
+    # hydrogen-like
+    el[3] = 20.0 / np.sqrt(1.0 + E / 1e5)
+    ca[3] = 0.33 * inv_v
+    # absorber-like
+    el[4] = 2.0
+    ca[4] = 3840.0 * inv_v
+    return dict(grid=E, nuc_A=A, nuc_el=el, nuc_c=ca, nuc_f=fi)
+
+
+def config5(n_particles=1_000_000, seed=1, n_grid=50_000, jitter=False, absorber=1.0e-4, data_seed=5):
+    """C5: CE time-dependent infinite pin cell; stand-in for the paper's UO2 pin cell with the
+    OpenMC data library, which is not in this container."""
+    P = geom_pincell(fuel=0, mod=1)
+    P["cell_bin"][:] = 0
+    P["n_bins"] = 1
+    P.update(ce_nuclides(data_seed, n_grid, jitter))
+    P["mode"] = "ce"
+    P["n_mat"] = 2
+    P["mat_nuc_off"] = np.array([0, 3, 5], np.int32)
+    P["mat_nuc_id"] = np.array([0, 1, 2, 3, 4], np.int32)
+    P["mat_nuc_dens"] = np.array([5.5e-4, 2.24e-2, 4.6e-2, 6.68e-2, absorber], np.float64)
+    P.update(nu0=2.4, nu1=0.1, watt_a=0.988, watt_b=2.249)
+    P["t_edges"] = np.concatenate([[0.0], 10.0 ** (-8.0 + 0.5 * np.arange(1, 11))])
+    P["e_edges"] = np.exp(np.linspace(np.log(1e-5), np.log(2e7), 101))
+    P["e_edges"][0], P["e_edges"][-1] = 1e-5, 2e7
+    P.update(_src([-0.63, -0.63, 0], [0.63, 0.63, 0], E=2.0e6, t=0.0))
+    P["run"] = dict(kind="fixed", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "C5"
+    return P
+
+
+# --------------------------------------------------------------------------- pin problems (closed forms)
+def slab_beam(L=2.0, sig_t=1.3, n_particles=100_000, seed=7):
+    """Pure absorber slab, mono-directional normal beam born on x=0+: leakage = exp(-Sigma_t L)."""
+    P = geom_slab(L)
+    P.update(_mg_pack([one_group_material(sig_t=sig_t, sig_s=0.0, sig_f=0.0, nu=0.0)]))
+    P.update(_src([1e-12, 0, 0], [1e-12, 0, 0], G=1, iso=False, direction=(1.0, 0.0, 0.0)))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "slab"
+    return P
+
+
+def sphere_absorber(r=1.5, sig_t=0.8, n_particles=100_000, seed=11):
+    """Pure absorber sphere, isotropic point source at the centre: leakage = exp(-Sigma_t r)."""
+    P = geom_sphere(r)
+    P.update(_mg_pack([one_group_material(sig_t=sig_t, sig_s=0.0, sig_f=0.0, nu=0.0)]))
+    P.update(_src([0, 0, 0], [0, 0, 0], G=1))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "sphere"
+    return P
+
+
+def ce_one_over_v(lam=2.0e5, n_particles=100_000, seed=13, E0=1.0e3, n_grid=2000):
+    """Single nuclide, pure 1/v absorber (Sigma_a v = lam [1/s]), no scatter, infinite medium:
+    track length in [t1,t2] per source neutron = (v/lam)(exp(-lam t1)-exp(-lam t2))."""
+    P = geom_infinite()
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    E[0], E[-1] = 1e-5, 2e7
+    c_cm = 2.99792458e10
+    v = c_cm * np.sqrt(2.0 * E / 939.56542052e6)
+    P.update(mode="ce", n_mat=1, grid=E, nuc_A=np.array([10.0]), nuc_el=np.zeros((1, n_grid)),
+             nuc_c=(lam / v)[None, :].copy(), nuc_f=np.zeros((1, n_grid)),
+             mat_nuc_off=np.array([0, 1], np.int32), mat_nuc_id=np.array([0], np.int32),
+             mat_nuc_dens=np.array([1.0]), nu0=0.0, nu1=0.0, watt_a=0.988, watt_b=2.249)
+    P["t_edges"] = np.concatenate([[0.0], 10.0 ** (-6.5 + 0.25 * np.arange(1, 9))])
+    P["e_edges"] = np.array([1e-5, 1.0, 2e7])
+    P.update(_src([0, 0, 0], [0, 0, 0], E=E0, t=0.0))
+    P["run"] = dict(kind="fixed", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "ce_1v"
+    return P
+
+
+def ce_single_scatterer(A=16.0, n_particles=50_000, seed=17, E0=1.0e6, sig_el=0.5, sig_c=0.5, n_grid=500):
+    """One nuclide with flat elastic + flat capture in an infinite medium (elastic-kinematics pin:
+    the first-collision energy/angle moments are read from the event trace)."""
+    P = geom_infinite()
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    E[0], E[-1] = 1e-5, 2e7
+    P.update(mode="ce", n_mat=1, grid=E, nuc_A=np.array([float(A)]), nuc_el=np.full((1, n_grid), sig_el),
+             nuc_c=np.full((1, n_grid), sig_c), nuc_f=np.zeros((1, n_grid)),
+             mat_nuc_off=np.array([0, 1], np.int32), mat_nuc_id=np.array([0], np.int32),
+             mat_nuc_dens=np.array([1.0]), nu0=0.0, nu1=0.0, watt_a=0.988, watt_b=2.249)
+    P["t_edges"] = np.array([0.0, 1.0])
+    P["e_edges"] = np.array([1e-5, 2e7])
+    P.update(_src([0, 0, 0], [0, 0, 0], E=E0, t=0.0))
+    P["run"] = dict(kind="fixed", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "ce_scatter"
+    return P
+
+
+def ce_pure_fission(n_particles=50_000, seed=19, E0=1.0e6, n_grid=500):
+    """One nuclide whose only reaction is fission, children killed by the first time edge
+    (Watt/nu pin: child energies and multiplicities are read from the trace/counters)."""
+    P = ce_single_scatterer(A=235.0, n_particles=n_particles, seed=seed, E0=E0, n_grid=n_grid)
+    P["nuc_el"][:] = 0.0
+    P["nuc_c"][:] = 0.0
+    P["nuc_f"][:] = 1.0
+    P.update(nu0=2.4, nu1=0.1)
+    P["t_edges"] = np.array([0.0, 1.0e-12])
+    P["name"] = "ce_fission"
+    return P
+
+
+CONFIGS = dict(C1=config1, C2=config2, C3=config3, C4=config4, C5=config5)
