@@ -732,6 +732,7 @@ static void transport(orc_problem *p, particle *q)
             trace(p, q, ev, loc[0], loc[1], loc[2], hit, gi, d, E_flight);
         } else {
             q->tbin++;
+            q->last_surf = -1; /* R11: the particle has moved off the surface it sat on */
             if (q->tbin == in->n_t) { ev = ORC_EV_CUTOFF; q->alive = 0; } else ev = ORC_EV_TIME_EDGE;
             trace(p, q, ev, loc[0], loc[1], loc[2], -1, gi, d, E_flight);
         }
@@ -872,10 +873,13 @@ int orc_run_fixed_source(orc_problem *p, uint64_t N, uint64_t seed)
         if (q.alive) transport(p, &q); else p->counters[0]++;
         while (p->n_stack > 0) {
             if (p->n_stack > p->counters[12]) p->counters[12] = p->n_stack;
+            /* R25: the prompt chain must be subcritical; more than 64 N secondaries = bank overflow */
+            if (p->counters[11] > 64 * N + 4096) { p->error = -3; p->n_stack = 0; break; }
             particle c = p->stack[--p->n_stack];
             transport(p, &c);
         }
     }
+    if (p->error == -3) return p->error;
     accumulate_cycle(p, N, 1);
     return p->error;
 }
