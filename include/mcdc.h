@@ -1,0 +1,226 @@
+/* mcdc.h -- C-ABI of the B200-native event-based Monte Carlo neutron transport library.
+ *
+ * What it computes: the data-parallel hot path of the transport loop named in arxiv 2501.05440
+ * ("continuous and multi-group energy neutron transport physics with constructive solid
+ * geometry modeling using surface tracking ... k-eigenvalue and fully dynamic simulations ...
+ * replicable random number generation"; PAPER.md:51 one "segment" = one event; PAPER.md:55 dual
+ * particle banks; PAPER.md:57 per-event kernels; PAPER.md:124 inactive/active cycles
+ * time-dependent fixed source).  The paper prints no formulas; every step follows the readings
+ * R1..R31 of DESIGN.md section 3 (= SURVEY.md 8c).
+ *
+ * Conventions for every call
+ *   - plain C: pointers + sizes only.  All INPUT pointers are HOST pointers; the library copies what
+ *     it needs during the call (the caller may free them as soon as the call returns).  All OUTPUT
+ *     pointers are HOST pointers to caller-allocated arrays of the documented length.
+ *   - the only DEVICE pointer is mcdc_device.workspace: device memory owned by the caller (the Python
+ *     binding allocates it with torch.empty); the library never calls cudaMalloc/cudaFree.  All kernels
+ *     are launched on mcdc_device.stream (a cudaStream_t; NULL = the legacy default stream).
+ *   - every call returns 0 or a negative MCDC_E* code; mcdc_last_error() gives a thread-local
+ *     message.  Nothing throws or aborts across the ABI; a failed run leaves earlier tallies intact.
+ *   - all floating point is float64.
+ */
+#ifndef MCDC_H
+#define MCDC_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { MCDC_OK = 0, MCDC_EINVAL = -1, MCDC_EGEOM = -2, MCDC_EBANK = -3, MCDC_ELOST = -4, MCDC_ECUDA = -5,
+       MCDC_ENOMEM = -6 };
+
+/* surface types / boundary conditions (R11-R13) */
+enum { MCDC_PLANE_X = 0, MCDC_PLANE_Y, MCDC_PLANE_Z, MCDC_PLANE, MCDC_CYL_X, MCDC_CYL_Y, MCDC_CYL_Z, MCDC_SPHERE };
+enum { MCDC_BC_TRANSMIT = 0, MCDC_BC_REFLECT = 1, MCDC_BC_VACUUM = 2 };
+
+/* event codes of the trace and of the event counters (one event per segment) */
+enum { MCDC_EV_SCATTER = 1, MCDC_EV_FISSION, MCDC_EV_CAPTURE, MCDC_EV_TRANSMIT, MCDC_EV_REFLECT, MCDC_EV_LEAK,
+       MCDC_EV_LATTICE, MCDC_EV_TIME_EDGE, MCDC_EV_CUTOFF, MCDC_EV_LOST };
+/* counters[0] tracks started, [1..10] events by code, [11] children banked, [12] bank high-water mark,
+ * [13] sweeps (kernel rounds), [14] tail-kernel histories, [15] reserved */
+#define MCDC_N_COUNTERS 16
+
+/* CSG geometry: surfaces, conjunctive cells grouped by universe, one optional rectangular lattice
+ * (R11-R16).  surf_param[s][4]: PLANE_X/Y/Z (p,-,-,-); PLANE (a,b,c,d): a x+b y+c z = d; CYL_Z (x0,y0,r,-)
+ * (CYL_X (y0,z0,r), CYL_Y (x0,z0,r)); SPHERE (x0,y0,z0,r).  Cells of universe u are
+ * [univ_cell_off[u], univ_cell_off[u+1]); universe 0 is the root.  cell_fill_type 0: cell_fill = material
+ * id; 1: the cell is filled by the lattice (at most one such cell, in the root universe).  lat_univ[iy][ix]
+ * names the universe of element (ix,iy); its cells are written in element-centred coordinates. */
+typedef struct {
+    int32_t n_surf;
+    const int32_t *surf_type;
+    const double *surf_param;
+    const int32_t *surf_bc;
+    int32_t n_cell;
+    const int32_t *cell_surf_off;   /* [n_cell+1] */
+    const int32_t *cell_surf_id;    /* [cell_surf_off[n_cell]] */
+    const int32_t *cell_surf_sense; /* +1: f(x) > 0 side, -1: f(x) < 0 side */
+    const int32_t *cell_fill_type;
+    const int32_t *cell_fill;
+    int32_t n_univ;
+    const int32_t *univ_cell_off; /* [n_univ+1] */
+    int32_t has_lattice;
+    double lat_x0, lat_y0, lat_px, lat_py;
+    int32_t lat_nx, lat_ny;
+    const int32_t *lat_univ; /* [lat_ny][lat_nx] */
+} mcdc_geometry;
+
+/* multi-group materials (R3-R5, R30): arrays [n_mat][G]; S[n_mat][G][G], row = incident group.
+ * Sigma_s = row sum of S; Sigma_c = Sigma_t - Sigma_s - Sigma_f.  Pass NULL for a continuous-energy problem. */
+typedef struct {
+    int32_t n_mat, G;
+    const double *sig_t, *sig_f, *nu, *chi, *S;
+} mcdc_materials;
+
+/* continuous-energy data (R19-R23): union grid [n_grid] (eV, strictly increasing), microscopic elastic /
+ * capture / fission per nuclide [n_nuc][n_grid] (barns), materials as (nuclide, atom density 1/(b cm)) lists,
+ * nu(E) = nu0 + nu1 E[MeV], Watt(a [MeV], b [1/MeV]).  Pass NULL for a multi-group problem.
+ * search: 0 binary search on the grid, 1 hashed search (exponent/mantissa-keyed buckets, then bisection);
+ * both return the same index. */
+typedef struct {
+    int32_t n_mat;
+    int32_t n_grid;
+    const double *grid;
+    int32_t n_nuc;
+    const double *nuc_A;
+    const double *nuc_el, *nuc_c, *nuc_f;
+    const int32_t *mat_nuc_off; /* [n_mat+1] */
+    const int32_t *mat_nuc_id;
+    const double *mat_nuc_dens;
+    double nu0, nu1, watt_a, watt_b;
+    int32_t search;
+} mcdc_xs;
+
+/* source: uniform in the box [lo,hi], isotropic or fixed direction; MG: group pdf [G]; CE: mono-energetic E
+ * (eV) at time t (s).  Birth always consumes six draws (draw budget table of DESIGN.md). */
+typedef struct {
+    double lo[3], hi[3];
+    int32_t isotropic;
+    double dir[3];
+    const double *group_pdf;
+    double E, t;
+} mcdc_source;
+
+/* track-length flux tally (R17, R24): spatial bin of a particle = cell_bin[cell] (+ lat_bin[element] inside
+ * the lattice); MG: flux[bin][g]; CE: flux[bin][time bin][energy bin] with explicit edges. */
+typedef struct {
+    int32_t n_bins;
+    const int32_t *cell_bin; /* [n_cell] */
+    const int32_t *lat_bin;  /* [lat_ny][lat_nx] or NULL */
+    int32_t n_t;
+    const double *t_edges; /* [n_t+1], CE only */
+    int32_t n_e;
+    const double *e_edges; /* [n_e+1], CE only */
+} mcdc_tally_spec;
+
+/* device resources handed in by the caller.  schedule: 0 = per-event kernels over compacted index queues
+ * (default), 1 = monolithic one-segment-per-launch kernel over every bank slot, no compaction (the paper's
+ * PAPER.md:51-55 design, kept for the divergence comparison).  tail_threshold: when at most this many
+ * particles are alive the remaining histories are finished inside one kernel (0 = library default,
+ * negative = never). */
+typedef struct {
+    void *workspace; /* DEVICE pointer, 256-byte aligned */
+    uint64_t workspace_bytes;
+    void *stream; /* cudaStream_t */
+    int32_t device;
+    int32_t schedule;
+    int32_t tail_threshold;
+    int32_t reserved;
+} mcdc_device;
+
+typedef struct {
+    int32_t mode; /* 0 MG, 1 CE */
+    int32_t n_tally; /* length of flux_mean / flux_sdev */
+    int32_t n_cycles; /* cycles run so far (fixed source: 1) */
+    int32_t n_active;
+    uint64_t bank_count; /* sites in the current source bank */
+} mcdc_dims;
+
+typedef struct {
+    double *k_cycle;   /* [n_cycles] */
+    double *flux_mean; /* [n_tally] */
+    double *flux_sdev; /* [n_tally] */
+    uint64_t *counters; /* [MCDC_N_COUNTERS] */
+    double k_mean, k_sdev, leak_mean, leak_sdev;
+} mcdc_tallies;
+
+/* one record per event of a traced particle: location BEFORE the event (root cell c0, lattice element or -1,
+ * local cell c1 or -1), surface hit (or -1; n_surf+k for lattice wall k), group / grid index, position and time
+ * AFTER the move, flight distance d and flight energy E. */
+typedef struct {
+    uint64_t id;
+    uint32_t cycle, seq;
+    int32_t ev, c0, elem, c1, surf, gi;
+    double x, y, z, d, E, t;
+} mcdc_trace_rec;
+
+/* fission-bank site (R5: the parent samples group and direction) */
+typedef struct {
+    double x, y, z, ux, uy, uz;
+    int32_t g;
+    int32_t pad;
+} mcdc_site;
+
+typedef struct mcdc_problem mcdc_problem;
+
+/* bytes of device workspace needed for runs of up to n_particles nominal particles per cycle. */
+int mcdc_workspace_bytes(const mcdc_geometry *geo, const mcdc_materials *mat, const mcdc_xs *xs,
+                         const mcdc_tally_spec *tally, uint64_t n_particles, uint64_t *bytes);
+
+/* validate + copy all inputs, build derived tables (cumulative scatter rows, chi CDF, macroscopic CE rows,
+ * hash buckets), upload them into the workspace.  Exactly one of mat / xs is non-NULL. */
+int mcdc_create(const mcdc_geometry *geo, const mcdc_materials *mat, const mcdc_xs *xs, const mcdc_source *src,
+                const mcdc_tally_spec *tally, const mcdc_device *dev, uint64_t max_particles, mcdc_problem **out);
+
+/* k-eigenvalue power iteration (R6, R7): n_inactive + n_active cycles of n_particles nominal
+ * histories; cycle 0 samples the source, later cycles start from the fission bank with weight N/M. */
+int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, int32_t n_inactive, int32_t n_active, uint64_t seed);
+
+/* one power-iteration cycle (cycle 0 resets the run and samples the source); returns the cycle's
+ * track-length k.  active != 0 accumulates the flux / leakage / k statistics. */
+int mcdc_run_cycle(mcdc_problem *p, uint64_t n_particles, uint32_t cycle, int32_t active, uint64_t seed,
+                   double *k_cycle);
+
+/* host-buffer form of one cycle (the end-to-end path): uploads n_in source sites from HOST memory (NULL/0:
+ * sample the source), transports them as cycle `cycle` with k_prev, downloads the produced fission bank
+ * (at most max_out sites; *n_out = produced count) and this cycle's per-source-particle flux [n_tally]. */
+int mcdc_run_cycle_host(mcdc_problem *p, uint64_t n_particles, uint32_t cycle, uint64_t seed, double k_prev,
+                        const mcdc_site *sites_in, uint64_t n_in, mcdc_site *sites_out, uint64_t max_out,
+                        uint64_t *n_out, double *flux_cycle, double *k_cycle, double *leak_cycle);
+
+/* time-dependent fixed source, continuous energy (R24, R25): n_particles source particles and
+ * all their prompt fission secondaries, to the last time edge. */
+int mcdc_run_fixed_source(mcdc_problem *p, uint64_t n_particles, uint64_t seed);
+
+int mcdc_get_dims(const mcdc_problem *p, mcdc_dims *dims);
+int mcdc_get_tallies(const mcdc_problem *p, mcdc_tallies *out);
+/* current source bank (after a cycle: the sorted fission bank), at most max sites; returns the count via *n */
+int mcdc_get_bank(const mcdc_problem *p, mcdc_site *out, uint64_t max, uint64_t *n);
+
+/* record the events of particles first_id .. first_id+n_ids-1 (at most max_events each, per cycle) */
+int mcdc_set_trace(mcdc_problem *p, uint64_t first_id, uint32_t n_ids, uint32_t max_events);
+/* copies at most max records (ordered by cycle, id, seq); *n = records available */
+int mcdc_get_trace(const mcdc_problem *p, mcdc_trace_rec *out, uint64_t max, uint64_t *n);
+
+/* unit-level entry points (device kernels behind them; used by the parity tests):
+ * n uniform draws of stream (seed, id[i], domain, cycle) at index draw[i] */
+int mcdc_test_draws(mcdc_problem *p, uint64_t seed, uint32_t domain, uint32_t cycle, const uint64_t *id,
+                    const uint32_t *draw, uint64_t n, double *out);
+/* union-grid index of E[i] with the binary (out_bin) and the hashed (out_hash) search */
+int mcdc_test_grid_index(mcdc_problem *p, const double *E, uint64_t n, int32_t *out_bin, int32_t *out_hash);
+/* locate + nearest boundary for n points: loc[i][3] = (c0, elem, c1), dist[i], surf[i] */
+int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64_t n, int32_t *loc, double *dist,
+                       int32_t *surf);
+
+/* device time (ms, CUDA events on the library's stream) of the transport part of the last run call, and the
+ * number of kernels it launched */
+int mcdc_get_timing(const mcdc_problem *p, double *ms_transport, uint64_t *n_launches);
+
+void mcdc_destroy(mcdc_problem *p);
+const char *mcdc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,525 @@
+// mcdc_kernels.cuh -- the kernels of the event-based transport loop.
+//
+// Event schedule (default): per sweep three kernels regroup the live particles by next event
+//   k_advance  (a2/a3 XS lookup, a5 nearest boundary, a6 distance to collision, a7 move + tallies, reaction
+//               choice) over the live queue; each block appends its scatter events to the FRONT and its
+//               surface / lattice / time-edge events to the BACK of the next queue with ballot + prefix-sum
+//               compaction and one atomic per block and queue (a11);
+//   k_scatter  (a8) over the front region;   k_surface (a9) over the back region.
+// Fission and capture end a history inside k_advance; the children are produced at the end of the cycle
+// by count -> exclusive scan -> write (a10/a12), which yields the bank sorted by (parent id, child index)
+// without atomics or a sort.  k_segment is the paper's monolithic design: one whole
+// segment for every bank slot per launch, no compaction.  k_finish ends the last few histories in registers.
+#pragma once
+#include "mcdc_device.cuh"
+
+namespace mcdc {
+
+constexpr int BS = 256;  // threads per block of every transport kernel
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ------------------------------------------------------------------ bank access
+template <bool CE>
+__device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr)
+{
+    p.x = B.x[i]; p.y = B.y[i]; p.z = B.z[i];
+    p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i];
+    p.cell = B.cell[i]; p.elem = B.elem[i];
+    int gl = B.gl[i];
+    p.g = gl & 0xffff; p.last = (gl >> 16) - 1;
+    ctr = B.ctr[i];
+    if (CE) { p.E = B.E[i]; p.t = B.t[i]; p.tbin = B.tbin[i]; p.id = B.id[i]; }
+    else { p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = i; }
+}
+
+__device__ __forceinline__ int pack_gl(int g, int last) { return (g & 0xffff) | ((last + 1) << 16); }
+
+// per-block flush of the thread accumulators: k numerator, leakage, event counters
+__device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
+{
+    __shared__ double s_k[BS / 32], s_l[BS / 32];
+    __shared__ unsigned int s_ev[11];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x < 11) s_ev[threadIdx.x] = 0;
+    double k = warp_sum(acc.knum), l = warp_sum(acc.leak);
+    if (lane == 0) { s_k[w] = k; s_l[w] = l; }
+    __syncthreads();
+#pragma unroll
+    for (int e = 1; e < 11; e++) {
+        unsigned int n = acc.n_ev[e];
+        n = __reduce_add_sync(0xffffffffu, n);
+        if (lane == 0 && n) atomicAdd(&s_ev[e], n);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double ks = 0.0, ls = 0.0;
+        for (int i = 0; i < BS / 32; i++) { ks += s_k[i]; ls += s_l[i]; }
+        if (ks != 0.0) atomicAdd(c.scal + 0, ks);
+        if (ls != 0.0) atomicAdd(c.scal + 1, ls);
+    }
+    if (threadIdx.x >= 1 && threadIdx.x < 11 && s_ev[threadIdx.x])
+        atomicAdd(c.counters + threadIdx.x, (unsigned long long)s_ev[threadIdx.x]);
+}
+
+// shared-memory tally columns (one per thread) -> one float64 atomic per bin and block
+__device__ __forceinline__ void flush_private_flux(const Ctx &c, const double *s_flux)
+{
+    __syncthreads();
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int b = w; b < c.n_tally; b += BS / 32) {
+        double v = 0.0;
+        for (int t = lane; t < BS; t += 32) v += s_flux[b * BS + t];
+        v = warp_sum(v);
+        if (lane == 0 && v != 0.0) atomicAdd(c.flux + b, v);
+    }
+}
+
+// ballot + prefix-sum compaction of one block's events into the two ends of the next queue (a11)
+__device__ __forceinline__ void block_push(bool to_front, bool to_back, unsigned int idx, unsigned int *qout, QCount *oc,
+                                           unsigned int q_cap)
+{
+    __shared__ unsigned int s_n[2][BS / 32];
+    __shared__ unsigned int s_base[2];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned int mf = __ballot_sync(0xffffffffu, to_front), mb = __ballot_sync(0xffffffffu, to_back);
+    if (lane == 0) { s_n[0][w] = __popc(mf); s_n[1][w] = __popc(mb); }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        unsigned int tot = 0;
+        for (int i = 0; i < BS / 32; i++) { unsigned int n = s_n[threadIdx.x][i]; s_n[threadIdx.x][i] = tot; tot += n; }
+        s_base[threadIdx.x] = tot ? atomicAdd(threadIdx.x == 0 ? &oc->n_scat : &oc->n_surf, tot) : 0u;
+    }
+    __syncthreads();
+    unsigned int lt = (1u << lane) - 1u;
+    if (to_front) qout[s_base[0] + s_n[0][w] + __popc(mf & lt)] = idx;
+    if (to_back) qout[q_cap - 1u - (s_base[1] + s_n[1][w] + __popc(mb & lt))] = idx;
+    __syncthreads();
+}
+
+__device__ __forceinline__ unsigned int queue_entry(const unsigned int *qin, unsigned int q_cap, unsigned int n_front,
+                                                    unsigned int t)
+{
+    return t < n_front ? qin[t] : qin[q_cap - 1u - (t - n_front)];
+}
+
+// ------------------------------------------------------------------ a1: source
+template <bool CE>
+__global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
+{
+    unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Bank &B = c.bank[c.cur];
+    Rng rng;
+    rng.init(c.seed, i, 0u, c.cycle, 0u);
+    double xi[6];
+#pragma unroll
+    for (int k = 0; k < 6; k++) xi[k] = rng.next();  // always six draws
+    double x = c.src_lo[0] + xi[0] * (c.src_hi[0] - c.src_lo[0]);
+    double y = c.src_lo[1] + xi[1] * (c.src_hi[1] - c.src_lo[1]);
+    double z = c.src_lo[2] + xi[2] * (c.src_hi[2] - c.src_lo[2]);
+    double ux = c.src_dir[0], uy = c.src_dir[1], uz = c.src_dir[2];
+    if (c.src_iso) iso_dir(xi[3], xi[4], ux, uy, uz);
+    int g = 0;
+    if (!CE) g = pick(c.mg.src_cum, c.mg.G, xi[5] * __ldg(c.mg.src_cum + c.mg.G - 1));
+    int cell, elem;
+    if (!locate(c.geo, x, y, z, ux, uy, uz, -1, cell, elem)) { atomicExch(c.err, -2); cell = -1; }
+    B.x[i] = x; B.y[i] = y; B.z[i] = z; B.ux[i] = ux; B.uy[i] = uy; B.uz[i] = uz;
+    B.cell[i] = cell; B.elem[i] = elem; B.gl[i] = pack_gl(g, -1); B.ctr[i] = 6u;
+    B.ev[i] = cell < 0 ? EV_DEAD : 0; B.fis_n[i] = 0;
+    if (CE) {
+        B.E[i] = c.src_E; B.t[i] = c.src_t; B.tbin[i] = edge_bin(c.ce.t_edges, c.ce.n_t, c.src_t); B.id[i] = i;
+    }
+}
+
+struct Site { double x, y, z, ux, uy, uz; int g, pad; };
+
+// source particles from a bank of sites handed in by the host (no draws at birth)
+__global__ void __launch_bounds__(BS) k_load_sites(Ctx c, const Site *sites, unsigned int n)
+{
+    unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Bank &B = c.bank[c.cur];
+    Site s = sites[i];
+    int cell, elem;
+    if (!locate(c.geo, s.x, s.y, s.z, s.ux, s.uy, s.uz, -1, cell, elem)) { atomicExch(c.err, -2); cell = -1; }
+    B.x[i] = s.x; B.y[i] = s.y; B.z[i] = s.z; B.ux[i] = s.ux; B.uy[i] = s.uy; B.uz[i] = s.uz;
+    B.cell[i] = cell; B.elem[i] = elem; B.gl[i] = pack_gl(s.g, -1); B.ctr[i] = 0u;
+    B.ev[i] = cell < 0 ? EV_DEAD : 0; B.fis_n[i] = 0;
+}
+
+__global__ void __launch_bounds__(BS) k_store_sites(Ctx c, Site *sites, unsigned int n)
+{
+    unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Bank &B = c.bank[c.cur];
+    Site s;
+    s.x = B.x[i]; s.y = B.y[i]; s.z = B.z[i]; s.ux = B.ux[i]; s.uy = B.uy[i]; s.uz = B.uz[i];
+    s.g = B.gl[i] & 0xffff; s.pad = 0;
+    sites[i] = s;
+}
+
+// ------------------------------------------------------------------ per-event kernels
+template <bool CE, bool PRIVATE>
+__global__ void __launch_bounds__(BS) k_advance(Ctx c, unsigned int s, unsigned int n0)
+{
+    extern __shared__ double s_flux[];
+    unsigned int n_front = 0, n_in = n0;
+    const unsigned int *qin = c.q[s & 1];
+    if (s > 0) {
+        QCount pc = c.qc[(s - 1) % RING];
+        n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
+    }
+    unsigned int *qout = c.q[(s + 1) & 1];
+    QCount *oc = c.qc + (s % RING);
+    if (PRIVATE) {
+        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
+        __syncthreads();
+    }
+    Acc acc;
+    acc.knum = acc.leak = 0.0;
+#pragma unroll
+    for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
+    const Bank &B = c.bank[c.cur];
+    for (unsigned int base = blockIdx.x * BS; base < n_in; base += gridDim.x * BS) {
+        unsigned int t = base + threadIdx.x, i = 0;
+        int code = ADV_DEAD;
+        if (t < n_in) {
+            i = s == 0 ? t : queue_entry(qin, c.q_cap, n_front, t);
+            int cell = B.cell[i];
+            if (cell >= 0) {
+                Particle p;
+                uint32_t ctr;
+                load_full<CE>(B, i, p, ctr);
+                const int last0 = p.last, tbin0 = p.tbin;
+                Rng rng;
+                rng.init(c.seed, p.id, 0u, c.cycle, ctr);
+                int aux = 0;
+                code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+                B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z;
+                B.ctr[i] = rng.ctr;
+                if (code == ADV_FISSION) { B.fis_n[i] = aux; code = ADV_DEAD; }
+                else if (code != ADV_DEAD) B.ev[i] = aux;
+                if (p.last != last0) B.gl[i] = pack_gl(p.g, p.last);
+                if (CE) { B.t[i] = p.t; if (p.tbin != tbin0) B.tbin[i] = p.tbin; }
+            }
+        }
+        block_push(code == ADV_SCATTER, code == ADV_SURFACE, i, qout, oc, c.q_cap);
+    }
+    if (PRIVATE) flush_private_flux(c, s_flux);
+    flush_acc(c, acc);
+}
+
+template <bool CE>
+__global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
+{
+    const QCount oc = c.qc[s % RING];
+    const unsigned int *q = c.q[(s + 1) & 1];
+    const Bank &B = c.bank[c.cur];
+    // queue-counter housekeeping: clear the set the next sweep appends to
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        QCount z = {0u, 0u, 0u, 0u};
+        c.qc[(s + 1) % RING] = z;
+    }
+    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_scat; t += gridDim.x * BS) {
+        unsigned int i = q[t];
+        Particle p;
+        int gl = B.gl[i];
+        p.g = gl & 0xffff;
+        p.cell = B.cell[i];
+        p.id = CE ? B.id[i] : i;
+        if (CE) { p.E = B.E[i]; p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i]; }
+        Rng rng;
+        rng.init(c.seed, p.id, 0u, c.cycle, B.ctr[i]);
+        do_scatter<CE>(c, p, rng, B.ev[i]);
+        B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
+        B.gl[i] = pack_gl(p.g, -1);
+        B.ctr[i] = rng.ctr;
+        if (CE) B.E[i] = p.E;
+    }
+}
+
+__global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
+{
+    const QCount oc = c.qc[s % RING];
+    const unsigned int *q = c.q[(s + 1) & 1];
+    const Bank &B = c.bank[c.cur];
+    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_surf; t += gridDim.x * BS) {
+        unsigned int i = q[c.q_cap - 1u - t];
+        int hit = B.ev[i];
+        if (hit == HIT_TIME_EDGE) continue;
+        Particle p;
+        p.x = B.x[i]; p.y = B.y[i]; p.z = B.z[i];
+        p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i];
+        p.cell = B.cell[i]; p.elem = B.elem[i];
+        int gl = B.gl[i];
+        p.g = gl & 0xffff; p.last = (gl >> 16) - 1;
+        const int cell0 = p.cell, elem0 = p.elem;
+        const double ux0 = p.ux, uy0 = p.uy, uz0 = p.uz;
+        if (!do_surface(c, p, hit)) {
+            atomicExch(c.err, -2);
+            atomicAdd(c.counters + 10, 1ull);
+            p.cell = -1;
+        }
+        if (p.cell != cell0) B.cell[i] = p.cell;
+        if (p.elem != elem0) B.elem[i] = p.elem;
+        B.gl[i] = pack_gl(p.g, p.last);
+        if (p.ux != ux0) B.ux[i] = p.ux;
+        if (p.uy != uy0) B.uy[i] = p.uy;
+        if (p.uz != uz0) B.uz[i] = p.uz;
+    }
+}
+
+// whole segment in registers (shared by the monolithic schedule and the tail kernel)
+template <bool CE, bool PRIVATE>
+__device__ __forceinline__ bool segment(const Ctx &c, const Bank &B, unsigned int i, Particle &p, Rng &rng, Acc &acc,
+                                        double *s_flux)
+{
+    int aux = 0;
+    int code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+    if (code == ADV_SCATTER) { do_scatter<CE>(c, p, rng, aux); return true; }
+    if (code == ADV_SURFACE) {
+        if (!do_surface(c, p, aux)) {
+            atomicExch(c.err, -2);
+            atomicAdd(c.counters + 10, 1ull);
+            p.cell = -1;
+            return false;
+        }
+        return true;
+    }
+    if (code == ADV_FISSION) B.fis_n[i] = aux;
+    return false;
+}
+
+template <bool CE>
+__device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr)
+{
+    B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z; B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
+    B.cell[i] = p.cell; B.elem[i] = p.elem; B.gl[i] = pack_gl(p.g, p.last); B.ctr[i] = ctr;
+    if (CE) { B.E[i] = p.E; B.t[i] = p.t; B.tbin[i] = p.tbin; }
+}
+
+// monolithic schedule: every slot, one segment, no compaction; counts the survivors
+template <bool CE, bool PRIVATE>
+__global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned int n)
+{
+    extern __shared__ double s_flux[];
+    if (PRIVATE) {
+        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
+        __syncthreads();
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        QCount z = {0u, 0u, 0u, 0u};
+        c.qc[(s + 1) % RING] = z;
+    }
+    Acc acc;
+    acc.knum = acc.leak = 0.0;
+#pragma unroll
+    for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
+    const Bank &B = c.bank[c.cur];
+    unsigned int alive = 0;
+    for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
+        if (B.ev[i] == EV_DEAD) continue;
+        Particle p;
+        uint32_t ctr;
+        load_full<CE>(B, i, p, ctr);
+        Rng rng;
+        rng.init(c.seed, p.id, 0u, c.cycle, ctr);
+        bool live = segment<CE, PRIVATE>(c, B, i, p, rng, acc, s_flux);
+        store_full<CE>(B, i, p, rng.ctr);
+        if (!live) B.ev[i] = EV_DEAD; else alive++;
+    }
+    alive = __reduce_add_sync(0xffffffffu, alive);
+    if ((threadIdx.x & 31) == 0 && alive) atomicAdd(&c.qc[s % RING].n_alive, alive);
+    if (PRIVATE) flush_private_flux(c, s_flux);
+    flush_acc(c, acc);
+}
+
+// tail: finish the few remaining histories of the live queue inside one kernel
+template <bool CE, bool PRIVATE>
+__global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned int n0)
+{
+    extern __shared__ double s_flux[];
+    if (PRIVATE) {
+        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
+        __syncthreads();
+    }
+    unsigned int n_front = 0, n_in = n0;
+    const unsigned int *qin = c.q[s & 1];
+    if (s > 0) {
+        QCount pc = c.qc[(s - 1) % RING];
+        n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
+    }
+    Acc acc;
+    acc.knum = acc.leak = 0.0;
+#pragma unroll
+    for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
+    const Bank &B = c.bank[c.cur];
+    unsigned int done = 0;
+    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < n_in; t += gridDim.x * BS) {
+        unsigned int i = s == 0 ? t : queue_entry(qin, c.q_cap, n_front, t);
+        if (B.cell[i] < 0) continue;
+        Particle p;
+        uint32_t ctr;
+        load_full<CE>(B, i, p, ctr);
+        Rng rng;
+        rng.init(c.seed, p.id, 0u, c.cycle, ctr);
+        unsigned int guard = 0;
+        while (segment<CE, PRIVATE>(c, B, i, p, rng, acc, s_flux)) {
+            if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
+        }
+        store_full<CE>(B, i, p, rng.ctr);
+        done++;
+    }
+    done = __reduce_add_sync(0xffffffffu, done);
+    if ((threadIdx.x & 31) == 0 && done) atomicAdd(c.counters + 14, (unsigned long long)done);
+    if (PRIVATE) flush_private_flux(c, s_flux);
+    flush_acc(c, acc);
+}
+
+// ------------------------------------------------------------------ a10/a12: fission bank by count-scan-write
+__global__ void __launch_bounds__(BS) k_scan_partial(Ctx c, unsigned int n, unsigned int *part)
+{
+    __shared__ unsigned int s_w[BS / 32];
+    unsigned int i = blockIdx.x * BS + threadIdx.x;
+    unsigned int v = i < n ? (unsigned int)c.bank[c.cur].fis_n[i] : 0u;
+    v = __reduce_add_sync(0xffffffffu, v);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int t = 0;
+        for (int k = 0; k < BS / 32; k++) t += s_w[k];
+        part[blockIdx.x] = t;
+    }
+}
+
+// exclusive scan of the per-block counts by one block; total -> part[nb]
+__global__ void __launch_bounds__(1024) k_scan_top(unsigned int *part, unsigned int nb)
+{
+    __shared__ unsigned int s_sum[1024];
+    unsigned int per = (nb + 1023u) / 1024u;
+    unsigned int lo = threadIdx.x * per, hi = lo + per < nb ? lo + per : nb;
+    unsigned int t = 0;
+    for (unsigned int k = lo; k < hi; k++) t += part[k];
+    s_sum[threadIdx.x] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int run = 0;
+        for (int k = 0; k < 1024; k++) { unsigned int v = s_sum[k]; s_sum[k] = run; run += v; }
+        part[nb] = run;
+    }
+    __syncthreads();
+    unsigned int run = s_sum[threadIdx.x];
+    for (unsigned int k = lo; k < hi; k++) { unsigned int v = part[k]; part[k] = run; run += v; }
+}
+
+// every fission parent writes its children into the next bank at [offset(parent), +n): sorted by (parent id,
+// child index) by construction.  MG: child group ~ chi, isotropic direction (1 + 2 draws per child) from the
+// parent's stream (R5).  CE: Watt energy (4 draws) + direction (2 draws), own id from the domain-1 block (R10).
+template <bool CE>
+__global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsigned int *part, unsigned int cap)
+{
+    __shared__ unsigned int s_w[BS / 32];
+    const Bank &B = c.bank[c.cur];
+    const Bank &O = c.bank[1 - c.cur];
+    unsigned int i = blockIdx.x * BS + threadIdx.x;
+    int nc = i < n ? B.fis_n[i] : 0;
+    // block exclusive scan
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned int incl = (unsigned int)nc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) s_w[w] = incl;
+    __syncthreads();
+    unsigned int wbase = 0;
+    for (int k = 0; k < w; k++) wbase += s_w[k];
+    unsigned int off = part[blockIdx.x] + wbase + incl - (unsigned int)nc;
+    if (nc <= 0) return;
+    if (off + (unsigned int)nc > cap) { atomicExch(c.err, -3); return; }  // bank overflow (R6)
+    double x = B.x[i], y = B.y[i], z = B.z[i];
+    int cell = B.cell[i], elem = B.elem[i];
+    const int mat = __ldg(c.geo.cfill + cell);
+    unsigned long long pid = CE ? B.id[i] : (unsigned long long)i;
+    uint32_t ctr0 = B.ctr[i];
+    Rng rng;
+    rng.init(c.seed, pid, 0u, c.cycle, ctr0);
+    for (int j = 0; j < nc; j++) {
+        unsigned int o = off + j;
+        double ux, uy, uz;
+        int g = 0;
+        if (!CE) {
+            const double *cc = c.mg.cumchi + (size_t)mat * c.mg.G;
+            g = pick(cc, c.mg.G, rng.next() * __ldg(cc + c.mg.G - 1));
+            double a = rng.next(), b = rng.next();
+            iso_dir(a, b, ux, uy, uz);
+        } else {
+            double a1 = rng.next(), a2 = rng.next(), a3 = rng.next(), a4 = rng.next();
+            double En = 1e6 * watt(c.ce.watt_a, c.ce.watt_b, a1, a2, a3, a4);
+            if (En < c.ce.E_min) En = c.ce.E_min;
+            if (En > c.ce.E_max) En = c.ce.E_max;
+            double a = rng.next(), b = rng.next();
+            iso_dir(a, b, ux, uy, uz);
+            O.E[o] = En; O.t[o] = B.t[i]; O.tbin[o] = B.tbin[i];
+            O.id[o] = child_id(c.seed, pid, ctr0, (uint32_t)j);
+        }
+        O.x[o] = x; O.y[o] = y; O.z[o] = z; O.ux[o] = ux; O.uy[o] = uy; O.uz[o] = uz;
+        O.cell[o] = cell; O.elem[o] = elem; O.gl[o] = pack_gl(g, -1); O.ctr[o] = 0u;
+        O.ev[o] = 0; O.fis_n[o] = 0;
+    }
+}
+
+// cycle end: per-source-particle flux into the running mean / mean-square, clear the per-cycle tally (R17)
+__global__ void __launch_bounds__(BS) k_accumulate(double *flux, double *acc, double *acc2, int n_tally, double inv_n,
+                                                   int active)
+{
+    int i = blockIdx.x * BS + threadIdx.x;
+    if (i >= n_tally) return;
+    double f = flux[i] * inv_n;
+    if (active) { acc[i] += f; acc2[i] += f * f; }
+    flux[i] = 0.0;
+}
+
+// ------------------------------------------------------------------ unit-level test kernels
+__global__ void k_test_draws(unsigned long long seed, uint32_t domain, uint32_t cycle, const unsigned long long *id,
+                             const uint32_t *draw, unsigned long long n, double *out)
+{
+    unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Rng rng;
+    rng.init(seed, id[i], domain, cycle, draw[i]);
+    out[i] = rng.next();
+}
+
+__global__ void k_test_grid(Ctx c, const double *E, unsigned long long n, int *ob, int *oh)
+{
+    unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    ob[i] = grid_index_binary(c.ce, E[i]);
+    oh[i] = grid_index_hash(c.ce, E[i]);
+}
+
+__global__ void k_test_geometry(Ctx c, const double *x, const double *u, unsigned long long n, int *loc, double *dist,
+                                int *surf)
+{
+    unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int cell, elem, hit = -1;
+    bool ok = locate(c.geo, x[3 * i], x[3 * i + 1], x[3 * i + 2], u[3 * i], u[3 * i + 1], u[3 * i + 2], -1, cell, elem);
+    double d = -1.0;
+    if (ok) d = nearest(c.geo, x[3 * i], x[3 * i + 1], x[3 * i + 2], u[3 * i], u[3 * i + 1], u[3 * i + 2], cell, elem, -1, hit);
+    loc[3 * i] = !ok ? -1 : (elem >= 0 ? c.geo.lat_cell : cell);
+    loc[3 * i + 1] = ok ? elem : -1;
+    loc[3 * i + 2] = ok && elem >= 0 ? cell : -1;
+    dist[i] = d;
+    surf[i] = hit;
+}
+
+}  // namespace mcdc
