@@ -1,0 +1,82 @@
+"""GPU parity for the continuous-energy time-dependent path (C5 and its closed-form reductions)."""
+import numpy as np
+import pytest
+
+from paper_2501_05440_b200 import inputs
+from tests.test_gpu_parity import compare_traces
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    from paper_2501_05440_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def compare_ce(r, ro, rtol=1e-9):
+    assert np.allclose(r["k_cycle"], ro["k_cycle"], rtol=rtol)
+    scale = np.abs(ro["flux_mean"]).max()
+    assert np.allclose(r["flux_mean"], ro["flux_mean"], rtol=rtol, atol=1e-13 * scale)
+    # events by type, tracks started and children banked are integers: exact
+    assert (r["counters"][:12] == ro["counters"][:12]).all(), (r["counters"], ro["counters"])
+
+
+CE_CASES = {
+    "C5": lambda: inputs.config5(n_particles=1500, n_grid=50_000),
+    "C5jitter": lambda: inputs.config5(n_particles=1201, n_grid=7000, jitter=True),
+    "ce_1v": lambda: inputs.ce_one_over_v(n_particles=20000),
+    "ce_scatter": lambda: inputs.ce_single_scatterer(A=16.0, n_particles=5000),
+    "ce_scatterH": lambda: inputs.ce_single_scatterer(A=1.0, n_particles=5000),
+    "ce_fission": lambda: _fis(),
+}
+
+
+def _fis():
+    P = inputs.ce_pure_fission(2000)
+    P["t_edges"] = np.array([0.0, 1.0e-9])
+    return P
+
+
+@pytest.mark.parametrize("name", list(CE_CASES))
+@pytest.mark.parametrize("schedule,tail,search", [(0, 0, 0), (0, -1, 1), (0, 1 << 30, 1), (1, 0, 0)])
+def test_ce_parity(gpu, orc, name, schedule, tail, search):
+    P = CE_CASES[name]()
+    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, search=search)
+    r = g.run()
+    o = orc.Oracle(P)
+    rc, ro = o.run()
+    assert rc == 0
+    compare_ce(r, ro)
+    g.close()
+
+
+@pytest.mark.parametrize("schedule,tail,search", [(0, -1, 0), (0, 0, 1), (1, 0, 1)])
+def test_ce_traces_identical(gpu, orc, schedule, tail, search):
+    """Source particles 0..99 of C5: identical event sequences incl. grid index, time, energy."""
+    P = inputs.config5(n_particles=400, n_grid=20_000)
+    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, search=search)
+    g.set_trace(0, 100, 4096)
+    r = g.run()
+    o = orc.Oracle(P)
+    o.set_trace(0, 100, 2_000_000)
+    rc, ro = o.run()
+    compare_traces(g.trace(), o.trace())
+    compare_ce(r, ro)
+    g.close()
+
+
+@pytest.mark.parametrize("jitter", [False, True])
+def test_grid_search_binary_equals_hash_equals_numpy(gpu, jitter):
+    P = inputs.config5(n_particles=10, n_grid=50_000, jitter=jitter)
+    g = gpu.Problem(P)
+    grid = P["grid"]
+    rng = np.random.default_rng(3)
+    E = np.concatenate([np.exp(rng.uniform(np.log(1e-6), np.log(1e8), 200_000)), grid, np.nextafter(grid, 0),
+                        np.nextafter(grid, np.inf), [1e-7, 5e7, grid[0], grid[-1]]])
+    ref = np.clip(np.searchsorted(grid, E, side="right") - 1, 0, len(grid) - 2)
+    ob, oh = g.grid_index(E)
+    assert (ob == ref).all()
+    assert (oh == ref).all()
+    g.close()
