@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the event-based Monte Carlo transport hot path on B200 (one JSON line).
+
+Workload (BASELINE.json): the largest multi-group configuration, C4 = 2-D quarter core, 7 groups, 10^7
+particles per cycle.  A "step" is one power-iteration cycle: the whole hot path (source bank -> XS lookup ->
+distance -> move + tally -> collision / surface events -> fission bank) over one batch of 10^7 histories.
+metric = active particle histories per second (whole job); events/s, the per-kernel roofline of the dominant
+kernel and the CPU oracle timed on this box's host cores are reported beside it.  Synthetic seeded inputs
+(paper_2501_05440_b200.inputs); the particle bank (> 1.2 GB) is larger than L2.
+
+    python bench.py --gpus 1 --steps K --warmup W            # our CUDA path
+    python bench.py --impl reference --steps K --warmup W     # the CPU oracle on a bounded sample
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "active particle histories/sec"
+UNIT = "histories/s"
+B_ALG_MG = 176.0      # algorithmic bytes per MG event, whole event
+B_ADV_MG = 112.0      # part of it moved by k_advance
+B_ALG_CE = 374.0
+B_ADV_CE = 310.0
+FALLBACK_HBM_GBS = 6650.0
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def workload(args):
+    from paper_2501_05440_b200 import inputs
+    N = args.particles
+    return inputs.config4(n_particles=N, n_inactive=args.warmup, n_active=args.steps), N
+
+
+def events_of(counters):
+    return int(counters[1:10].sum())
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    from paper_2501_05440_b200 import inputs
+    n = args.ref_particles
+    P = inputs.config4(n_particles=n, n_inactive=args.warmup, n_active=args.steps)
+    o = oracle.Oracle(P)
+    L = o.L
+    # the oracle has no per-cycle entry point: time (W+K) cycles minus W cycles
+    t0 = time.perf_counter(); L.orc_run_eigenvalue(o.h, n, args.warmup, 0, 1); tw = time.perf_counter() - t0
+    t0 = time.perf_counter(); rc = L.orc_run_eigenvalue(o.h, n, args.warmup, args.steps, 1); tt = time.perf_counter() - t0
+    o.n_cycles = args.warmup + args.steps
+    dt = max(tt - tw, 1e-9)
+    val = args.steps * n / dt
+    sample = f"C4 quarter core at {n} particles/cycle (full: 1e7), {args.steps} active cycles after {args.warmup}"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C4 2-D quarter core, 7 groups (bounded sample)", "particles_per_cycle": n},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2501_05440_b200 import binding, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    P, N = workload(args)
+    seed = 1 + rank  # replicas only: independent problems, no data-path collective
+    g = binding.Problem(P, device=local, search=1)
+    K, W = args.steps, args.warmup
+
+    # ---- device-resident throughput: W warm-up cycles, then exactly K timed cycles
+    for c in range(W):
+        g.run_cycle(N, c, 0, seed)
+    c0 = g.results()["counters"].copy()
+    ms0, nl0 = g.timing()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for c in range(W, W + K):
+        g.run_cycle(N, c, 1, seed)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    res = g.results()
+    c1 = res["counters"]
+    ms1, nl1 = g.timing()
+    events = events_of(c1) - events_of(c0)
+    tracks = int(c1[0] - c0[0])
+    value = world * K * N / (ms * 1e-3)
+    ev_per_s = world * events / (ms * 1e-3)
+
+    # ---- per-kernel timing of the same cycles' successors (event pairs around each launch; separate pass)
+    g.set_profile(True)
+    cb = g.results()["counters"].copy()
+    n_prof = max(1, min(K, 3))
+    for c in range(W + K, W + K + n_prof):
+        g.run_cycle(N, c, 1, seed)
+    prof = g.profile()
+    g.set_profile(False)
+    ca = g.results()["counters"]
+    ev_prof = events_of(ca) - events_of(cb)
+    adv = prof["advance"]
+    peak, peak_src = peaks()
+    tot_ms = sum(v["ms"] for v in prof.values())
+    roof = None
+    if adv["launches"]:
+        bytes_per_launch = B_ADV_MG * ev_prof / adv["launches"]
+        dur = adv["ms"] * 1e-3 / adv["launches"]
+        ach = bytes_per_launch / dur / 1e9
+        roof = {"bound": "hbm", "kernel": "k_advance<MG>", "achieved": ach, "peak": peak, "unit": "GB/s",
+                "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                "bytes_per_event": B_ADV_MG, "events_per_launch": ev_prof / adv["launches"],
+                "avg_launch_ms": 1e3 * dur, "share_of_step": adv["ms"] / tot_ms if tot_ms else None,
+                "whole_event": {"bytes_per_event": B_ALG_MG, "achieved": ev_per_s / world * B_ALG_MG / 1e9,
+                                "frac": ev_per_s / world * B_ALG_MG / 1e9 / peak},
+                "kernel_ms": {k: round(v["ms"] / n_prof, 3) for k, v in prof.items() if v["launches"]}}
+        tr = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tr):
+            try:
+                roof["traffic"] = json.load(open(tr)).get("k_advance_bytes_per_launch")
+            except Exception:
+                pass
+
+    # ---- end to end through the host-buffer C-ABI call: source bank H2D, fission bank + flux D2H every step
+    cap = 2 * N + 1024
+    sites_a = torch.empty(cap * 56, dtype=torch.uint8, pin_memory=True).numpy().view(binding.SITE_DTYPE)
+    sites_b = torch.empty(cap * 56, dtype=torch.uint8, pin_memory=True).numpy().view(binding.SITE_DTYPE)
+    flux = torch.empty(g.n_tally, dtype=torch.float64, pin_memory=True).numpy()
+    k, leak, n = g.run_cycle_host(N, 0, seed, 1.0, None, sites_a, flux)
+    for c in range(1, max(W, 1)):
+        k, leak, n = g.run_cycle_host(N, c, seed, k, sites_a[:n], sites_b, flux)
+        sites_a, sites_b = sites_b, sites_a
+    barrier()
+    t0 = time.perf_counter()
+    h2d = d2h = 0
+    for c in range(max(W, 1), max(W, 1) + K):
+        h2d += n * 56
+        k, leak, n = g.run_cycle_host(N, c, seed, k, sites_a[:n], sites_b, flux)
+        d2h += n * 56 + g.n_tally * 8 + 24
+        sites_a, sites_b = sites_b, sites_a
+    barrier()
+    dt = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([dt], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+    e2e = {"value": world * K * N / dt, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
+           "api": "mcdc_run_cycle_host"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "C4: 2-D quarter core, 7 groups, 2x2 17x17-pin assemblies + reflector, k-eigenvalue cycle",
+                   "particles_per_cycle": N, "step": "one power-iteration cycle", "parallelism": "replicas only",
+                   "l2": "particle bank (>1.2 GB) larger than L2", "schedule": "event queues + tail kernel",
+                   "k_mean": res["k_mean"]},
+        "events_per_sec": ev_per_s, "events_per_history": events / max(tracks, 1),
+        "roofline": roof, "e2e": e2e, "gpu_launches": int(nl1 - nl0), "clocks": clocks,
+    }
+
+    if rank == 0 and not args.no_cpu_baseline:
+        import oracle
+        n = args.ref_particles
+        Pc = inputs.config4(n_particles=n, n_inactive=1, n_active=args.ref_cycles)
+        o = oracle.Oracle(Pc)
+        t0 = time.perf_counter(); o.L.orc_run_eigenvalue(o.h, n, 1, 0, 1); tw = time.perf_counter() - t0
+        t0 = time.perf_counter(); o.L.orc_run_eigenvalue(o.h, n, 1, args.ref_cycles, 1); tt = time.perf_counter() - t0
+        o.n_cycles = 1 + args.ref_cycles
+        cnt = o.results()["counters"]
+        dtc = max(tt - tw, 1e-9)
+        out["cpu_baseline"] = {"value": args.ref_cycles * n / dtc, "unit": UNIT, "cores": 1, "kind": "oracle",
+                               "sample": f"C4 at {n} particles/cycle, {args.ref_cycles} active cycles after 1 (full: 1e7/cycle)",
+                               "events_per_sec": events_of(cnt) / tt, "host_cores_available": os.cpu_count()}
+
+    if rank == 0 and args.ce:
+        out["secondary"] = bench_ce(binding, inputs, args, peak)
+    g.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def bench_ce(binding, inputs, args, peak):
+    """Largest continuous-energy configuration (C5: 1e6 source particles) -- reported beside the headline."""
+    import torch
+    P = inputs.config5(n_particles=args.ce_particles)
+    g = binding.Problem(P, search=1)
+    g.run()  # warm-up
+    torch.cuda.synchronize()
+    best = None
+    for _ in range(2):
+        t0 = time.perf_counter()
+        r = g.run()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        ms, _ = g.timing()
+        best = ms if best is None else min(best, ms)
+    ev = events_of(r["counters"])
+    g.set_profile(True)
+    g.run()
+    prof = g.profile()
+    g.set_profile(False)
+    g.close()
+    adv = prof["advance"]
+    ach = B_ADV_CE * ev / (adv["ms"] * 1e-3) / 1e9 if adv["ms"] else None
+    return {"workload": "C5: continuous-energy time-dependent pin cell", "source_particles": args.ce_particles,
+            "histories_per_sec": args.ce_particles / (best * 1e-3), "tracks": int(r["counters"][0]),
+            "events_per_sec": ev / (best * 1e-3), "ms": best,
+            "roofline": {"bound": "hbm", "kernel": "k_advance<CE>", "achieved": ach, "peak": peak, "unit": "GB/s",
+                         "frac": ach / peak if ach else None, "bytes_per_event": B_ADV_CE,
+                         "whole_event": {"bytes_per_event": B_ALG_CE, "frac": ev / (best * 1e-3) * B_ALG_CE / 1e9 / peak}},
+            "kernel_ms": {k: round(v["ms"], 3) for k, v in prof.items() if v["launches"]}}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--particles", type=int, default=10_000_000)
+    ap.add_argument("--ref-particles", type=int, default=100_000)
+    ap.add_argument("--ref-cycles", type=int, default=8)
+    ap.add_argument("--ce-particles", type=int, default=1_000_000)
+    ap.add_argument("--no-ce", dest="ce", action="store_false")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 1)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -217,6 +217,14 @@ int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64
  * number of kernels it launched */
 int mcdc_get_timing(const mcdc_problem *p, double *ms_transport, uint64_t *n_launches);
 
+/* per-kernel-class device timing: when on, every launch is bracketed by a CUDA event pair on the library's
+ * stream (costs a few microseconds per launch, so it is off for throughput runs).  mcdc_get_profile fills
+ * ms[MCDC_N_PROFILE] and launches[MCDC_N_PROFILE] accumulated since mcdc_set_profile. */
+enum { MCDC_PROF_ADVANCE = 0, MCDC_PROF_SCATTER, MCDC_PROF_SURFACE, MCDC_PROF_TAIL, MCDC_PROF_SEGMENT, MCDC_PROF_BANK,
+       MCDC_N_PROFILE };
+int mcdc_set_profile(mcdc_problem *p, int32_t on);
+int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches);
+
 void mcdc_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);
 

@@ -24,7 +24,7 @@ EV_NAMES = {1: "scatter", 2: "fission", 3: "capture", 4: "transmit", 5: "reflect
 SYMBOLS = ["mcdc_workspace_bytes", "mcdc_create", "mcdc_run_eigenvalue", "mcdc_run_cycle", "mcdc_run_cycle_host",
            "mcdc_run_fixed_source", "mcdc_get_dims", "mcdc_get_tallies", "mcdc_get_bank", "mcdc_set_trace",
            "mcdc_get_trace", "mcdc_test_draws", "mcdc_test_grid_index", "mcdc_test_geometry", "mcdc_get_timing",
-           "mcdc_destroy", "mcdc_last_error"]
+           "mcdc_set_profile", "mcdc_get_profile", "mcdc_destroy", "mcdc_last_error"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -128,6 +128,8 @@ def load_library():
     L.mcdc_test_grid_index.argtypes = [vp, _dp, u64, _ip, _ip]
     L.mcdc_test_geometry.argtypes = [vp, _dp, _dp, u64, _ip, _dp, _ip]
     L.mcdc_get_timing.argtypes = [vp, _dp, P(u64)]
+    L.mcdc_set_profile.argtypes = [vp, i32]
+    L.mcdc_get_profile.argtypes = [vp, _dp, P(u64)]
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -294,6 +296,16 @@ class Problem:
         ms, nl = C.c_double(), C.c_uint64()
         self._check(self.L.mcdc_get_timing(self.h, C.byref(ms), C.byref(nl)))
         return ms.value, nl.value
+
+    PROFILE_CLASSES = ("advance", "scatter", "surface", "tail", "segment", "bank")
+
+    def set_profile(self, on=True):
+        self._check(self.L.mcdc_set_profile(self.h, int(on)))
+
+    def profile(self):
+        ms, nl = np.zeros(6), np.zeros(6, np.uint64)
+        self._check(self.L.mcdc_get_profile(self.h, ms.ctypes.data_as(_dp), nl.ctypes.data_as(C.POINTER(C.c_uint64))))
+        return {k: dict(ms=float(m), launches=int(n)) for k, m, n in zip(self.PROFILE_CLASSES, ms, nl)}
 
     def bank(self):
         n = C.c_uint64()

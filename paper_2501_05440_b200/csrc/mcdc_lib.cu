@@ -71,7 +71,44 @@ struct mcdc_problem {
     uint32_t trace_n_ids, trace_max_events;
     uint32_t trace_cap_slots;
     uint64_t last_N;
+    // optional per-kernel-class timing (mcdc_set_profile): event pairs around every launch
+    int profile;
+    std::vector<cudaEvent_t> pool;
+    std::vector<int> pool_class;  // class of pair k (events 2k, 2k+1)
+    double prof_ms[MCDC_N_PROFILE];
+    uint64_t prof_launches[MCDC_N_PROFILE];
 };
+
+// RAII-free helper: record an event pair around one launch when profiling is on
+struct ProfScope {
+    mcdc_problem *p;
+    size_t k;
+    ProfScope(mcdc_problem *p_, int cls) : p(p_), k((size_t)-1)
+    {
+        if (!p->profile) return;
+        k = p->pool_class.size();
+        if (p->pool.size() < 2 * (k + 1)) {
+            cudaEvent_t a, b;
+            cudaEventCreate(&a); cudaEventCreate(&b);
+            p->pool.push_back(a); p->pool.push_back(b);
+        }
+        p->pool_class.push_back(cls);
+        cudaEventRecord(p->pool[2 * k], p->stream);
+    }
+    ~ProfScope() { if (k != (size_t)-1) cudaEventRecord(p->pool[2 * k + 1], p->stream); }
+};
+
+static void profile_collect(mcdc_problem *p)  // call after a stream synchronize
+{
+    for (size_t k = 0; k < p->pool_class.size(); k++) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p->pool[2 * k], p->pool[2 * k + 1]) == cudaSuccess) {
+            p->prof_ms[p->pool_class[k]] += ms;
+            p->prof_launches[p->pool_class[k]]++;
+        }
+    }
+    p->pool_class.clear();
+}
 
 // ------------------------------------------------------------------ workspace layout
 struct Carver {
@@ -428,6 +465,8 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     p->k_acc = p->k_acc2 = p->leak_acc = p->leak_acc2 = 0.0;
     memset(p->host_counters, 0, sizeof p->host_counters);
     p->ms_transport = 0.0; p->n_launches = 0; p->last_N = 0;
+    p->profile = 0;
+    memset(p->prof_ms, 0, sizeof p->prof_ms); memset(p->prof_launches, 0, sizeof p->prof_launches);
     *out = p;
     return 0;
 }
@@ -437,6 +476,7 @@ extern "C" void mcdc_destroy(mcdc_problem *p)
     if (!p) return;
     cudaStreamSynchronize(p->stream);
     for (int k = 0; k < RING; k++) cudaEventDestroy(p->ev[k]);
+    for (cudaEvent_t e : p->pool) cudaEventDestroy(e);
     cudaEventDestroy(p->t0); cudaEventDestroy(p->t1);
     cudaFreeHost(p->pin);
     delete p;
@@ -486,19 +526,19 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
     while (upper > 0) {
         if (s > 4000000u) return fail(MCDC_ELOST, "sweep guard exceeded");
         if (p->schedule == 0 && p->tail > 0 && upper <= (uint64_t)p->tail) {
-            k_finish<CE, PRIV><<<grid_for(upper), BS, smem, st>>>(c, s, n0);
+            { ProfScope ps(p, MCDC_PROF_TAIL); k_finish<CE, PRIV><<<grid_for(upper), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
             p->host_counters[13]++;
             break;
         }
         unsigned int gr = grid_for(upper);
         if (p->schedule == 0) {
-            k_advance<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0);
-            k_scatter<CE><<<gr, BS, 0, st>>>(c, s);
-            k_surface<<<gr, BS, 0, st>>>(c, s);
+            { ProfScope ps(p, MCDC_PROF_ADVANCE); k_advance<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, 0, st>>>(c, s); }
+            { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, 0, st>>>(c, s); }
             p->n_launches += 3;
         } else {
-            k_segment<CE, PRIV><<<grid_for(M), BS, smem, st>>>(c, s, n0);
+            { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
         }
         p->host_counters[13]++;
@@ -534,16 +574,20 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
     unsigned int nb = (unsigned int)((M + BS - 1) / BS);
+    {
+    ProfScope ps(p, MCDC_PROF_BANK);
     k_scan_partial<<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part);
     k_scan_top<<<1, 1024, 0, st>>>(p->part, nb);
     if (p->mode == 0) k_emit<false><<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part, (unsigned int)p->cap);
     else k_emit<true><<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part, (unsigned int)p->cap);
+    }
     p->n_launches += 3;
     CUDA_OK(cudaMemcpyAsync(&p->pin->total, p->part + nb, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(&p->pin->err, c.err, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaStreamSynchronize(st));
     CUDA_OK(cudaGetLastError());
+    profile_collect(p);
     *total = p->pin->total;
     return 0;
 }
@@ -804,6 +848,21 @@ extern "C" int mcdc_get_trace(const mcdc_problem *p, mcdc_trace_rec *out, uint64
         for (unsigned int j = 0; j < k && written < max; j++) memcpy(&out[written++], &buf[j], sizeof(TraceRec));
     }
     *n = total;
+    return 0;
+}
+
+extern "C" int mcdc_set_profile(mcdc_problem *p, int32_t on)
+{
+    if (!p) return fail(MCDC_EINVAL, "null");
+    p->profile = on ? 1 : 0;
+    memset(p->prof_ms, 0, sizeof p->prof_ms); memset(p->prof_launches, 0, sizeof p->prof_launches);
+    return 0;
+}
+
+extern "C" int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches)
+{
+    if (!p || !ms || !launches) return fail(MCDC_EINVAL, "null");
+    for (int k = 0; k < MCDC_N_PROFILE; k++) { ms[k] = p->prof_ms[k]; launches[k] = p->prof_launches[k]; }
     return 0;
 }
 

@@ -43,7 +43,9 @@ def _fis():
 @pytest.mark.parametrize("schedule,tail,search", [(0, 0, 0), (0, -1, 1), (0, 1 << 30, 1), (1, 0, 0)])
 def test_ce_parity(gpu, orc, name, schedule, tail, search):
     P = CE_CASES[name]()
-    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, search=search)
+    # the supercritical pure-fission pin grows by generation: give its waves room (capacity = 2 max + 1024)
+    mp = 100_000 if name == "ce_fission" else None
+    g = gpu.Problem(P, max_particles=mp, schedule=schedule, tail_threshold=tail, search=search)
     r = g.run()
     o = orc.Oracle(P)
     rc, ro = o.run()
@@ -70,7 +72,7 @@ def test_ce_traces_identical(gpu, orc, schedule, tail, search):
 @pytest.mark.parametrize("jitter", [False, True])
 def test_grid_search_binary_equals_hash_equals_numpy(gpu, jitter):
     P = inputs.config5(n_particles=10, n_grid=50_000, jitter=jitter)
-    g = gpu.Problem(P)
+    g = gpu.Problem(P, max_particles=400_000)
     grid = P["grid"]
     rng = np.random.default_rng(3)
     E = np.concatenate([np.exp(rng.uniform(np.log(1e-6), np.log(1e8), 200_000)), grid, np.nextafter(grid, 0),
