@@ -40,11 +40,24 @@ struct CETab {
     double nu0, nu1, watt_a, watt_b, E_min, E_max;
 };
 
-// Particle bank: structure of arrays, slot = particle index inside the cycle / wave (R6: id = slot in
-// eigenvalue mode).  gl packs the group (low 16 bits) and last_surf+1 (high 16 bits).
+// Particle banks ("dual particle banks"): two dense structure-of-arrays banks.  A sweep reads the
+// live particles of bank[s&1] (scatter-bound ones packed at the FRONT, surface-bound ones at the BACK) and
+// k_advance writes every survivor, whole, to the front or the back of bank[(s+1)&1]: the queues hold the
+// particles themselves, so every load and store of every kernel is coalesced.
+// gl packs the group (low 16 bits) and last_surf+1 (high 16 bits); ev = pending event code (or EV_DEAD in the
+// monolithic schedule); slot = index of the particle inside its cycle / wave (= its id in eigenvalue mode, R6).
 struct Bank {
     double *x, *y, *z, *ux, *uy, *uz, *E, *t;
-    int *cell, *elem, *gl, *tbin, *ev, *fis_n;
+    int *cell, *elem, *gl, *tbin, *ev;
+    uint32_t *ctr, *slot;
+    uint64_t *id;
+};
+
+// What a fission leaves behind, indexed by the parent's slot: number of children, the site, the parent's
+// location and draw counter (the parent's stream continues in k_emit, R5).
+struct FisRec {
+    int *n, *cell, *elem, *tbin;
+    double *x, *y, *z, *t;
     uint32_t *ctr;
     uint64_t *id;
 };
@@ -65,16 +78,15 @@ struct Ctx {
     MGTab mg;
     CETab ce;
     Bank bank[2];
-    int cur;            // bank holding the particles in flight
+    FisRec fis;
+    unsigned int cap;   // slots per bank
     int mode;           // 0 MG, 1 CE
     int n_tally, n_bins;
     double *flux;       // [n_tally] per-cycle track-length tally
     double *scal;       // [0] k numerator, [1] leakage weight
     unsigned long long *counters;  // [16]
     int *err;           // device error flag
-    unsigned int *q[2];  // index queues, capacity q_cap each; scatter events grow from the front, surface
-    unsigned int q_cap;  // events from the back
-    QCount *qc;          // [RING]
+    QCount *qc;          // [RING] per-sweep counts of the front / back regions
     Trace tr;
     unsigned long long seed;
     unsigned int cycle;

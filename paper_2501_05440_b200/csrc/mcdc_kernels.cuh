@@ -2,14 +2,16 @@
 //
 // Event schedule (default): per sweep three kernels regroup the live particles by next event
 //   k_advance  (a2/a3 XS lookup, a5 nearest boundary, a6 distance to collision, a7 move + tallies, reaction
-//               choice) over the live queue; each block appends its scatter events to the FRONT and its
-//               surface / lattice / time-edge events to the BACK of the next queue with ballot + prefix-sum
-//               compaction and one atomic per block and queue (a11);
-//   k_scatter  (a8) over the front region;   k_surface (a9) over the back region.
-// Fission and capture end a history inside k_advance; the children are produced at the end of the cycle
-// by count -> exclusive scan -> write (a10/a12), which yields the bank sorted by (parent id, child index)
-// without atomics or a sort.  k_segment is the paper's monolithic design: one whole
-// segment for every bank slot per launch, no compaction.  k_finish ends the last few histories in registers.
+//               choice) reads the live particles of bank[s&1] and writes every survivor, whole, into
+//               bank[(s+1)&1]: scatter events packed at the FRONT, surface / lattice / time-edge events at the
+//               BACK, positions from ballot + prefix-sum compaction with one atomic per block and queue (a11);
+//   k_scatter  (a8) over the front region, in place;   k_surface (a9) over the back region, in place.
+// The queues are the particles themselves (PAPER.md:55 dual banks), so all bank traffic is coalesced.
+// Fission and capture end a history inside k_advance; a fission leaves a record at the parent's slot and the
+// children are produced at the end of the cycle by count -> exclusive scan -> write (a10/a12), which yields
+// the bank sorted by (parent id, child index) without atomics or a sort.  k_segment is the paper's monolithic
+// design: one whole segment for every bank slot per launch, no compaction.  k_finish ends the
+// last few histories in registers.
 #pragma once
 #include "mcdc_device.cuh"
 
@@ -24,9 +26,11 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// ------------------------------------------------------------------ bank access
+__device__ __forceinline__ int pack_gl(int g, int last) { return (g & 0xffff) | ((last + 1) << 16); }
+
+// ------------------------------------------------------------------ bank access (dense, position-indexed)
 template <bool CE>
-__device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr)
+__device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr, uint32_t &slot)
 {
     p.x = B.x[i]; p.y = B.y[i]; p.z = B.z[i];
     p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i];
@@ -34,11 +38,38 @@ __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particl
     int gl = B.gl[i];
     p.g = gl & 0xffff; p.last = (gl >> 16) - 1;
     ctr = B.ctr[i];
+    slot = B.slot[i];
     if (CE) { p.E = B.E[i]; p.t = B.t[i]; p.tbin = B.tbin[i]; p.id = B.id[i]; }
-    else { p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = i; }
+    else { p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = slot; }
 }
 
-__device__ __forceinline__ int pack_gl(int g, int last) { return (g & 0xffff) | ((last + 1) << 16); }
+template <bool CE>
+__device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr, uint32_t slot,
+                                           int ev)
+{
+    B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z; B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
+    B.cell[i] = p.cell; B.elem[i] = p.elem; B.gl[i] = pack_gl(p.g, p.last); B.ctr[i] = ctr; B.slot[i] = slot;
+    B.ev[i] = ev;
+    if (CE) { B.E[i] = p.E; B.t[i] = p.t; B.tbin[i] = p.tbin; B.id[i] = p.id; }
+}
+
+// a fission ends the history: leave what k_emit needs at the parent's slot
+template <bool CE>
+__device__ __forceinline__ void record_fission(const Ctx &c, const Particle &p, uint32_t ctr, uint32_t slot, int n)
+{
+    const FisRec &F = c.fis;
+    F.n[slot] = n;
+    if (n <= 0) return;
+    F.x[slot] = p.x; F.y[slot] = p.y; F.z[slot] = p.z;
+    F.cell[slot] = p.cell; F.elem[slot] = p.elem; F.ctr[slot] = ctr;
+    if (CE) { F.t[slot] = p.t; F.tbin[slot] = p.tbin; F.id[slot] = p.id; }
+}
+
+// position of live particle t of a sweep's input bank: front region first, then the back region
+__device__ __forceinline__ unsigned int live_pos(unsigned int cap, unsigned int n_front, unsigned int t)
+{
+    return t < n_front ? t : cap - 1u - (t - n_front);
+}
 
 // per-block flush of the thread accumulators: k numerator, leakage, event counters
 __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
@@ -80,9 +111,9 @@ __device__ __forceinline__ void flush_private_flux(const Ctx &c, const double *s
     }
 }
 
-// ballot + prefix-sum compaction of one block's events into the two ends of the next queue (a11)
-__device__ __forceinline__ void block_push(bool to_front, bool to_back, unsigned int idx, unsigned int *qout, QCount *oc,
-                                           unsigned int q_cap)
+// ballot + prefix-sum compaction (a11): output position of this thread's particle in the next bank, front
+// region for scatter events, back region for surface events; one atomic per block and region.
+__device__ __forceinline__ unsigned int block_slot(bool to_front, bool to_back, QCount *oc, unsigned int cap)
 {
     __shared__ unsigned int s_n[2][BS / 32];
     __shared__ unsigned int s_base[2];
@@ -97,15 +128,11 @@ __device__ __forceinline__ void block_push(bool to_front, bool to_back, unsigned
     }
     __syncthreads();
     unsigned int lt = (1u << lane) - 1u;
-    if (to_front) qout[s_base[0] + s_n[0][w] + __popc(mf & lt)] = idx;
-    if (to_back) qout[q_cap - 1u - (s_base[1] + s_n[1][w] + __popc(mb & lt))] = idx;
+    unsigned int pos = 0xffffffffu;
+    if (to_front) pos = s_base[0] + s_n[0][w] + __popc(mf & lt);
+    if (to_back) pos = cap - 1u - (s_base[1] + s_n[1][w] + __popc(mb & lt));
     __syncthreads();
-}
-
-__device__ __forceinline__ unsigned int queue_entry(const unsigned int *qin, unsigned int q_cap, unsigned int n_front,
-                                                    unsigned int t)
-{
-    return t < n_front ? qin[t] : qin[q_cap - 1u - (t - n_front)];
+    return pos;
 }
 
 // ------------------------------------------------------------------ a1: source
@@ -114,27 +141,26 @@ __global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[0];
     Rng rng;
     rng.init(c.seed, i, 0u, c.cycle, 0u);
     double xi[6];
 #pragma unroll
     for (int k = 0; k < 6; k++) xi[k] = rng.next();  // always six draws
-    double x = c.src_lo[0] + xi[0] * (c.src_hi[0] - c.src_lo[0]);
-    double y = c.src_lo[1] + xi[1] * (c.src_hi[1] - c.src_lo[1]);
-    double z = c.src_lo[2] + xi[2] * (c.src_hi[2] - c.src_lo[2]);
-    double ux = c.src_dir[0], uy = c.src_dir[1], uz = c.src_dir[2];
-    if (c.src_iso) iso_dir(xi[3], xi[4], ux, uy, uz);
-    int g = 0;
-    if (!CE) g = pick(c.mg.src_cum, c.mg.G, xi[5] * __ldg(c.mg.src_cum + c.mg.G - 1));
-    int cell, elem;
-    if (!locate(c.geo, x, y, z, ux, uy, uz, -1, cell, elem)) { atomicExch(c.err, -2); cell = -1; }
-    B.x[i] = x; B.y[i] = y; B.z[i] = z; B.ux[i] = ux; B.uy[i] = uy; B.uz[i] = uz;
-    B.cell[i] = cell; B.elem[i] = elem; B.gl[i] = pack_gl(g, -1); B.ctr[i] = 6u;
-    B.ev[i] = cell < 0 ? EV_DEAD : 0; B.fis_n[i] = 0;
-    if (CE) {
-        B.E[i] = c.src_E; B.t[i] = c.src_t; B.tbin[i] = edge_bin(c.ce.t_edges, c.ce.n_t, c.src_t); B.id[i] = i;
-    }
+    Particle p;
+    p.x = c.src_lo[0] + xi[0] * (c.src_hi[0] - c.src_lo[0]);
+    p.y = c.src_lo[1] + xi[1] * (c.src_hi[1] - c.src_lo[1]);
+    p.z = c.src_lo[2] + xi[2] * (c.src_hi[2] - c.src_lo[2]);
+    p.ux = c.src_dir[0]; p.uy = c.src_dir[1]; p.uz = c.src_dir[2];
+    if (c.src_iso) iso_dir(xi[3], xi[4], p.ux, p.uy, p.uz);
+    p.g = 0;
+    if (!CE) p.g = pick(c.mg.src_cum, c.mg.G, xi[5] * __ldg(c.mg.src_cum + c.mg.G - 1));
+    if (!locate(c.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, -1, p.cell, p.elem)) { atomicExch(c.err, -2); p.cell = -1; }
+    p.last = -1; p.id = i;
+    p.E = c.src_E; p.t = c.src_t; p.tbin = 0;
+    if (CE) p.tbin = edge_bin(c.ce.t_edges, c.ce.n_t, c.src_t);
+    store_full<CE>(B, i, p, 6u, i, p.cell < 0 ? EV_DEAD : 0);
+    c.fis.n[i] = 0;
 }
 
 struct Site { double x, y, z, ux, uy, uz; int g, pad; };
@@ -144,20 +170,20 @@ __global__ void __launch_bounds__(BS) k_load_sites(Ctx c, const Site *sites, uns
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const Bank &B = c.bank[c.cur];
     Site s = sites[i];
-    int cell, elem;
-    if (!locate(c.geo, s.x, s.y, s.z, s.ux, s.uy, s.uz, -1, cell, elem)) { atomicExch(c.err, -2); cell = -1; }
-    B.x[i] = s.x; B.y[i] = s.y; B.z[i] = s.z; B.ux[i] = s.ux; B.uy[i] = s.uy; B.uz[i] = s.uz;
-    B.cell[i] = cell; B.elem[i] = elem; B.gl[i] = pack_gl(s.g, -1); B.ctr[i] = 0u;
-    B.ev[i] = cell < 0 ? EV_DEAD : 0; B.fis_n[i] = 0;
+    Particle p;
+    p.x = s.x; p.y = s.y; p.z = s.z; p.ux = s.ux; p.uy = s.uy; p.uz = s.uz; p.g = s.g; p.last = -1; p.id = i;
+    p.E = 0.0; p.t = 0.0; p.tbin = 0;
+    if (!locate(c.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, -1, p.cell, p.elem)) { atomicExch(c.err, -2); p.cell = -1; }
+    store_full<false>(c.bank[0], i, p, 0u, i, p.cell < 0 ? EV_DEAD : 0);
+    c.fis.n[i] = 0;
 }
 
 __global__ void __launch_bounds__(BS) k_store_sites(Ctx c, Site *sites, unsigned int n)
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[0];
     Site s;
     s.x = B.x[i]; s.y = B.y[i]; s.z = B.z[i]; s.ux = B.ux[i]; s.uy = B.uy[i]; s.uz = B.uz[i];
     s.g = B.gl[i] & 0xffff; s.pad = 0;
@@ -169,13 +195,11 @@ template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS) k_advance(Ctx c, unsigned int s, unsigned int n0)
 {
     extern __shared__ double s_flux[];
-    unsigned int n_front = 0, n_in = n0;
-    const unsigned int *qin = c.q[s & 1];
+    unsigned int n_front = n0, n_in = n0;
     if (s > 0) {
         QCount pc = c.qc[(s - 1) % RING];
         n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
     }
-    unsigned int *qout = c.q[(s + 1) & 1];
     QCount *oc = c.qc + (s % RING);
     if (PRIVATE) {
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
@@ -185,31 +209,25 @@ __global__ void __launch_bounds__(BS) k_advance(Ctx c, unsigned int s, unsigned 
     acc.knum = acc.leak = 0.0;
 #pragma unroll
     for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[s & 1];
+    const Bank &O = c.bank[(s + 1) & 1];
     for (unsigned int base = blockIdx.x * BS; base < n_in; base += gridDim.x * BS) {
-        unsigned int t = base + threadIdx.x, i = 0;
-        int code = ADV_DEAD;
+        unsigned int t = base + threadIdx.x;
+        int code = ADV_DEAD, aux = 0;
+        Particle p;
+        uint32_t ctr = 0, slot = 0;
+        Rng rng;
         if (t < n_in) {
-            i = s == 0 ? t : queue_entry(qin, c.q_cap, n_front, t);
-            int cell = B.cell[i];
-            if (cell >= 0) {
-                Particle p;
-                uint32_t ctr;
-                load_full<CE>(B, i, p, ctr);
-                const int last0 = p.last, tbin0 = p.tbin;
-                Rng rng;
+            unsigned int i = live_pos(c.cap, n_front, t);
+            if (B.cell[i] >= 0) {
+                load_full<CE>(B, i, p, ctr, slot);
                 rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-                int aux = 0;
                 code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
-                B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z;
-                B.ctr[i] = rng.ctr;
-                if (code == ADV_FISSION) { B.fis_n[i] = aux; code = ADV_DEAD; }
-                else if (code != ADV_DEAD) B.ev[i] = aux;
-                if (p.last != last0) B.gl[i] = pack_gl(p.g, p.last);
-                if (CE) { B.t[i] = p.t; if (p.tbin != tbin0) B.tbin[i] = p.tbin; }
+                if (code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
-        block_push(code == ADV_SCATTER, code == ADV_SURFACE, i, qout, oc, c.q_cap);
+        unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap);
+        if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot, aux);
     }
     if (PRIVATE) flush_private_flux(c, s_flux);
     flush_acc(c, acc);
@@ -219,20 +237,18 @@ template <bool CE>
 __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
 {
     const QCount oc = c.qc[s % RING];
-    const unsigned int *q = c.q[(s + 1) & 1];
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[(s + 1) & 1];
     // queue-counter housekeeping: clear the set the next sweep appends to
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         QCount z = {0u, 0u, 0u, 0u};
         c.qc[(s + 1) % RING] = z;
     }
-    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_scat; t += gridDim.x * BS) {
-        unsigned int i = q[t];
+    for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < oc.n_scat; i += gridDim.x * BS) {
         Particle p;
         int gl = B.gl[i];
         p.g = gl & 0xffff;
         p.cell = B.cell[i];
-        p.id = CE ? B.id[i] : i;
+        p.id = CE ? B.id[i] : (unsigned long long)B.slot[i];
         if (CE) { p.E = B.E[i]; p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i]; }
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, B.ctr[i]);
@@ -247,10 +263,9 @@ __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
 __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 {
     const QCount oc = c.qc[s % RING];
-    const unsigned int *q = c.q[(s + 1) & 1];
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[(s + 1) & 1];
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_surf; t += gridDim.x * BS) {
-        unsigned int i = q[c.q_cap - 1u - t];
+        unsigned int i = c.cap - 1u - t;
         int hit = B.ev[i];
         if (hit == HIT_TIME_EDGE) continue;
         Particle p;
@@ -277,8 +292,7 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 
 // whole segment in registers (shared by the monolithic schedule and the tail kernel)
 template <bool CE, bool PRIVATE>
-__device__ __forceinline__ bool segment(const Ctx &c, const Bank &B, unsigned int i, Particle &p, Rng &rng, Acc &acc,
-                                        double *s_flux)
+__device__ __forceinline__ bool segment(const Ctx &c, Particle &p, Rng &rng, uint32_t slot, Acc &acc, double *s_flux)
 {
     int aux = 0;
     int code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
@@ -292,19 +306,11 @@ __device__ __forceinline__ bool segment(const Ctx &c, const Bank &B, unsigned in
         }
         return true;
     }
-    if (code == ADV_FISSION) B.fis_n[i] = aux;
+    if (code == ADV_FISSION) record_fission<CE>(c, p, rng.ctr, slot, aux);
     return false;
 }
 
-template <bool CE>
-__device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr)
-{
-    B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z; B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
-    B.cell[i] = p.cell; B.elem[i] = p.elem; B.gl[i] = pack_gl(p.g, p.last); B.ctr[i] = ctr;
-    if (CE) { B.E[i] = p.E; B.t[i] = p.t; B.tbin[i] = p.tbin; }
-}
-
-// monolithic schedule: every slot, one segment, no compaction; counts the survivors
+// monolithic schedule: every slot of bank 0, one segment, no compaction; counts the survivors
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned int n)
 {
@@ -321,18 +327,18 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
     acc.knum = acc.leak = 0.0;
 #pragma unroll
     for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[0];
     unsigned int alive = 0;
     for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
         if (B.ev[i] == EV_DEAD) continue;
         Particle p;
-        uint32_t ctr;
-        load_full<CE>(B, i, p, ctr);
+        uint32_t ctr, slot;
+        load_full<CE>(B, i, p, ctr, slot);
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-        bool live = segment<CE, PRIVATE>(c, B, i, p, rng, acc, s_flux);
-        store_full<CE>(B, i, p, rng.ctr);
-        if (!live) B.ev[i] = EV_DEAD; else alive++;
+        bool live = segment<CE, PRIVATE>(c, p, rng, slot, acc, s_flux);
+        store_full<CE>(B, i, p, rng.ctr, slot, live ? 0 : EV_DEAD);
+        if (live) alive++;
     }
     alive = __reduce_add_sync(0xffffffffu, alive);
     if ((threadIdx.x & 31) == 0 && alive) atomicAdd(&c.qc[s % RING].n_alive, alive);
@@ -340,7 +346,7 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
     flush_acc(c, acc);
 }
 
-// tail: finish the few remaining histories of the live queue inside one kernel
+// tail: finish the few remaining histories of the live regions inside one kernel
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned int n0)
 {
@@ -349,8 +355,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
     }
-    unsigned int n_front = 0, n_in = n0;
-    const unsigned int *qin = c.q[s & 1];
+    unsigned int n_front = n0, n_in = n0;
     if (s > 0) {
         QCount pc = c.qc[(s - 1) % RING];
         n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
@@ -359,21 +364,20 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
     acc.knum = acc.leak = 0.0;
 #pragma unroll
     for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
-    const Bank &B = c.bank[c.cur];
+    const Bank &B = c.bank[s & 1];
     unsigned int done = 0;
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < n_in; t += gridDim.x * BS) {
-        unsigned int i = s == 0 ? t : queue_entry(qin, c.q_cap, n_front, t);
+        unsigned int i = live_pos(c.cap, n_front, t);
         if (B.cell[i] < 0) continue;
         Particle p;
-        uint32_t ctr;
-        load_full<CE>(B, i, p, ctr);
+        uint32_t ctr, slot;
+        load_full<CE>(B, i, p, ctr, slot);
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, ctr);
         unsigned int guard = 0;
-        while (segment<CE, PRIVATE>(c, B, i, p, rng, acc, s_flux)) {
+        while (segment<CE, PRIVATE>(c, p, rng, slot, acc, s_flux)) {
             if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
         }
-        store_full<CE>(B, i, p, rng.ctr);
         done++;
     }
     done = __reduce_add_sync(0xffffffffu, done);
@@ -387,7 +391,7 @@ __global__ void __launch_bounds__(BS) k_scan_partial(Ctx c, unsigned int n, unsi
 {
     __shared__ unsigned int s_w[BS / 32];
     unsigned int i = blockIdx.x * BS + threadIdx.x;
-    unsigned int v = i < n ? (unsigned int)c.bank[c.cur].fis_n[i] : 0u;
+    unsigned int v = i < n ? (unsigned int)c.fis.n[i] : 0u;
     v = __reduce_add_sync(0xffffffffu, v);
     if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = v;
     __syncthreads();
@@ -418,18 +422,18 @@ __global__ void __launch_bounds__(1024) k_scan_top(unsigned int *part, unsigned 
     for (unsigned int k = lo; k < hi; k++) { unsigned int v = part[k]; part[k] = run; run += v; }
 }
 
-// every fission parent writes its children into the next bank at [offset(parent), +n): sorted by (parent id,
-// child index) by construction.  MG: child group ~ chi, isotropic direction (1 + 2 draws per child) from the
-// parent's stream (R5).  CE: Watt energy (4 draws) + direction (2 draws), own id from the domain-1 block (R10).
+// every fission parent writes its children into bank 0 at [offset(parent), +n): sorted by (parent id, child
+// index) by construction.  MG: child group ~ chi, isotropic direction (1 + 2 draws per child) from the parent's
+// stream (R5).  CE: Watt energy (4 draws) + direction (2 draws), own id from the domain-1 block (R10).
+// The children's fission counts are cleared through a second array (nn) because n is still being read.
 template <bool CE>
 __global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsigned int *part, unsigned int cap)
 {
     __shared__ unsigned int s_w[BS / 32];
-    const Bank &B = c.bank[c.cur];
-    const Bank &O = c.bank[1 - c.cur];
+    const FisRec &F = c.fis;
+    const Bank &O = c.bank[0];
     unsigned int i = blockIdx.x * BS + threadIdx.x;
-    int nc = i < n ? B.fis_n[i] : 0;
-    // block exclusive scan
+    int nc = i < n ? F.n[i] : 0;
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned int incl = (unsigned int)nc;
 #pragma unroll
@@ -444,36 +448,42 @@ __global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsign
     unsigned int off = part[blockIdx.x] + wbase + incl - (unsigned int)nc;
     if (nc <= 0) return;
     if (off + (unsigned int)nc > cap) { atomicExch(c.err, -3); return; }  // bank overflow (R6)
-    double x = B.x[i], y = B.y[i], z = B.z[i];
-    int cell = B.cell[i], elem = B.elem[i];
-    const int mat = __ldg(c.geo.cfill + cell);
-    unsigned long long pid = CE ? B.id[i] : (unsigned long long)i;
-    uint32_t ctr0 = B.ctr[i];
+    Particle p;
+    p.x = F.x[i]; p.y = F.y[i]; p.z = F.z[i];
+    p.cell = F.cell[i]; p.elem = F.elem[i];
+    p.last = -1; p.g = 0; p.E = 0.0; p.t = 0.0; p.tbin = 0;
+    if (CE) { p.t = F.t[i]; p.tbin = F.tbin[i]; }
+    const int mat = __ldg(c.geo.cfill + p.cell);
+    unsigned long long pid = CE ? F.id[i] : (unsigned long long)i;
+    uint32_t ctr0 = F.ctr[i];
     Rng rng;
     rng.init(c.seed, pid, 0u, c.cycle, ctr0);
     for (int j = 0; j < nc; j++) {
         unsigned int o = off + j;
-        double ux, uy, uz;
-        int g = 0;
         if (!CE) {
             const double *cc = c.mg.cumchi + (size_t)mat * c.mg.G;
-            g = pick(cc, c.mg.G, rng.next() * __ldg(cc + c.mg.G - 1));
+            p.g = pick(cc, c.mg.G, rng.next() * __ldg(cc + c.mg.G - 1));
             double a = rng.next(), b = rng.next();
-            iso_dir(a, b, ux, uy, uz);
+            iso_dir(a, b, p.ux, p.uy, p.uz);
+            p.id = o;
         } else {
             double a1 = rng.next(), a2 = rng.next(), a3 = rng.next(), a4 = rng.next();
             double En = 1e6 * watt(c.ce.watt_a, c.ce.watt_b, a1, a2, a3, a4);
             if (En < c.ce.E_min) En = c.ce.E_min;
             if (En > c.ce.E_max) En = c.ce.E_max;
             double a = rng.next(), b = rng.next();
-            iso_dir(a, b, ux, uy, uz);
-            O.E[o] = En; O.t[o] = B.t[i]; O.tbin[o] = B.tbin[i];
-            O.id[o] = child_id(c.seed, pid, ctr0, (uint32_t)j);
+            iso_dir(a, b, p.ux, p.uy, p.uz);
+            p.E = En;
+            p.id = child_id(c.seed, pid, ctr0, (uint32_t)j);
         }
-        O.x[o] = x; O.y[o] = y; O.z[o] = z; O.ux[o] = ux; O.uy[o] = uy; O.uz[o] = uz;
-        O.cell[o] = cell; O.elem[o] = elem; O.gl[o] = pack_gl(g, -1); O.ctr[o] = 0u;
-        O.ev[o] = 0; O.fis_n[o] = 0;
+        store_full<CE>(O, o, p, 0u, o, 0);
     }
+}
+
+__global__ void __launch_bounds__(BS) k_clear_counts(int *n, unsigned int m)
+{
+    unsigned int i = blockIdx.x * BS + threadIdx.x;
+    if (i < m) n[i] = 0;
 }
 
 // cycle end: per-source-particle flux into the running mean / mean-square, clear the per-cycle tally (R17)

@@ -132,7 +132,7 @@ struct Layout {  // everything carved from the workspace, in order
     double *grid, *tab, *colA, *t_edges, *e_edges;
     int *ncol, *hash;
     Bank bank[2];
-    unsigned int *q[2];
+    FisRec fis;
     QCount *qc;
     double *flux, *flux_acc, *flux_acc2, *scal;
     unsigned long long *counters;
@@ -199,11 +199,19 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         B.E = ce ? C.take<double>(cap) : nullptr; B.t = ce ? C.take<double>(cap) : nullptr;
         B.cell = C.take<int>(cap); B.elem = C.take<int>(cap); B.gl = C.take<int>(cap);
         B.tbin = ce ? C.take<int>(cap) : nullptr;
-        B.ev = C.take<int>(cap); B.fis_n = C.take<int>(cap);
-        B.ctr = C.take<uint32_t>(cap);
+        B.ev = C.take<int>(cap);
+        B.ctr = C.take<uint32_t>(cap); B.slot = C.take<uint32_t>(cap);
         B.id = ce ? C.take<uint64_t>(cap) : nullptr;
     }
-    L.q[0] = C.take<unsigned int>(cap); L.q[1] = C.take<unsigned int>(cap);
+    {
+        FisRec &F = L.fis;
+        F.n = C.take<int>(cap); F.cell = C.take<int>(cap); F.elem = C.take<int>(cap);
+        F.tbin = ce ? C.take<int>(cap) : nullptr;
+        F.x = C.take<double>(cap); F.y = C.take<double>(cap); F.z = C.take<double>(cap);
+        F.t = ce ? C.take<double>(cap) : nullptr;
+        F.ctr = C.take<uint32_t>(cap);
+        F.id = ce ? C.take<uint64_t>(cap) : nullptr;
+    }
     L.qc = C.take<QCount>(RING);
     uint64_t nt = n_tally_of(m, t);
     L.flux = C.take<double>(nt); L.flux_acc = C.take<double>(nt); L.flux_acc2 = C.take<double>(nt);
@@ -433,8 +441,9 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
         c.n_tally = t->n_bins * t->n_t * t->n_e;
     }
     c.n_bins = t->n_bins;
-    for (int b = 0; b < 2; b++) { c.bank[b] = L.bank[b]; c.q[b] = L.q[b]; }
-    c.q_cap = (unsigned int)cap;
+    for (int b = 0; b < 2; b++) c.bank[b] = L.bank[b];
+    c.fis = L.fis;
+    c.cap = (unsigned int)cap;
     c.qc = L.qc; c.flux = L.flux; c.scal = L.scal; c.counters = L.counters; c.err = L.err;
     c.tr.rec = nullptr;
     for (int k = 0; k < 3; k++) { c.src_lo[k] = s->lo[k]; c.src_hi[k] = s->hi[k]; c.src_dir[k] = s->dir[k]; }
@@ -501,6 +510,7 @@ static int reset_run(mcdc_problem *p)
     CUDA_OK(cudaMemsetAsync(p->flux_acc2, 0, sizeof(double) * c.n_tally, st));
     CUDA_OK(cudaMemsetAsync(c.counters, 0, 8 * MCDC_N_COUNTERS, st));
     CUDA_OK(cudaMemsetAsync(c.err, 0, 16, st));
+    CUDA_OK(cudaMemsetAsync(c.fis.n, 0, sizeof(int) * (size_t)p->cap, st));
     if (c.tr.rec) CUDA_OK(cudaMemsetAsync(c.tr.count, 0, sizeof(unsigned int) * c.tr.cap_slots, st));
     p->k_cycle.clear();
     p->n_active = 0;
@@ -580,8 +590,9 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
     k_scan_top<<<1, 1024, 0, st>>>(p->part, nb);
     if (p->mode == 0) k_emit<false><<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part, (unsigned int)p->cap);
     else k_emit<true><<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part, (unsigned int)p->cap);
+    k_clear_counts<<<nb, BS, 0, st>>>(c.fis.n, (unsigned int)M);
     }
-    p->n_launches += 3;
+    p->n_launches += 4;
     CUDA_OK(cudaMemcpyAsync(&p->pin->total, p->part + nb, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(&p->pin->err, c.err, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -647,7 +658,6 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     p->host_counters[0] += M;
     p->host_counters[11] += total;
     if (total > p->host_counters[12]) p->host_counters[12] = total;
-    c.cur = 1 - c.cur;
     p->bank_count = total;
     p->last_N = N;
     return 0;
@@ -738,7 +748,6 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
         if (total > p->host_counters[12]) p->host_counters[12] = total;
         secondaries += total;
         if (secondaries > 64 * N + 4096) return fail(MCDC_EBANK, "prompt fission chain does not die out (R25)");
-        c.cur = 1 - c.cur;
         M = total;
     }
     CUDA_OK(cudaEventRecord(p->t1, st));
