@@ -14,7 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
-_SO = os.path.join(_HERE, "libmcdc_b200.so")
+_SO = os.environ.get("MCDC_LIB") or os.path.join(_HERE, "libmcdc_b200.so")  # MCDC_LIB: A/B-test another build
 _SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cuh", "mcdc_device.cuh")]
 _HDR = os.path.join(_ROOT, "include", "mcdc.h")
 

@@ -16,6 +16,7 @@ constexpr int RING = 8;            // per-sweep queue-counter sets kept alive fo
 // Geometry and small tables: plain arrays in the workspace (read-only, L1/L2 resident).
 struct Geo {
     int n_surf, n_cell, n_univ, has_lat, lat_nx, lat_ny, lat_cell;
+    unsigned int lat_magic;  // floor(2^32 / lat_nx) + 1: elem / lat_nx == umulhi(elem, lat_magic) (elem * lat_nx < 2^32)
     double lat_x0, lat_y0, lat_px, lat_py;
     const int *surf_type, *surf_bc;
     const double *surf_param;  // [n_surf][4]
@@ -82,7 +83,9 @@ struct Ctx {
     unsigned int cap;   // slots per bank
     int mode;           // 0 MG, 1 CE
     int n_tally, n_bins;
-    double *flux;       // [n_tally] per-cycle track-length tally
+    int flux_aggregate;  // global tally flavour: 1 = warp-aggregate equal bins before the atomic
+    int flux_copy_mask;  // R - 1: the per-cycle tally is kept in R copies, copy = block index & mask
+    double *flux;       // [R][n_tally] per-cycle track-length tally
     double *scal;       // [0] k numerator, [1] leakage weight
     unsigned long long *counters;  // [16]
     int *err;           // device error flag
@@ -290,10 +293,18 @@ __device__ __forceinline__ int find_cell(const Geo &G, int univ, double x, doubl
     return -1;
 }
 
+// lattice element -> (ix, iy) without an integer division
+__device__ __forceinline__ void elem_xy(const Geo &G, int elem, int &ix, int &iy)
+{
+    iy = (int)__umulhi((unsigned int)elem, G.lat_magic);
+    ix = elem - iy * G.lat_nx;
+}
+
 // element-centred coordinates, recomputed from the global position every time (R14)
 __device__ __forceinline__ void local_xy(const Geo &G, int elem, double x, double y, double &xl, double &yl)
 {
-    int ix = elem % G.lat_nx, iy = elem / G.lat_nx;
+    int ix, iy;
+    elem_xy(G, elem, ix, iy);
     xl = x - (G.lat_x0 + (ix + 0.5) * G.lat_px);
     yl = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
 }
@@ -320,8 +331,9 @@ __device__ __forceinline__ bool locate(const Geo &G, double x, double y, double 
 }
 
 // positive ray distance to surface s (infinity = miss); on: the particle sits on s (R11-R13)
+// inv_ux, inv_uy = 1/ux, 1/uy computed once per segment (axis planes and lattice walls share them)
 __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, double y, double z, double ux, double uy,
-                                                double uz, bool on)
+                                                double uz, bool on, double inv_ux, double inv_uy)
 {
     const double INF = __longlong_as_double(0x7ff0000000000000LL);
     const double *q = G.surf_param + 4 * s;
@@ -329,13 +341,16 @@ __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, d
     double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2), q3 = __ldg(q + 3);
     if (t <= 3) {
         if (on) return INF;
-        double num, den;
-        if (t == 0) { num = q0 - x; den = ux; }
-        else if (t == 1) { num = q0 - y; den = uy; }
-        else if (t == 2) { num = q0 - z; den = uz; }
-        else { num = q3 - (q0 * x + q1 * y + q2 * z); den = q0 * ux + q1 * uy + q2 * uz; }
-        if (den == 0.0) return INF;
-        double d = num / den;
+        double d;
+        if (t == 0) { if (ux == 0.0) return INF; d = (q0 - x) * inv_ux; }
+        else if (t == 1) { if (uy == 0.0) return INF; d = (q0 - y) * inv_uy; }
+        else {
+            double num, den;
+            if (t == 2) { num = q0 - z; den = uz; }
+            else { num = q3 - (q0 * x + q1 * y + q2 * z); den = q0 * ux + q1 * uy + q2 * uz; }
+            if (den == 0.0) return INF;
+            d = num / den;
+        }
         return d > 0.0 ? d : INF;
     }
     double a, k, c;
@@ -374,38 +389,40 @@ __device__ __forceinline__ double nearest(const Geo &G, double x, double y, doub
 {
     double best = __longlong_as_double(0x7ff0000000000000LL);
     hit = -1;
+    const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;  // +-inf when the component is zero: guarded at use
     int c0 = elem >= 0 ? G.lat_cell : cell;
     int k1 = __ldg(G.cso + c0 + 1);
     for (int k = __ldg(G.cso + c0); k < k1; k++) {
         int s = __ldg(G.csi + k);
-        double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last);
+        double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
         if (d < best) { best = d; hit = s; }
     }
     if (elem >= 0) {
-        double xl, yl;
-        local_xy(G, elem, x, y, xl, yl);
+        int ix, iy;
+        elem_xy(G, elem, ix, iy);
+        const double xl = x - (G.lat_x0 + (ix + 0.5) * G.lat_px);
+        const double yl = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
         k1 = __ldg(G.cso + cell + 1);
         for (int k = __ldg(G.cso + cell); k < k1; k++) {
             int s = __ldg(G.csi + k);
-            double d = surf_distance(G, s, xl, yl, z, ux, uy, uz, s == last);
+            double d = surf_distance(G, s, xl, yl, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
-        int ix = elem % G.lat_nx, iy = elem / G.lat_nx;
         // only the wall ahead on each axis; the lattice's outermost walls are never events (R14)
         if (ux < 0.0 && ix > 0) {
-            double d = (G.lat_x0 + ix * G.lat_px - x) / ux;
+            double d = (G.lat_x0 + ix * G.lat_px - x) * inv_ux;
             if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 0; }
         }
         if (ux > 0.0 && ix + 1 < G.lat_nx) {
-            double d = (G.lat_x0 + (ix + 1) * G.lat_px - x) / ux;
+            double d = (G.lat_x0 + (ix + 1) * G.lat_px - x) * inv_ux;
             if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 1; }
         }
         if (uy < 0.0 && iy > 0) {
-            double d = (G.lat_y0 + iy * G.lat_py - y) / uy;
+            double d = (G.lat_y0 + iy * G.lat_py - y) * inv_uy;
             if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 2; }
         }
         if (uy > 0.0 && iy + 1 < G.lat_ny) {
-            double d = (G.lat_y0 + (iy + 1) * G.lat_py - y) / uy;
+            double d = (G.lat_y0 + (iy + 1) * G.lat_py - y) * inv_uy;
             if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 3; }
         }
     }
@@ -427,11 +444,38 @@ struct Particle {
     unsigned long long id;
 };
 
-// per-thread accumulators reduced once per kernel
+// per-thread accumulators reduced once per kernel.  Event counts by code 1..10 are packed as 16-bit fields of
+// three 64-bit registers (a dynamically indexed array would live in local memory); a thread that nears
+// 65535 events spills its fields to the global counters.
 struct Acc {
     double knum, leak;
-    unsigned int n_ev[11];  // events by code 1..10 (index 0 unused)
+    unsigned long long pk0, pk1, pk2;
+    unsigned int since;
+    __device__ __forceinline__ void clear() { knum = leak = 0.0; pk0 = pk1 = pk2 = 0ull; since = 0u; }
+    __device__ __forceinline__ unsigned int field(int e) const
+    {
+        unsigned long long w = (e >> 2) == 0 ? pk0 : ((e >> 2) == 1 ? pk1 : pk2);
+        return (unsigned int)(w >> ((e & 3) * 16)) & 0xffffu;
+    }
 };
+
+__device__ __forceinline__ void count_event(unsigned long long *counters, Acc &acc, int ev)
+{
+    unsigned long long inc = 1ull << ((ev & 3) * 16);
+    int w = ev >> 2;
+    acc.pk0 += w == 0 ? inc : 0ull;
+    acc.pk1 += w == 1 ? inc : 0ull;
+    acc.pk2 += w == 2 ? inc : 0ull;
+    if (++acc.since >= 65000u) {
+#pragma unroll
+        for (int e = 1; e < 11; e++) {
+            unsigned int n = acc.field(e);
+            if (n) atomicAdd(counters + e, (unsigned long long)n);
+        }
+        acc.pk0 = acc.pk1 = acc.pk2 = 0ull;
+        acc.since = 0u;
+    }
+}
 
 enum { ADV_DEAD = 0, ADV_SCATTER = 1, ADV_SURFACE = 2, ADV_FISSION = 3 };
 constexpr int HIT_TIME_EDGE = 0x3fff0000;  // aux code of a time-edge event in the surface queue
@@ -470,13 +514,15 @@ __device__ __forceinline__ void flux_add(const Ctx &c, double *s_flux, long long
     if (PRIVATE) {
         s_flux[tix * blockDim.x + threadIdx.x] += v;
     } else {
+        double *dst = c.flux + (size_t)(blockIdx.x & c.flux_copy_mask) * c.n_tally + tix;
+        if (!c.flux_aggregate) { atomicAdd(dst, v); return; }
         // warp-aggregated: lanes that hit the same bin elect a leader which adds the group's sum
         unsigned int act = __activemask();
         unsigned int grp = __match_any_sync(act, tix);
         int leader = __ffs(grp) - 1;
         int lane = threadIdx.x & 31;
         if (grp == (1u << lane)) {
-            atomicAdd(c.flux + tix, v);
+            atomicAdd(dst, v);
         } else {
             // tree over the ranks inside the group: rank r receives from rank r + step
             double sum = v;
@@ -489,7 +535,7 @@ __device__ __forceinline__ void flux_add(const Ctx &c, double *s_flux, long long
                 if (lane == leader) sum += o;
                 rest &= rest - 1;
             }
-            if (lane == leader) atomicAdd(c.flux + tix, sum);
+            if (lane == leader) atomicAdd(dst, sum);
         }
     }
 }
@@ -596,7 +642,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         else { ev = 8; code = ADV_SURFACE; aux = HIT_TIME_EDGE; }
         trace_event(c, p, ev, cell0, elem0, -1, gi, d, E_flight);
     }
-    acc.n_ev[ev]++;
+    count_event(c.counters, acc, ev);
     return code;
 }
 
@@ -651,7 +697,8 @@ __device__ __forceinline__ bool do_surface(const Ctx &c, Particle &p, int hit)
     if (hit == HIT_TIME_EDGE) return true;
     if (hit >= G.n_surf) {
         int w = hit - G.n_surf;
-        int ix = p.elem % G.lat_nx, iy = p.elem / G.lat_nx;
+        int ix, iy;
+        elem_xy(G, p.elem, ix, iy);
         if (w == 0) ix--; else if (w == 1) ix++; else if (w == 2) iy--; else iy++;
         p.elem = iy * G.lat_nx + ix;
         p.last = -1;

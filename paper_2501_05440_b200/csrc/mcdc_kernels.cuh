@@ -83,7 +83,7 @@ __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
     __syncthreads();
 #pragma unroll
     for (int e = 1; e < 11; e++) {
-        unsigned int n = acc.n_ev[e];
+        unsigned int n = acc.field(e);
         n = __reduce_add_sync(0xffffffffu, n);
         if (lane == 0 && n) atomicAdd(&s_ev[e], n);
     }
@@ -107,31 +107,37 @@ __device__ __forceinline__ void flush_private_flux(const Ctx &c, const double *s
         double v = 0.0;
         for (int t = lane; t < BS; t += 32) v += s_flux[b * BS + t];
         v = warp_sum(v);
-        if (lane == 0 && v != 0.0) atomicAdd(c.flux + b, v);
+        if (lane == 0 && v != 0.0) atomicAdd(c.flux + (size_t)(blockIdx.x & c.flux_copy_mask) * c.n_tally + b, v);
     }
 }
 
 // ballot + prefix-sum compaction (a11): output position of this thread's particle in the next bank, front
 // region for scatter events, back region for surface events; one atomic per block and region.
-__device__ __forceinline__ unsigned int block_slot(bool to_front, bool to_back, QCount *oc, unsigned int cap)
+// `par` alternates 0/1 between consecutive calls of a block: two scratch sets make two barriers per call enough.
+__device__ __forceinline__ unsigned int block_slot(bool to_front, bool to_back, QCount *oc, unsigned int cap, int par)
 {
-    __shared__ unsigned int s_n[2][BS / 32];
-    __shared__ unsigned int s_base[2];
+    __shared__ unsigned int s_n[2][2][BS / 32];
+    __shared__ unsigned int s_base[2][2];
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned int mf = __ballot_sync(0xffffffffu, to_front), mb = __ballot_sync(0xffffffffu, to_back);
-    if (lane == 0) { s_n[0][w] = __popc(mf); s_n[1][w] = __popc(mb); }
+    if (lane == 0) { s_n[par][0][w] = __popc(mf); s_n[par][1][w] = __popc(mb); }
     __syncthreads();
     if (threadIdx.x < 2) {
-        unsigned int tot = 0;
-        for (int i = 0; i < BS / 32; i++) { unsigned int n = s_n[threadIdx.x][i]; s_n[threadIdx.x][i] = tot; tot += n; }
-        s_base[threadIdx.x] = tot ? atomicAdd(threadIdx.x == 0 ? &oc->n_scat : &oc->n_surf, tot) : 0u;
+        unsigned int tot = 0, n_w[BS / 32];
+#pragma unroll
+        for (int i = 0; i < BS / 32; i++) { n_w[i] = s_n[par][threadIdx.x][i]; tot += n_w[i]; }
+        s_base[par][threadIdx.x] = tot ? atomicAdd(threadIdx.x == 0 ? &oc->n_scat : &oc->n_surf, tot) : 0u;
     }
     __syncthreads();
     unsigned int lt = (1u << lane) - 1u;
     unsigned int pos = 0xffffffffu;
-    if (to_front) pos = s_base[0] + s_n[0][w] + __popc(mf & lt);
-    if (to_back) pos = cap - 1u - (s_base[1] + s_n[1][w] + __popc(mb & lt));
-    __syncthreads();
+    if (to_front || to_back) {
+        int q = to_front ? 0 : 1;
+        unsigned int off = 0;
+        for (int i = 0; i < w; i++) off += s_n[par][q][i];
+        off += s_base[par][q] + __popc((to_front ? mf : mb) & lt);
+        pos = to_front ? off : cap - 1u - off;
+    }
     return pos;
 }
 
@@ -191,8 +197,11 @@ __global__ void __launch_bounds__(BS) k_store_sites(Ctx c, Site *sites, unsigned
 }
 
 // ------------------------------------------------------------------ per-event kernels
+#ifndef MCDC_ADV_MINBLOCKS
+#define MCDC_ADV_MINBLOCKS 3
+#endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS) k_advance(Ctx c, unsigned int s, unsigned int n0)
+__global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsigned int s, unsigned int n0)
 {
     extern __shared__ double s_flux[];
     unsigned int n_front = n0, n_in = n0;
@@ -206,12 +215,11 @@ __global__ void __launch_bounds__(BS) k_advance(Ctx c, unsigned int s, unsigned 
         __syncthreads();
     }
     Acc acc;
-    acc.knum = acc.leak = 0.0;
-#pragma unroll
-    for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
+    acc.clear();
     const Bank &B = c.bank[s & 1];
     const Bank &O = c.bank[(s + 1) & 1];
-    for (unsigned int base = blockIdx.x * BS; base < n_in; base += gridDim.x * BS) {
+    int par = 0;
+    for (unsigned int base = blockIdx.x * BS; base < n_in; base += gridDim.x * BS, par ^= 1) {
         unsigned int t = base + threadIdx.x;
         int code = ADV_DEAD, aux = 0;
         Particle p;
@@ -226,7 +234,7 @@ __global__ void __launch_bounds__(BS) k_advance(Ctx c, unsigned int s, unsigned 
                 if (code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
-        unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap);
+        unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap, par);
         if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot, aux);
     }
     if (PRIVATE) flush_private_flux(c, s_flux);
@@ -324,9 +332,7 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         c.qc[(s + 1) % RING] = z;
     }
     Acc acc;
-    acc.knum = acc.leak = 0.0;
-#pragma unroll
-    for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
+    acc.clear();
     const Bank &B = c.bank[0];
     unsigned int alive = 0;
     for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
@@ -361,9 +367,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
         n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
     }
     Acc acc;
-    acc.knum = acc.leak = 0.0;
-#pragma unroll
-    for (int e = 0; e < 11; e++) acc.n_ev[e] = 0;
+    acc.clear();
     const Bank &B = c.bank[s & 1];
     unsigned int done = 0;
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < n_in; t += gridDim.x * BS) {
@@ -487,14 +491,19 @@ __global__ void __launch_bounds__(BS) k_clear_counts(int *n, unsigned int m)
 }
 
 // cycle end: per-source-particle flux into the running mean / mean-square, clear the per-cycle tally (R17)
-__global__ void __launch_bounds__(BS) k_accumulate(double *flux, double *acc, double *acc2, int n_tally, double inv_n,
-                                                   int active)
+__global__ void __launch_bounds__(BS) k_accumulate(double *flux, int copies, double *flux_cycle, double *acc, double *acc2,
+                                                   int n_tally, double inv_n, int active)
 {
     int i = blockIdx.x * BS + threadIdx.x;
     if (i >= n_tally) return;
-    double f = flux[i] * inv_n;
+    double f = 0.0;
+    for (int r = 0; r < copies; r++) {  // the replicated per-cycle tally (see flux_add)
+        f += flux[(size_t)r * n_tally + i];
+        flux[(size_t)r * n_tally + i] = 0.0;
+    }
+    f *= inv_n;
+    flux_cycle[i] = f;
     if (active) { acc[i] += f; acc2[i] += f * f; }
-    flux[i] = 0.0;
 }
 
 // ------------------------------------------------------------------ unit-level test kernels

@@ -33,6 +33,10 @@ static int fail(int code, const char *fmt, ...)
 static const int LAG = 3;                 // sweeps the host may run ahead of the queue-count read-back
 static const int DEFAULT_TAIL = 32768;    // live particles at which the tail kernel takes over
 static const uint64_t TRACE_BYTES = 48ull << 20;
+#ifndef MCDC_AGG_MAX
+#define MCDC_AGG_MAX 4096
+#endif
+static const int AGGREGATE_TALLY_MAX = MCDC_AGG_MAX;  // above this, equal bins inside a warp are rare: plain float64 atomics
 static const int PRIVATE_TALLY_MAX = 20;  // bins for which the one-column-per-thread tally fits (20*256*8 = 40 KB)
 
 struct HostPinned {
@@ -50,7 +54,8 @@ struct mcdc_problem {
     int schedule, tail;
     uint64_t cap;  // bank slots
     // workspace pieces not in ctx
-    double *flux_acc, *flux_acc2;
+    double *flux_acc, *flux_acc2, *flux_cycle;
+    int flux_copies;
     unsigned int *part;
     Site *sites;
     char *trace_base;
@@ -134,7 +139,7 @@ struct Layout {  // everything carved from the workspace, in order
     Bank bank[2];
     FisRec fis;
     QCount *qc;
-    double *flux, *flux_acc, *flux_acc2, *scal;
+    double *flux, *flux_acc, *flux_acc2, *flux_cycle, *scal;
     unsigned long long *counters;
     int *err;
     unsigned int *part;
@@ -143,6 +148,15 @@ struct Layout {  // everything carved from the workspace, in order
     unsigned int *trace_count;
     uint64_t bytes;
 };
+
+// The per-cycle tally is replicated (copy = block index mod R) so that hot bins (e.g. one reflector bin that a
+// large share of all segments hits) do not serialise on one L2 address; k_accumulate sums the copies.
+static int flux_copies_for(uint64_t n_tally)
+{
+    int r = 64;
+    while (r > 1 && (uint64_t)r * n_tally * 8 > (4ull << 20)) r >>= 1;
+    return r;
+}
 
 static uint64_t n_tally_of(const mcdc_materials *mat, const mcdc_tally_spec *t)
 {
@@ -214,7 +228,8 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     }
     L.qc = C.take<QCount>(RING);
     uint64_t nt = n_tally_of(m, t);
-    L.flux = C.take<double>(nt); L.flux_acc = C.take<double>(nt); L.flux_acc2 = C.take<double>(nt);
+    L.flux = C.take<double>(nt * flux_copies_for(nt)); L.flux_acc = C.take<double>(nt); L.flux_acc2 = C.take<double>(nt);
+    L.flux_cycle = C.take<double>(nt);
     L.scal = C.take<double>(8);
     L.counters = C.take<unsigned long long>(MCDC_N_COUNTERS);
     L.err = C.take<int>(4);
@@ -255,6 +270,7 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
     if (g->has_lattice) {
         if (n_lat_cells != 1) return fail(MCDC_EGEOM, "exactly one lattice-filled cell is supported");
         if (g->lat_nx < 1 || g->lat_ny < 1 || !(g->lat_px > 0) || !(g->lat_py > 0)) return fail(MCDC_EGEOM, "lattice shape");
+        if ((unsigned long long)g->lat_nx * g->lat_nx * g->lat_ny >= 0x100000000ull) return fail(MCDC_EGEOM, "lattice too large (nx*nx*ny must be < 2^32)");
         if (!t->lat_bin) return fail(MCDC_EINVAL, "lat_bin missing");
         for (int e = 0; e < g->lat_nx * g->lat_ny; e++) {
             if (g->lat_univ[e] < 1 || g->lat_univ[e] >= g->n_univ) return fail(MCDC_EGEOM, "lattice element %d names universe %d", e, g->lat_univ[e]);
@@ -345,6 +361,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     G.lat_nx = g->has_lattice ? g->lat_nx : 1; G.lat_ny = g->has_lattice ? g->lat_ny : 1;
     G.lat_x0 = g->lat_x0; G.lat_y0 = g->lat_y0; G.lat_px = g->lat_px; G.lat_py = g->lat_py;
     G.lat_cell = -1;
+    G.lat_magic = (unsigned int)(0x100000000ull / (unsigned long long)G.lat_nx) + 1u;
     for (int cc = 0; cc < g->n_cell; cc++) if (g->cell_fill_type[cc] == 1) G.lat_cell = cc;
     G.surf_type = L.surf_type; G.surf_bc = L.surf_bc; G.surf_param = L.surf_param;
     G.cso = L.cso; G.csi = L.csi; G.css = L.css; G.cft = L.cft; G.cfill = L.cfill; G.cbin = L.cbin; G.uco = L.uco;
@@ -449,10 +466,14 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     for (int k = 0; k < 3; k++) { c.src_lo[k] = s->lo[k]; c.src_hi[k] = s->hi[k]; c.src_dir[k] = s->dir[k]; }
     c.src_iso = s->isotropic; c.src_E = s->E; c.src_t = s->t;
     c.w0 = 1.0; c.k_prev = 1.0;
-    p->flux_acc = L.flux_acc; p->flux_acc2 = L.flux_acc2; p->part = L.part; p->sites = L.sites;
+    p->flux_acc = L.flux_acc; p->flux_acc2 = L.flux_acc2; p->flux_cycle = L.flux_cycle;
+    p->flux_copies = flux_copies_for((uint64_t)c.n_tally);
+    c.flux_copy_mask = p->flux_copies - 1;
+    p->part = L.part; p->sites = L.sites;
     p->trace_base = L.trace; p->trace_count = L.trace_count;
     p->tally_private = c.n_tally <= PRIVATE_TALLY_MAX;
-    if (e == cudaSuccess) e = cudaMemsetAsync(L.flux, 0, sizeof(double) * c.n_tally, st);
+    c.flux_aggregate = c.n_tally <= AGGREGATE_TALLY_MAX ? 1 : 0;
+    if (e == cudaSuccess) e = cudaMemsetAsync(L.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc, 0, sizeof(double) * c.n_tally, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc2, 0, sizeof(double) * c.n_tally, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.scal, 0, 64, st);
@@ -505,7 +526,7 @@ static int reset_run(mcdc_problem *p)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
-    CUDA_OK(cudaMemsetAsync(c.flux, 0, sizeof(double) * c.n_tally, st));
+    CUDA_OK(cudaMemsetAsync(c.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st));
     CUDA_OK(cudaMemsetAsync(p->flux_acc, 0, sizeof(double) * c.n_tally, st));
     CUDA_OK(cudaMemsetAsync(p->flux_acc2, 0, sizeof(double) * c.n_tally, st));
     CUDA_OK(cudaMemsetAsync(c.counters, 0, 8 * MCDC_N_COUNTERS, st));
@@ -637,8 +658,8 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     rc = emit_children(p, M, &total);
     if (rc) return rc;
     CUDA_OK(cudaEventRecord(p->t1, st));
-    if (flux_cycle_host) CUDA_OK(cudaMemcpyAsync(flux_cycle_host, c.flux, sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, st));
-    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_acc, p->flux_acc2, c.n_tally, 1.0 / (double)N, active);
+    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc, p->flux_acc2, c.n_tally, 1.0 / (double)N, active);
+    if (flux_cycle_host) CUDA_OK(cudaMemcpyAsync(flux_cycle_host, p->flux_cycle, sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, st));
     p->n_launches++;
     CUDA_OK(cudaStreamSynchronize(st));
     float ms = 0.f;
@@ -646,7 +667,6 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     p->ms_transport += ms;
     rc = device_error(p);
     if (rc) return rc;
-    if (flux_cycle_host) for (int i = 0; i < c.n_tally; i++) flux_cycle_host[i] /= (double)N;
     double k_c = p->pin->scal[0] / (double)N, leak = p->pin->scal[1] / (double)N;
     p->k_cycle.push_back(k_c);
     if (active) {
@@ -751,7 +771,7 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
         M = total;
     }
     CUDA_OK(cudaEventRecord(p->t1, st));
-    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_acc, p->flux_acc2, c.n_tally, 1.0 / (double)N, 1);
+    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc, p->flux_acc2, c.n_tally, 1.0 / (double)N, 1);
     p->n_launches++;
     CUDA_OK(cudaStreamSynchronize(st));
     float ms = 0.f;
