@@ -21,8 +21,9 @@ struct Geo {
     const int *surf_type, *surf_bc;
     const double *surf_param;  // [n_surf][4]
     const int *cso, *csi, *css, *cft, *cfill, *cbin, *uco;
-    const int *lat_univ, *lat_bin;
-};
+    const int *lat_univ, *lat_bin;  // lat_bin bit 30: the enclosing cell's surfaces can be the nearest boundary
+};                                  // from inside this element (create() proves when they cannot)
+constexpr int LAT_ROOT_FLAG = 1 << 30;
 
 struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi running chi sums
     int G, n_mat;
@@ -385,18 +386,19 @@ __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, d
 // nearest boundary of the current location; candidate order: enclosing-cell surfaces, local-cell surfaces,
 // lattice walls -x,+x,-y,+y; ties keep the first (R12, R14).  hit = surface id, or n_surf+k for wall k.
 __device__ __forceinline__ double nearest(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int cell,
-                                          int elem, int last, int &hit)
+                                          int elem, int last, int &hit, bool root_needed = true)
 {
     double best = __longlong_as_double(0x7ff0000000000000LL);
     hit = -1;
     const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;  // +-inf when the component is zero: guarded at use
     int c0 = elem >= 0 ? G.lat_cell : cell;
     int k1 = __ldg(G.cso + c0 + 1);
-    for (int k = __ldg(G.cso + c0); k < k1; k++) {
-        int s = __ldg(G.csi + k);
-        double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
-        if (d < best) { best = d; hit = s; }
-    }
+    if (root_needed)
+        for (int k = __ldg(G.cso + c0); k < k1; k++) {
+            int s = __ldg(G.csi + k);
+            double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
+            if (d < best) { best = d; hit = s; }
+        }
     if (elem >= 0) {
         int ix, iy;
         elem_xy(G, elem, ix, iy);
@@ -550,7 +552,12 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     const int cell0 = p.cell, elem0 = p.elem;
     const int mat = __ldg(G.cfill + p.cell);
     int bin = __ldg(G.cbin + p.cell);
-    if (p.elem >= 0) bin += __ldg(G.lat_bin + p.elem);
+    bool root_needed = true;
+    if (p.elem >= 0) {
+        int lb = __ldg(G.lat_bin + p.elem);
+        root_needed = (lb & LAT_ROOT_FLAG) != 0;
+        bin += lb & (LAT_ROOT_FLAG - 1);
+    }
 
     double sig_t, nusf, cum[MAX_CE_COL];
     int gi, ncol = 0;
@@ -580,7 +587,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     // candidate distances: collision (one draw every segment), boundary, time edge (R12)
     double d_coll = -log(rng.next()) / sig_t;
     int hit;
-    double d_surf = nearest(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit);
+    double d_surf = nearest(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_needed);
     double v = 0.0, d_time = __longlong_as_double(0x7ff0000000000000LL);
     if (CE) {
         v = speed_of(p.E);

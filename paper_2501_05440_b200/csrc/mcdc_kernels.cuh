@@ -122,10 +122,10 @@ __device__ __forceinline__ unsigned int block_slot(bool to_front, bool to_back, 
     unsigned int mf = __ballot_sync(0xffffffffu, to_front), mb = __ballot_sync(0xffffffffu, to_back);
     if (lane == 0) { s_n[par][0][w] = __popc(mf); s_n[par][1][w] = __popc(mb); }
     __syncthreads();
-    if (threadIdx.x < 2) {
-        unsigned int tot = 0, n_w[BS / 32];
+    if (threadIdx.x < 2) {  // exclusive prefix over the warps, then the block's base in the region
+        unsigned int tot = 0;
 #pragma unroll
-        for (int i = 0; i < BS / 32; i++) { n_w[i] = s_n[par][threadIdx.x][i]; tot += n_w[i]; }
+        for (int i = 0; i < BS / 32; i++) { unsigned int n = s_n[par][threadIdx.x][i]; s_n[par][threadIdx.x][i] = tot; tot += n; }
         s_base[par][threadIdx.x] = tot ? atomicAdd(threadIdx.x == 0 ? &oc->n_scat : &oc->n_surf, tot) : 0u;
     }
     __syncthreads();
@@ -133,9 +133,7 @@ __device__ __forceinline__ unsigned int block_slot(bool to_front, bool to_back, 
     unsigned int pos = 0xffffffffu;
     if (to_front || to_back) {
         int q = to_front ? 0 : 1;
-        unsigned int off = 0;
-        for (int i = 0; i < w; i++) off += s_n[par][q][i];
-        off += s_base[par][q] + __popc((to_front ? mf : mb) & lt);
+        unsigned int off = s_base[par][q] + s_n[par][q][w] + __popc((to_front ? mf : mb) & lt);
         pos = to_front ? off : cap - 1u - off;
     }
     return pos;

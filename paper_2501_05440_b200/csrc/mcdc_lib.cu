@@ -377,7 +377,31 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     UP(L.cso, g->cell_surf_off, g->n_cell + 1); UP(L.csi, g->cell_surf_id, nref); UP(L.css, g->cell_surf_sense, nref);
     UP(L.cft, g->cell_fill_type, g->n_cell); UP(L.cfill, h_cfill.data(), g->n_cell); UP(L.cbin, t->cell_bin, g->n_cell);
     UP(L.uco, g->univ_cell_off, g->n_univ + 1);
-    if (nlat) { UP(L.lat_univ, g->lat_univ, nlat); UP(L.lat_bin, t->lat_bin, nlat); }
+    // lattice element -> tally bin, plus the flag "the enclosing cell's surfaces must be tested from inside this
+    // element".  It may be dropped only where it is provably never the nearest candidate: an interior element
+    // (all four walls are events, R14) whose closed x/y range contains none of the enclosing cell's surfaces;
+    // only axis planes x = p / y = p can be excluded that way, any other surface type keeps the flag set.
+    std::vector<int> h_latbin(nlat);
+    if (nlat) {
+        int lc = G.lat_cell;
+        for (int iy = 0; iy < g->lat_ny; iy++)
+            for (int ix = 0; ix < g->lat_nx; ix++) {
+                bool need = ix == 0 || iy == 0 || ix == g->lat_nx - 1 || iy == g->lat_ny - 1;
+                double xlo = g->lat_x0 + ix * g->lat_px, xhi = g->lat_x0 + (ix + 1) * g->lat_px;
+                double ylo = g->lat_y0 + iy * g->lat_py, yhi = g->lat_y0 + (iy + 1) * g->lat_py;
+                double tx = 1e-9 * g->lat_px, ty = 1e-9 * g->lat_py;
+                for (int k = g->cell_surf_off[lc]; k < g->cell_surf_off[lc + 1] && !need; k++) {
+                    int sidx = g->cell_surf_id[k];
+                    double pp = g->surf_param[4 * sidx];
+                    if (g->surf_type[sidx] == MCDC_PLANE_X) need = pp > xlo - tx && pp < xhi + tx;
+                    else if (g->surf_type[sidx] == MCDC_PLANE_Y) need = pp > ylo - ty && pp < yhi + ty;
+                    else need = true;
+                }
+                int e_ = iy * g->lat_nx + ix;
+                h_latbin[e_] = t->lat_bin[e_] | (need ? LAT_ROOT_FLAG : 0);
+            }
+        UP(L.lat_univ, g->lat_univ, nlat); UP(L.lat_bin, h_latbin.data(), nlat);
+    }
 
     // ---- cross sections: derived tables built here, in plain left-to-right float64 sums
     if (m) {
