@@ -149,7 +149,8 @@ def run_ours(args):
 
     P, N = workload(args)
     seed = 1 + rank  # replicas only: independent problems, no data-path collective
-    g = binding.Problem(P, device=local, search=1, tail_threshold=args.tail, schedule=args.schedule)
+    g = binding.Problem(P, device=local, search=1, tail_threshold=args.tail, schedule=args.schedule,
+                        fuse_threshold=args.fuse, fuse_segments=args.fuse_segments)
     K, W = args.steps, args.warmup
 
     # ---- device-resident throughput: W warm-up cycles, then exactly K timed cycles
@@ -278,7 +279,8 @@ def bench_ce(binding, inputs, args, peak):
     """Largest continuous-energy configuration (C5: 1e6 source particles) -- reported beside the headline."""
     import torch
     P = inputs.config5(n_particles=args.ce_particles)
-    g = binding.Problem(P, search=1, tail_threshold=args.tail, schedule=args.schedule)
+    g = binding.Problem(P, search=1, tail_threshold=args.tail, schedule=args.schedule,
+                        fuse_threshold=args.fuse, fuse_segments=args.fuse_segments)
     g.run()  # warm-up
     torch.cuda.synchronize()
     best = None
@@ -319,6 +321,8 @@ def main():
     ap.add_argument("--no-ce", dest="ce", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tail", type=int, default=0, help="tail-kernel threshold (0 = library default, <0 = off)")
+    ap.add_argument("--fuse", type=int, default=0, help="fused-sweep threshold (0 = default, <0 = off)")
+    ap.add_argument("--fuse-segments", type=int, default=0)
     ap.add_argument("--schedule", type=int, default=0, help="0 event queues (default), 1 monolithic")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 1)

@@ -126,6 +126,9 @@ typedef struct {
     int32_t device;
     int32_t schedule;
     int32_t tail_threshold;
+    int32_t fuse_threshold; /* at most this many alive: one fused launch does fuse_segments whole segments per
+                               particle, then compacts (0 = library default, negative = never) */
+    int32_t fuse_segments;  /* 0 = library default */
     int32_t reserved;
 } mcdc_device;
 
@@ -221,7 +224,7 @@ int mcdc_get_timing(const mcdc_problem *p, double *ms_transport, uint64_t *n_lau
  * stream (costs a few microseconds per launch, so it is off for throughput runs).  mcdc_get_profile fills
  * ms[MCDC_N_PROFILE] and launches[MCDC_N_PROFILE] accumulated since mcdc_set_profile. */
 enum { MCDC_PROF_ADVANCE = 0, MCDC_PROF_SCATTER, MCDC_PROF_SURFACE, MCDC_PROF_TAIL, MCDC_PROF_SEGMENT, MCDC_PROF_BANK,
-       MCDC_N_PROFILE };
+       MCDC_PROF_FUSED, MCDC_N_PROFILE };
 int mcdc_set_profile(mcdc_problem *p, int32_t on);
 int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches);
 

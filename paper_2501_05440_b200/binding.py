@@ -68,7 +68,8 @@ class TallySpec(C.Structure):
 
 class Device(C.Structure):
     _fields_ = [("workspace", C.c_void_p), ("workspace_bytes", C.c_uint64), ("stream", C.c_void_p),
-                ("device", C.c_int32), ("schedule", C.c_int32), ("tail_threshold", C.c_int32), ("reserved", C.c_int32)]
+                ("device", C.c_int32), ("schedule", C.c_int32), ("tail_threshold", C.c_int32), ("fuse_threshold", C.c_int32),
+                ("fuse_segments", C.c_int32), ("reserved", C.c_int32)]
 
 
 class Dims(C.Structure):
@@ -148,7 +149,8 @@ def _i(a):
 class Problem:
     """One transport problem on one CUDA device, built from a problem dict (see ``inputs``)."""
 
-    def __init__(self, P: dict, max_particles=None, device=0, schedule=0, tail_threshold=0, search=0):
+    def __init__(self, P: dict, max_particles=None, device=0, schedule=0, tail_threshold=0, search=0,
+                 fuse_threshold=0, fuse_segments=0):
         import torch
 
         if not torch.cuda.is_available():
@@ -224,6 +226,7 @@ class Problem:
         d.workspace, d.workspace_bytes = base, nbytes.value
         d.stream, d.device = self.stream.cuda_stream, device
         d.schedule, d.tail_threshold = int(schedule), int(tail_threshold)
+        d.fuse_threshold, d.fuse_segments = int(fuse_threshold), int(fuse_segments)
         h = C.c_void_p()
         self._check(self.L.mcdc_create(C.byref(g), mp, xp, C.byref(s), C.byref(t), C.byref(d), self.max_particles, C.byref(h)))
         self.h = h
@@ -297,13 +300,13 @@ class Problem:
         self._check(self.L.mcdc_get_timing(self.h, C.byref(ms), C.byref(nl)))
         return ms.value, nl.value
 
-    PROFILE_CLASSES = ("advance", "scatter", "surface", "tail", "segment", "bank")
+    PROFILE_CLASSES = ("advance", "scatter", "surface", "tail", "segment", "bank", "fused")
 
     def set_profile(self, on=True):
         self._check(self.L.mcdc_set_profile(self.h, int(on)))
 
     def profile(self):
-        ms, nl = np.zeros(6), np.zeros(6, np.uint64)
+        ms, nl = np.zeros(7), np.zeros(7, np.uint64)
         self._check(self.L.mcdc_get_profile(self.h, ms.ctypes.data_as(_dp), nl.ctypes.data_as(C.POINTER(C.c_uint64))))
         return {k: dict(ms=float(m), launches=int(n)) for k, m, n in zip(self.PROFILE_CLASSES, ms, nl)}
 

@@ -64,6 +64,17 @@ struct FisRec {
     uint64_t *id;
 };
 
+// Tail kernel, continuous energy: a thread follows its particle AND the prompt-fission subtree below it depth
+// first; pending siblings wait on a small per-thread stack in HBM.  If the stack is full the fission is left as
+// an ordinary record in the overflow part of FisRec ([M, M + over_cap)) and its children run in the next wave.
+struct StackRec {
+    double x, y, z, ux, uy, uz, E, t;
+    int cell, elem, tbin, pad;
+    unsigned long long id;
+};
+constexpr int STACK_DEPTH = 24;
+constexpr unsigned int OVER_CAP = 65536;
+
 struct QCount {  // one set per sweep (ring of RING)
     unsigned int n_scat, n_surf, n_alive, pad;
 };
@@ -91,6 +102,9 @@ struct Ctx {
     unsigned long long *counters;  // [16]
     int *err;           // device error flag
     QCount *qc;          // [RING] per-sweep counts of the front / back regions
+    StackRec *stack;     // [stack_threads][STACK_DEPTH]
+    unsigned int stack_threads;
+    unsigned int *n_over;  // overflow fission records of the running wave
     Trace tr;
     unsigned long long seed;
     unsigned int cycle;
@@ -481,6 +495,7 @@ __device__ __forceinline__ void count_event(unsigned long long *counters, Acc &a
 
 enum { ADV_DEAD = 0, ADV_SCATTER = 1, ADV_SURFACE = 2, ADV_FISSION = 3 };
 constexpr int HIT_TIME_EDGE = 0x3fff0000;  // aux code of a time-edge event in the surface queue
+constexpr int HIT_NEWBORN = 0x3fff0001;    // aux code of a prompt secondary just written to the back region
 
 struct TraceRec {  // = mcdc_trace_rec
     unsigned long long id;

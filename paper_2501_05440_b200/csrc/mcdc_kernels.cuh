@@ -139,6 +139,34 @@ __device__ __forceinline__ unsigned int block_slot(bool to_front, bool to_back, 
     return pos;
 }
 
+// same with a COUNT of back-region slots per thread (a continuous-energy fission puts its n children, alive, into
+// the next bank: secondaries carry their own id-keyed streams, so they simply join the running population)
+__device__ __forceinline__ void block_slot_n(bool to_front, unsigned int n_back, QCount *oc, unsigned int cap, int par,
+                                             unsigned int &pos_front, unsigned int &off_back)
+{
+    __shared__ unsigned int s_n[2][2][BS / 32];
+    __shared__ unsigned int s_base[2][2];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned int mf = __ballot_sync(0xffffffffu, to_front);
+    unsigned int incl = n_back;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) { s_n[par][0][w] = __popc(mf); s_n[par][1][w] = incl; }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        unsigned int tot = 0;
+#pragma unroll
+        for (int i = 0; i < BS / 32; i++) { unsigned int n = s_n[par][threadIdx.x][i]; s_n[par][threadIdx.x][i] = tot; tot += n; }
+        s_base[par][threadIdx.x] = tot ? atomicAdd(threadIdx.x == 0 ? &oc->n_scat : &oc->n_surf, tot) : 0u;
+    }
+    __syncthreads();
+    pos_front = s_base[par][0] + s_n[par][0][w] + __popc(mf & ((1u << lane) - 1u));
+    off_back = s_base[par][1] + s_n[par][1][w] + incl - n_back;  // slot k of this thread = cap - 1 - (off_back + k)
+}
+
 // ------------------------------------------------------------------ a1: source
 template <bool CE>
 __global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
@@ -194,6 +222,31 @@ __global__ void __launch_bounds__(BS) k_store_sites(Ctx c, Site *sites, unsigned
     sites[i] = s;
 }
 
+// child j of a fission at the parent's site, drawn from the parent's stream (R5).  MG: group ~ chi and an
+// isotropic direction (1 + 2 draws).  CE: Watt energy (4 draws) + direction (2 draws), own id from the domain-1
+// block keyed by (parent id, parent draw counter after the multiplicity draw, j) (R10).
+template <bool CE>
+__device__ __forceinline__ void make_child(const Ctx &c, Rng &rng, int mat, unsigned long long pid, uint32_t ctr0, int j,
+                                           Particle &p)
+{
+    if (!CE) {
+        const double *cc = c.mg.cumchi + (size_t)mat * c.mg.G;
+        p.g = pick(cc, c.mg.G, rng.next() * __ldg(cc + c.mg.G - 1));
+        double a = rng.next(), b = rng.next();
+        iso_dir(a, b, p.ux, p.uy, p.uz);
+    } else {
+        double a1 = rng.next(), a2 = rng.next(), a3 = rng.next(), a4 = rng.next();
+        double En = 1e6 * watt(c.ce.watt_a, c.ce.watt_b, a1, a2, a3, a4);
+        if (En < c.ce.E_min) En = c.ce.E_min;
+        if (En > c.ce.E_max) En = c.ce.E_max;
+        double a = rng.next(), b = rng.next();
+        iso_dir(a, b, p.ux, p.uy, p.uz);
+        p.E = En;
+        p.id = child_id(c.seed, pid, ctr0, (uint32_t)j);
+    }
+    p.last = -1;
+}
+
 // ------------------------------------------------------------------ per-event kernels
 #ifndef MCDC_ADV_MINBLOCKS
 #define MCDC_ADV_MINBLOCKS 3
@@ -229,11 +282,30 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
                 load_full<CE>(B, i, p, ctr, slot);
                 rng.init(c.seed, p.id, 0u, c.cycle, ctr);
                 code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
-                if (code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
+                if (!CE && code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
-        unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap, par);
-        if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot, aux);
+        if (!CE) {
+            unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap, par);
+            if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot, aux);
+        } else {
+            unsigned int nb = code == ADV_SURFACE ? 1u : (code == ADV_FISSION ? (unsigned int)aux : 0u);
+            unsigned int pf, ob;
+            block_slot_n(code == ADV_SCATTER, nb, oc, c.cap, par, pf, ob);
+            if (code == ADV_SCATTER) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot, aux); }
+            else if (code == ADV_SURFACE) { if (ob < c.cap) store_full<CE>(O, c.cap - 1u - ob, p, rng.ctr, slot, aux); }
+            else if (code == ADV_FISSION && nb) {
+                // prompt secondaries: born alive at the parent's site, first segment in the next sweep
+                const int mat = __ldg(c.geo.cfill + p.cell);
+                const unsigned long long pid = p.id;
+                const uint32_t ctr0 = rng.ctr;
+                for (unsigned int j = 0; j < nb; j++) {
+                    make_child<CE>(c, rng, mat, pid, ctr0, (int)j, p);
+                    if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot, HIT_NEWBORN);
+                }
+                atomicAdd(c.counters + 15, (unsigned long long)nb);
+            }
+        }
     }
     if (PRIVATE) flush_private_flux(c, s_flux);
     flush_acc(c, acc);
@@ -248,8 +320,9 @@ __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         QCount z = {0u, 0u, 0u, 0u};
         c.qc[(s + 1) % RING] = z;
+        if ((unsigned long long)oc.n_scat + oc.n_surf > c.cap) atomicExch(c.err, -3);  // the two regions met
     }
-    for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < oc.n_scat; i += gridDim.x * BS) {
+    for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < oc.n_scat && i < c.cap; i += gridDim.x * BS) {
         Particle p;
         int gl = B.gl[i];
         p.g = gl & 0xffff;
@@ -273,7 +346,7 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_surf; t += gridDim.x * BS) {
         unsigned int i = c.cap - 1u - t;
         int hit = B.ev[i];
-        if (hit == HIT_TIME_EDGE) continue;
+        if (hit == HIT_TIME_EDGE || hit == HIT_NEWBORN) continue;
         Particle p;
         p.x = B.x[i]; p.y = B.y[i]; p.z = B.z[i];
         p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i];
@@ -296,24 +369,88 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
     }
 }
 
-// whole segment in registers (shared by the monolithic schedule and the tail kernel)
+// whole segment in registers (shared by the monolithic schedule and the tail kernel):
+// returns 1 = still alive, 0 = history ended, 2 = ended in a fission with n_children
 template <bool CE, bool PRIVATE>
-__device__ __forceinline__ bool segment(const Ctx &c, Particle &p, Rng &rng, uint32_t slot, Acc &acc, double *s_flux)
+__device__ __forceinline__ int segment(const Ctx &c, Particle &p, Rng &rng, Acc &acc, double *s_flux, int &n_children)
 {
     int aux = 0;
     int code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
-    if (code == ADV_SCATTER) { do_scatter<CE>(c, p, rng, aux); return true; }
+    if (code == ADV_SCATTER) { do_scatter<CE>(c, p, rng, aux); return 1; }
     if (code == ADV_SURFACE) {
         if (!do_surface(c, p, aux)) {
             atomicExch(c.err, -2);
             atomicAdd(c.counters + 10, 1ull);
             p.cell = -1;
-            return false;
+            return 0;
         }
-        return true;
+        return 1;
     }
-    if (code == ADV_FISSION) record_fission<CE>(c, p, rng.ctr, slot, aux);
-    return false;
+    if (code == ADV_FISSION) { n_children = aux; return 2; }
+    return 0;
+}
+
+// Fused sweep for a thinned-out population: up to max_seg whole segments per particle in registers, then the same
+// ballot / prefix-sum compaction of the survivors into the next bank (front region; continuous-energy fission
+// children go, alive, to the back region).  One launch replaces 3 * max_seg launches of the per-event kernels
+// when a sweep is launch-latency bound; divergence is irrelevant at these sizes.
+template <bool CE, bool PRIVATE>
+__global__ void __launch_bounds__(BS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
+{
+    extern __shared__ double s_flux[];
+    unsigned int n_front = n0, n_in = n0;
+    if (s > 0) {
+        QCount pc = c.qc[(s - 1) % RING];
+        n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
+    }
+    QCount *oc = c.qc + (s % RING);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        QCount z = {0u, 0u, 0u, 0u};
+        c.qc[(s + 1) % RING] = z;
+        if (n_in > c.cap) atomicExch(c.err, -3);
+    }
+    if (PRIVATE) {
+        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
+        __syncthreads();
+    }
+    Acc acc;
+    acc.clear();
+    const Bank &B = c.bank[s & 1];
+    const Bank &O = c.bank[(s + 1) & 1];
+    int par = 0;
+    for (unsigned int base = blockIdx.x * BS; base < n_in; base += gridDim.x * BS, par ^= 1) {
+        unsigned int t = base + threadIdx.x;
+        int st = 0, nch = 0;
+        Particle p;
+        uint32_t ctr = 0, slot = 0;
+        Rng rng;
+        if (t < n_in && t < c.cap) {
+            unsigned int i = live_pos(c.cap, n_front, t);
+            if (B.cell[i] >= 0) {
+                load_full<CE>(B, i, p, ctr, slot);
+                rng.init(c.seed, p.id, 0u, c.cycle, ctr);
+                unsigned int k = 0;
+                do { st = segment<CE, PRIVATE>(c, p, rng, acc, s_flux, nch); } while (st == 1 && ++k < max_seg);
+                if (!CE && st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
+            }
+        }
+        unsigned int nb = (CE && st == 2) ? (unsigned int)nch : 0u;
+        unsigned int pf, ob;
+        block_slot_n(st == 1, nb, oc, c.cap, par, pf, ob);
+        if (st == 1) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot, 0); }
+        else if (nb) {
+            const int mat = __ldg(c.geo.cfill + p.cell);
+            const unsigned long long pid = p.id;
+            const uint32_t ctr0 = rng.ctr;
+            for (unsigned int j = 0; j < nb; j++) {
+                make_child<CE>(c, rng, mat, pid, ctr0, (int)j, p);
+                if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot, HIT_NEWBORN);
+            }
+            atomicAdd(c.counters + 15, (unsigned long long)nb);
+        }
+    }
+    if (PRIVATE) flush_private_flux(c, s_flux);
+    flush_acc(c, acc);
 }
 
 // monolithic schedule: every slot of bank 0, one segment, no compaction; counts the survivors
@@ -340,9 +477,11 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         load_full<CE>(B, i, p, ctr, slot);
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-        bool live = segment<CE, PRIVATE>(c, p, rng, slot, acc, s_flux);
-        store_full<CE>(B, i, p, rng.ctr, slot, live ? 0 : EV_DEAD);
-        if (live) alive++;
+        int nch = 0;
+        int st = segment<CE, PRIVATE>(c, p, rng, acc, s_flux, nch);
+        if (st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
+        store_full<CE>(B, i, p, rng.ctr, slot, st == 1 ? 0 : EV_DEAD);
+        if (st == 1) alive++;
     }
     alive = __reduce_add_sync(0xffffffffu, alive);
     if ((threadIdx.x & 31) == 0 && alive) atomicAdd(&c.qc[s % RING].n_alive, alive);
@@ -367,7 +506,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
     Acc acc;
     acc.clear();
     const Bank &B = c.bank[s & 1];
-    unsigned int done = 0;
+    unsigned int done = 0, born = 0, pops = 0;
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < n_in; t += gridDim.x * BS) {
         unsigned int i = live_pos(c.cap, n_front, t);
         if (B.cell[i] < 0) continue;
@@ -376,22 +515,66 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
         load_full<CE>(B, i, p, ctr, slot);
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-        unsigned int guard = 0;
-        while (segment<CE, PRIVATE>(c, p, rng, slot, acc, s_flux)) {
-            if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
+        unsigned int guard = 0, depth = 0;
+        StackRec *stk = CE ? c.stack + (size_t)(blockIdx.x * BS + threadIdx.x) * STACK_DEPTH : nullptr;
+        for (;;) {
+            int nch = 0, st;
+            while ((st = segment<CE, PRIVATE>(c, p, rng, acc, s_flux, nch)) == 1) {
+                if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
+            }
+            done++;
+            if (st == 2) {
+                if (!CE) record_fission<CE>(c, p, rng.ctr, slot, nch);
+                else if (nch > 0) {
+                    if (depth + (unsigned int)nch <= STACK_DEPTH) {
+                        const int mat = __ldg(c.geo.cfill + p.cell);
+                        const unsigned long long pid = p.id;
+                        const uint32_t ctr0 = rng.ctr;
+                        Particle ch = p;
+                        for (int j = 0; j < nch; j++) {
+                            make_child<CE>(c, rng, mat, pid, ctr0, j, ch);
+                            StackRec r;
+                            r.x = ch.x; r.y = ch.y; r.z = ch.z; r.ux = ch.ux; r.uy = ch.uy; r.uz = ch.uz; r.E = ch.E; r.t = ch.t;
+                            r.cell = ch.cell; r.elem = ch.elem; r.tbin = ch.tbin; r.pad = 0; r.id = ch.id;
+                            stk[depth++] = r;
+                        }
+                        born += (unsigned int)nch;
+                    } else {  // stack full: an ordinary fission record in the overflow region, next wave
+                        unsigned int k = atomicAdd(c.n_over, 1u);
+                        if (k < OVER_CAP) record_fission<CE>(c, p, rng.ctr, n0 + k, nch);
+                        else atomicExch(c.err, -3);
+                    }
+                }
+            }
+            if (!CE || depth == 0) break;
+            if (++pops > 4000000u) { atomicExch(c.err, -3); break; }  // R25a: diverging chain
+            StackRec r = stk[--depth];
+            p.x = r.x; p.y = r.y; p.z = r.z; p.ux = r.ux; p.uy = r.uy; p.uz = r.uz; p.E = r.E; p.t = r.t;
+            p.cell = r.cell; p.elem = r.elem; p.tbin = r.tbin; p.id = r.id; p.last = -1; p.g = 0;
+            rng.init(c.seed, p.id, 0u, c.cycle, 0u);
+            guard = 0;
         }
-        done++;
     }
     done = __reduce_add_sync(0xffffffffu, done);
+    born = __reduce_add_sync(0xffffffffu, born);
     if ((threadIdx.x & 31) == 0 && done) atomicAdd(c.counters + 14, (unsigned long long)done);
+    if ((threadIdx.x & 31) == 0 && born) atomicAdd(c.counters + 15, (unsigned long long)born);
     if (PRIVATE) flush_private_flux(c, s_flux);
     flush_acc(c, acc);
 }
 
 // ------------------------------------------------------------------ a10/a12: fission bank by count-scan-write
-__global__ void __launch_bounds__(BS) k_scan_partial(Ctx c, unsigned int n, unsigned int *part)
+// number of fission-record slots of the running wave: its M particles plus the overflow records
+__device__ __forceinline__ unsigned int record_count(const Ctx &c, unsigned int m)
+{
+    unsigned int k = *c.n_over;
+    return m + (k < OVER_CAP ? k : OVER_CAP);
+}
+
+__global__ void __launch_bounds__(BS) k_scan_partial(Ctx c, unsigned int m, unsigned int *part)
 {
     __shared__ unsigned int s_w[BS / 32];
+    const unsigned int n = record_count(c, m);
     unsigned int i = blockIdx.x * BS + threadIdx.x;
     unsigned int v = i < n ? (unsigned int)c.fis.n[i] : 0u;
     v = __reduce_add_sync(0xffffffffu, v);
@@ -429,11 +612,12 @@ __global__ void __launch_bounds__(1024) k_scan_top(unsigned int *part, unsigned 
 // stream (R5).  CE: Watt energy (4 draws) + direction (2 draws), own id from the domain-1 block (R10).
 // The children's fission counts are cleared through a second array (nn) because n is still being read.
 template <bool CE>
-__global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsigned int *part, unsigned int cap)
+__global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int m, const unsigned int *part, unsigned int cap)
 {
     __shared__ unsigned int s_w[BS / 32];
     const FisRec &F = c.fis;
     const Bank &O = c.bank[0];
+    const unsigned int n = record_count(c, m);
     unsigned int i = blockIdx.x * BS + threadIdx.x;
     int nc = i < n ? F.n[i] : 0;
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -453,7 +637,7 @@ __global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsign
     Particle p;
     p.x = F.x[i]; p.y = F.y[i]; p.z = F.z[i];
     p.cell = F.cell[i]; p.elem = F.elem[i];
-    p.last = -1; p.g = 0; p.E = 0.0; p.t = 0.0; p.tbin = 0;
+    p.last = -1; p.g = 0; p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = 0;
     if (CE) { p.t = F.t[i]; p.tbin = F.tbin[i]; }
     const int mat = __ldg(c.geo.cfill + p.cell);
     unsigned long long pid = CE ? F.id[i] : (unsigned long long)i;
@@ -461,31 +645,15 @@ __global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsign
     Rng rng;
     rng.init(c.seed, pid, 0u, c.cycle, ctr0);
     for (int j = 0; j < nc; j++) {
-        unsigned int o = off + j;
-        if (!CE) {
-            const double *cc = c.mg.cumchi + (size_t)mat * c.mg.G;
-            p.g = pick(cc, c.mg.G, rng.next() * __ldg(cc + c.mg.G - 1));
-            double a = rng.next(), b = rng.next();
-            iso_dir(a, b, p.ux, p.uy, p.uz);
-            p.id = o;
-        } else {
-            double a1 = rng.next(), a2 = rng.next(), a3 = rng.next(), a4 = rng.next();
-            double En = 1e6 * watt(c.ce.watt_a, c.ce.watt_b, a1, a2, a3, a4);
-            if (En < c.ce.E_min) En = c.ce.E_min;
-            if (En > c.ce.E_max) En = c.ce.E_max;
-            double a = rng.next(), b = rng.next();
-            iso_dir(a, b, p.ux, p.uy, p.uz);
-            p.E = En;
-            p.id = child_id(c.seed, pid, ctr0, (uint32_t)j);
-        }
-        store_full<CE>(O, o, p, 0u, o, 0);
+        make_child<CE>(c, rng, mat, pid, ctr0, j, p);
+        store_full<CE>(O, off + j, p, 0u, off + j, 0);
     }
 }
 
-__global__ void __launch_bounds__(BS) k_clear_counts(int *n, unsigned int m)
+__global__ void __launch_bounds__(BS) k_clear_counts(Ctx c, unsigned int m)
 {
     unsigned int i = blockIdx.x * BS + threadIdx.x;
-    if (i < m) n[i] = 0;
+    if (i < record_count(c, m)) c.fis.n[i] = 0;
 }
 
 // cycle end: per-source-particle flux into the running mean / mean-square, clear the per-cycle tally (R17)

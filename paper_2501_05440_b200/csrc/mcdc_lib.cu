@@ -31,7 +31,11 @@ static int fail(int code, const char *fmt, ...)
     } while (0)
 
 static const int LAG = 3;                 // sweeps the host may run ahead of the queue-count read-back
-static const int DEFAULT_TAIL = 32768;    // live particles at which the tail kernel takes over
+static const int DEFAULT_TAIL = 32768;    // live particles at which the tail kernel takes over (multi-group)
+static const int DEFAULT_TAIL_CE = 64;    // continuous energy: the tail thread also follows its prompt subtree
+// live particles below which a sweep is one fused multi-segment launch (measured on B200, profiles/r01_step4*.md)
+static const int DEFAULT_FUSE = 2000000, DEFAULT_FUSE_CE = 4000000;
+static const int DEFAULT_FUSE_SEGMENTS = 8, DEFAULT_FUSE_SEGMENTS_CE = 16;
 static const uint64_t TRACE_BYTES = 48ull << 20;
 #ifndef MCDC_AGG_MAX
 #define MCDC_AGG_MAX 4096
@@ -51,7 +55,7 @@ struct mcdc_problem {
     int mode;
     cudaStream_t stream;
     int device;
-    int schedule, tail;
+    int schedule, tail, fuse, fuse_segments;
     uint64_t cap;  // bank slots
     // workspace pieces not in ctx
     double *flux_acc, *flux_acc2, *flux_cycle;
@@ -138,6 +142,8 @@ struct Layout {  // everything carved from the workspace, in order
     int *ncol, *hash;
     Bank bank[2];
     FisRec fis;
+    StackRec *stack;
+    uint64_t stack_threads;
     QCount *qc;
     double *flux, *flux_acc, *flux_acc2, *flux_cycle, *scal;
     unsigned long long *counters;
@@ -219,13 +225,16 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     }
     {
         FisRec &F = L.fis;
-        F.n = C.take<int>(cap); F.cell = C.take<int>(cap); F.elem = C.take<int>(cap);
-        F.tbin = ce ? C.take<int>(cap) : nullptr;
-        F.x = C.take<double>(cap); F.y = C.take<double>(cap); F.z = C.take<double>(cap);
-        F.t = ce ? C.take<double>(cap) : nullptr;
-        F.ctr = C.take<uint32_t>(cap);
-        F.id = ce ? C.take<uint64_t>(cap) : nullptr;
+        const uint64_t fc = cap + OVER_CAP;  // the wave's slots + the tail kernel's overflow records
+        F.n = C.take<int>(fc); F.cell = C.take<int>(fc); F.elem = C.take<int>(fc);
+        F.tbin = ce ? C.take<int>(fc) : nullptr;
+        F.x = C.take<double>(fc); F.y = C.take<double>(fc); F.z = C.take<double>(fc);
+        F.t = ce ? C.take<double>(fc) : nullptr;
+        F.ctr = C.take<uint32_t>(fc);
+        F.id = ce ? C.take<uint64_t>(fc) : nullptr;
     }
+    L.stack_threads = ce ? std::min<uint64_t>(148ull * 16ull * BS, (cap + BS - 1) / BS * BS) : 0;
+    L.stack = C.take<StackRec>(L.stack_threads * STACK_DEPTH);
     L.qc = C.take<QCount>(RING);
     uint64_t nt = n_tally_of(m, t);
     L.flux = C.take<double>(nt * flux_copies_for(nt)); L.flux_acc = C.take<double>(nt); L.flux_acc2 = C.take<double>(nt);
@@ -233,7 +242,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     L.scal = C.take<double>(8);
     L.counters = C.take<unsigned long long>(MCDC_N_COUNTERS);
     L.err = C.take<int>(4);
-    L.part = C.take<unsigned int>(cap / BS + 4);
+    L.part = C.take<unsigned int>((cap + OVER_CAP) / BS + 4);
     L.sites = C.take<Site>(cap);
     L.trace = C.take<char>(TRACE_BYTES);
     L.trace_count = C.take<unsigned int>(TRACE_BYTES / sizeof(TraceRec) + 1);
@@ -348,7 +357,9 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     p->stream = st;
     p->device = dev->device;
     p->schedule = dev->schedule;
-    p->tail = dev->tail_threshold == 0 ? DEFAULT_TAIL : dev->tail_threshold;
+    p->tail = dev->tail_threshold == 0 ? (x ? DEFAULT_TAIL_CE : DEFAULT_TAIL) : dev->tail_threshold;
+    p->fuse = dev->fuse_threshold == 0 ? (x ? DEFAULT_FUSE_CE : DEFAULT_FUSE) : dev->fuse_threshold;
+    p->fuse_segments = dev->fuse_segments <= 0 ? (x ? DEFAULT_FUSE_SEGMENTS_CE : DEFAULT_FUSE_SEGMENTS) : dev->fuse_segments;
     p->cap = cap;
     Ctx &c = p->ctx;
     c.mode = p->mode;
@@ -484,6 +495,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     c.n_bins = t->n_bins;
     for (int b = 0; b < 2; b++) c.bank[b] = L.bank[b];
     c.fis = L.fis;
+    c.stack = L.stack; c.stack_threads = (unsigned int)L.stack_threads; c.n_over = (unsigned int *)(L.err + 1);
     c.cap = (unsigned int)cap;
     c.qc = L.qc; c.flux = L.flux; c.scal = L.scal; c.counters = L.counters; c.err = L.err;
     c.tr.rec = nullptr;
@@ -555,7 +567,7 @@ static int reset_run(mcdc_problem *p)
     CUDA_OK(cudaMemsetAsync(p->flux_acc2, 0, sizeof(double) * c.n_tally, st));
     CUDA_OK(cudaMemsetAsync(c.counters, 0, 8 * MCDC_N_COUNTERS, st));
     CUDA_OK(cudaMemsetAsync(c.err, 0, 16, st));
-    CUDA_OK(cudaMemsetAsync(c.fis.n, 0, sizeof(int) * (size_t)p->cap, st));
+    CUDA_OK(cudaMemsetAsync(c.fis.n, 0, sizeof(int) * (size_t)(p->cap + OVER_CAP), st));
     if (c.tr.rec) CUDA_OK(cudaMemsetAsync(c.tr.count, 0, sizeof(unsigned int) * c.tr.cap_slots, st));
     p->k_cycle.clear();
     p->n_active = 0;
@@ -574,6 +586,7 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
     cudaStream_t st = p->stream;
     const size_t smem = PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0;
     CUDA_OK(cudaMemsetAsync(c.qc, 0, sizeof(QCount) * RING, st));
+    CUDA_OK(cudaMemsetAsync(c.n_over, 0, sizeof(unsigned int), st));
     uint64_t upper = M;
     long long known = -1;  // newest sweep whose counts the host has seen
     unsigned int s = 0;
@@ -587,7 +600,11 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
             break;
         }
         unsigned int gr = grid_for(upper);
-        if (p->schedule == 0) {
+        if (p->schedule == 0 && p->fuse > 0 && upper <= (uint64_t)p->fuse) {
+            ProfScope ps(p, MCDC_PROF_FUSED);
+            k_multi<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0, (unsigned int)p->fuse_segments);
+            p->n_launches++;
+        } else if (p->schedule == 0) {
             { ProfScope ps(p, MCDC_PROF_ADVANCE); k_advance<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
             { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, 0, st>>>(c, s); }
             { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, 0, st>>>(c, s); }
@@ -628,14 +645,14 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
-    unsigned int nb = (unsigned int)((M + BS - 1) / BS);
+    unsigned int nb = (unsigned int)((M + (p->mode == 1 ? OVER_CAP : 0) + BS - 1) / BS);
     {
     ProfScope ps(p, MCDC_PROF_BANK);
     k_scan_partial<<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part);
     k_scan_top<<<1, 1024, 0, st>>>(p->part, nb);
     if (p->mode == 0) k_emit<false><<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part, (unsigned int)p->cap);
     else k_emit<true><<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part, (unsigned int)p->cap);
-    k_clear_counts<<<nb, BS, 0, st>>>(c.fis.n, (unsigned int)M);
+    k_clear_counts<<<nb, BS, 0, st>>>(c, (unsigned int)M);
     }
     p->n_launches += 4;
     CUDA_OK(cudaMemcpyAsync(&p->pin->total, p->part + nb, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
@@ -846,7 +863,9 @@ extern "C" int mcdc_get_tallies(const mcdc_problem *p, mcdc_tallies *out)
     }
     if (out->counters) {
         for (int i = 0; i < MCDC_N_COUNTERS; i++) out->counters[i] = dc[i];
-        out->counters[0] = p->host_counters[0]; out->counters[11] = p->host_counters[11];
+        // histories started / children made inside the tail kernel (continuous energy) are counted on the device
+        out->counters[0] = p->host_counters[0] + dc[15]; out->counters[11] = p->host_counters[11] + dc[15];
+        out->counters[15] = 0;
         out->counters[12] = p->host_counters[12]; out->counters[13] = p->host_counters[13];
     }
     return 0;

@@ -26,7 +26,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_binding_struct_sizes_match_header():
     """Field-by-field layouts are plain C; spot-check sizes the header implies (LP64)."""
-    assert ctypes.sizeof(binding.Device) == 40
+    assert ctypes.sizeof(binding.Device) == 48
     assert ctypes.sizeof(binding.Dims) == 24
     assert binding.TRACE_DTYPE.itemsize == 88 and binding.SITE_DTYPE.itemsize == 56
     assert ctypes.sizeof(binding.Source) == 3 * 8 * 3 + 8 + 8 + 16

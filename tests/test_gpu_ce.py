@@ -40,12 +40,14 @@ def _fis():
 
 
 @pytest.mark.parametrize("name", list(CE_CASES))
-@pytest.mark.parametrize("schedule,tail,search", [(0, 0, 0), (0, -1, 1), (0, 1 << 30, 1), (1, 0, 0)])
-def test_ce_parity(gpu, orc, name, schedule, tail, search):
+@pytest.mark.parametrize("schedule,tail,search,fuse", [(0, 0, 0, 0), (0, -1, 1, -1), (0, 1 << 30, 1, 0), (1, 0, 0, 0), (0, -1, 1, 1 << 30),
+                                                       (0, 100, 0, 1000)])
+def test_ce_parity(gpu, orc, name, schedule, tail, search, fuse):
     P = CE_CASES[name]()
     # the supercritical pure-fission pin grows by generation: give its waves room (capacity = 2 max + 1024)
     mp = 100_000 if name == "ce_fission" else None
-    g = gpu.Problem(P, max_particles=mp, schedule=schedule, tail_threshold=tail, search=search)
+    g = gpu.Problem(P, max_particles=mp, schedule=schedule, tail_threshold=tail, search=search, fuse_threshold=fuse,
+                    fuse_segments=5)
     r = g.run()
     o = orc.Oracle(P)
     rc, ro = o.run()
@@ -54,11 +56,11 @@ def test_ce_parity(gpu, orc, name, schedule, tail, search):
     g.close()
 
 
-@pytest.mark.parametrize("schedule,tail,search", [(0, -1, 0), (0, 0, 1), (1, 0, 1)])
-def test_ce_traces_identical(gpu, orc, schedule, tail, search):
+@pytest.mark.parametrize("schedule,tail,search,fuse", [(0, -1, 0, -1), (0, 0, 1, 0), (1, 0, 1, 0), (0, 50, 1, 200)])
+def test_ce_traces_identical(gpu, orc, schedule, tail, search, fuse):
     """Source particles 0..99 of C5: identical event sequences incl. grid index, time, energy."""
     P = inputs.config5(n_particles=400, n_grid=20_000)
-    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, search=search)
+    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, search=search, fuse_threshold=fuse)
     g.set_trace(0, 100, 4096)
     r = g.run()
     o = orc.Oracle(P)

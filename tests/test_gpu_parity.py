@@ -56,12 +56,12 @@ CASES = {
 
 
 @pytest.mark.parametrize("name", list(CASES))
-@pytest.mark.parametrize("schedule,tail", [(0, 0), (0, -1), (0, 1 << 30), (1, 0)])
-def test_mg_parity(gpu, orc, name, schedule, tail):
-    """Event schedule with the default tail, with no tail kernel (pure per-event kernels), tail-only
-    (histories in registers) and the monolithic schedule all reproduce the oracle."""
+@pytest.mark.parametrize("schedule,tail,fuse", [(0, 0, 0), (0, -1, -1), (0, 1 << 30, 0), (1, 0, 0), (0, -1, 1 << 30), (0, 300, 2000)])
+def test_mg_parity(gpu, orc, name, schedule, tail, fuse):
+    """Default schedule, pure per-event kernels (no tail, no fused sweeps), tail-only (histories in registers),
+    the monolithic schedule, fused sweeps only, and a mix of all three stages all reproduce the oracle."""
     P = CASES[name]()
-    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail)
+    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, fuse_threshold=fuse, fuse_segments=3)
     r = g.run()
     o = orc.Oracle(P)
     rc, ro = o.run()
@@ -76,12 +76,12 @@ def test_mg_parity(gpu, orc, name, schedule, tail):
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small"])
-@pytest.mark.parametrize("schedule,tail", [(0, -1), (0, 0), (1, 0)])
-def test_mg_traces_identical(gpu, orc, name, schedule, tail):
+@pytest.mark.parametrize("schedule,tail,fuse", [(0, -1, -1), (0, 0, 0), (1, 0, 0), (0, 100, 500)])
+def test_mg_traces_identical(gpu, orc, name, schedule, tail, fuse):
     """100 particles x 2 cycles: identical per-particle event sequences (SURVEY.md 8d parity protocol 1)."""
     P = CASES[name]()
     N = 1000
-    g = gpu.Problem(P, max_particles=N, schedule=schedule, tail_threshold=tail)
+    g = gpu.Problem(P, max_particles=N, schedule=schedule, tail_threshold=tail, fuse_threshold=fuse)
     g.set_trace(0, 100, 1024)
     r = g.run(n_particles=N, n_inactive=0, n_active=2)
     o = orc.Oracle(P)
