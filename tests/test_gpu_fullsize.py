@@ -1,0 +1,139 @@
+"""Full-size parity (BASELINE.json sizes, in the launch configuration bench.py times): sampled per-particle event
+sequences the oracle can compute one by one, invariants that hold at any size, k within 3 combined sigma of the
+closed form (C1, C2) or of the oracle at reduced N (C3, C4), C5 flux per time bin within 4 sigma."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2501_05440_b200 import inputs
+from tests.test_gpu_parity import compare_results, compare_traces
+from tests.test_oracle_transport import EV, kinf_dense
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    from paper_2501_05440_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def invariants(r, n_hist_expected=None):
+    c = r["counters"].astype(np.int64)
+    assert c[EV["lost"]] == 0
+    assert c[EV["capture"]] + c[EV["fission"]] + c[EV["leak"]] + c[EV["cutoff"]] == c[0]
+    assert np.isfinite(r["flux_mean"]).all() and (r["flux_mean"] >= 0).all()
+    if n_hist_expected is not None:
+        assert c[0] == n_hist_expected
+
+
+def test_c1_full(gpu, orc):
+    P = inputs.config1()
+    g = gpu.Problem(P)
+    r = g.run()
+    rc, ro = orc.Oracle(P).run()
+    compare_results(r, ro)
+    invariants(r)
+    assert abs(r["k_mean"] - 1.3) < 3 * r["k_sdev"]
+    g.close()
+
+
+def test_c2_full(gpu, orc):
+    P = inputs.config2()
+    g = gpu.Problem(P)
+    r = g.run()
+    rc, ro = orc.Oracle(P).run()
+    compare_results(r, ro)
+    invariants(r)
+    assert abs(r["k_mean"] - kinf_dense(P)) < 3 * r["k_sdev"]
+    g.close()
+
+
+def test_c3_full(gpu, orc):
+    """10^6 particles x (20 + 80) cycles on the GPU; oracle at 5*10^4 x (10 + 30)."""
+    P = inputs.config3()
+    g = gpu.Problem(P)
+    r = g.run()
+    invariants(r)
+    assert len(r["k_cycle"]) == 100
+    Po = inputs.config3(n_particles=50_000, n_inactive=10, n_active=30)
+    rc, ro = orc.Oracle(Po).run()
+    assert abs(r["k_mean"] - ro["k_mean"]) < 3 * math.hypot(r["k_sdev"], ro["k_sdev"])
+    comb = np.hypot(r["flux_sdev"], ro["flux_sdev"])
+    assert (np.abs(r["flux_mean"] - ro["flux_mean"]) < 4.5 * comb + 1e-12).all()
+    # sum over cycles of source weight = N per cycle: flux per source particle is O(1/Sigma_a)
+    assert 1.0 < r["flux_mean"].sum() < 100.0
+    g.close()
+
+
+@pytest.mark.parametrize("first", [0, 250_000])
+def test_c4_full_sampled_traces(gpu, orc, first):
+    """C4 at 10^7 particles per cycle (bench configuration): the event sequences of 150 sampled histories of
+    cycle 0 equal the oracle's, which can follow them one by one (cycle-0 histories depend on (seed, id) only)."""
+    P = inputs.config4()
+    g = gpu.Problem(P)
+    g.set_trace(first, 150, 2048)
+    k0 = g.run_cycle(10_000_000, 0, 1, 1)
+    tg = g.trace()
+    r = g.results()
+    invariants(r, 10_000_000)
+    o = orc.Oracle(P)
+    o.set_trace(first, 150, 1_000_000)
+    o.run(n_particles=first + 150, n_inactive=0, n_active=1)
+    compare_traces(tg, o.trace())
+    assert 1.0 < k0 < 2.0
+    g.close()
+
+
+def test_c4_full_k_and_flux(gpu, orc):
+    """10^7 x (3 + 6) cycles on the GPU against the oracle at 10^5 x (3 + 6): k within 3 combined sigma, total
+    flux per source particle within 4 sigma, leakage tiny and consistent."""
+    P = inputs.config4(n_inactive=3, n_active=6)
+    g = gpu.Problem(P)
+    r = g.run()
+    invariants(r)
+    Po = inputs.config4(n_particles=100_000, n_inactive=3, n_active=6)  # same cycles: the source is still converging
+    rc, ro = orc.Oracle(Po).run()
+    assert abs(r["k_mean"] - ro["k_mean"]) < 3 * math.hypot(r["k_sdev"], ro["k_sdev"]) + 2e-3
+    fg, fo = r["flux_mean"].reshape(-1, 7), ro["flux_mean"].reshape(-1, 7)
+    tg, to = fg.sum(), fo.sum()
+    assert abs(tg - to) / to < 0.01
+    # per-group spectrum summed over space
+    assert np.allclose(fg.sum(0) / tg, fo.sum(0) / to, atol=3e-3)
+    assert r["leak_mean"] < 1e-2
+    g.close()
+
+
+def test_c5_full(gpu, orc):
+    """10^6 source particles: sampled source histories identical to the oracle's; flux per time bin within 4 sigma of
+    the oracle at 2*10^4 (sigma from 8 independent GPU seeds at that size)."""
+    P = inputs.config5()
+    g = gpu.Problem(P, search=1)
+    g.set_trace(0, 60, 8192)
+    r = g.run()
+    invariants(r)
+    tg = g.trace()
+    o = orc.Oracle(P)
+    o.set_trace(0, 60, 2_000_000)
+    o.run(n_particles=60)
+    compare_traces(tg, o.trace())
+    g.close()
+    n = 20_000
+    Ps = inputs.config5(n_particles=n)
+    gs = gpu.Problem(Ps, search=1)
+    per_t = []
+    for seed in range(2, 10):
+        rs = gs.run(seed=seed)
+        per_t.append(rs["flux_mean"].reshape(10, 100).sum(1))
+    gs.close()
+    sig = np.std(per_t, axis=0, ddof=1)
+    rc, ro = orc.Oracle(Ps).run()
+    ft_o = ro["flux_mean"].reshape(10, 100).sum(1)
+    ft_g = r["flux_mean"].reshape(10, 100).sum(1)
+    assert (np.abs(ft_g - ft_o) < 4 * sig * math.sqrt(1 + n / 1e6) + 1e-12).all()
+    # tracks per source history (prompt chain k) agree statistically
+    kg = r["counters"][11] / r["counters"][0]
+    ko = ro["counters"][11] / ro["counters"][0]
+    assert abs(kg - ko) < 0.02
