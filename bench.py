@@ -91,6 +91,22 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """Timing rule: the job's time is the slowest rank's (torch.distributed all-reduce MAX; identity at world 1)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(units_per_rank: float, world: int, seconds_max: float) -> float:
+    """Replicas only: every rank processes units_per_rank; whole-job throughput."""
+    return world * units_per_rank / seconds_max
+
+
 def workload(args):
     from paper_2501_05440_b200 import inputs
     N = args.particles
@@ -170,17 +186,14 @@ def run_ours(args):
     barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     res = g.results()
     c1 = res["counters"]
     ms1, nl1 = g.timing()
     events = events_of(c1) - events_of(c0)
     tracks = int(c1[0] - c0[0])
-    value = world * K * N / (ms * 1e-3)
-    ev_per_s = world * events / (ms * 1e-3)
+    value = job_value(K * N, world, ms * 1e-3)
+    ev_per_s = job_value(events, world, ms * 1e-3)
 
     # ---- per-kernel timing of the same cycles' successors (event pairs around each launch; separate pass)
     g.set_profile(True)
@@ -233,11 +246,8 @@ def run_ours(args):
         sites_a, sites_b = sites_b, sites_a
     barrier()
     dt = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([dt], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = float(t.item())
-    e2e = {"value": world * K * N / dt, "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
+    dt = max_over_ranks(dt, world, "cuda")
+    e2e = {"value": job_value(K * N, world, dt), "unit": UNIT, "h2d_bytes_per_step": h2d // K, "d2h_bytes_per_step": d2h // K,
            "api": "mcdc_run_cycle_host"}
 
     out = {
