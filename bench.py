@@ -223,7 +223,7 @@ def run_ours(args):
         tr = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tr):
             try:
-                roof["traffic"] = json.load(open(tr)).get("k_advance_bytes_per_launch")
+                roof["traffic"] = json.load(open(tr))["k_advance_bytes_per_event"] * ev_prof / adv["launches"]
             except Exception:
                 pass
 

@@ -249,7 +249,7 @@ __device__ __forceinline__ void make_child(const Ctx &c, Rng &rng, int mat, unsi
 
 // ------------------------------------------------------------------ per-event kernels
 #ifndef MCDC_ADV_MINBLOCKS
-#define MCDC_ADV_MINBLOCKS 3
+#define MCDC_ADV_MINBLOCKS 4  // measured on B200: 2 -> 30.2, 3 -> 25.2, 4 -> 22.5, 5 -> 24.1 ms of k_advance per C4 cycle
 #endif
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsigned int s, unsigned int n0)
@@ -394,8 +394,11 @@ __device__ __forceinline__ int segment(const Ctx &c, Particle &p, Rng &rng, Acc 
 // ballot / prefix-sum compaction of the survivors into the next bank (front region; continuous-energy fission
 // children go, alive, to the back region).  One launch replaces 3 * max_seg launches of the per-event kernels
 // when a sweep is launch-latency bound; divergence is irrelevant at these sizes.
+#ifndef MCDC_MULTI_MINBLOCKS
+#define MCDC_MULTI_MINBLOCKS 3  // measured: 2 -> 11.4, 3 -> 9.7, 4 -> 9.6 ms of fused sweeps per C4 cycle
+#endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
+__global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
 {
     extern __shared__ double s_flux[];
     unsigned int n_front = n0, n_in = n0;
