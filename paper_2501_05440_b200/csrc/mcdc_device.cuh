@@ -460,38 +460,16 @@ struct Particle {
     unsigned long long id;
 };
 
-// per-thread accumulators reduced once per kernel.  Event counts by code 1..10 are packed as 16-bit fields of
-// three 64-bit registers (a dynamically indexed array would live in local memory); a thread that nears
-// 65535 events spills its fields to the global counters.
+// Per-thread accumulator (k numerator) reduced once per kernel; event counts by code go to a block-shared
+// counter array (integer shared-memory atomics) and leakage straight to the global scalar: both are kept out
+// of the registers, which is what limits the occupancy of the latency-bound transport kernels.
 struct Acc {
-    double knum, leak;
-    unsigned long long pk0, pk1, pk2;
-    unsigned int since;
-    __device__ __forceinline__ void clear() { knum = leak = 0.0; pk0 = pk1 = pk2 = 0ull; since = 0u; }
-    __device__ __forceinline__ unsigned int field(int e) const
-    {
-        unsigned long long w = (e >> 2) == 0 ? pk0 : ((e >> 2) == 1 ? pk1 : pk2);
-        return (unsigned int)(w >> ((e & 3) * 16)) & 0xffffu;
-    }
+    double knum;
+    unsigned int *s_ev;  // [16] in shared memory
+    __device__ __forceinline__ void clear(unsigned int *ev) { knum = 0.0; s_ev = ev; }
 };
 
-__device__ __forceinline__ void count_event(unsigned long long *counters, Acc &acc, int ev)
-{
-    unsigned long long inc = 1ull << ((ev & 3) * 16);
-    int w = ev >> 2;
-    acc.pk0 += w == 0 ? inc : 0ull;
-    acc.pk1 += w == 1 ? inc : 0ull;
-    acc.pk2 += w == 2 ? inc : 0ull;
-    if (++acc.since >= 65000u) {
-#pragma unroll
-        for (int e = 1; e < 11; e++) {
-            unsigned int n = acc.field(e);
-            if (n) atomicAdd(counters + e, (unsigned long long)n);
-        }
-        acc.pk0 = acc.pk1 = acc.pk2 = 0ull;
-        acc.since = 0u;
-    }
-}
+__device__ __forceinline__ void count_event(Acc &acc, int ev) { atomicAdd(acc.s_ev + ev, 1u); }
 
 enum { ADV_DEAD = 0, ADV_SCATTER = 1, ADV_SURFACE = 2, ADV_FISSION = 3 };
 constexpr int HIT_TIME_EDGE = 0x3fff0000;  // aux code of a time-edge event in the surface queue
@@ -652,7 +630,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         if (hit >= G.n_surf) { ev = 7; code = ADV_SURFACE; aux = hit; }
         else {
             int bc = __ldg(G.surf_bc + hit);
-            if (bc == 2) { ev = 6; code = ADV_DEAD; acc.leak += c.w0; }
+            if (bc == 2) { ev = 6; code = ADV_DEAD; atomicAdd(c.scal + 1, c.w0); }
             else { ev = bc == 1 ? 5 : 4; code = ADV_SURFACE; aux = hit; }
         }
         trace_event(c, p, ev, cell0, elem0, hit, gi, d, E_flight);
@@ -664,7 +642,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         else { ev = 8; code = ADV_SURFACE; aux = HIT_TIME_EDGE; }
         trace_event(c, p, ev, cell0, elem0, -1, gi, d, E_flight);
     }
-    count_event(c.counters, acc, ev);
+    count_event(acc, ev);
     return code;
 }
 

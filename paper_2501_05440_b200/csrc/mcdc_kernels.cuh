@@ -71,32 +71,30 @@ __device__ __forceinline__ unsigned int live_pos(unsigned int cap, unsigned int 
     return t < n_front ? t : cap - 1u - (t - n_front);
 }
 
-// per-block flush of the thread accumulators: k numerator, leakage, event counters
+// per-block flush: k numerator (warp shuffles + one atomic per block) and the shared event counters
 __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
 {
-    __shared__ double s_k[BS / 32], s_l[BS / 32];
-    __shared__ unsigned int s_ev[11];
+    __shared__ double s_k[BS / 32];
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (threadIdx.x < 11) s_ev[threadIdx.x] = 0;
-    double k = warp_sum(acc.knum), l = warp_sum(acc.leak);
-    if (lane == 0) { s_k[w] = k; s_l[w] = l; }
-    __syncthreads();
-#pragma unroll
-    for (int e = 1; e < 11; e++) {
-        unsigned int n = acc.field(e);
-        n = __reduce_add_sync(0xffffffffu, n);
-        if (lane == 0 && n) atomicAdd(&s_ev[e], n);
-    }
+    double k = warp_sum(acc.knum);
+    if (lane == 0) s_k[w] = k;
     __syncthreads();
     if (threadIdx.x == 0) {
-        double ks = 0.0, ls = 0.0;
-        for (int i = 0; i < BS / 32; i++) { ks += s_k[i]; ls += s_l[i]; }
+        double ks = 0.0;
+        for (int i = 0; i < BS / 32; i++) ks += s_k[i];
         if (ks != 0.0) atomicAdd(c.scal + 0, ks);
-        if (ls != 0.0) atomicAdd(c.scal + 1, ls);
     }
-    if (threadIdx.x >= 1 && threadIdx.x < 11 && s_ev[threadIdx.x])
-        atomicAdd(c.counters + threadIdx.x, (unsigned long long)s_ev[threadIdx.x]);
+    if (threadIdx.x >= 1 && threadIdx.x < 11 && acc.s_ev[threadIdx.x])
+        atomicAdd(c.counters + threadIdx.x, (unsigned long long)acc.s_ev[threadIdx.x]);
 }
+
+// block-shared event counters: declare + clear (call at kernel start, before any event is counted)
+#define MCDC_EVENT_COUNTERS(acc)                         \
+    __shared__ unsigned int s_evc[16];                   \
+    if (threadIdx.x < 16) s_evc[threadIdx.x] = 0u;       \
+    __syncthreads();                                     \
+    Acc acc;                                             \
+    acc.clear(s_evc)
 
 // shared-memory tally columns (one per thread) -> one float64 atomic per bin and block
 __device__ __forceinline__ void flush_private_flux(const Ctx &c, const double *s_flux)
@@ -265,8 +263,7 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
     }
-    Acc acc;
-    acc.clear();
+    MCDC_EVENT_COUNTERS(acc);
     const Bank &B = c.bank[s & 1];
     const Bank &O = c.bank[(s + 1) & 1];
     int par = 0;
@@ -416,8 +413,7 @@ __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsig
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
     }
-    Acc acc;
-    acc.clear();
+    MCDC_EVENT_COUNTERS(acc);
     const Bank &B = c.bank[s & 1];
     const Bank &O = c.bank[(s + 1) & 1];
     int par = 0;
@@ -469,8 +465,7 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         QCount z = {0u, 0u, 0u, 0u};
         c.qc[(s + 1) % RING] = z;
     }
-    Acc acc;
-    acc.clear();
+    MCDC_EVENT_COUNTERS(acc);
     const Bank &B = c.bank[0];
     unsigned int alive = 0;
     for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
@@ -506,8 +501,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
         QCount pc = c.qc[(s - 1) % RING];
         n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
     }
-    Acc acc;
-    acc.clear();
+    MCDC_EVENT_COUNTERS(acc);
     const Bank &B = c.bank[s & 1];
     unsigned int done = 0, born = 0, pops = 0;
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < n_in; t += gridDim.x * BS) {
