@@ -25,8 +25,11 @@ struct Geo {
 };                                  // from inside this element (create() proves when they cannot)
 constexpr int LAT_ROOT_FLAG = 1 << 30;
 
+// All multi-group tables are one contiguous blob (blob, blob_doubles); the transport kernels copy it to shared
+// memory at start-up and run on rebased pointers (stage_mg) when it fits.
 struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi running chi sums
-    int G, n_mat;
+    int G, n_mat, blob_doubles;
+    const double *blob;
     const double *sig_t, *sig_s, *sig_f, *nu, *nusf, *cumS, *cumchi, *src_cum;
 };
 
@@ -95,6 +98,7 @@ struct Ctx {
     unsigned int cap;   // slots per bank
     int mode;           // 0 MG, 1 CE
     int n_tally, n_bins;
+    int mg_stage;        // doubles of the multi-group table blob staged in shared memory by every transport kernel (0: none)
     int flux_aggregate;  // global tally flavour: 1 = warp-aggregate equal bins before the atomic
     int flux_copy_mask;  // R - 1: the per-cycle tally is kept in R copies, copy = block index & mask
     double *flux;       // [R][n_tally] per-cycle track-length tally
@@ -187,7 +191,7 @@ __device__ __forceinline__ void iso_dir(double xi_mu, double xi_phi, double &ux,
 __device__ __forceinline__ int pick(const double *__restrict__ cum, int n, double v)
 {
     int i = 0;
-    while (i < n - 1 && !(__ldg(cum + i) > v)) i++;
+    while (i < n - 1 && !(cum[i] > v)) i++;
     return i;
 }
 
@@ -539,7 +543,8 @@ __device__ __forceinline__ void flux_add(const Ctx &c, double *s_flux, long long
 // reaction choice of a8): cross sections, distance to collision, nearest boundary, time edge, move, tallies.
 // Returns ADV_*; aux = elastic column (scatter), hit code (surface / time edge) or number of children (fission).
 template <bool CE, bool PRIVATE>
-__device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int &aux, Acc &acc, double *s_flux)
+__device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int &aux, Acc &acc,
+                                       double *s_flux)
 {
     const Geo &G = c.geo;
     const int cell0 = p.cell, elem0 = p.elem;
@@ -556,8 +561,8 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     int gi, ncol = 0;
     if (!CE) {
         gi = p.g;
-        sig_t = __ldg(c.mg.sig_t + mat * c.mg.G + p.g);
-        nusf = __ldg(c.mg.nusf + mat * c.mg.G + p.g);
+        sig_t = mg.sig_t[mat * mg.G + p.g];
+        nusf = mg.nusf[mat * mg.G + p.g];
     } else {
         gi = grid_index(c.ce, p.E);
         double g0 = __ldg(c.ce.grid + gi), g1 = __ldg(c.ce.grid + gi + 1);
@@ -596,7 +601,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
     const double E_flight = CE ? p.E : 0.0;
     long long tix;
-    if (!CE) tix = (long long)bin * c.mg.G + p.g;
+    if (!CE) tix = (long long)bin * mg.G + p.g;
     else {
         tix = ((long long)bin * c.ce.n_t + p.tbin) * c.ce.n_e + edge_bin(c.ce.e_edges, c.ce.n_e, p.E);
         if (kind == 2) p.t = __ldg(c.ce.t_edges + p.tbin + 1); else p.t += d / v;
@@ -609,11 +614,11 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         p.last = -1;
         double uu = rng.next() * sig_t;
         if (!CE) {
-            double sig_s = __ldg(c.mg.sig_s + mat * c.mg.G + p.g), sig_f = __ldg(c.mg.sig_f + mat * c.mg.G + p.g);
+            double sig_s = mg.sig_s[mat * mg.G + p.g], sig_f = mg.sig_f[mat * mg.G + p.g];
             if (uu < sig_s) { ev = 1; code = ADV_SCATTER; aux = 0; }
             else if (uu < sig_s + sig_f) {
                 ev = 2; code = ADV_FISSION;
-                aux = (int)floor(c.w0 * __ldg(c.mg.nu + mat * c.mg.G + p.g) / c.k_prev + rng.next());
+                aux = (int)floor(c.w0 * mg.nu[mat * mg.G + p.g] / c.k_prev + rng.next());
             } else { ev = 3; code = ADV_DEAD; }
         } else {
             int r = 0;
@@ -649,14 +654,14 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
 // Scatter event (a8).  MG: new group from the cumulative scatter row, isotropic direction (1 + 2 draws).
 // CE: elastic off a target at rest with mass ratio A: mu_cm, azimuth (2 draws), rotation, energy clamp (R19, R21).
 template <bool CE>
-__device__ __forceinline__ void do_scatter(const Ctx &c, Particle &p, Rng &rng, int col)
+__device__ __forceinline__ void do_scatter(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int col)
 {
     const int mat = __ldg(c.geo.cfill + p.cell);
     if (!CE) {
-        const int G = c.mg.G;
-        double sig_s = __ldg(c.mg.sig_s + mat * G + p.g);
+        const int G = mg.G;
+        double sig_s = mg.sig_s[mat * G + p.g];
         double vv = rng.next() * sig_s;
-        p.g = pick(c.mg.cumS + ((size_t)mat * G + p.g) * G, G, vv);
+        p.g = pick(mg.cumS + (mat * G + p.g) * G, G, vv);
         double a = rng.next(), b = rng.next();
         iso_dir(a, b, p.ux, p.uy, p.uz);
     } else {

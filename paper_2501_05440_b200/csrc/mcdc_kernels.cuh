@@ -28,6 +28,24 @@ __device__ __forceinline__ double warp_sum(double v)
 
 __device__ __forceinline__ int pack_gl(int g, int last) { return (g & 0xffff) | ((last + 1) << 16); }
 
+// ------------------------------------------------------------------ a2: multi-group tables in shared memory
+// Copies the table blob to shared memory (all threads of the block; ends with a barrier) and returns the table
+// descriptor rebased onto the copy; `smem` is where the copy goes, n_stage its size in doubles (0: not staged,
+// the tables are then read from global memory through L1).
+__device__ __forceinline__ MGTab stage_mg(const Ctx &c, double *smem, int n_stage)
+{
+    MGTab mg = c.mg;
+    if (n_stage > 0) {
+        for (int k = threadIdx.x; k < n_stage; k += blockDim.x) smem[k] = __ldg(c.mg.blob + k);
+        mg.sig_t = smem + (c.mg.sig_t - c.mg.blob); mg.sig_s = smem + (c.mg.sig_s - c.mg.blob);
+        mg.sig_f = smem + (c.mg.sig_f - c.mg.blob); mg.nu = smem + (c.mg.nu - c.mg.blob);
+        mg.nusf = smem + (c.mg.nusf - c.mg.blob); mg.cumS = smem + (c.mg.cumS - c.mg.blob);
+        mg.cumchi = smem + (c.mg.cumchi - c.mg.blob); mg.src_cum = smem + (c.mg.src_cum - c.mg.blob);
+        __syncthreads();
+    }
+    return mg;
+}
+
 // ------------------------------------------------------------------ bank access (dense, position-indexed)
 template <bool CE>
 __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr, uint32_t &slot)
@@ -252,7 +270,9 @@ __device__ __forceinline__ void make_child(const Ctx &c, Rng &rng, int mat, unsi
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsigned int s, unsigned int n0)
 {
-    extern __shared__ double s_flux[];
+    extern __shared__ double s_dyn[];
+    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
     unsigned int n_front = n0, n_in = n0;
     if (s > 0) {
         QCount pc = c.qc[(s - 1) % RING];
@@ -278,7 +298,7 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
             if (B.cell[i] >= 0) {
                 load_full<CE>(B, i, p, ctr, slot);
                 rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-                code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+                code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux);
                 if (!CE && code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
@@ -311,6 +331,8 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
 template <bool CE>
 __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
 {
+    extern __shared__ double s_dyn[];
+    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
     const QCount oc = c.qc[s % RING];
     const Bank &B = c.bank[(s + 1) & 1];
     // queue-counter housekeeping: clear the set the next sweep appends to
@@ -328,7 +350,7 @@ __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
         if (CE) { p.E = B.E[i]; p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i]; }
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, B.ctr[i]);
-        do_scatter<CE>(c, p, rng, B.ev[i]);
+        do_scatter<CE>(c, mg, p, rng, B.ev[i]);
         B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
         B.gl[i] = pack_gl(p.g, -1);
         B.ctr[i] = rng.ctr;
@@ -369,11 +391,12 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 // whole segment in registers (shared by the monolithic schedule and the tail kernel):
 // returns 1 = still alive, 0 = history ended, 2 = ended in a fission with n_children
 template <bool CE, bool PRIVATE>
-__device__ __forceinline__ int segment(const Ctx &c, Particle &p, Rng &rng, Acc &acc, double *s_flux, int &n_children)
+__device__ __forceinline__ int segment(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, Acc &acc, double *s_flux,
+                                       int &n_children)
 {
     int aux = 0;
-    int code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
-    if (code == ADV_SCATTER) { do_scatter<CE>(c, p, rng, aux); return 1; }
+    int code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux);
+    if (code == ADV_SCATTER) { do_scatter<CE>(c, mg, p, rng, aux); return 1; }
     if (code == ADV_SURFACE) {
         if (!do_surface(c, p, aux)) {
             atomicExch(c.err, -2);
@@ -397,7 +420,9 @@ __device__ __forceinline__ int segment(const Ctx &c, Particle &p, Rng &rng, Acc 
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
 {
-    extern __shared__ double s_flux[];
+    extern __shared__ double s_dyn[];
+    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
     unsigned int n_front = n0, n_in = n0;
     if (s > 0) {
         QCount pc = c.qc[(s - 1) % RING];
@@ -429,7 +454,7 @@ __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsig
                 load_full<CE>(B, i, p, ctr, slot);
                 rng.init(c.seed, p.id, 0u, c.cycle, ctr);
                 unsigned int k = 0;
-                do { st = segment<CE, PRIVATE>(c, p, rng, acc, s_flux, nch); } while (st == 1 && ++k < max_seg);
+                do { st = segment<CE, PRIVATE>(c, mg, p, rng, acc, s_flux, nch); } while (st == 1 && ++k < max_seg);
                 if (!CE && st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
             }
         }
@@ -456,7 +481,9 @@ __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsig
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned int n)
 {
-    extern __shared__ double s_flux[];
+    extern __shared__ double s_dyn[];
+    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
     if (PRIVATE) {
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
@@ -476,7 +503,7 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, ctr);
         int nch = 0;
-        int st = segment<CE, PRIVATE>(c, p, rng, acc, s_flux, nch);
+        int st = segment<CE, PRIVATE>(c, mg, p, rng, acc, s_flux, nch);
         if (st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
         store_full<CE>(B, i, p, rng.ctr, slot, st == 1 ? 0 : EV_DEAD);
         if (st == 1) alive++;
@@ -491,7 +518,9 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned int n0)
 {
-    extern __shared__ double s_flux[];
+    extern __shared__ double s_dyn[];
+    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
     if (PRIVATE) {
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
@@ -516,7 +545,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
         StackRec *stk = CE ? c.stack + (size_t)(blockIdx.x * BS + threadIdx.x) * STACK_DEPTH : nullptr;
         for (;;) {
             int nch = 0, st;
-            while ((st = segment<CE, PRIVATE>(c, p, rng, acc, s_flux, nch)) == 1) {
+            while ((st = segment<CE, PRIVATE>(c, mg, p, rng, acc, s_flux, nch)) == 1) {
                 if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
             }
             done++;

@@ -41,6 +41,7 @@ static const uint64_t TRACE_BYTES = 48ull << 20;
 #define MCDC_AGG_MAX 4096
 #endif
 static const int AGGREGATE_TALLY_MAX = MCDC_AGG_MAX;  // above this, equal bins inside a warp are rare: plain float64 atomics
+static const uint64_t MG_STAGE_MAX_BYTES = 16384;  // multi-group tables up to this size are staged in shared memory
 static const int PRIVATE_TALLY_MAX = 20;  // bins for which the one-column-per-thread tally fits (20*256*8 = 40 KB)
 
 struct HostPinned {
@@ -140,6 +141,7 @@ struct Layout {  // everything carved from the workspace, in order
     double *sig_t, *sig_s, *sig_f, *nu, *nusf, *cumS, *cumchi, *src_cum;
     double *grid, *tab, *colA, *t_edges, *e_edges;
     int *ncol, *hash;
+    uint64_t mg_doubles;
     Bank bank[2];
     FisRec fis;
     StackRec *stack;
@@ -197,9 +199,11 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     bool ce = x != nullptr;
     if (!ce) {
         uint64_t mg = (uint64_t)m->n_mat * m->G;
-        L.sig_t = C.take<double>(mg); L.sig_s = C.take<double>(mg); L.sig_f = C.take<double>(mg);
-        L.nu = C.take<double>(mg); L.nusf = C.take<double>(mg); L.cumS = C.take<double>(mg * m->G);
-        L.cumchi = C.take<double>(mg); L.src_cum = C.take<double>(m->G);
+        // one contiguous blob (staged in shared memory by the kernels): six [n_mat][G] tables, cumS, src_cum
+        L.mg_doubles = 6 * mg + mg * m->G + m->G;
+        L.sig_t = C.take<double>(L.mg_doubles);
+        L.sig_s = L.sig_t + mg; L.sig_f = L.sig_s + mg; L.nu = L.sig_f + mg; L.nusf = L.nu + mg; L.cumchi = L.nusf + mg;
+        L.cumS = L.cumchi + mg; L.src_cum = L.cumS + mg * m->G;
         L.grid = L.tab = L.colA = L.t_edges = L.e_edges = nullptr; L.ncol = L.hash = nullptr;
     } else {
         int sh, lo, nh;
@@ -211,6 +215,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         L.hash = C.take<int>(nh + 2);
         L.t_edges = C.take<double>(t->n_t + 1); L.e_edges = C.take<double>(t->n_e + 1);
         L.sig_t = L.sig_s = L.sig_f = L.nu = L.nusf = L.cumS = L.cumchi = L.src_cum = nullptr;
+        L.mg_doubles = 0;
     }
     for (int b = 0; b < 2; b++) {
         Bank &B = L.bank[b];
@@ -440,7 +445,8 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
         UP(L.sig_s, h_sig_s.data(), nm * Gn); UP(L.nusf, h_nusf.data(), nm * Gn);
         UP(L.cumS, h_cumS.data(), (size_t)nm * Gn * Gn); UP(L.cumchi, h_cumchi.data(), nm * Gn);
         UP(L.src_cum, h_srccum.data(), Gn);
-        c.mg.G = Gn; c.mg.n_mat = nm;
+        c.mg.G = Gn; c.mg.n_mat = nm; c.mg.blob = L.sig_t; c.mg.blob_doubles = (int)L.mg_doubles;
+        c.mg_stage = L.mg_doubles * 8 <= MG_STAGE_MAX_BYTES ? (int)L.mg_doubles : 0;
         c.mg.sig_t = L.sig_t; c.mg.sig_s = L.sig_s; c.mg.sig_f = L.sig_f; c.mg.nu = L.nu; c.mg.nusf = L.nusf;
         c.mg.cumS = L.cumS; c.mg.cumchi = L.cumchi; c.mg.src_cum = L.src_cum;
         c.n_tally = t->n_bins * Gn;
@@ -508,6 +514,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     p->part = L.part; p->sites = L.sites;
     p->trace_base = L.trace; p->trace_count = L.trace_count;
     p->tally_private = c.n_tally <= PRIVATE_TALLY_MAX;
+    if (p->tally_private && (size_t)c.mg_stage * 8 + (size_t)c.n_tally * BS * 8 > 48 * 1024) c.mg_stage = 0;  // 48 KB default limit
     c.flux_aggregate = c.n_tally <= AGGREGATE_TALLY_MAX ? 1 : 0;
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc, 0, sizeof(double) * c.n_tally, st);
@@ -584,7 +591,8 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
-    const size_t smem = PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0;
+    const size_t smem_mg = CE ? 0 : (size_t)c.mg_stage * sizeof(double);
+    const size_t smem = smem_mg + (PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0);
     CUDA_OK(cudaMemsetAsync(c.qc, 0, sizeof(QCount) * RING, st));
     CUDA_OK(cudaMemsetAsync(c.n_over, 0, sizeof(unsigned int), st));
     uint64_t upper = M;
@@ -606,7 +614,7 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
             p->n_launches++;
         } else if (p->schedule == 0) {
             { ProfScope ps(p, MCDC_PROF_ADVANCE); k_advance<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
-            { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, 0, st>>>(c, s); }
+            { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, smem_mg, st>>>(c, s); }
             { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, 0, st>>>(c, s); }
             p->n_launches += 3;
         } else {
