@@ -21,6 +21,8 @@ struct Geo {
     const int *surf_type, *surf_bc;
     const double *surf_param;  // [n_surf][4]
     const int *cso, *csi, *css, *cft, *cfill, *cbin, *uco;
+    const char *blob;  // surfaces, cells and universes are one contiguous blob (staged in shared memory)
+    int blob_words;    // its size in 4-byte words
     const int *lat_univ, *lat_bin;  // lat_bin bit 30: the enclosing cell's surfaces can be the nearest boundary
 };                                  // from inside this element (create() proves when they cannot)
 constexpr int LAT_ROOT_FLAG = 1 << 30;
@@ -98,6 +100,7 @@ struct Ctx {
     unsigned int cap;   // slots per bank
     int mode;           // 0 MG, 1 CE
     int n_tally, n_bins;
+    int geo_stage;       // 4-byte words of the geometry blob staged in shared memory (0: none)
     int mg_stage;        // doubles of the multi-group table blob staged in shared memory by every transport kernel (0: none)
     int flux_aggregate;  // global tally flavour: 1 = warp-aggregate equal bins before the atomic
     int flux_copy_mask;  // R - 1: the per-cycle tally is kept in R copies, copy = block index & mask
@@ -251,8 +254,8 @@ __device__ __forceinline__ int grid_index(const CETab &ce, double E)
 __device__ __forceinline__ double surf_f(const Geo &G, int s, double x, double y, double z)
 {
     const double *q = G.surf_param + 4 * s;
-    int t = __ldg(G.surf_type + s);
-    double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2), q3 = __ldg(q + 3);
+    int t = G.surf_type[s];
+    double q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3];
     switch (t) {
     case 0: return x - q0;
     case 1: return y - q0;
@@ -270,8 +273,8 @@ __device__ __forceinline__ void surf_normal(const Geo &G, int s, double x, doubl
                                             double &nz)
 {
     const double *q = G.surf_param + 4 * s;
-    int t = __ldg(G.surf_type + s);
-    double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2);
+    int t = G.surf_type[s];
+    double q0 = q[0], q1 = q[1], q2 = q[2];
     nx = ny = nz = 0.0;
     switch (t) {
     case 0: nx = 1.0; break;
@@ -301,12 +304,12 @@ __device__ __forceinline__ int sense_of(const Geo &G, int s, double x, double y,
 __device__ __forceinline__ int find_cell(const Geo &G, int univ, double x, double y, double z, double ux, double uy,
                                          double uz, int last)
 {
-    int c1 = __ldg(G.uco + univ + 1);
-    for (int c = __ldg(G.uco + univ); c < c1; c++) {
+    int c1 = G.uco[univ + 1];
+    for (int c = G.uco[univ]; c < c1; c++) {
         bool ok = true;
-        int k1 = __ldg(G.cso + c + 1);
-        for (int k = __ldg(G.cso + c); k < k1; k++)
-            if (sense_of(G, __ldg(G.csi + k), x, y, z, ux, uy, uz, last) != __ldg(G.css + k)) { ok = false; break; }
+        int k1 = G.cso[c + 1];
+        for (int k = G.cso[c]; k < k1; k++)
+            if (sense_of(G, G.csi[k], x, y, z, ux, uy, uz, last) != G.css[k]) { ok = false; break; }
         if (ok) return c;
     }
     return -1;
@@ -336,7 +339,7 @@ __device__ __forceinline__ bool locate(const Geo &G, double x, double y, double 
     elem = -1;
     cell = find_cell(G, 0, x, y, z, ux, uy, uz, last);
     if (cell < 0) return false;
-    if (__ldg(G.cft + cell) == 1) {
+    if (G.cft[cell] == 1) {
         int ix = (int)floor((x - G.lat_x0) / G.lat_px);
         int iy = (int)floor((y - G.lat_y0) / G.lat_py);
         if (ix < 0 || iy < 0 || ix >= G.lat_nx || iy >= G.lat_ny) { cell = -1; return false; }
@@ -356,8 +359,8 @@ __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, d
 {
     const double INF = __longlong_as_double(0x7ff0000000000000LL);
     const double *q = G.surf_param + 4 * s;
-    int t = __ldg(G.surf_type + s);
-    double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2), q3 = __ldg(q + 3);
+    int t = G.surf_type[s];
+    double q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3];
     if (t <= 3) {
         if (on) return INF;
         double d;
@@ -410,10 +413,10 @@ __device__ __forceinline__ double nearest(const Geo &G, double x, double y, doub
     hit = -1;
     const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;  // +-inf when the component is zero: guarded at use
     int c0 = elem >= 0 ? G.lat_cell : cell;
-    int k1 = __ldg(G.cso + c0 + 1);
+    int k1 = G.cso[c0 + 1];
     if (root_needed)
-        for (int k = __ldg(G.cso + c0); k < k1; k++) {
-            int s = __ldg(G.csi + k);
+        for (int k = G.cso[c0]; k < k1; k++) {
+            int s = G.csi[k];
             double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
@@ -422,9 +425,9 @@ __device__ __forceinline__ double nearest(const Geo &G, double x, double y, doub
         elem_xy(G, elem, ix, iy);
         const double xl = x - (G.lat_x0 + (ix + 0.5) * G.lat_px);
         const double yl = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
-        k1 = __ldg(G.cso + cell + 1);
-        for (int k = __ldg(G.cso + cell); k < k1; k++) {
-            int s = __ldg(G.csi + k);
+        k1 = G.cso[cell + 1];
+        for (int k = G.cso[cell]; k < k1; k++) {
+            int s = G.csi[k];
             double d = surf_distance(G, s, xl, yl, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
@@ -451,9 +454,9 @@ __device__ __forceinline__ double nearest(const Geo &G, double x, double y, doub
 
 __device__ __forceinline__ bool surface_in_cell(const Geo &G, int c, int s)
 {
-    int k1 = __ldg(G.cso + c + 1);
-    for (int k = __ldg(G.cso + c); k < k1; k++)
-        if (__ldg(G.csi + k) == s) return true;
+    int k1 = G.cso[c + 1];
+    for (int k = G.cso[c]; k < k1; k++)
+        if (G.csi[k] == s) return true;
     return false;
 }
 
@@ -544,12 +547,11 @@ __device__ __forceinline__ void flux_add(const Ctx &c, double *s_flux, long long
 // Returns ADV_*; aux = elastic column (scatter), hit code (surface / time edge) or number of children (fission).
 template <bool CE, bool PRIVATE>
 __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int &aux, Acc &acc,
-                                       double *s_flux)
+                                       double *s_flux, const Geo &G)
 {
-    const Geo &G = c.geo;
     const int cell0 = p.cell, elem0 = p.elem;
-    const int mat = __ldg(G.cfill + p.cell);
-    int bin = __ldg(G.cbin + p.cell);
+    const int mat = G.cfill[p.cell];
+    int bin = G.cbin[p.cell];
     bool root_needed = true;
     if (p.elem >= 0) {
         int lb = __ldg(G.lat_bin + p.elem);
@@ -634,7 +636,7 @@ __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &
     } else if (kind == 1) {
         if (hit >= G.n_surf) { ev = 7; code = ADV_SURFACE; aux = hit; }
         else {
-            int bc = __ldg(G.surf_bc + hit);
+            int bc = G.surf_bc[hit];
             if (bc == 2) { ev = 6; code = ADV_DEAD; atomicAdd(c.scal + 1, c.w0); }
             else { ev = bc == 1 ? 5 : 4; code = ADV_SURFACE; aux = hit; }
         }
@@ -654,9 +656,9 @@ __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &
 // Scatter event (a8).  MG: new group from the cumulative scatter row, isotropic direction (1 + 2 draws).
 // CE: elastic off a target at rest with mass ratio A: mu_cm, azimuth (2 draws), rotation, energy clamp (R19, R21).
 template <bool CE>
-__device__ __forceinline__ void do_scatter(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int col)
+__device__ __forceinline__ void do_scatter(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int col, const Geo &G)
 {
-    const int mat = __ldg(c.geo.cfill + p.cell);
+    const int mat = G.cfill[p.cell];
     if (!CE) {
         const int G = mg.G;
         double sig_s = mg.sig_s[mat * G + p.g];
@@ -696,9 +698,8 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const MGTab &mg, Partic
 
 // Surface event (a9): lattice wall -> neighbour element; reflect; transmit -> neighbour cell by the side being
 // entered (R11, R14).  Time-edge events need no geometry work.  Returns false if the particle got lost.
-__device__ __forceinline__ bool do_surface(const Ctx &c, Particle &p, int hit)
+__device__ __forceinline__ bool do_surface(const Geo &G, Particle &p, int hit)
 {
-    const Geo &G = c.geo;
     if (hit == HIT_TIME_EDGE) return true;
     if (hit >= G.n_surf) {
         int w = hit - G.n_surf;
@@ -712,13 +713,13 @@ __device__ __forceinline__ bool do_surface(const Ctx &c, Particle &p, int hit)
         p.cell = find_cell(G, __ldg(G.lat_univ + p.elem), xl, yl, p.z, p.ux, p.uy, p.uz, -1);
         return p.cell >= 0;
     }
-    int bc = __ldg(G.surf_bc + hit);
+    int bc = G.surf_bc[hit];
     bool local = p.elem >= 0 && !surface_in_cell(G, G.lat_cell, hit);
     double xl = p.x, yl = p.y;
     if (local) local_xy(G, p.elem, p.x, p.y, xl, yl);
     p.last = hit;
     if (bc == 1) {
-        int t = __ldg(G.surf_type + hit);
+        int t = G.surf_type[hit];
         if (t == 0) p.ux = -p.ux;
         else if (t == 1) p.uy = -p.uy;
         else if (t == 2) p.uz = -p.uz;

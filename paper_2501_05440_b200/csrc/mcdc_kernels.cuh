@@ -46,6 +46,29 @@ __device__ __forceinline__ MGTab stage_mg(const Ctx &c, double *smem, int n_stag
     return mg;
 }
 
+// a4/a5: the CSG tables (surfaces, cell -> surface lists, fills, bins, universes) in shared memory, same scheme;
+// `smem` must be 8-byte aligned; the lattice maps stay in global memory (L1/L2)
+__device__ __forceinline__ Geo stage_geo(const Ctx &c, void *smem, int n_words)
+{
+    Geo G = c.geo;
+    if (n_words > 0) {
+        int *dst = (int *)smem;
+        const int *src = (const int *)c.geo.blob;
+        for (int k = threadIdx.x; k < n_words; k += blockDim.x) dst[k] = __ldg(src + k);
+        const char *b = c.geo.blob;
+        char *d = (char *)smem;
+        G.surf_param = (const double *)(d + ((const char *)c.geo.surf_param - b));
+        G.surf_type = (const int *)(d + ((const char *)c.geo.surf_type - b));
+        G.surf_bc = (const int *)(d + ((const char *)c.geo.surf_bc - b));
+        G.cso = (const int *)(d + ((const char *)c.geo.cso - b)); G.csi = (const int *)(d + ((const char *)c.geo.csi - b));
+        G.css = (const int *)(d + ((const char *)c.geo.css - b)); G.cft = (const int *)(d + ((const char *)c.geo.cft - b));
+        G.cfill = (const int *)(d + ((const char *)c.geo.cfill - b)); G.cbin = (const int *)(d + ((const char *)c.geo.cbin - b));
+        G.uco = (const int *)(d + ((const char *)c.geo.uco - b));
+        __syncthreads();
+    }
+    return G;
+}
+
 // ------------------------------------------------------------------ bank access (dense, position-indexed)
 template <bool CE>
 __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr, uint32_t &slot)
@@ -272,7 +295,8 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
+    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
     unsigned int n_front = n0, n_in = n0;
     if (s > 0) {
         QCount pc = c.qc[(s - 1) % RING];
@@ -298,7 +322,7 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
             if (B.cell[i] >= 0) {
                 load_full<CE>(B, i, p, ctr, slot);
                 rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-                code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux);
+                code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux, geo);
                 if (!CE && code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
@@ -313,7 +337,7 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
             else if (code == ADV_SURFACE) { if (ob < c.cap) store_full<CE>(O, c.cap - 1u - ob, p, rng.ctr, slot, aux); }
             else if (code == ADV_FISSION && nb) {
                 // prompt secondaries: born alive at the parent's site, first segment in the next sweep
-                const int mat = __ldg(c.geo.cfill + p.cell);
+                const int mat = c.geo.cfill[p.cell];
                 const unsigned long long pid = p.id;
                 const uint32_t ctr0 = rng.ctr;
                 for (unsigned int j = 0; j < nb; j++) {
@@ -350,7 +374,7 @@ __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
         if (CE) { p.E = B.E[i]; p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i]; }
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, B.ctr[i]);
-        do_scatter<CE>(c, mg, p, rng, B.ev[i]);
+        do_scatter<CE>(c, mg, p, rng, B.ev[i], c.geo);
         B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
         B.gl[i] = pack_gl(p.g, -1);
         B.ctr[i] = rng.ctr;
@@ -360,6 +384,8 @@ __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
 
 __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 {
+    extern __shared__ double s_dyn[];
+    const Geo geo = stage_geo(c, s_dyn, c.geo_stage);
     const QCount oc = c.qc[s % RING];
     const Bank &B = c.bank[(s + 1) & 1];
     for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_surf; t += gridDim.x * BS) {
@@ -374,7 +400,7 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
         p.g = gl & 0xffff; p.last = (gl >> 16) - 1;
         const int cell0 = p.cell, elem0 = p.elem;
         const double ux0 = p.ux, uy0 = p.uy, uz0 = p.uz;
-        if (!do_surface(c, p, hit)) {
+        if (!do_surface(geo, p, hit)) {
             atomicExch(c.err, -2);
             atomicAdd(c.counters + 10, 1ull);
             p.cell = -1;
@@ -391,14 +417,14 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 // whole segment in registers (shared by the monolithic schedule and the tail kernel):
 // returns 1 = still alive, 0 = history ended, 2 = ended in a fission with n_children
 template <bool CE, bool PRIVATE>
-__device__ __forceinline__ int segment(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, Acc &acc, double *s_flux,
-                                       int &n_children)
+__device__ __forceinline__ int segment(const Ctx &c, const MGTab &mg, const Geo &G, Particle &p, Rng &rng, Acc &acc,
+                                       double *s_flux, int &n_children)
 {
     int aux = 0;
-    int code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux);
-    if (code == ADV_SCATTER) { do_scatter<CE>(c, mg, p, rng, aux); return 1; }
+    int code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux, G);
+    if (code == ADV_SCATTER) { do_scatter<CE>(c, mg, p, rng, aux, G); return 1; }
     if (code == ADV_SURFACE) {
-        if (!do_surface(c, p, aux)) {
+        if (!do_surface(G, p, aux)) {
             atomicExch(c.err, -2);
             atomicAdd(c.counters + 10, 1ull);
             p.cell = -1;
@@ -422,7 +448,8 @@ __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsig
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
+    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
     unsigned int n_front = n0, n_in = n0;
     if (s > 0) {
         QCount pc = c.qc[(s - 1) % RING];
@@ -454,7 +481,7 @@ __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsig
                 load_full<CE>(B, i, p, ctr, slot);
                 rng.init(c.seed, p.id, 0u, c.cycle, ctr);
                 unsigned int k = 0;
-                do { st = segment<CE, PRIVATE>(c, mg, p, rng, acc, s_flux, nch); } while (st == 1 && ++k < max_seg);
+                do { st = segment<CE, PRIVATE>(c, mg, geo, p, rng, acc, s_flux, nch); } while (st == 1 && ++k < max_seg);
                 if (!CE && st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
             }
         }
@@ -463,7 +490,7 @@ __global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsig
         block_slot_n(st == 1, nb, oc, c.cap, par, pf, ob);
         if (st == 1) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot, 0); }
         else if (nb) {
-            const int mat = __ldg(c.geo.cfill + p.cell);
+            const int mat = c.geo.cfill[p.cell];
             const unsigned long long pid = p.id;
             const uint32_t ctr0 = rng.ctr;
             for (unsigned int j = 0; j < nb; j++) {
@@ -483,7 +510,8 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
+    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
     if (PRIVATE) {
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
@@ -503,7 +531,7 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         Rng rng;
         rng.init(c.seed, p.id, 0u, c.cycle, ctr);
         int nch = 0;
-        int st = segment<CE, PRIVATE>(c, mg, p, rng, acc, s_flux, nch);
+        int st = segment<CE, PRIVATE>(c, mg, geo, p, rng, acc, s_flux, nch);
         if (st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
         store_full<CE>(B, i, p, rng.ctr, slot, st == 1 ? 0 : EV_DEAD);
         if (st == 1) alive++;
@@ -520,7 +548,8 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);
+    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
     if (PRIVATE) {
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();
@@ -545,7 +574,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
         StackRec *stk = CE ? c.stack + (size_t)(blockIdx.x * BS + threadIdx.x) * STACK_DEPTH : nullptr;
         for (;;) {
             int nch = 0, st;
-            while ((st = segment<CE, PRIVATE>(c, mg, p, rng, acc, s_flux, nch)) == 1) {
+            while ((st = segment<CE, PRIVATE>(c, mg, geo, p, rng, acc, s_flux, nch)) == 1) {
                 if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
             }
             done++;
@@ -553,7 +582,7 @@ __global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned i
                 if (!CE) record_fission<CE>(c, p, rng.ctr, slot, nch);
                 else if (nch > 0) {
                     if (depth + (unsigned int)nch <= STACK_DEPTH) {
-                        const int mat = __ldg(c.geo.cfill + p.cell);
+                        const int mat = c.geo.cfill[p.cell];
                         const unsigned long long pid = p.id;
                         const uint32_t ctr0 = rng.ctr;
                         Particle ch = p;
@@ -665,7 +694,7 @@ __global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int m, const unsign
     p.cell = F.cell[i]; p.elem = F.elem[i];
     p.last = -1; p.g = 0; p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = 0;
     if (CE) { p.t = F.t[i]; p.tbin = F.tbin[i]; }
-    const int mat = __ldg(c.geo.cfill + p.cell);
+    const int mat = c.geo.cfill[p.cell];
     unsigned long long pid = CE ? F.id[i] : (unsigned long long)i;
     uint32_t ctr0 = F.ctr[i];
     Rng rng;

@@ -41,6 +41,7 @@ static const uint64_t TRACE_BYTES = 48ull << 20;
 #define MCDC_AGG_MAX 4096
 #endif
 static const int AGGREGATE_TALLY_MAX = MCDC_AGG_MAX;  // above this, equal bins inside a warp are rare: plain float64 atomics
+static const uint64_t GEO_STAGE_MAX_BYTES = 8192;  // CSG tables up to this size are staged in shared memory
 static const uint64_t MG_STAGE_MAX_BYTES = 16384;  // multi-group tables up to this size are staged in shared memory
 static const int PRIVATE_TALLY_MAX = 20;  // bins for which the one-column-per-thread tally fits (20*256*8 = 40 KB)
 
@@ -141,7 +142,7 @@ struct Layout {  // everything carved from the workspace, in order
     double *sig_t, *sig_s, *sig_f, *nu, *nusf, *cumS, *cumchi, *src_cum;
     double *grid, *tab, *colA, *t_edges, *e_edges;
     int *ncol, *hash;
-    uint64_t mg_doubles;
+    uint64_t mg_doubles, geo_words;
     Bank bank[2];
     FisRec fis;
     StackRec *stack;
@@ -190,11 +191,19 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     Carver C(ws);
     int nref = g->cell_surf_off[g->n_cell];
     int nlat = g->has_lattice ? g->lat_nx * g->lat_ny : 0;
-    L.surf_type = C.take<int>(g->n_surf); L.surf_bc = C.take<int>(g->n_surf);
-    L.surf_param = C.take<double>(4 * (uint64_t)g->n_surf);
-    L.cso = C.take<int>(g->n_cell + 1); L.csi = C.take<int>(nref); L.css = C.take<int>(nref);
-    L.cft = C.take<int>(g->n_cell); L.cfill = C.take<int>(g->n_cell); L.cbin = C.take<int>(g->n_cell);
-    L.uco = C.take<int>(g->n_univ + 1);
+    // one contiguous blob (staged in shared memory by the kernels): surface parameters first (8-byte aligned),
+    // then the int tables
+    {
+        uint64_t ns = g->n_surf, nc = g->n_cell;
+        uint64_t n_int = 2 * ns + (nc + 1) + 2 * (uint64_t)nref + 3 * nc + (g->n_univ + 1);
+        L.geo_words = 8 * ns + n_int;
+        L.surf_param = C.take<double>(4 * ns + (n_int + 1) / 2);
+        int *ip = (int *)(L.surf_param + 4 * ns);
+        L.surf_type = ip; ip += ns; L.surf_bc = ip; ip += ns;
+        L.cso = ip; ip += nc + 1; L.csi = ip; ip += nref; L.css = ip; ip += nref;
+        L.cft = ip; ip += nc; L.cfill = ip; ip += nc; L.cbin = ip; ip += nc;
+        L.uco = ip;
+    }
     L.lat_univ = C.take<int>(nlat); L.lat_bin = C.take<int>(nlat);
     bool ce = x != nullptr;
     if (!ce) {
@@ -382,6 +391,8 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     G.surf_type = L.surf_type; G.surf_bc = L.surf_bc; G.surf_param = L.surf_param;
     G.cso = L.cso; G.csi = L.csi; G.css = L.css; G.cft = L.cft; G.cfill = L.cfill; G.cbin = L.cbin; G.uco = L.uco;
     G.lat_univ = L.lat_univ; G.lat_bin = L.lat_bin;
+    G.blob = (const char *)L.surf_param; G.blob_words = (int)L.geo_words;
+    c.geo_stage = L.geo_words * 4 <= GEO_STAGE_MAX_BYTES ? (int)L.geo_words : 0;
     // host staging must outlive the async copies: keep vectors until the sync at the end
     std::vector<double> h_sig_s, h_nusf, h_cumS, h_cumchi, h_srccum, h_tab, h_colA;
     std::vector<int> h_ncol, h_hash, h_cfill(g->cell_fill, g->cell_fill + g->n_cell);
@@ -514,7 +525,8 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     p->part = L.part; p->sites = L.sites;
     p->trace_base = L.trace; p->trace_count = L.trace_count;
     p->tally_private = c.n_tally <= PRIVATE_TALLY_MAX;
-    if (p->tally_private && (size_t)c.mg_stage * 8 + (size_t)c.n_tally * BS * 8 > 48 * 1024) c.mg_stage = 0;  // 48 KB default limit
+    if (p->tally_private && (size_t)c.mg_stage * 8 + (size_t)c.geo_stage * 4 + 8 + (size_t)c.n_tally * BS * 8 > 48 * 1024)
+        c.mg_stage = c.geo_stage = 0;  // 48 KB default dynamic shared memory limit
     c.flux_aggregate = c.n_tally <= AGGREGATE_TALLY_MAX ? 1 : 0;
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc, 0, sizeof(double) * c.n_tally, st);
@@ -592,7 +604,8 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
     const size_t smem_mg = CE ? 0 : (size_t)c.mg_stage * sizeof(double);
-    const size_t smem = smem_mg + (PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0);
+    const size_t smem_geo = (size_t)((c.geo_stage + 1) / 2) * sizeof(double);
+    const size_t smem = smem_mg + smem_geo + (PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0);
     CUDA_OK(cudaMemsetAsync(c.qc, 0, sizeof(QCount) * RING, st));
     CUDA_OK(cudaMemsetAsync(c.n_over, 0, sizeof(unsigned int), st));
     uint64_t upper = M;
@@ -615,7 +628,7 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
         } else if (p->schedule == 0) {
             { ProfScope ps(p, MCDC_PROF_ADVANCE); k_advance<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
             { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, smem_mg, st>>>(c, s); }
-            { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, 0, st>>>(c, s); }
+            { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, smem_geo, st>>>(c, s); }
             p->n_launches += 3;
         } else {
             { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
