@@ -222,11 +222,12 @@ int mcdc_get_timing(const mcdc_problem *p, double *ms_transport, uint64_t *n_lau
 
 /* per-kernel-class device timing: when on, every launch is bracketed by a CUDA event pair on the library's
  * stream (costs a few microseconds per launch, so it is off for throughput runs).  mcdc_get_profile fills
- * ms[MCDC_N_PROFILE] and launches[MCDC_N_PROFILE] accumulated since mcdc_set_profile. */
+ * ms[MCDC_N_PROFILE] and launches[MCDC_N_PROFILE] accumulated since mcdc_set_profile, and the number of events
+ * (live particles) the k_advance launches processed in that time. */
 enum { MCDC_PROF_ADVANCE = 0, MCDC_PROF_SCATTER, MCDC_PROF_SURFACE, MCDC_PROF_TAIL, MCDC_PROF_SEGMENT, MCDC_PROF_BANK,
        MCDC_PROF_FUSED, MCDC_N_PROFILE };
 int mcdc_set_profile(mcdc_problem *p, int32_t on);
-int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches);
+int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *advance_events);
 
 void mcdc_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);

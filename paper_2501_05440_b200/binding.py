@@ -130,7 +130,7 @@ def load_library():
     L.mcdc_test_geometry.argtypes = [vp, _dp, _dp, u64, _ip, _dp, _ip]
     L.mcdc_get_timing.argtypes = [vp, _dp, P(u64)]
     L.mcdc_set_profile.argtypes = [vp, i32]
-    L.mcdc_get_profile.argtypes = [vp, _dp, P(u64)]
+    L.mcdc_get_profile.argtypes = [vp, _dp, P(u64), P(u64)]
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -307,8 +307,11 @@ class Problem:
 
     def profile(self):
         ms, nl = np.zeros(7), np.zeros(7, np.uint64)
-        self._check(self.L.mcdc_get_profile(self.h, ms.ctypes.data_as(_dp), nl.ctypes.data_as(C.POINTER(C.c_uint64))))
-        return {k: dict(ms=float(m), launches=int(n)) for k, m, n in zip(self.PROFILE_CLASSES, ms, nl)}
+        ev = C.c_uint64()
+        self._check(self.L.mcdc_get_profile(self.h, ms.ctypes.data_as(_dp), nl.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(ev)))
+        out = {k: dict(ms=float(m), launches=int(n)) for k, m, n in zip(self.PROFILE_CLASSES, ms, nl)}
+        out["advance"]["events"] = int(ev.value)
+        return out
 
     def bank(self):
         n = C.c_uint64()

@@ -303,6 +303,7 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsig
         n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
     }
     QCount *oc = c.qc + (s % RING);
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(c.counters + 12, (unsigned long long)n_in);  // events of k_advance
     if (PRIVATE) {
         for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
         __syncthreads();

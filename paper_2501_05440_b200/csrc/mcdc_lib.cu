@@ -88,6 +88,7 @@ struct mcdc_problem {
     std::vector<int> pool_class;  // class of pair k (events 2k, 2k+1)
     double prof_ms[MCDC_N_PROFILE];
     uint64_t prof_launches[MCDC_N_PROFILE];
+    uint64_t prof_adv_base;  // device counter 12 (events processed by k_advance) when profiling was switched on
 };
 
 // RAII-free helper: record an event pair around one launch when profiling is on
@@ -948,14 +949,22 @@ extern "C" int mcdc_set_profile(mcdc_problem *p, int32_t on)
 {
     if (!p) return fail(MCDC_EINVAL, "null");
     p->profile = on ? 1 : 0;
+    unsigned long long b = 0;
+    CUDA_OK(cudaMemcpy(&b, p->ctx.counters + 12, sizeof b, cudaMemcpyDeviceToHost));
+    p->prof_adv_base = b;
     memset(p->prof_ms, 0, sizeof p->prof_ms); memset(p->prof_launches, 0, sizeof p->prof_launches);
     return 0;
 }
 
-extern "C" int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches)
+extern "C" int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *advance_events)
 {
     if (!p || !ms || !launches) return fail(MCDC_EINVAL, "null");
     for (int k = 0; k < MCDC_N_PROFILE; k++) { ms[k] = p->prof_ms[k]; launches[k] = p->prof_launches[k]; }
+    if (advance_events) {
+        unsigned long long b = 0;
+        CUDA_OK(cudaMemcpy(&b, p->ctx.counters + 12, sizeof b, cudaMemcpyDeviceToHost));
+        *advance_events = b - p->prof_adv_base;
+    }
     return 0;
 }
 
