@@ -444,8 +444,11 @@ __device__ __forceinline__ int segment(const Ctx &c, const MGTab &mg, const Geo 
 #ifndef MCDC_MULTI_MINBLOCKS
 #define MCDC_MULTI_MINBLOCKS 3  // measured: 2 -> 11.4, 3 -> 9.7, 4 -> 9.6 ms of fused sweeps per C4 cycle
 #endif
+#ifndef MCDC_MULTI_MINBLOCKS_CE
+#define MCDC_MULTI_MINBLOCKS_CE 3
+#endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS, MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
+__global__ void __launch_bounds__(BS, CE ? MCDC_MULTI_MINBLOCKS_CE : MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
