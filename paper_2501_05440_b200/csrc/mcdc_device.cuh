@@ -23,6 +23,8 @@ struct Geo {
     const int *cso, *csi, *css, *cft, *cfill, *cbin, *uco;
     const char *blob;  // surfaces, cells and universes are one contiguous blob (staged in shared memory)
     int blob_words;    // its size in 4-byte words
+    const unsigned int *lat_rmask;  // per element: bit j set = surface j of the enclosing cell's list can be the
+                                    // nearest boundary from inside the element (built exactly at create)
     const int *lat_univ, *lat_bin;  // lat_bin bit 30: the enclosing cell's surfaces can be the nearest boundary
 };                                  // from inside this element (create() proves when they cannot)
 constexpr int LAT_ROOT_FLAG = 1 << 30;
@@ -407,19 +409,29 @@ __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, d
 // nearest boundary of the current location; candidate order: enclosing-cell surfaces, local-cell surfaces,
 // lattice walls -x,+x,-y,+y; ties keep the first (R12, R14).  hit = surface id, or n_surf+k for wall k.
 __device__ __forceinline__ double nearest(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int cell,
-                                          int elem, int last, int &hit, bool root_needed = true)
+                                          int elem, int last, int &hit, unsigned int root_mask = 0xffffffffu)
 {
     double best = __longlong_as_double(0x7ff0000000000000LL);
     hit = -1;
     const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;  // +-inf when the component is zero: guarded at use
     int c0 = elem >= 0 ? G.lat_cell : cell;
     int k1 = G.cso[c0 + 1];
-    if (root_needed)
-        for (int k = G.cso[c0]; k < k1; k++) {
+    if (root_mask) {
+        // candidates in list order (ties keep the first, R12): the listed bits, then anything past the 32nd surface
+        const int k0 = G.cso[c0];
+        unsigned int m = k1 - k0 >= 32 ? root_mask : root_mask & ((1u << (k1 - k0)) - 1u);
+        while (m) {
+            int s = G.csi[k0 + __ffs(m) - 1];
+            m &= m - 1u;
+            double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
+            if (d < best) { best = d; hit = s; }
+        }
+        for (int k = k0 + 32; k < k1; k++) {
             int s = G.csi[k];
             double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
+    }
     if (elem >= 0) {
         int ix, iy;
         elem_xy(G, elem, ix, iy);
@@ -552,10 +564,10 @@ __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &
     const int cell0 = p.cell, elem0 = p.elem;
     const int mat = G.cfill[p.cell];
     int bin = G.cbin[p.cell];
-    bool root_needed = true;
+    unsigned int root_mask = 0xffffffffu;
     if (p.elem >= 0) {
         int lb = __ldg(G.lat_bin + p.elem);
-        root_needed = (lb & LAT_ROOT_FLAG) != 0;
+        root_mask = (lb & LAT_ROOT_FLAG) ? __ldg(G.lat_rmask + p.elem) : 0u;
         bin += lb & (LAT_ROOT_FLAG - 1);
     }
 
@@ -587,7 +599,7 @@ __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &
     // candidate distances: collision (one draw every segment), boundary, time edge (R12)
     double d_coll = -log(rng.next()) / sig_t;
     int hit;
-    double d_surf = nearest(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_needed);
+    double d_surf = nearest(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_mask);
     double v = 0.0, d_time = __longlong_as_double(0x7ff0000000000000LL);
     if (CE) {
         v = speed_of(p.E);

@@ -139,6 +139,7 @@ struct Carver {
 struct Layout {  // everything carved from the workspace, in order
     // small tables
     int *surf_type, *surf_bc, *cso, *csi, *css, *cft, *cfill, *cbin, *uco, *lat_univ, *lat_bin;
+    unsigned int *lat_rmask;
     double *surf_param;
     double *sig_t, *sig_s, *sig_f, *nu, *nusf, *cumS, *cumchi, *src_cum;
     double *grid, *tab, *colA, *t_edges, *e_edges;
@@ -205,7 +206,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         L.cft = ip; ip += nc; L.cfill = ip; ip += nc; L.cbin = ip; ip += nc;
         L.uco = ip;
     }
-    L.lat_univ = C.take<int>(nlat); L.lat_bin = C.take<int>(nlat);
+    L.lat_univ = C.take<int>(nlat); L.lat_bin = C.take<int>(nlat); L.lat_rmask = C.take<unsigned int>(nlat);
     bool ce = x != nullptr;
     if (!ce) {
         uint64_t mg = (uint64_t)m->n_mat * m->G;
@@ -391,7 +392,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     for (int cc = 0; cc < g->n_cell; cc++) if (g->cell_fill_type[cc] == 1) G.lat_cell = cc;
     G.surf_type = L.surf_type; G.surf_bc = L.surf_bc; G.surf_param = L.surf_param;
     G.cso = L.cso; G.csi = L.csi; G.css = L.css; G.cft = L.cft; G.cfill = L.cfill; G.cbin = L.cbin; G.uco = L.uco;
-    G.lat_univ = L.lat_univ; G.lat_bin = L.lat_bin;
+    G.lat_univ = L.lat_univ; G.lat_bin = L.lat_bin; G.lat_rmask = L.lat_rmask;
     G.blob = (const char *)L.surf_param; G.blob_words = (int)L.geo_words;
     c.geo_stage = L.geo_words * 4 <= GEO_STAGE_MAX_BYTES ? (int)L.geo_words : 0;
     // host staging must outlive the async copies: keep vectors until the sync at the end
@@ -405,30 +406,37 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     UP(L.cso, g->cell_surf_off, g->n_cell + 1); UP(L.csi, g->cell_surf_id, nref); UP(L.css, g->cell_surf_sense, nref);
     UP(L.cft, g->cell_fill_type, g->n_cell); UP(L.cfill, h_cfill.data(), g->n_cell); UP(L.cbin, t->cell_bin, g->n_cell);
     UP(L.uco, g->univ_cell_off, g->n_univ + 1);
-    // lattice element -> tally bin, plus the flag "the enclosing cell's surfaces must be tested from inside this
-    // element".  It may be dropped only where it is provably never the nearest candidate: an interior element
-    // (all four walls are events, R14) whose closed x/y range contains none of the enclosing cell's surfaces;
-    // only axis planes x = p / y = p can be excluded that way, any other surface type keeps the flag set.
+    // lattice element -> tally bin, plus which of the enclosing cell's surfaces must be tested from inside the
+    // element (bit mask over the cell's surface list; flag bit 30 of lat_bin = mask != 0).  A surface is dropped
+    // only where it is provably never the nearest candidate: an axis plane x = p (y = p) lying strictly beyond a
+    // wall of the element that is itself an event (an interior lattice wall, R14) -- the ray crosses that wall
+    // first.  Any other surface type, and planes beyond an outermost (non-event) wall, stay in the mask.
     std::vector<int> h_latbin(nlat);
+    std::vector<unsigned int> h_rmask(nlat);
     if (nlat) {
         int lc = G.lat_cell;
         for (int iy = 0; iy < g->lat_ny; iy++)
             for (int ix = 0; ix < g->lat_nx; ix++) {
-                bool need = ix == 0 || iy == 0 || ix == g->lat_nx - 1 || iy == g->lat_ny - 1;
+                unsigned int mask = 0u;
                 double xlo = g->lat_x0 + ix * g->lat_px, xhi = g->lat_x0 + (ix + 1) * g->lat_px;
                 double ylo = g->lat_y0 + iy * g->lat_py, yhi = g->lat_y0 + (iy + 1) * g->lat_py;
                 double tx = 1e-9 * g->lat_px, ty = 1e-9 * g->lat_py;
-                for (int k = g->cell_surf_off[lc]; k < g->cell_surf_off[lc + 1] && !need; k++) {
-                    int sidx = g->cell_surf_id[k];
+                for (int k = g->cell_surf_off[lc]; k < g->cell_surf_off[lc + 1]; k++) {
+                    int sidx = g->cell_surf_id[k], j = k - g->cell_surf_off[lc];
                     double pp = g->surf_param[4 * sidx];
-                    if (g->surf_type[sidx] == MCDC_PLANE_X) need = pp > xlo - tx && pp < xhi + tx;
-                    else if (g->surf_type[sidx] == MCDC_PLANE_Y) need = pp > ylo - ty && pp < yhi + ty;
-                    else need = true;
+                    bool need = true;
+                    if (g->surf_type[sidx] == MCDC_PLANE_X)
+                        need = !((pp > xhi + tx && ix + 1 < g->lat_nx) || (pp < xlo - tx && ix > 0));
+                    else if (g->surf_type[sidx] == MCDC_PLANE_Y)
+                        need = !((pp > yhi + ty && iy + 1 < g->lat_ny) || (pp < ylo - ty && iy > 0));
+                    if (j >= 32) { if (need) mask |= 0x80000000u; }  // past the 32nd surface: always tested
+                    else if (need) mask |= 1u << j;
                 }
                 int e_ = iy * g->lat_nx + ix;
-                h_latbin[e_] = t->lat_bin[e_] | (need ? LAT_ROOT_FLAG : 0);
+                h_rmask[e_] = mask;
+                h_latbin[e_] = t->lat_bin[e_] | (mask ? LAT_ROOT_FLAG : 0);
             }
-        UP(L.lat_univ, g->lat_univ, nlat); UP(L.lat_bin, h_latbin.data(), nlat);
+        UP(L.lat_univ, g->lat_univ, nlat); UP(L.lat_bin, h_latbin.data(), nlat); UP(L.lat_rmask, h_rmask.data(), nlat);
     }
 
     // ---- cross sections: derived tables built here, in plain left-to-right float64 sums
