@@ -17,7 +17,10 @@
 
 namespace mcdc {
 
-constexpr int BS = 256;  // threads per block of every transport kernel
+#ifndef MCDC_BS
+#define MCDC_BS 256
+#endif
+constexpr int BS = MCDC_BS;  // threads per block of every transport kernel
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -291,7 +294,7 @@ __device__ __forceinline__ void make_child(const Ctx &c, Rng &rng, int mat, unsi
 #define MCDC_ADV_MINBLOCKS 4  // measured on B200: 2 -> 30.2, 3 -> 25.2, 4 -> 22.5, 5 -> 24.1 ms of k_advance per C4 cycle
 #endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS) k_advance(Ctx c, unsigned int s, unsigned int n0)
+__global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS * 256 / BS) k_advance(Ctx c, unsigned int s, unsigned int n0)
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
@@ -448,7 +451,7 @@ __device__ __forceinline__ int segment(const Ctx &c, const MGTab &mg, const Geo 
 #define MCDC_MULTI_MINBLOCKS_CE 3
 #endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS, CE ? MCDC_MULTI_MINBLOCKS_CE : MCDC_MULTI_MINBLOCKS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
+__global__ void __launch_bounds__(BS, (CE ? MCDC_MULTI_MINBLOCKS_CE : MCDC_MULTI_MINBLOCKS) * 256 / BS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
 {
     extern __shared__ double s_dyn[];
     const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);

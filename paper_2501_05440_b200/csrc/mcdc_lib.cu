@@ -249,7 +249,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         F.ctr = C.take<uint32_t>(fc);
         F.id = ce ? C.take<uint64_t>(fc) : nullptr;
     }
-    L.stack_threads = ce ? std::min<uint64_t>(148ull * 16ull * BS, (cap + BS - 1) / BS * BS) : 0;
+    L.stack_threads = ce ? std::min<uint64_t>(148ull * 16ull * 256, (cap + BS - 1) / BS * BS) : 0;
     L.stack = C.take<StackRec>(L.stack_threads * STACK_DEPTH);
     L.qc = C.take<QCount>(RING);
     uint64_t nt = n_tally_of(m, t);
@@ -582,7 +582,7 @@ extern "C" const char *mcdc_last_error(void) { return g_err.c_str(); }
 static unsigned int grid_for(uint64_t n)
 {
     uint64_t b = (n + BS - 1) / BS;
-    const uint64_t cap = 148ull * 16ull;  // persistent-style: at most 16 resident-block waves' worth per SM
+    const uint64_t cap = 148ull * 16ull * 256 / BS;  // persistent-style: at most 16 x 256 threads' worth per SM
     return (unsigned int)std::max<uint64_t>(1, std::min(b, cap));
 }
 
