@@ -137,6 +137,40 @@ def geom_pincell(pitch=1.26, r=0.54, fuel=0, mod=1):
     return g.finish(n_bins=2)
 
 
+def geom_mixed(material_a=0, material_b=1):
+    """Every surface type in one problem (parity / pin geometry, not a BASELINE config): a reflecting box
+    [-2,2]^3 (PLANE_X/Y/Z) holding a sphere (r = 0.9 at (0.3,-0.2,0.1)), an x-axis cylinder (CYL_X, r = 0.5 through
+    (y,z) = (-1.3, 1.3)), a y-axis cylinder (CYL_Y, r = 0.4 through (x,z) = (1.2,-1.1)), and a general plane
+    x + 2y - z = 0.8 that splits the remaining volume in two cells; vacuum on the +z face."""
+    g = _Geom()
+    xm = g.surf(PLANE_X, [-2.0], REFLECT); xp = g.surf(PLANE_X, [2.0], REFLECT)
+    ym = g.surf(PLANE_Y, [-2.0], REFLECT); yp = g.surf(PLANE_Y, [2.0], REFLECT)
+    zm = g.surf(PLANE_Z, [-2.0], REFLECT); zp = g.surf(PLANE_Z, [2.0], VACUUM)
+    sp = g.surf(SPHERE, [0.3, -0.2, 0.1, 0.9])
+    cx = g.surf(CYL_X, [-1.3, 1.3, 0.5])
+    cy = g.surf(CYL_Y, [1.2, -1.1, 0.4])
+    pl = g.surf(PLANE, [1.0, 2.0, -1.0, 0.8])
+    box = [(xm, +1), (xp, -1), (ym, +1), (yp, -1), (zm, +1), (zp, -1)]
+    g.cell(0, [(sp, -1)], material_a, bin_=0)
+    g.cell(0, [(cx, -1), (xm, +1), (xp, -1)], material_a, bin_=1)
+    g.cell(0, [(cy, -1), (ym, +1), (yp, -1)], material_b, bin_=2)
+    g.cell(0, box + [(sp, +1), (cx, +1), (cy, +1), (pl, -1)], material_b, bin_=3)
+    g.cell(0, box + [(sp, +1), (cx, +1), (cy, +1), (pl, +1)], material_a, bin_=4)
+    return g.finish(n_bins=5)
+
+
+def mixed_surfaces(n_particles=20_000, n_inactive=1, n_active=3, seed=23, G=3):
+    """Two synthetic 3-group materials in geom_mixed(); eigenvalue run."""
+    rng = np.random.default_rng(6)
+    mats = [mg_fuel(rng, G, 1.4), mg_moderator(rng, G)]
+    P = geom_mixed()
+    P.update(_mg_pack(mats))
+    P.update(_src([-1.9, -1.9, -1.9], [1.9, 1.9, 1.9], G=G, pdf=mats[0]["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "mixed"
+    return P
+
+
 def tube_positions():
     """25 moderator-filled tube positions of a 17x17 assembly: our own 8-fold-symmetric
     choice (a regular 5x5 sub-grid, spacing 3) -- NOT any published benchmark's pin map."""

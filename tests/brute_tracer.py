@@ -119,10 +119,16 @@ def trace_cycle0(P, seed, n_hist, k_prev=1.0):
         g = _pick(pdf, r[5] * sum(pdf))
         w, seq, alive = 1.0, 0, True
         while alive:
-            cands = [(d, s) for s in range(ns) for d in _roots(P, s, x, u) if d > 1e-9]
-            d_surf, s_hit = min(cands) if cands else (math.inf, -1)
-            probe = min(d_surf, 1.0) * 0.5 if cands else 0.0
+            cands = sorted((d, s) for s in range(ns) for d in _roots(P, s, x, u) if d > 1e-9)
+            probe = min(cands[0][0], 1.0) * 0.5 if cands else 0.0
             cell = _cell_at(P, [x[i] + probe * 1e-3 * u[i] for i in range(3)])
+            # the event is the first crossing that changes the cell (or meets a boundary condition): a surface
+            # that merely passes through a cell which does not list it is not a boundary there
+            d_surf, s_hit = math.inf, -1
+            for dc, sc in cands:
+                if int(P["surf_bc"][sc]) != 0 or _cell_at(P, [x[i] + (dc + 1e-7) * u[i] for i in range(3)]) != cell:
+                    d_surf, s_hit = dc, sc
+                    break
             m = int(P["cell_fill"][cell])
             st = float(P["mg_sig_t"][m][g])
             d_coll = -math.log(xi()) / st

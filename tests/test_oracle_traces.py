@@ -39,6 +39,11 @@ def test_trace_sphere_and_slab_vs_brute_force(orc):
     _compare(orc, P, 60, 60)
 
 
+def test_trace_all_surface_types_vs_brute_force(orc):
+    """PLANE, PLANE_Z, SPHERE, CYL_X, CYL_Y, reflect + vacuum + transmit in one geometry."""
+    _compare(orc, inputs.mixed_surfaces(), 150, 150)
+
+
 def test_geometry_brute_force_quarter_core(orc):
     """Lattice fast path (element walls + local cell + enclosing cell) vs brute force: the distance returned
     must be the smallest positive distance to ANY pin cylinder / lattice line / outer plane along the ray that
