@@ -110,7 +110,11 @@ def load_library():
     if _lib is not None:
         return _lib
     if not os.path.exists(_SO):
-        raise McdcError(-5, f"{_SO} is missing: run `python -c 'import __graft_entry__ as g; g.build()'`")
+        try:  # build the product in-tree if the toolchain is there; never fall back to anything else
+            build()
+        except Exception as e:
+            raise McdcError(-5, f"{_SO} is missing and could not be built ({e}): run "
+                                "`python -c 'import __graft_entry__ as g; g.build()'`")
     L = C.CDLL(_SO)
     vp, u64, u32, i32 = C.c_void_p, C.c_uint64, C.c_uint32, C.c_int32
     P = C.POINTER
