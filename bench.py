@@ -332,13 +332,17 @@ def main():
     ap.add_argument("--ce-particles", type=int, default=1_000_000)
     ap.add_argument("--no-ce", dest="ce", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ce-only", action="store_true", help="run only the C5 continuous-energy configuration")
     ap.add_argument("--tail", type=int, default=0, help="tail-kernel threshold (0 = library default, <0 = off)")
     ap.add_argument("--fuse", type=int, default=0, help="fused-sweep threshold (0 = default, <0 = off)")
     ap.add_argument("--fuse-segments", type=int, default=0)
     ap.add_argument("--schedule", type=int, default=0, help="0 event queues (default), 1 monolithic")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 1)
-    if args.impl == "reference":
+    if args.ce_only:  # the continuous-energy configuration alone (profiling aid)
+        from paper_2501_05440_b200 import binding, inputs
+        print(json.dumps(bench_ce(binding, inputs, args, peaks()[0])))
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
