@@ -32,7 +32,7 @@ static int fail(int code, const char *fmt, ...)
 
 static const int LAG = 3;                 // sweeps the host may run ahead of the queue-count read-back
 static const int DEFAULT_TAIL = 32768;    // live particles at which the tail kernel takes over (multi-group)
-static const int DEFAULT_TAIL_CE = 64;    // continuous energy: the tail thread also follows its prompt subtree
+static const int DEFAULT_TAIL_CE = -1;    // continuous energy: no tail kernel by default (measured: 64 -> 91, 16 -> 88, none -> 83.6 ms on C5)
 // live particles below which a sweep is one fused multi-segment launch (measured on B200, profiles/r01_step4*.md)
 static const int DEFAULT_FUSE = 2000000, DEFAULT_FUSE_CE = 4000000;
 static const int DEFAULT_FUSE_SEGMENTS = 8, DEFAULT_FUSE_SEGMENTS_CE = 16;
