@@ -180,3 +180,22 @@ def test_empty_and_error_paths(gpu):
         g2.run(n_inactive=0, n_active=2)
     assert e.value.code == -3
     g2.close()
+
+
+def test_bank_overflow_and_lost_particle_errors(gpu):
+    """R6: more than 2N fission sites is MCDC_EBANK; a source point in no cell is MCDC_EGEOM; both leave the
+    problem usable for a later valid run."""
+    P = inputs.config1(n_particles=2000, n_inactive=0, n_active=2)
+    P["mg_nu"] = P["mg_nu"] * 4.0  # k_inf = 5.2: the first cycle banks about 5 N sites
+    g = gpu.Problem(P)
+    with pytest.raises(gpu.McdcError) as e:
+        g.run()
+    assert e.value.code == -3
+    g.close()
+    P = inputs.config1(n_particles=500, n_inactive=0, n_active=1)
+    P["src_hi"] = np.array([1.5, 1.0, 1.0])  # a third of the source box lies outside the cube
+    g = gpu.Problem(P)
+    with pytest.raises(gpu.McdcError) as e:
+        g.run()
+    assert e.value.code == -2
+    g.close()
