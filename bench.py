@@ -277,6 +277,8 @@ def run_ours(args):
         out["cpu_baseline"] = {"value": args.ref_cycles * n / dtc, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": f"C4 at {n} particles/cycle, {args.ref_cycles} active cycles after 1 (full: 1e7/cycle)",
                                "events_per_sec": events_of(cnt) / tt, "host_cores_available": os.cpu_count()}
+        # PAPER.md:118-120 Eq. (1): CPU cores one GPU is worth = (cores x CPU time) / (GPUs x GPU time) on the same work
+        out["core_equivalency_eq1"] = value / world / (out["cpu_baseline"]["value"] / out["cpu_baseline"]["cores"])
 
     if rank == 0 and args.ce:
         out["secondary"] = bench_ce(binding, inputs, args, peak)
