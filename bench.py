@@ -107,10 +107,19 @@ def job_value(units_per_rank: float, world: int, seconds_max: float) -> float:
     return world * units_per_rank / seconds_max
 
 
+WORKLOADS = {"C1": ("C1: 1-group infinite medium (reflecting unit cube)", 10_000),
+             "C2": ("C2: 7-group infinite medium (reflecting unit cube)", 100_000),
+             "C3": ("C3: 2-D pin cell, 7 groups", 1_000_000),
+             "C4": ("C4: 2-D quarter core, 7 groups, 2x2 17x17-pin assemblies + reflector, k-eigenvalue cycle", 10_000_000)}
+
+
 def workload(args):
+    """The bench workload is C4 (the largest multi-group configuration); --config C1..C3 times the smaller
+    BASELINE.json configurations with the same code path (documentation runs, not the headline)."""
     from paper_2501_05440_b200 import inputs
-    N = args.particles
-    return inputs.config4(n_particles=N, n_inactive=args.warmup, n_active=args.steps), N
+    N = args.particles if args.particles else WORKLOADS[args.config][1]
+    fn = {"C1": inputs.config1, "C2": inputs.config2, "C3": inputs.config3, "C4": inputs.config4}[args.config]
+    return fn(n_particles=N, n_inactive=args.warmup, n_active=args.steps), N
 
 
 def events_of(counters):
@@ -256,9 +265,9 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": "C4: 2-D quarter core, 7 groups, 2x2 17x17-pin assemblies + reflector, k-eigenvalue cycle",
+        "config": {"workload": WORKLOADS[args.config][0],
                    "particles_per_cycle": N, "step": "one power-iteration cycle", "parallelism": "replicas only",
-                   "l2": "particle bank (>1.2 GB) larger than L2", "schedule": "per-event kernels above 2e6 live particles, fused 8-segment sweeps below, tail kernel below 32768",
+                   "l2": "particle bank (>1.2 GB) larger than L2" if N >= 2_000_000 else "bank fits in L2 (small configuration)", "schedule": "per-event kernels above 2e6 live particles, fused 8-segment sweeps below, tail kernel below 32768",
                    "k_mean": res["k_mean"]},
         "events_per_sec": ev_per_s, "events_per_history": events / max(tracks, 1),
         "roofline": roof, "e2e": e2e, "gpu_launches": int(nl1 - nl0), "clocks": clocks,
@@ -328,7 +337,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--particles", type=int, default=10_000_000)
+    ap.add_argument("--particles", type=int, default=0, help="particles per cycle (0 = the configuration's own)")
+    ap.add_argument("--config", default="C4", choices=list(WORKLOADS))
     ap.add_argument("--ref-particles", type=int, default=100_000)
     ap.add_argument("--ref-cycles", type=int, default=8)
     ap.add_argument("--ce-particles", type=int, default=1_000_000)
