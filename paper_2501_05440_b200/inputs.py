@@ -177,7 +177,7 @@ def tube_positions():
     return [(8 + i, 8 + j) for i in (-6, -3, 0, 3, 6) for j in (-6, -3, 0, 3, 6)]
 
 
-def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_reflect=False):
+def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_reflect=False, height=None):
     """C4: one (n_asm*n_pin+n_refl)^2 lattice; elements [0,n_asm*n_pin)^2
     are fuelled assemblies, the rest moderator 'reflector' elements.  x=0,y=0 REFLECT,
     outer faces VACUUM.  Materials: 0,1,2 fuel variants; 3,4 alternate fuel; 5 tube fill; 6 moderator.
@@ -192,7 +192,12 @@ def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_refl
     y0 = g.surf(PLANE_Y, [0.0], REFLECT)
     y1 = g.surf(PLANE_Y, [side], outer)
     cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
-    g.cell(0, [(x0, +1), (x1, -1), (y0, +1), (y1, -1)], 0, lattice=True)
+    root = [(x0, +1), (x1, -1), (y0, +1), (y1, -1)]
+    if height is not None:  # finite height: reflecting mid-plane at z = 0, vacuum top at z = height
+        z0 = g.surf(PLANE_Z, [0.0], REFLECT)
+        z1 = g.surf(PLANE_Z, [float(height)], outer)
+        root += [(z0, +1), (z1, -1)]
+    g.cell(0, root, 0, lattice=True)
     for u in range(1, 7):
         g.cell(u, [(cy, -1)], u - 1)
         g.cell(u, [(cy, +1)], 6)
@@ -336,7 +341,7 @@ def config3(n_particles=1_000_000, n_inactive=20, n_active=80, seed=1, same_mate
 
 
 def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform=False,
-            n_asm=2, n_pin=17, n_refl=17, G=7):
+            n_asm=2, n_pin=17, n_refl=17, G=7, height=None):
     """C4: 2-D quarter core stand-in for the paper's C5G7 workload: 7 synthetic
     materials from seed 4.  uniform=True: all materials identical + all faces reflecting (pin)."""
     rng = np.random.default_rng(4)
@@ -345,10 +350,10 @@ def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform
     mats += [mg_moderator(rng, G), mg_moderator(rng, G)]
     if uniform:
         mats = [mg_fuel(np.random.default_rng(2), G, 1.2)] * 7
-    P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform)
+    P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform, height=height)
     P.update(_mg_pack(mats))
     side = n_asm * n_pin * 1.26
-    P.update(_src([0, 0, 0], [side, side, 0], G=G, pdf=mats[0]["chi"]))
+    P.update(_src([0, 0, 0], [side, side, 0.9 * height if height else 0], G=G, pdf=mats[0]["chi"]))
     P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
     P["name"] = "C4"
     return P

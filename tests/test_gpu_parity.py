@@ -51,6 +51,7 @@ CASES = {
     "C4": lambda: inputs.config4(n_particles=6000, n_inactive=1, n_active=2),
     "C4small": lambda: inputs.config4(n_particles=3001, n_inactive=1, n_active=2, n_asm=1, n_pin=3, n_refl=1),
     "mixed": lambda: inputs.mixed_surfaces(n_particles=4000),
+    "C4_3d": lambda: inputs.config4(n_particles=4000, n_inactive=1, n_active=2, n_asm=1, n_pin=4, n_refl=1, height=6.0),
     "slab": lambda: inputs.slab_beam(n_particles=5000),
     "sphere": lambda: inputs.sphere_absorber(n_particles=5000),
 }
@@ -76,7 +77,7 @@ def test_mg_parity(gpu, orc, name, schedule, tail, fuse):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d"])
 @pytest.mark.parametrize("schedule,tail,fuse", [(0, -1, -1), (0, 0, 0), (1, 0, 0), (0, 100, 500)])
 def test_mg_traces_identical(gpu, orc, name, schedule, tail, fuse):
     """100 particles x 2 cycles: identical per-particle event sequences (SURVEY.md 8d parity protocol 1)."""

@@ -305,3 +305,24 @@ def test_c5_subcritical_and_bounded(orc):
     # flux tallies: total track length per source history = sum over bins; positive, finite
     f = r["flux_mean"]
     assert np.isfinite(f).all() and f.sum() > 0
+
+
+def test_quarter_core_finite_height_leakage(orc):
+    """Lattice inside z planes (reflecting z = 0, vacuum top): pure absorber, beam along +z from z = 0+: leakage
+    through the top = exp(-Sigma_t * height); no lattice wall is ever crossed."""
+    hgt, st = 3.0, 0.5
+    P = inputs.config4(n_particles=40000, n_inactive=0, n_active=1, n_asm=1, n_pin=2, n_refl=1, G=1, height=hgt)
+    for k in ("mg_sig_t", "mg_sig_c"):
+        P[k][:] = st
+    for k in ("mg_sig_f", "mg_nu", "mg_S"):
+        P[k][:] = 0.0
+    P["mg_chi"][:] = 1.0
+    P["src_lo"][:] = [0.1, 0.1, 1e-9]
+    P["src_hi"][:] = [3.6, 3.6, 1e-9]
+    P["src_iso"] = 0
+    P["src_dir"][:] = [0.0, 0.0, 1.0]
+    rc, r = orc.Oracle(P).run()
+    assert rc == 0
+    p = math.exp(-st * hgt)
+    assert abs(r["leak_mean"] - p) < 3 * math.sqrt(p * (1 - p) / 40000)
+    assert r["counters"][EV["lattice"]] == 0
