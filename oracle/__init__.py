@@ -56,7 +56,7 @@ SITE_DTYPE = np.dtype([("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("ux", "<f8"), 
 def build(force: bool = False) -> str:
     """Compile the oracle (gcc -O2).  Building the checker is not using it."""
     if force or not os.path.exists(_SO) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC):
-        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", _SO, _SRC[0], "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", _SO, _SRC[0], "-lm"])
     return _SO
 
 
@@ -72,6 +72,7 @@ def lib():
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_set_trace.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64]
         L.orc_run_eigenvalue.argtypes = [C.c_void_p, C.c_uint64, C.c_int, C.c_int, C.c_uint64]
+        L.orc_run_eigenvalue_mt.argtypes = [C.c_void_p, C.c_uint64, C.c_int, C.c_int, C.c_uint64, C.c_int]
         L.orc_run_fixed_source.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
         L.orc_n_tally.restype = C.c_int64
         L.orc_n_tally.argtypes = [C.c_void_p]
@@ -180,6 +181,17 @@ class Oracle:
     def set_trace(self, first_id=0, n_ids=100, max_records=1_000_000):
         self.L.orc_set_trace(self.h, first_id, n_ids, max_records)
         self._tr_max = max_records
+
+    def run_mt(self, n_threads, n_particles=None, n_inactive=None, n_active=None, seed=None):
+        """All-core timing variant of the eigenvalue run (see mcdc_oracle.c); not used by the parity tests."""
+        r = self.P["run"]
+        N = int(n_particles if n_particles is not None else r["n_particles"])
+        ni = int(n_inactive if n_inactive is not None else r["n_inactive"])
+        na = int(n_active if n_active is not None else r["n_active"])
+        sd = int(seed if seed is not None else r["seed"])
+        rc = self.L.orc_run_eigenvalue_mt(self.h, N, ni, na, sd, int(n_threads))
+        self.n_cycles = ni + na
+        return rc, self.results()
 
     def run(self, n_particles=None, n_inactive=None, n_active=None, seed=None):
         r = self.P["run"]

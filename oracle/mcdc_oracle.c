@@ -855,6 +855,76 @@ int orc_run_eigenvalue(orc_problem *p, uint64_t N, int n_inactive, int n_active,
     return p->error;
 }
 
+/* All-core timing variant of the eigenvalue run (bench.py's cpu_baseline only; the parity tests use the serial
+ * run above): the source particles of a cycle are split in n_threads contiguous id ranges, each followed by its own
+ * thread into thread-private tallies and a private piece of the fission bank; pieces and tallies are joined in
+ * thread order, so the bank stays sorted by (parent id, child index) and the result is reproducible for a fixed
+ * n_threads (it differs from the serial run by float64 summation order only).  No tracing. */
+int orc_run_eigenvalue_mt(orc_problem *p, uint64_t N, int n_inactive, int n_active, uint64_t seed, int n_threads)
+{
+    if (p->in.mode != 0 || n_threads < 1) return -1;
+    int64_t nt = orc_n_tally(p);
+    reset_results(p, n_inactive + n_active);
+    p->seed = seed; p->fixed = 0; p->k_prev = 1.0;
+    p->cap_bank = 2 * N + 16;
+    free(p->bank); free(p->newbank);
+    p->bank = (orc_site *)calloc((size_t)p->cap_bank, sizeof(orc_site));
+    p->newbank = (orc_site *)calloc((size_t)p->cap_bank, sizeof(orc_site));
+    p->n_bank = 0;
+    free(p->trace); p->trace = NULL;
+    orc_problem *th = (orc_problem *)calloc((size_t)n_threads, sizeof(orc_problem));
+    for (int t = 0; t < n_threads; t++) {
+        th[t] = *p; /* shares the read-only inputs and derived tables */
+        th[t].flux_c = (double *)calloc((size_t)nt, sizeof(double));
+        th[t].cap_bank = p->cap_bank; /* worst case: one thread banks everything */
+        th[t].newbank = (orc_site *)calloc((size_t)p->cap_bank, sizeof(orc_site));
+    }
+    for (int c = 0; c < n_inactive + n_active; c++) {
+        p->cycle = (uint32_t)c;
+        uint64_t M = c == 0 ? N : p->n_bank;
+        double w0 = c == 0 ? 1.0 : (M > 0 ? (double)N / (double)M : 0.0);
+        #pragma omp parallel for num_threads(n_threads) schedule(static, 1)
+        for (int t = 0; t < n_threads; t++) {
+            orc_problem *q = &th[t];
+            q->cycle = p->cycle; q->seed = seed; q->k_prev = p->k_prev; q->bank = p->bank;
+            memset(q->flux_c, 0, (size_t)nt * sizeof(double));
+            memset(q->counters, 0, sizeof(q->counters));
+            q->k_num = 0.0; q->leak_c = 0.0; q->n_newbank = 0; q->error = 0;
+            uint64_t lo = M * (uint64_t)t / (uint64_t)n_threads, hi = M * (uint64_t)(t + 1) / (uint64_t)n_threads;
+            for (uint64_t i = lo; i < hi; i++) {
+                particle pt;
+                memset(&pt, 0, sizeof pt);
+                pt.id = i; pt.w = w0;
+                if (c == 0) sample_source(q, &pt);
+                else {
+                    const orc_site *s = &p->bank[i];
+                    pt.x = s->x; pt.y = s->y; pt.z = s->z; pt.ux = s->ux; pt.uy = s->uy; pt.uz = s->uz; pt.g = s->g;
+                }
+                place(q, &pt);
+                if (pt.alive) transport(q, &pt); else q->counters[0]++;
+            }
+        }
+        memset(p->flux_c, 0, (size_t)nt * sizeof(double));
+        p->k_num = 0.0; p->leak_c = 0.0; p->n_newbank = 0;
+        for (int t = 0; t < n_threads; t++) { /* join in thread order */
+            for (int64_t i = 0; i < nt; i++) p->flux_c[i] += th[t].flux_c[i];
+            p->k_num += th[t].k_num; p->leak_c += th[t].leak_c;
+            for (int k = 0; k < ORC_N_COUNTERS; k++) p->counters[k] += th[t].counters[k];
+            if (th[t].error && !p->error) p->error = th[t].error;
+            if (p->n_newbank + th[t].n_newbank > p->cap_bank) { p->error = -3; th[t].n_newbank = p->cap_bank - p->n_newbank; }
+            memcpy(p->newbank + p->n_newbank, th[t].newbank, (size_t)th[t].n_newbank * sizeof(orc_site));
+            p->n_newbank += th[t].n_newbank;
+        }
+        orc_site *tmp = p->bank; p->bank = p->newbank; p->newbank = tmp;
+        p->n_bank = p->n_newbank;
+        if (p->n_bank > p->counters[12]) p->counters[12] = p->n_bank;
+        accumulate_cycle(p, N, c >= n_inactive);
+    }
+    for (int t = 0; t < n_threads; t++) { free(th[t].flux_c); free(th[t].newbank); }
+    free(th);
+    return p->error;
+}
+
 /* time-dependent fixed source: every source particle, then its secondaries LIFO */
 int orc_run_fixed_source(orc_problem *p, uint64_t N, uint64_t seed)
 {

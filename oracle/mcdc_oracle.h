@@ -89,6 +89,8 @@ orc_problem *orc_create(const orc_input *in);
 void orc_destroy(orc_problem *p);
 int orc_set_trace(orc_problem *p, uint64_t first_id, uint64_t n_ids, uint64_t max_records);
 int orc_run_eigenvalue(orc_problem *p, uint64_t n_particles, int n_inactive, int n_active, uint64_t seed);
+/* all-core timing variant (bench.py cpu_baseline): n_threads contiguous id ranges, joined in thread order */
+int orc_run_eigenvalue_mt(orc_problem *p, uint64_t n_particles, int n_inactive, int n_active, uint64_t seed, int n_threads);
 int orc_run_fixed_source(orc_problem *p, uint64_t n_particles, uint64_t seed);
 /* results; arrays sized by the caller: k_cycle[n_cycles], flux_*[n_tally], counters[ORC_N_COUNTERS] */
 int64_t orc_n_tally(const orc_problem *p);

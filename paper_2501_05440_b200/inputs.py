@@ -141,7 +141,8 @@ def geom_mixed(material_a=0, material_b=1):
     """Every surface type in one problem (parity / pin geometry, not a BASELINE config): a reflecting box
     [-2,2]^3 (PLANE_X/Y/Z) holding a sphere (r = 0.9 at (0.3,-0.2,0.1)), an x-axis cylinder (CYL_X, r = 0.5 through
     (y,z) = (-1.3, 1.3)), a y-axis cylinder (CYL_Y, r = 0.4 through (x,z) = (1.2,-1.1)), and a general plane
-    x + 2y - z = 0.8 that splits the remaining volume in two cells; vacuum on the +z face."""
+    x + 2y - z = 0.8 that splits the remaining volume in two cells; vacuum on the +z face; a REFLECTING general plane
+    x + y + z = 5 cuts off the (+,+,+) corner (non-axis reflection)."""
     g = _Geom()
     xm = g.surf(PLANE_X, [-2.0], REFLECT); xp = g.surf(PLANE_X, [2.0], REFLECT)
     ym = g.surf(PLANE_Y, [-2.0], REFLECT); yp = g.surf(PLANE_Y, [2.0], REFLECT)
@@ -150,7 +151,8 @@ def geom_mixed(material_a=0, material_b=1):
     cx = g.surf(CYL_X, [-1.3, 1.3, 0.5])
     cy = g.surf(CYL_Y, [1.2, -1.1, 0.4])
     pl = g.surf(PLANE, [1.0, 2.0, -1.0, 0.8])
-    box = [(xm, +1), (xp, -1), (ym, +1), (yp, -1), (zm, +1), (zp, -1)]
+    mir = g.surf(PLANE, [1.0, 1.0, 1.0, 5.0], REFLECT)  # a mirror that cuts the (+,+,+) corner off the box
+    box = [(xm, +1), (xp, -1), (ym, +1), (yp, -1), (zm, +1), (zp, -1), (mir, -1)]
     g.cell(0, [(sp, -1)], material_a, bin_=0)
     g.cell(0, [(cx, -1), (xm, +1), (xp, -1)], material_a, bin_=1)
     g.cell(0, [(cy, -1), (ym, +1), (yp, -1)], material_b, bin_=2)
@@ -165,9 +167,43 @@ def mixed_surfaces(n_particles=20_000, n_inactive=1, n_active=3, seed=23, G=3):
     mats = [mg_fuel(rng, G, 1.4), mg_moderator(rng, G)]
     P = geom_mixed()
     P.update(_mg_pack(mats))
-    P.update(_src([-1.9, -1.9, -1.9], [1.9, 1.9, 1.9], G=G, pdf=mats[0]["chi"]))
+    P.update(_src([-1.9, -1.9, -1.9], [1.6, 1.6, 1.6], G=G, pdf=mats[0]["chi"]))
     P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
     P["name"] = "mixed"
+    return P
+
+
+def geom_mirror(kind, r=1.0, r_in=0.6):
+    """Homogeneous medium inside ONE reflecting curved surface (non-axis specular reflection, R13): 'sphere' (radius
+    r), 'cyl_z' / 'cyl_x' / 'cyl_y' (radius r, closed by two reflecting axis planes at +-1).  A concentric transmitting
+    surface of radius r_in splits it in two tally bins (same material): with specular walls the flux stays uniform, so
+    the bins' track lengths are in the ratio of their volumes."""
+    g = _Geom()
+    if kind == "sphere":
+        so = g.surf(SPHERE, [0.0, 0.0, 0.0, r], REFLECT)
+        si = g.surf(SPHERE, [0.0, 0.0, 0.0, r_in])
+        caps = []
+    else:
+        typ = dict(cyl_x=CYL_X, cyl_y=CYL_Y, cyl_z=CYL_Z)[kind]
+        ptyp = dict(cyl_x=PLANE_X, cyl_y=PLANE_Y, cyl_z=PLANE_Z)[kind]
+        so = g.surf(typ, [0.0, 0.0, r], REFLECT)
+        si = g.surf(typ, [0.0, 0.0, r_in])
+        c0 = g.surf(ptyp, [-1.0], REFLECT)
+        c1 = g.surf(ptyp, [1.0], REFLECT)
+        caps = [(c0, +1), (c1, -1)]
+    g.cell(0, [(si, -1)] + caps, 0, bin_=0)
+    g.cell(0, [(si, +1), (so, -1)] + caps, 0, bin_=1)
+    return g.finish(n_bins=2)
+
+
+def curved_mirror(kind="sphere", n_particles=20_000, n_inactive=2, n_active=10, seed=31):
+    """C1's one-group material inside geom_mirror(kind): leakage 0, k -> 1.3, flux ratio = volume ratio.  The source
+    is a small box at the centre (the inner cell); the fission source spreads out over the cycles."""
+    P = geom_mirror(kind)
+    P.update(_mg_pack([one_group_material()]))
+    P.update(_src([-0.3, -0.3, -0.3], [0.3, 0.3, 0.3], G=1))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "mirror_" + kind
     return P
 
 
@@ -220,6 +256,38 @@ def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_refl
             bins[iy, ix] = iy * nfuel + ix
     lat = dict(x0=0.0, y0=0.0, px=float(pitch), py=float(pitch), nx=n, ny=n, univ=univ, bin=bins)
     return g.finish(lat=lat, n_bins=nfuel * nfuel + 1)
+
+
+def geom_rect_lattice(nx, ny, pitch=1.26, r=0.54, x_hi=VACUUM, y_hi=REFLECT):
+    """nx x ny pin lattice filling the box [0, nx p] x [0, ny p] (parity geometry for non-square and one-column /
+    one-row lattices): universes 1 = fuel pin (material 0 in a cylinder, 1 outside), 2 = moderator only, in a
+    checker pattern; x = 0 and y = 0 reflect; one tally bin per element."""
+    g = _Geom()
+    x0 = g.surf(PLANE_X, [0.0], REFLECT)
+    x1 = g.surf(PLANE_X, [nx * pitch], x_hi)
+    y0 = g.surf(PLANE_Y, [0.0], REFLECT)
+    y1 = g.surf(PLANE_Y, [ny * pitch], y_hi)
+    cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
+    g.cell(0, [(x0, +1), (x1, -1), (y0, +1), (y1, -1)], 0, lattice=True)
+    g.cell(1, [(cy, -1)], 0)
+    g.cell(1, [(cy, +1)], 1)
+    g.cell(2, [], 1)
+    univ = np.array([[1 if (ix + 2 * iy) % 3 else 2 for ix in range(nx)] for iy in range(ny)], np.int32)
+    bins = np.arange(nx * ny, dtype=np.int32).reshape(ny, nx)
+    lat = dict(x0=0.0, y0=0.0, px=float(pitch), py=float(pitch), nx=nx, ny=ny, univ=univ, bin=bins)
+    return g.finish(lat=lat, n_bins=nx * ny)
+
+
+def rect_lattice(nx, ny, n_particles=4000, n_inactive=1, n_active=2, seed=29, G=3):
+    """Two synthetic 3-group materials in geom_rect_lattice(nx, ny); eigenvalue run."""
+    rng = np.random.default_rng(7)
+    mats = [mg_fuel(rng, G, 1.5), mg_moderator(rng, G)]
+    P = geom_rect_lattice(nx, ny)
+    P.update(_mg_pack(mats))
+    P.update(_src([0, 0, 0], [nx * 1.26, ny * 1.26, 0], G=G, pdf=mats[0]["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = f"lat{nx}x{ny}"
+    return P
 
 
 # --------------------------------------------------------------------------- MG materials
@@ -376,7 +444,6 @@ def ce_nuclides(seed=5, n_grid=50_000, jitter=False, n_res=200):
         E0 = np.exp(rng.uniform(np.log(1.0), np.log(1e4), n_res))
         gam = E0 * np.exp(rng.uniform(np.log(3e-3), np.log(1e-2), n_res))
         pk = np.exp(rng.uniform(np.log(lo_pk), np.log(hi_pk), n_res)) / np.sqrt(E0)
-        pk *= np.sqrt(1.0)  # peaks in barns at E0 (x E0^-1/2 as the recipe states)
         out = np.zeros_like(E)
         for e0, gm, p in zip(E0, gam, pk):
             out += p / (1.0 + ((E - e0) / (0.5 * gm)) ** 2)
@@ -487,6 +554,56 @@ def ce_single_scatterer(A=16.0, n_particles=50_000, seed=17, E0=1.0e6, sig_el=0.
     P.update(_src([0, 0, 0], [0, 0, 0], E=E0, t=0.0))
     P["run"] = dict(kind="fixed", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
     P["name"] = "ce_scatter"
+    return P
+
+
+def ce_two_nuclide_mix(n_particles=20_000, seed=37, E0=1.0e6, E_cut=1.0e3, p_light=0.3, n_grid=4000):
+    """Elastic-branch pin of the transport loop: a mixture of a light (A = 1) and a heavy (A = 238) nuclide with flat
+    elastic cross sections (light share p_light of Sigma_el), listed in the material in the order [light, heavy] while
+    the nuclide table holds [heavy, dummy A = 16, light] -- so the column -> nuclide map matters.  Capture (on the
+    heavy nuclide) is zero above E_cut and overwhelming below: a history slows down by elastic collisions only and is
+    captured at its first collision below E_cut."""
+    P = geom_infinite()
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    E[0], E[-1] = 1e-5, 2e7
+    el = np.zeros((3, n_grid))
+    ca = np.zeros((3, n_grid))
+    el[0] = 1.0 - p_light      # heavy
+    el[1] = 123.0              # never used by the material
+    el[2] = p_light            # light
+    ca[0] = np.where(E < E_cut, 1.0e7, 0.0)
+    P.update(mode="ce", n_mat=1, grid=E, nuc_A=np.array([238.0, 16.0, 1.0]), nuc_el=el, nuc_c=ca,
+             nuc_f=np.zeros((3, n_grid)), mat_nuc_off=np.array([0, 2], np.int32), mat_nuc_id=np.array([2, 0], np.int32),
+             mat_nuc_dens=np.array([1.0, 1.0]), nu0=0.0, nu1=0.0, watt_a=0.988, watt_b=2.249)
+    P["t_edges"] = np.array([0.0, 1.0e3])
+    P["e_edges"] = np.exp(np.linspace(np.log(1e-5), np.log(2e7), 101))
+    P["e_edges"][0], P["e_edges"][-1] = 1e-5, 2e7
+    P.update(_src([0, 0, 0], [0, 0, 0], E=E0, t=0.0))
+    P["run"] = dict(kind="fixed", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "ce_mix"
+    return P
+
+
+def ce_scatter_clock(lam=3.0e6, T=4.0e-6, A=1.0, n_particles=20_000, seed=41, E0=1.0e5, n_grid=6000):
+    """Time pin of the elastic branch: one nuclide (mass ratio A) whose only reaction is elastic scattering with
+    Sigma_el(E) = lam / v(E), in an infinite medium, run to the single time edge T.  The collision rate per unit TIME
+    is then lam whatever the energy history, so collisions per history ~ Poisson(lam T) -- only if every flight
+    advances the clock by d / v(E of that flight).  (Lin-lin interpolation of a 1/v curve on the fine log grid is
+    accurate to < 1e-6 relative; the energy floor E_min is never reached: the mean lethargy gain lam T is far less than
+    ln(E0 / E_min).)"""
+    P = geom_infinite()
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    E[0], E[-1] = 1e-5, 2e7
+    v = 2.99792458e10 * np.sqrt(2.0 * E / 939.56542052e6)
+    P.update(mode="ce", n_mat=1, grid=E, nuc_A=np.array([float(A)]), nuc_el=(lam / v)[None, :].copy(),
+             nuc_c=np.zeros((1, n_grid)), nuc_f=np.zeros((1, n_grid)), mat_nuc_off=np.array([0, 1], np.int32),
+             mat_nuc_id=np.array([0], np.int32), mat_nuc_dens=np.array([1.0]), nu0=0.0, nu1=0.0, watt_a=0.988,
+             watt_b=2.249)
+    P["t_edges"] = np.array([0.0, float(T)])
+    P["e_edges"] = np.array([1e-5, 2e7])
+    P.update(_src([0, 0, 0], [0, 0, 0], E=E0, t=0.0))
+    P["run"] = dict(kind="fixed", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = "ce_clock"
     return P
 
 

@@ -21,8 +21,10 @@ def _compare(orc, P, n_hist, N):
     assert len(tr) == len(ref) and len(ref) >= n_hist
     for a, b in zip(tr, ref):
         assert (int(a["id"]), int(a["seq"]), int(a["ev"]), int(a["surf"]), int(a["gi"])) == b[:5]
+        assert (int(a["elem"]), int(a["c1"])) == b[9:11]
         assert a["x"] == pytest.approx(b[5], abs=1e-11) and a["y"] == pytest.approx(b[6], abs=1e-11)
         assert a["z"] == pytest.approx(b[7], abs=1e-9) and a["d"] == pytest.approx(b[8], rel=1e-9, abs=1e-12)
+    return tr
 
 
 def test_trace_c1_vs_brute_force(orc):
@@ -40,8 +42,70 @@ def test_trace_sphere_and_slab_vs_brute_force(orc):
 
 
 def test_trace_all_surface_types_vs_brute_force(orc):
-    """PLANE, PLANE_Z, SPHERE, CYL_X, CYL_Y, reflect + vacuum + transmit in one geometry."""
-    _compare(orc, inputs.mixed_surfaces(), 150, 150)
+    """PLANE, PLANE_Z, SPHERE, CYL_X, CYL_Y, reflect + vacuum + transmit in one geometry, incl. reflections off the
+    general plane x + y + z = 5 (surface 10: non-axis branch of the oracle's reflect())."""
+    tr = _compare(orc, inputs.mixed_surfaces(), 400, 400)
+    assert ((tr["ev"] == 5) & (tr["surf"] == 10)).sum() >= 5
+
+
+@pytest.mark.parametrize("kind", ["sphere", "cyl_z", "cyl_x", "cyl_y"])
+def test_trace_curved_mirrors_vs_brute_force(orc, kind):
+    """Specular reflection off a sphere and off cylinders along each axis (non-axis branch of reflect(): normal
+    from the gradient, Omega' = Omega - 2 (Omega.n) n), event by event against the brute-force tracer."""
+    tr = _compare(orc, inputs.curved_mirror(kind), 120, 120)
+    curved = 0  # the reflecting quadric is surface 0 in geom_mirror
+    assert ((tr["ev"] == 5) & (tr["surf"] == curved)).sum() >= 100
+
+
+@pytest.mark.parametrize("case", ["C4small", "C4_3d", "lat1x6", "lat5x1", "lat3x5", "C4edge"])
+def test_trace_lattice_vs_brute_force(orc, case):
+    """One-level lattices, event by event (incl. element and local cell of every event): the oracle's neighbour /
+    wall-ahead logic (R14) against brute force over every grid line and every pin of the lattice."""
+    P = dict(C4small=lambda: inputs.config4(n_particles=60, n_asm=1, n_pin=3, n_refl=1),
+             C4_3d=lambda: inputs.config4(n_particles=60, n_asm=1, n_pin=4, n_refl=1, height=6.0),
+             lat1x6=lambda: inputs.rect_lattice(1, 6), lat5x1=lambda: inputs.rect_lattice(5, 1),
+             lat3x5=lambda: inputs.rect_lattice(3, 5),
+             C4edge=lambda: inputs.config4(n_particles=40, n_asm=2, n_pin=5, n_refl=2))[case]()
+    tr = _compare(orc, P, 60, 60)
+    assert (tr["ev"] == 7).sum() >= 50  # lattice-wall events
+
+
+def _compare_ce(orc, P, n_src):
+    """CE time-dependent fixed source: source histories event by event, integer event counters of ALL tracks (source
+    particles and every prompt secondary below them) and the (time bin x energy bin) flux tally."""
+    o = orc.Oracle(P)
+    o.set_trace(0, n_src, 2_000_000)
+    rc, r = o.run(n_particles=n_src)
+    assert rc == 0
+    tr = o.trace()
+    ev, cnt, flux = brute_tracer.trace_ce(P, P["run"]["seed"], n_src)
+    assert len(tr) == len(ev) and len(ev) >= n_src
+    for a, b in zip(tr, ev):
+        assert (int(a["id"]), int(a["seq"]), int(a["ev"]), int(a["surf"]), int(a["gi"])) == b[:5]
+        for k, f in enumerate(("x", "y", "z", "d", "E", "t")):
+            assert a[f] == pytest.approx(b[5 + k], rel=1e-9, abs=1e-11), f
+    assert [int(v) for v in r["counters"][:12]] == cnt[:12]
+    got = r["flux_mean"].reshape(len(flux), -1) * n_src
+    want = np.array(flux)
+    assert np.allclose(got, want, rtol=1e-9, atol=1e-13 * want.max())
+    return tr, r
+
+
+def test_trace_ce_c5_vs_brute_force(orc):
+    """C5 (pin cell, 5 nuclides, resonances, Watt fission, 10 time x 100 energy bins): 25 source histories and their
+    whole prompt-fission families against the pure-Python tracer.  Pins, inside the transport loop: the column ->
+    nuclide map of the elastic branch, the energy clamp, t += d / v, the time-edge logic, edge_bin() over 100 bins
+    (every track length lands in the bin numpy-style bisection names), secondaries' ids and streams."""
+    P = inputs.config5(n_particles=25, n_grid=3000)
+    tr, r = _compare_ce(orc, P, 25)
+    assert r["counters"][11] > 10 and (tr["ev"] == 8).sum() > 5
+
+
+def test_trace_ce_jittered_grid_and_light_nuclide(orc):
+    P = inputs.config5(n_particles=12, n_grid=1500, jitter=True)
+    _compare_ce(orc, P, 12)
+    P = inputs.ce_two_nuclide_mix(n_particles=15, n_grid=800)
+    _compare_ce(orc, P, 15)
 
 
 def test_geometry_brute_force_quarter_core(orc):

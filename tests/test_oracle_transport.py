@@ -326,3 +326,21 @@ def test_quarter_core_finite_height_leakage(orc):
     p = math.exp(-st * hgt)
     assert abs(r["leak_mean"] - p) < 3 * math.sqrt(p * (1 - p) / 40000)
     assert r["counters"][EV["lattice"]] == 0
+
+
+def test_all_core_variant_equals_serial_run(orc):
+    """orc_run_eigenvalue_mt (bench.py's all-core cpu_baseline) splits the source particles in contiguous id ranges:
+    identical integer counters and bank, tallies equal to summation order; one thread = the serial run bit for bit."""
+    P = inputs.config4(n_particles=6000, n_inactive=1, n_active=2, n_asm=1, n_pin=5, n_refl=2)
+    o = orc.Oracle(P)
+    rc, r1 = o.run()
+    b1 = o.bank().copy()
+    rc3, r3 = o.run_mt(3)
+    b3 = o.bank().copy()
+    assert rc == 0 and rc3 == 0
+    assert (r1["counters"] == r3["counters"]).all()
+    assert len(b1) == len(b3) and (b1["x"] == b3["x"]).all() and (b1["g"] == b3["g"]).all()
+    assert np.allclose(r1["k_cycle"], r3["k_cycle"], rtol=1e-12)
+    assert np.allclose(r1["flux_mean"], r3["flux_mean"], rtol=1e-11, atol=1e-15)
+    rc1, r1b = o.run_mt(1)
+    assert (r1["k_cycle"] == r1b["k_cycle"]).all() and (r1["flux_mean"] == r1b["flux_mean"]).all()
