@@ -174,8 +174,7 @@ def run_ours(args):
 
     P, N = workload(args)
     seed = 1 + rank  # replicas only: independent problems, no data-path collective
-    g = binding.Problem(P, device=local, search=1, tail_threshold=args.tail, schedule=args.schedule,
-                        fuse_threshold=args.fuse, fuse_segments=args.fuse_segments)
+    g = binding.Problem(P, device=local, search=1, persist_threshold=args.persist, schedule=args.schedule)
     K, W = args.steps, args.warmup
 
     # ---- device-resident throughput: W warm-up cycles, then exactly K timed cycles
@@ -214,7 +213,7 @@ def run_ours(args):
     g.set_profile(False)
     ca = g.results()["counters"]
     ev_prof = events_of(ca) - events_of(cb)
-    adv = prof["advance"]
+    adv = prof["sweep"]
     peak, peak_src = peaks()
     tot_ms = sum(v["ms"] for v in prof.values())
     roof = None
@@ -223,7 +222,7 @@ def run_ours(args):
         bytes_per_launch = B_ADV_MG * ev_adv / adv["launches"]
         dur = adv["ms"] * 1e-3 / adv["launches"]
         ach = bytes_per_launch / dur / 1e9
-        roof = {"bound": "hbm", "kernel": "k_advance<MG>", "achieved": ach, "peak": peak, "unit": "GB/s",
+        roof = {"bound": "hbm", "kernel": "k_sweep<MG>", "achieved": ach, "peak": peak, "unit": "GB/s",
                 "frac": ach / peak, "traffic": None, "peak_source": peak_src,
                 "bytes_per_event": B_ADV_MG, "events_per_launch": ev_adv / adv["launches"],
                 "share_of_events": ev_adv / max(ev_prof, 1),
@@ -267,7 +266,7 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config][0],
                    "particles_per_cycle": N, "step": "one power-iteration cycle", "parallelism": "replicas only",
-                   "l2": "particle bank (>1.2 GB) larger than L2" if N >= 2_000_000 else "bank fits in L2 (small configuration)", "schedule": "per-event kernels above 2e6 live particles, fused 8-segment sweeps below, tail kernel below 32768",
+                   "l2": "particle bank (>1.2 GB) larger than L2" if N >= 2_000_000 else "bank fits in L2 (small configuration)", "schedule": "event sweeps over dense queues regrouped by next event; persistent asynchronous kernel below the library's live-particle threshold",
                    "k_mean": res["k_mean"]},
         "events_per_sec": ev_per_s, "events_per_history": events / max(tracks, 1),
         "roofline": roof, "e2e": e2e, "gpu_launches": int(nl1 - nl0), "clocks": clocks,
@@ -302,8 +301,7 @@ def bench_ce(binding, inputs, args, peak):
     """Largest continuous-energy configuration (C5: 1e6 source particles) -- reported beside the headline."""
     import torch
     P = inputs.config5(n_particles=args.ce_particles)
-    g = binding.Problem(P, search=1, tail_threshold=args.tail, schedule=args.schedule,
-                        fuse_threshold=args.fuse, fuse_segments=args.fuse_segments)
+    g = binding.Problem(P, search=1, persist_threshold=args.persist_ce, schedule=args.schedule)
     g.run()  # warm-up
     torch.cuda.synchronize()
     best = None
@@ -320,12 +318,12 @@ def bench_ce(binding, inputs, args, peak):
     prof = g.profile()
     g.set_profile(False)
     g.close()
-    adv = prof["advance"]
+    adv = prof["sweep"]
     ach = B_ADV_CE * adv["events"] / (adv["ms"] * 1e-3) / 1e9 if adv["ms"] else None
     return {"workload": "C5: continuous-energy time-dependent pin cell", "source_particles": args.ce_particles,
             "histories_per_sec": args.ce_particles / (best * 1e-3), "tracks": int(r["counters"][0]),
             "events_per_sec": ev / (best * 1e-3), "ms": best,
-            "roofline": {"bound": "hbm", "kernel": "k_advance<CE>", "achieved": ach, "peak": peak, "unit": "GB/s",
+            "roofline": {"bound": "hbm", "kernel": "k_sweep<CE>", "achieved": ach, "peak": peak, "unit": "GB/s",
                          "frac": ach / peak if ach else None, "bytes_per_event": B_ADV_CE,
                          "whole_event": {"bytes_per_event": B_ALG_CE, "frac": ev / (best * 1e-3) * B_ALG_CE / 1e9 / peak}},
             "kernel_ms": {k: round(v["ms"], 3) for k, v in prof.items() if v["launches"]}}
@@ -345,10 +343,10 @@ def main():
     ap.add_argument("--no-ce", dest="ce", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ce-only", action="store_true", help="run only the C5 continuous-energy configuration")
-    ap.add_argument("--tail", type=int, default=0, help="tail-kernel threshold (0 = library default, <0 = off)")
-    ap.add_argument("--fuse", type=int, default=0, help="fused-sweep threshold (0 = default, <0 = off)")
-    ap.add_argument("--fuse-segments", type=int, default=0)
-    ap.add_argument("--schedule", type=int, default=0, help="0 event queues (default), 1 monolithic")
+    ap.add_argument("--persist", type=int, default=0, help="live particles at which the persistent kernel takes over "
+                    "(0 = library default, <0 = never, 2147483647 = from the start)")
+    ap.add_argument("--persist-ce", type=int, default=0, help="the same for the continuous-energy configuration")
+    ap.add_argument("--schedule", type=int, default=0, help="0 event sweeps + persistent kernel (default), 1 monolithic, 2 split per-event kernels")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 1)
     if args.ce_only:  # the continuous-energy configuration alone (profiling aid)

@@ -16,7 +16,9 @@
  *     binding allocates it with torch.empty); the library never calls cudaMalloc/cudaFree.  All kernels
  *     are launched on mcdc_device.stream (a cudaStream_t; NULL = the legacy default stream).
  *   - every call returns 0 or a negative MCDC_E* code; mcdc_last_error() gives a thread-local
- *     message.  Nothing throws or aborts across the ABI; a failed run leaves earlier tallies intact.
+ *     message.  Nothing throws or aborts across the ABI.  A failed run call leaves the results of the last
+ *     successful call readable (mcdc_get_dims / mcdc_get_tallies keep reporting them) and the problem usable: the
+ *     next run has to start again from cycle 0.
  *   - all floating point is float64.
  */
 #ifndef MCDC_H
@@ -37,11 +39,12 @@ enum { MCDC_BC_TRANSMIT = 0, MCDC_BC_REFLECT = 1, MCDC_BC_VACUUM = 2 };
 /* event codes of the trace and of the event counters (one event per segment) */
 enum { MCDC_EV_SCATTER = 1, MCDC_EV_FISSION, MCDC_EV_CAPTURE, MCDC_EV_TRANSMIT, MCDC_EV_REFLECT, MCDC_EV_LEAK,
        MCDC_EV_LATTICE, MCDC_EV_TIME_EDGE, MCDC_EV_CUTOFF, MCDC_EV_LOST };
-/* counters[0] tracks started, [1..10] events by code, [11] children banked, [12] bank high-water mark,
- * [13] sweeps (kernel rounds), [14] tail-kernel histories, [15] reserved */
+/* counters[0] tracks started, [1..10] events by code, [11] children banked, [12] largest fission / secondary bank
+ * of the run (sites), [13] kernel rounds (sweeps + persistent launches), [14] particles the persistent kernel took
+ * from its work queue, [15] reserved */
 #define MCDC_N_COUNTERS 16
 
-/* CSG geometry: surfaces, conjunctive cells grouped by universe, one optional rectangular lattice
+/* CSG geometry: at most 3800 surfaces, conjunctive cells grouped by universe, one optional rectangular lattice
  * (R11-R16).  surf_param[s][4]: PLANE_X/Y/Z (p,-,-,-); PLANE (a,b,c,d): a x+b y+c z = d; CYL_Z (x0,y0,r,-)
  * (CYL_X (y0,z0,r), CYL_Y (x0,z0,r)); SPHERE (x0,y0,z0,r).  Cells of universe u are
  * [univ_cell_off[u], univ_cell_off[u+1]); universe 0 is the root.  cell_fill_type 0: cell_fill = material
@@ -114,22 +117,23 @@ typedef struct {
     const double *e_edges; /* [n_e+1], CE only */
 } mcdc_tally_spec;
 
-/* device resources handed in by the caller.  schedule: 0 = per-event kernels over compacted index queues
- * (default), 1 = monolithic one-segment-per-launch kernel over every bank slot, no compaction (the paper's
- * PAPER.md:51-55 design, kept for the divergence comparison).  tail_threshold: when at most this many
- * particles are alive the remaining histories are finished inside one kernel (0 = library default,
- * negative = never). */
+/* device resources handed in by the caller.
+ * schedule: 0 (default) = event-based sweeps over dense particle queues regrouped by next event, one kernel per sweep
+ *   (each particle's pending scatter / surface event is finished by the kernel that picks it up), and the persistent
+ *   asynchronous kernel once at most persist_threshold particles are alive;
+ *   1 = monolithic one-segment-per-launch kernel over every bank slot, no compaction (the paper's PAPER.md:51-55
+ *   design, kept for the divergence comparison);
+ *   2 = as 0, but the pending events are finished by two separate per-event kernels after every sweep (split
+ *   per-event kernels).
+ * persist_threshold: 0 = library default, negative = never use the persistent kernel, 2^31-1 = always. */
 typedef struct {
     void *workspace; /* DEVICE pointer, 256-byte aligned */
     uint64_t workspace_bytes;
     void *stream; /* cudaStream_t */
     int32_t device;
     int32_t schedule;
-    int32_t tail_threshold;
-    int32_t fuse_threshold; /* at most this many alive: one fused launch does fuse_segments whole segments per
-                               particle, then compacts (0 = library default, negative = never) */
-    int32_t fuse_segments;  /* 0 = library default */
-    int32_t reserved;
+    int32_t persist_threshold;
+    int32_t reserved[3];
 } mcdc_device;
 
 typedef struct {
@@ -172,7 +176,10 @@ int mcdc_workspace_bytes(const mcdc_geometry *geo, const mcdc_materials *mat, co
                          const mcdc_tally_spec *tally, uint64_t n_particles, uint64_t *bytes);
 
 /* validate + copy all inputs, build derived tables (cumulative scatter rows, chi CDF, macroscopic CE rows,
- * hash buckets), upload them into the workspace.  Exactly one of mat / xs is non-NULL. */
+ * hash buckets, per-lattice-element boundary codes), upload them into the workspace.  Exactly one of mat / xs is
+ * non-NULL.  Checked here: index ranges and monotone offset arrays, Sigma_s + Sigma_f <= Sigma_t, a strictly
+ * increasing grid and edges, cell_bin + lat_bin < n_bins, the source time inside the time edges, and that the source
+ * box lies inside the geometry (a 9 x 9 x 9 grid of its points must all be in a cell; MCDC_EGEOM otherwise). */
 int mcdc_create(const mcdc_geometry *geo, const mcdc_materials *mat, const mcdc_xs *xs, const mcdc_source *src,
                 const mcdc_tally_spec *tally, const mcdc_device *dev, uint64_t max_particles, mcdc_problem **out);
 
@@ -212,9 +219,12 @@ int mcdc_test_draws(mcdc_problem *p, uint64_t seed, uint32_t domain, uint32_t cy
                     const uint32_t *draw, uint64_t n, double *out);
 /* union-grid index of E[i] with the binary (out_bin) and the hashed (out_hash) search */
 int mcdc_test_grid_index(mcdc_problem *p, const double *E, uint64_t n, int32_t *out_bin, int32_t *out_hash);
-/* locate + nearest boundary for n points: loc[i][3] = (c0, elem, c1), dist[i], surf[i] */
-int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64_t n, int32_t *loc, double *dist,
-                       int32_t *surf);
+/* locate + nearest boundary for n points: loc[i][3] = (c0, elem, c1), dist[i], surf[i].  path 0: the code path the
+ * transport kernels take from that point (straight-line inside simple lattice elements, else the generic loops over
+ * the enclosing cell's surfaces that create() could not rule out); 1: generic loops with that pruned list; 2: generic
+ * loops over every surface (no pruning).  All three must agree. */
+int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64_t n, int32_t path, int32_t *loc,
+                       double *dist, int32_t *surf);
 
 /* device time (ms, CUDA events on the library's stream) of the transport part of the last run call, and the
  * number of kernels it launched */
@@ -222,12 +232,20 @@ int mcdc_get_timing(const mcdc_problem *p, double *ms_transport, uint64_t *n_lau
 
 /* per-kernel-class device timing: when on, every launch is bracketed by a CUDA event pair on the library's
  * stream (costs a few microseconds per launch, so it is off for throughput runs).  mcdc_get_profile fills
- * ms[MCDC_N_PROFILE] and launches[MCDC_N_PROFILE] accumulated since mcdc_set_profile, and the number of events
- * (live particles) the k_advance launches processed in that time. */
-enum { MCDC_PROF_ADVANCE = 0, MCDC_PROF_SCATTER, MCDC_PROF_SURFACE, MCDC_PROF_TAIL, MCDC_PROF_SEGMENT, MCDC_PROF_BANK,
-       MCDC_PROF_FUSED, MCDC_N_PROFILE };
+ * ms[MCDC_N_PROFILE] and launches[MCDC_N_PROFILE] accumulated since mcdc_set_profile, and the number of segments
+ * (= events) the sweep kernels ran in that time (the rest of the run's events ran in the persistent kernel). */
+enum { MCDC_PROF_SWEEP = 0, MCDC_PROF_SCATTER, MCDC_PROF_SURFACE, MCDC_PROF_PERSIST, MCDC_PROF_SEGMENT, MCDC_PROF_BANK,
+       MCDC_N_PROFILE };
 int mcdc_set_profile(mcdc_problem *p, int32_t on);
-int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *advance_events);
+int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *sweep_events);
+
+/* Arithmetic micro-benchmarks of this GPU (the ALU roofline's denominators): runs `iters` loop trips of
+ * independent register-only chains of one operation on 148 x 8 blocks of 256 threads; returns the device time of the
+ * launch and the thread-level operations it performed (FFMA / DFMA: fused multiply-adds; LOG, DIV, SQRT, SINCOSPI, RCP:
+ * float64 library calls; PHILOX: Philox4x32-10 blocks = two draws each). */
+enum { MCDC_MB_FFMA = 0, MCDC_MB_DFMA, MCDC_MB_LOG, MCDC_MB_DIV, MCDC_MB_SQRT, MCDC_MB_SINCOSPI, MCDC_MB_RCP, MCDC_MB_PHILOX,
+       MCDC_MB_COUNT };
+int mcdc_microbench(mcdc_problem *p, int32_t which, uint64_t iters, double *ms, double *ops);
 
 void mcdc_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);

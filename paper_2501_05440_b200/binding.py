@@ -14,17 +14,18 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
-_SO = os.environ.get("MCDC_LIB") or os.path.join(_HERE, "libmcdc_b200.so")  # MCDC_LIB: A/B-test another build
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cuh", "mcdc_device.cuh")]
+_SO = os.path.join(_HERE, "libmcdc_b200.so")
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cuh", "mcdc_device.cuh", "mcdc_microbench.cuh")]
 _HDR = os.path.join(_ROOT, "include", "mcdc.h")
 
 N_COUNTERS = 16
+ALWAYS = 0x7FFFFFFF  # persist_threshold: the persistent kernel runs the whole cycle
 EV_NAMES = {1: "scatter", 2: "fission", 3: "capture", 4: "transmit", 5: "reflect", 6: "leak", 7: "lattice",
             8: "time_edge", 9: "cutoff", 10: "lost"}
 SYMBOLS = ["mcdc_workspace_bytes", "mcdc_create", "mcdc_run_eigenvalue", "mcdc_run_cycle", "mcdc_run_cycle_host",
            "mcdc_run_fixed_source", "mcdc_get_dims", "mcdc_get_tallies", "mcdc_get_bank", "mcdc_set_trace",
            "mcdc_get_trace", "mcdc_test_draws", "mcdc_test_grid_index", "mcdc_test_geometry", "mcdc_get_timing",
-           "mcdc_set_profile", "mcdc_get_profile", "mcdc_destroy", "mcdc_last_error"]
+           "mcdc_set_profile", "mcdc_get_profile", "mcdc_microbench", "mcdc_destroy", "mcdc_last_error"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -68,8 +69,8 @@ class TallySpec(C.Structure):
 
 class Device(C.Structure):
     _fields_ = [("workspace", C.c_void_p), ("workspace_bytes", C.c_uint64), ("stream", C.c_void_p),
-                ("device", C.c_int32), ("schedule", C.c_int32), ("tail_threshold", C.c_int32), ("fuse_threshold", C.c_int32),
-                ("fuse_segments", C.c_int32), ("reserved", C.c_int32)]
+                ("device", C.c_int32), ("schedule", C.c_int32), ("persist_threshold", C.c_int32),
+                ("reserved", C.c_int32 * 3)]
 
 
 class Dims(C.Structure):
@@ -131,10 +132,11 @@ def load_library():
     L.mcdc_get_trace.argtypes = [vp, vp, u64, P(u64)]
     L.mcdc_test_draws.argtypes = [vp, u64, u32, u32, vp, vp, u64, _dp]
     L.mcdc_test_grid_index.argtypes = [vp, _dp, u64, _ip, _ip]
-    L.mcdc_test_geometry.argtypes = [vp, _dp, _dp, u64, _ip, _dp, _ip]
+    L.mcdc_test_geometry.argtypes = [vp, _dp, _dp, u64, i32, _ip, _dp, _ip]
     L.mcdc_get_timing.argtypes = [vp, _dp, P(u64)]
     L.mcdc_set_profile.argtypes = [vp, i32]
     L.mcdc_get_profile.argtypes = [vp, _dp, P(u64), P(u64)]
+    L.mcdc_microbench.argtypes = [vp, i32, u64, _dp, _dp]
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -153,8 +155,9 @@ def _i(a):
 class Problem:
     """One transport problem on one CUDA device, built from a problem dict (see ``inputs``)."""
 
-    def __init__(self, P: dict, max_particles=None, device=0, schedule=0, tail_threshold=0, search=0,
-                 fuse_threshold=0, fuse_segments=0):
+    def __init__(self, P: dict, max_particles=None, device=0, schedule=0, persist_threshold=0, search=0):
+        """schedule 0: event sweeps + persistent kernel below persist_threshold (0 = library default, < 0 = never,
+        ALWAYS = from the first segment); 1: monolithic; 2: split per-event kernels (see include/mcdc.h)."""
         import torch
 
         if not torch.cuda.is_available():
@@ -229,8 +232,7 @@ class Problem:
         d = Device()
         d.workspace, d.workspace_bytes = base, nbytes.value
         d.stream, d.device = self.stream.cuda_stream, device
-        d.schedule, d.tail_threshold = int(schedule), int(tail_threshold)
-        d.fuse_threshold, d.fuse_segments = int(fuse_threshold), int(fuse_segments)
+        d.schedule, d.persist_threshold = int(schedule), int(persist_threshold)
         h = C.c_void_p()
         self._check(self.L.mcdc_create(C.byref(g), mp, xp, C.byref(s), C.byref(t), C.byref(d), self.max_particles, C.byref(h)))
         self.h = h
@@ -304,18 +306,26 @@ class Problem:
         self._check(self.L.mcdc_get_timing(self.h, C.byref(ms), C.byref(nl)))
         return ms.value, nl.value
 
-    PROFILE_CLASSES = ("advance", "scatter", "surface", "tail", "segment", "bank", "fused")
+    PROFILE_CLASSES = ("sweep", "scatter", "surface", "persist", "segment", "bank")
 
     def set_profile(self, on=True):
         self._check(self.L.mcdc_set_profile(self.h, int(on)))
 
     def profile(self):
-        ms, nl = np.zeros(7), np.zeros(7, np.uint64)
+        ms, nl = np.zeros(6), np.zeros(6, np.uint64)
         ev = C.c_uint64()
         self._check(self.L.mcdc_get_profile(self.h, ms.ctypes.data_as(_dp), nl.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(ev)))
         out = {k: dict(ms=float(m), launches=int(n)) for k, m, n in zip(self.PROFILE_CLASSES, ms, nl)}
-        out["advance"]["events"] = int(ev.value)
+        out["sweep"]["events"] = int(ev.value)
         return out
+
+    MICROBENCH = ("ffma", "dfma", "log", "div", "sqrt", "sincospi", "rcp", "philox")
+
+    def microbench(self, which, iters=20000):
+        """Measured rate (thread-level operations per second) of one arithmetic micro-benchmark of the library."""
+        ms, ops = C.c_double(), C.c_double()
+        self._check(self.L.mcdc_microbench(self.h, self.MICROBENCH.index(which), int(iters), C.byref(ms), C.byref(ops)))
+        return ops.value / (ms.value * 1e-3)
 
     def bank(self):
         n = C.c_uint64()
@@ -351,10 +361,10 @@ class Problem:
         self._check(self.L.mcdc_test_grid_index(self.h, E.ctypes.data_as(_dp), len(E), ob.ctypes.data_as(_ip), oh.ctypes.data_as(_ip)))
         return ob, oh
 
-    def geometry(self, x, u):
+    def geometry(self, x, u, path=0):
         x, u = _d(x).reshape(-1, 3), _d(u).reshape(-1, 3)
         n = len(x)
         loc, dist, surf = np.zeros((n, 3), np.int32), np.zeros(n), np.zeros(n, np.int32)
-        self._check(self.L.mcdc_test_geometry(self.h, x.ctypes.data_as(_dp), u.ctypes.data_as(_dp), n, loc.ctypes.data_as(_ip),
+        self._check(self.L.mcdc_test_geometry(self.h, x.ctypes.data_as(_dp), u.ctypes.data_as(_dp), n, int(path), loc.ctypes.data_as(_ip),
                                               dist.ctypes.data_as(_dp), surf.ctypes.data_as(_ip)))
         return loc, dist, surf

@@ -1,5 +1,5 @@
 // mcdc_device.cuh -- device-side data layout and per-particle device functions of the B200 transport
-// library (include/mcdc.h).  Written from the readings R1..R31 of DESIGN.md section 3 (= SURVEY.md 8c);
+// library (include/mcdc.h).  Written from the readings R1..R40 of DESIGN.md section 3 (= SURVEY.md 8c);
 // shares no code with oracle/.  float64 everywhere.
 #pragma once
 #include <cuda_runtime.h>
@@ -9,56 +9,73 @@ namespace mcdc {
 
 constexpr int CE_ROW = 8;          // doubles per (material, grid point) row of the macroscopic CE table
 constexpr int MAX_CE_COL = 6;      // cumulative columns kept per row: [el_1..el_n, fission, capture], n <= 4
-constexpr int EV_DEAD = -0x40000000;  // status value of a finished history (monolithic schedule)
 constexpr int RING = 8;            // per-sweep queue-counter sets kept alive for the lagging host read-back
+constexpr unsigned int MAX_SEGMENTS = 1000000u;  // lost-particle guard (R11): segments per history
+
+// Pending event of a banked particle (low 12 bits of Bank::ev; the high 20 bits count the history's segments):
+// a surface / lattice-wall hit code (< PEND_SCATTER), an elastic / group-transfer scatter (PEND_SCATTER | column),
+// a time edge, or nothing.  The event is FINISHED by whichever kernel picks the particle up next.
+constexpr unsigned int PEND_SCATTER = 0xF00u, PEND_TIME = 0xFFEu, PEND_NONE = 0xFFFu, PEND_MASK = 0xFFFu;
+constexpr int MAX_SURFACES = 3800;  // hit codes 0 .. n_surf+3 must stay below PEND_SCATTER
 
 // ------------------------------------------------------------------ layout in HBM
-// Geometry and small tables: plain arrays in the workspace (read-only, L1/L2 resident).
+// Geometry: small read-only tables in the workspace (L1/L2 resident).
+// Straight-line geometry path: where the boundaries of the current location are axis planes (at most one per
+// direction of flight), lattice walls and at most one z-cylinder, the nearest boundary is found without loops:
+//   lat_info[e] (lattice element e; one 16-byte load per segment): x = universe of the element | LAT_FAST, y = tally
+//     bin of the element, z = boundary code per direction -x,+x,-y,+y (8 bits each), w = codes for -z,+z.
+//   cell_info[c] (cell c outside a lattice): x = CELL_FAST | the cell across the cylinder (or CELL_NO_NEIGHBOUR),
+//     y = the cell's z-cylinder (or -1), z / w = boundary codes as above.
+//   Code 0: nothing can be hit that way; 1: a lattice wall that is an event (R14); 2+j: axis plane j of the problem
+//   (ap_pos, ap_sid).  The cylinder of a lattice element is its universe's (ufast).
+// Locations without the flag use the generic loops; for lattice elements with lat_rmask (bit j = surface j of the
+// enclosing cell's list can be the nearest boundary; built at create).
 struct Geo {
-    int n_surf, n_cell, n_univ, has_lat, lat_nx, lat_ny, lat_cell;
-    unsigned int lat_magic;  // floor(2^32 / lat_nx) + 1: elem / lat_nx == umulhi(elem, lat_magic) (elem * lat_nx < 2^32)
+    int n_surf, n_cell, n_univ, has_lat, lat_nx, lat_ny, lat_cell, n_ap;
+    unsigned int lat_magic;  // floor(2^32 / lat_nx) + 1: elem / lat_nx == umulhi(elem, lat_magic) (lat_nx >= 2)
     double lat_x0, lat_y0, lat_px, lat_py;
     const int *surf_type, *surf_bc;
     const double *surf_param;  // [n_surf][4]
     const int *cso, *csi, *css, *cft, *cfill, *cbin, *uco;
-    const char *blob;  // surfaces, cells and universes are one contiguous blob (staged in shared memory)
-    int blob_words;    // its size in 4-byte words
-    const unsigned int *lat_rmask;  // per element: bit j set = surface j of the enclosing cell's list can be the
-                                    // nearest boundary from inside the element (built exactly at create)
-    const int *lat_univ, *lat_bin;  // lat_bin bit 30: the enclosing cell's surfaces can be the nearest boundary
-};                                  // from inside this element (create() proves when they cannot)
-constexpr int LAT_ROOT_FLAG = 1 << 30;
+    const int4 *lat_info, *cell_info;
+    const unsigned int *lat_rmask;
+    const int4 *ufast;      // per universe: x = 1 if it is one cell, or two cells split by one CYL_Z; y = that
+                            // cylinder (or -1); z = cell inside it (or the only cell); w = cell outside it
+    const double *ap_pos;   // [n_ap] position of axis plane j
+    const int *ap_sid;      // [n_ap] its surface id
+};
+constexpr int LAT_FAST = 1 << 30, CELL_FAST = 1 << 30, CELL_NO_NEIGHBOUR = (1 << 30) - 1;
 
-// All multi-group tables are one contiguous blob (blob, blob_doubles); the transport kernels copy it to shared
-// memory at start-up and run on rebased pointers (stage_mg) when it fits.
-struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi running chi sums
-    int G, n_mat, blob_doubles;
+struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi running chi sums.  One contiguous
+    int G, n_mat, blob_doubles;  // blob: the transport kernels copy it to shared memory when it fits
     const double *blob;
-    const double *sig_t, *sig_s, *sig_f, *nu, *nusf, *cumS, *cumchi, *src_cum;
+    int o_sig_t, o_sig_s, o_sig_f, o_nu, o_nusf, o_cumS, o_cumchi, o_src_cum;  // offsets (doubles) into the blob
 };
 
 struct CETab {
     int n_grid, n_mat, n_t, n_e, search;
     const double *grid;
-    const double *tab;    // [n_mat][n_grid][CE_ROW]: cumulative macroscopic columns, then Sigma_f in slot 7
+    const double *tab;    // [n_mat][n_grid][CE_ROW]: cumulative macroscopic columns, the grid energy in slot 6, Sigma_f in 7
     const int *ncol;      // [n_mat] number of cumulative columns (= n_nuclides + 2)
     const double *colA;   // [n_mat][CE_ROW] mass ratio A of the nuclide behind elastic column j
     const double *t_edges, *e_edges;
     const int *hash;      // [n_hash+1] bucket b -> last grid index <= lower edge of the bucket
     int hash_shift, hash_lo, n_hash;
+    const int *ehash;     // the same for the energy-bin edges of the tally: bucket -> last edge index <= its lower edge
+    int ehash_shift, ehash_lo, n_ehash;
     double nu0, nu1, watt_a, watt_b, E_min, E_max;
 };
 
 // Particle banks ("dual particle banks"): two dense structure-of-arrays banks.  A sweep reads the
-// live particles of bank[s&1] (scatter-bound ones packed at the FRONT, surface-bound ones at the BACK) and
-// k_advance writes every survivor, whole, to the front or the back of bank[(s+1)&1]: the queues hold the
-// particles themselves, so every load and store of every kernel is coalesced.
-// gl packs the group (low 16 bits) and last_surf+1 (high 16 bits); ev = pending event code (or EV_DEAD in the
-// monolithic schedule); slot = index of the particle inside its cycle / wave (= its id in eigenvalue mode, R6).
+// live particles of bank[s&1] (scatter-pending ones packed at the FRONT, surface-pending ones at the BACK) and
+// writes every survivor, whole, to the front or the back of bank[(s+1)&1]: the queues hold the particles
+// themselves, so every load and store is coalesced.
+// gl packs the group (low 16 bits) and last_surf+1 (high 16 bits); ev = pending event | segments << 12;
+// slot = index of the particle inside its cycle / wave (= its id in eigenvalue mode, R6).
 struct Bank {
     double *x, *y, *z, *ux, *uy, *uz, *E, *t;
-    int *cell, *elem, *gl, *tbin, *ev;
-    uint32_t *ctr, *slot;
+    int *cell, *elem, *gl, *tbin;
+    uint32_t *ev, *ctr, *slot;
     uint64_t *id;
 };
 
@@ -71,19 +88,8 @@ struct FisRec {
     uint64_t *id;
 };
 
-// Tail kernel, continuous energy: a thread follows its particle AND the prompt-fission subtree below it depth
-// first; pending siblings wait on a small per-thread stack in HBM.  If the stack is full the fission is left as
-// an ordinary record in the overflow part of FisRec ([M, M + over_cap)) and its children run in the next wave.
-struct StackRec {
-    double x, y, z, ux, uy, uz, E, t;
-    int cell, elem, tbin, pad;
-    unsigned long long id;
-};
-constexpr int STACK_DEPTH = 24;
-constexpr unsigned int OVER_CAP = 65536;
-
 struct QCount {  // one set per sweep (ring of RING)
-    unsigned int n_scat, n_surf, n_alive, pad;
+    unsigned int n_scat, n_surf, n_alive, err;
 };
 
 struct Trace {
@@ -102,7 +108,6 @@ struct Ctx {
     unsigned int cap;   // slots per bank
     int mode;           // 0 MG, 1 CE
     int n_tally, n_bins;
-    int geo_stage;       // 4-byte words of the geometry blob staged in shared memory (0: none)
     int mg_stage;        // doubles of the multi-group table blob staged in shared memory by every transport kernel (0: none)
     int flux_aggregate;  // global tally flavour: 1 = warp-aggregate equal bins before the atomic
     int flux_copy_mask;  // R - 1: the per-cycle tally is kept in R copies, copy = block index & mask
@@ -111,10 +116,10 @@ struct Ctx {
     unsigned long long *counters;  // [16]
     int *err;           // device error flag
     QCount *qc;          // [RING] per-sweep counts of the front / back regions
-    StackRec *stack;     // [stack_threads][STACK_DEPTH]
-    unsigned int stack_threads;
-    unsigned int *n_over;  // overflow fission records of the running wave
+    unsigned int *work;  // persistent kernel: queue head, secondaries pushed, histories ended, secondaries born
+    unsigned long long max_secondaries;  // R25a: more prompt secondaries than this = bank overflow
     Trace tr;
+    const Trace *tr_g;   // copy of tr in global memory for the out-of-line trace_event (see Acc::geo)
     unsigned long long seed;
     unsigned int cycle;
     double w0, k_prev;
@@ -141,27 +146,26 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
-// Stream (seed, id, domain, cycle): counter = (id_lo, id_hi, domain<<24 | cycle, draw/2); one block yields the
-// draws 2b (words 1:0) and 2b+1 (words 3:2); xi = ((u >> 11) + 0.5) 2^-53.  The block is kept in registers so
-// that two consecutive draws of one kernel cost one Philox evaluation.
+// Stream (seed, id, domain 0, cycle): counter = (id_lo, id_hi, cycle, draw/2); one block yields the draws 2b
+// (words 1:0) and 2b+1 (words 3:2); xi = ((u >> 11) + 0.5) 2^-53.  The block is kept in registers so that two
+// consecutive draws cost one Philox evaluation; seed and cycle are launch constants read from the Ctx at use.
+// (A buffer of the segment's 5 draws filled at one code site was measured: 3 instead of ~5 Philox evaluations per
+// warp and segment, but 8 more live registers and the selects to read it: 31.0 instead of 29.9 ms per C4 cycle.)
 struct Rng {
-    uint32_t id_lo, id_hi, w2, k0, k1, ctr, blk;
+    unsigned long long id;
+    uint32_t ctr, blk;
     uint64_t u0, u1;
-    __device__ __forceinline__ void init(unsigned long long seed, unsigned long long id, uint32_t domain, uint32_t cycle,
-                                         uint32_t ctr_)
+    __device__ __forceinline__ void init(unsigned long long id_, uint32_t ctr_)
     {
-        id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32);
-        w2 = (domain << 24) | cycle;
-        k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32);
-        ctr = ctr_;
-        blk = 0xFFFFFFFFu;
+        id = id_; ctr = ctr_; blk = 0xFFFFFFFFu;
     }
-    __device__ __forceinline__ double next()
+    __device__ __forceinline__ double next(const Ctx &c)
     {
         uint32_t b = ctr >> 1;
         if (b != blk) {
             uint32_t o0, o1, o2, o3;
-            philox4x32_10(id_lo, id_hi, w2, b, k0, k1, o0, o1, o2, o3);
+            philox4x32_10((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b, (uint32_t)c.seed, (uint32_t)(c.seed >> 32), o0, o1,
+                          o2, o3);
             u0 = ((uint64_t)o1 << 32) | o0;
             u1 = ((uint64_t)o3 << 32) | o2;
             blk = b;
@@ -171,6 +175,17 @@ struct Rng {
         return ((double)(u >> 11) + 0.5) * (1.0 / 9007199254740992.0);
     }
 };
+
+// one draw of an arbitrary stream (unit-level entry point)
+__device__ __forceinline__ double draw_at(unsigned long long seed, unsigned long long id, uint32_t domain, uint32_t cycle,
+                                          uint32_t index)
+{
+    uint32_t o0, o1, o2, o3;
+    philox4x32_10((uint32_t)id, (uint32_t)(id >> 32), (domain << 24) | cycle, index >> 1, (uint32_t)seed,
+                  (uint32_t)(seed >> 32), o0, o1, o2, o3);
+    uint64_t u = (index & 1u) ? (((uint64_t)o3 << 32) | o2) : (((uint64_t)o1 << 32) | o0);
+    return ((double)(u >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+}
 
 __device__ __forceinline__ unsigned long long child_id(unsigned long long seed, unsigned long long parent, uint32_t parent_ctr,
                                                        uint32_t j)
@@ -192,11 +207,11 @@ __device__ __forceinline__ void iso_dir(double xi_mu, double xi_phi, double &ux,
     ux = s * cp; uy = s * sp; uz = mu;
 }
 
-// first index with cum[i] > v, else n-1 (R3)
+// first index with cum[i] > v, else n-1 (R3); cum in global memory
 __device__ __forceinline__ int pick(const double *__restrict__ cum, int n, double v)
 {
     int i = 0;
-    while (i < n - 1 && !(cum[i] > v)) i++;
+    while (i < n - 1 && !(__ldg(cum + i) > v)) i++;
     return i;
 }
 
@@ -252,12 +267,29 @@ __device__ __forceinline__ int grid_index(const CETab &ce, double E)
     return ce.search ? grid_index_hash(ce, E) : grid_index_binary(ce, E);
 }
 
+// tally energy bin (R24: the largest b with e_edges[b] <= E, clamped): the same exact bucket key narrows the
+// bisection to the one or two edges that can fall in the bucket; equals edge_bin(e_edges, n_e, E) bit for bit
+__device__ __forceinline__ int energy_bin(const CETab &ce, double E)
+{
+    if (E < __ldg(ce.e_edges)) return 0;
+    if (E >= __ldg(ce.e_edges + ce.n_e)) return ce.n_e - 1;
+    int b = (int)(__double_as_longlong(E) >> ce.ehash_shift) - ce.ehash_lo;
+    int lo = __ldg(ce.ehash + b), hi = __ldg(ce.ehash + b + 1) + 1;
+    if (hi > ce.n_e) hi = ce.n_e;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(ce.e_edges + mid) <= E) lo = mid; else hi = mid;
+    }
+    return lo < ce.n_e - 1 ? lo : ce.n_e - 1;
+}
+
 // ------------------------------------------------------------------ geometry (R11-R14)
+struct Particle;
 __device__ __forceinline__ double surf_f(const Geo &G, int s, double x, double y, double z)
 {
     const double *q = G.surf_param + 4 * s;
-    int t = G.surf_type[s];
-    double q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3];
+    int t = __ldg(G.surf_type + s);
+    double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2), q3 = __ldg(q + 3);
     switch (t) {
     case 0: return x - q0;
     case 1: return y - q0;
@@ -275,8 +307,8 @@ __device__ __forceinline__ void surf_normal(const Geo &G, int s, double x, doubl
                                             double &nz)
 {
     const double *q = G.surf_param + 4 * s;
-    int t = G.surf_type[s];
-    double q0 = q[0], q1 = q[1], q2 = q[2];
+    int t = __ldg(G.surf_type + s);
+    double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2);
     nx = ny = nz = 0.0;
     switch (t) {
     case 0: nx = 1.0; break;
@@ -306,21 +338,21 @@ __device__ __forceinline__ int sense_of(const Geo &G, int s, double x, double y,
 __device__ __forceinline__ int find_cell(const Geo &G, int univ, double x, double y, double z, double ux, double uy,
                                          double uz, int last)
 {
-    int c1 = G.uco[univ + 1];
-    for (int c = G.uco[univ]; c < c1; c++) {
+    int c1 = __ldg(G.uco + univ + 1);
+    for (int c = __ldg(G.uco + univ); c < c1; c++) {
         bool ok = true;
-        int k1 = G.cso[c + 1];
-        for (int k = G.cso[c]; k < k1; k++)
-            if (sense_of(G, G.csi[k], x, y, z, ux, uy, uz, last) != G.css[k]) { ok = false; break; }
+        int k1 = __ldg(G.cso + c + 1);
+        for (int k = __ldg(G.cso + c); k < k1; k++)
+            if (sense_of(G, __ldg(G.csi + k), x, y, z, ux, uy, uz, last) != __ldg(G.css + k)) { ok = false; break; }
         if (ok) return c;
     }
     return -1;
 }
 
-// lattice element -> (ix, iy) without an integer division
+// lattice element -> (ix, iy) without an integer division (a one-column lattice has iy = elem)
 __device__ __forceinline__ void elem_xy(const Geo &G, int elem, int &ix, int &iy)
 {
-    iy = (int)__umulhi((unsigned int)elem, G.lat_magic);
+    iy = G.lat_nx == 1 ? elem : (int)__umulhi((unsigned int)elem, G.lat_magic);
     ix = elem - iy * G.lat_nx;
 }
 
@@ -333,6 +365,8 @@ __device__ __forceinline__ void local_xy(const Geo &G, int elem, double x, doubl
     yl = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
 }
 
+__device__ __forceinline__ int elem_universe(const Geo &G, int elem) { return __ldg(&G.lat_info[elem].x) & (LAT_FAST - 1); }
+
 // full point location from the root universe.  cell = material cell (root cell, or the local cell inside
 // lattice element elem); returns false if the point is in no cell.
 __device__ __forceinline__ bool locate(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int last,
@@ -341,14 +375,14 @@ __device__ __forceinline__ bool locate(const Geo &G, double x, double y, double 
     elem = -1;
     cell = find_cell(G, 0, x, y, z, ux, uy, uz, last);
     if (cell < 0) return false;
-    if (G.cft[cell] == 1) {
+    if (__ldg(G.cft + cell) == 1) {
         int ix = (int)floor((x - G.lat_x0) / G.lat_px);
         int iy = (int)floor((y - G.lat_y0) / G.lat_py);
         if (ix < 0 || iy < 0 || ix >= G.lat_nx || iy >= G.lat_ny) { cell = -1; return false; }
         elem = iy * G.lat_nx + ix;
         double xl, yl;
         local_xy(G, elem, x, y, xl, yl);
-        cell = find_cell(G, __ldg(G.lat_univ + elem), xl, yl, z, ux, uy, uz, last);
+        cell = find_cell(G, elem_universe(G, elem), xl, yl, z, ux, uy, uz, last);
         if (cell < 0) return false;
     }
     return true;
@@ -361,8 +395,8 @@ __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, d
 {
     const double INF = __longlong_as_double(0x7ff0000000000000LL);
     const double *q = G.surf_param + 4 * s;
-    int t = G.surf_type[s];
-    double q0 = q[0], q1 = q[1], q2 = q[2], q3 = q[3];
+    int t = __ldg(G.surf_type + s);
+    double q0 = __ldg(q), q1 = __ldg(q + 1), q2 = __ldg(q + 2), q3 = __ldg(q + 3);
     if (t <= 3) {
         if (on) return INF;
         double d;
@@ -406,28 +440,28 @@ __device__ __forceinline__ double surf_distance(const Geo &G, int s, double x, d
     return d > 0.0 ? d : INF;
 }
 
-// nearest boundary of the current location; candidate order: enclosing-cell surfaces, local-cell surfaces,
-// lattice walls -x,+x,-y,+y; ties keep the first (R12, R14).  hit = surface id, or n_surf+k for wall k.
-__device__ __forceinline__ double nearest(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int cell,
-                                          int elem, int last, int &hit, unsigned int root_mask = 0xffffffffu)
+// nearest boundary of the current location, generic path; candidate order: enclosing-cell surfaces, local-cell
+// surfaces, lattice walls -x,+x,-y,+y; ties keep the first (R12, R14).  hit = surface id, or n_surf+k for wall k.
+__device__ __noinline__ double nearest(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int cell,
+                                       int elem, int last, int &hit, unsigned int root_mask)
 {
     double best = __longlong_as_double(0x7ff0000000000000LL);
     hit = -1;
     const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;  // +-inf when the component is zero: guarded at use
     int c0 = elem >= 0 ? G.lat_cell : cell;
-    int k1 = G.cso[c0 + 1];
+    int k1 = __ldg(G.cso + c0 + 1);
     if (root_mask) {
         // candidates in list order (ties keep the first, R12): the listed bits, then anything past the 32nd surface
-        const int k0 = G.cso[c0];
+        const int k0 = __ldg(G.cso + c0);
         unsigned int m = k1 - k0 >= 32 ? root_mask : root_mask & ((1u << (k1 - k0)) - 1u);
         while (m) {
-            int s = G.csi[k0 + __ffs(m) - 1];
+            int s = __ldg(G.csi + k0 + __ffs(m) - 1);
             m &= m - 1u;
             double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
         for (int k = k0 + 32; k < k1; k++) {
-            int s = G.csi[k];
+            int s = __ldg(G.csi + k);
             double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
@@ -437,9 +471,9 @@ __device__ __forceinline__ double nearest(const Geo &G, double x, double y, doub
         elem_xy(G, elem, ix, iy);
         const double xl = x - (G.lat_x0 + (ix + 0.5) * G.lat_px);
         const double yl = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
-        k1 = G.cso[cell + 1];
-        for (int k = G.cso[cell]; k < k1; k++) {
-            int s = G.csi[k];
+        k1 = __ldg(G.cso + cell + 1);
+        for (int k = __ldg(G.cso + cell); k < k1; k++) {
+            int s = __ldg(G.csi + k);
             double d = surf_distance(G, s, xl, yl, z, ux, uy, uz, s == last, inv_ux, inv_uy);
             if (d < best) { best = d; hit = s; }
         }
@@ -464,18 +498,84 @@ __device__ __forceinline__ double nearest(const Geo &G, double x, double y, doub
     return best;
 }
 
+// Straight-line path (see Geo): per axis ONE candidate, named by the location's boundary code for the direction of
+// flight (lattice wall ahead, or an axis plane), plus at most one z-cylinder (centred on the lattice element, or in
+// global coordinates outside a lattice).  Same formulas and the same candidate order as `nearest` (planes of the
+// cell, cylinder, lattice walls); no loops, no surface-type switch: all lanes do the same work.
+__device__ __forceinline__ double nearest_fast(const Geo &G, int codes_xy, int codes_z, int cyl, double x, double y, double z,
+                                               double ux, double uy, double uz, int elem, int last, int &hit)
+{
+    const double INF = __longlong_as_double(0x7ff0000000000000LL);
+    int ix = 0, iy = 0;
+    double cx0 = 0.0, cy0 = 0.0;  // centre of the lattice element (origin of the cylinder's coordinates)
+    if (elem >= 0) {
+        elem_xy(G, elem, ix, iy);
+        cx0 = G.lat_x0 + (ix + 0.5) * G.lat_px;
+        cy0 = G.lat_y0 + (iy + 0.5) * G.lat_py;
+    }
+    const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;
+    const bool xp = ux > 0.0, yp = uy > 0.0, zp = uz > 0.0;
+    const int cx = (codes_xy >> (xp ? 8 : 0)) & 255, cy = (codes_xy >> (yp ? 24 : 16)) & 255, cz = (codes_z >> (zp ? 8 : 0)) & 255;
+    double px = G.lat_x0 + (ix + (xp ? 1 : 0)) * G.lat_px, py = G.lat_y0 + (iy + (yp ? 1 : 0)) * G.lat_py, pz = 0.0;
+    int hx = G.n_surf + (xp ? 1 : 0), hy = G.n_surf + (yp ? 3 : 2), hz = -1;
+    if (cx >= 2) { px = __ldg(G.ap_pos + cx - 2); hx = __ldg(G.ap_sid + cx - 2); }
+    if (cy >= 2) { py = __ldg(G.ap_pos + cy - 2); hy = __ldg(G.ap_sid + cy - 2); }
+    if (cz >= 2) { pz = __ldg(G.ap_pos + cz - 2); hz = __ldg(G.ap_sid + cz - 2); }
+    double dx = (px - x) * inv_ux, dy = (py - y) * inv_uy, dz = INF;
+    if (cz >= 2 && uz != 0.0 && hz != last) { dz = (pz - z) / uz; if (!(dz > 0.0)) dz = INF; }
+    if (cx == 0 || ux == 0.0 || hx == last || !(dx > 0.0)) dx = INF;
+    if (cy == 0 || uy == 0.0 || hy == last || !(dy > 0.0)) dy = INF;
+    double dc = INF;
+    if (cyl >= 0) {
+        const double *q = G.surf_param + 4 * cyl;
+        const double da = x - cx0 - __ldg(q);
+        const double db = y - cy0 - __ldg(q + 1);
+        const double r = __ldg(q + 2);
+        const double a = ux * ux + uy * uy, k = da * ux + db * uy;
+        // numerator of the root, then ONE division for every lane (on the cylinder: c is exactly 0, only the far root
+        // -2k / a, only when heading inward, R13)
+        double num = -1.0;
+        if (cyl == last) { if (k < 0.0) num = -2.0 * k; }
+        else {
+            const double cc = da * da + db * db - r * r;
+            const double disc = k * k - a * cc;
+            if (disc >= 0.0) {
+                const double sq = sqrt(disc);
+                num = cc < 0.0 ? sq - k : -k - sq;
+            }
+        }
+        if (a != 0.0 && num > 0.0) {
+            dc = num / a;
+            if (!(dc > 0.0)) dc = INF;
+        }
+    }
+    // candidate order (ties keep the first, R12): the cell's planes, the cylinder, lattice walls
+    double best = INF;
+    hit = -1;
+    if (cx >= 2 && dx < best) { best = dx; hit = hx; }
+    if (cy >= 2 && dy < best) { best = dy; hit = hy; }
+    if (dz < best) { best = dz; hit = hz; }
+    if (dc < best) { best = dc; hit = cyl; }
+    if (cx == 1 && dx < best) { best = dx; hit = hx; }
+    if (cy == 1 && dy < best) { best = dy; hit = hy; }
+    return best;
+}
+
 __device__ __forceinline__ bool surface_in_cell(const Geo &G, int c, int s)
 {
-    int k1 = G.cso[c + 1];
-    for (int k = G.cso[c]; k < k1; k++)
-        if (G.csi[k] == s) return true;
+    int k1 = __ldg(G.cso + c + 1);
+    for (int k = __ldg(G.cso + c); k < k1; k++)
+        if (__ldg(G.csi + k) == s) return true;
     return false;
 }
 
 // ------------------------------------------------------------------ particle in registers
 struct Particle {
     double x, y, z, ux, uy, uz, E, t;
+    double v;       // continuous energy: speed, union-grid index and tally energy bin of E (they change only when E
+    int gi, ebin;   // does: at birth and in a scatter), kept with the particle instead of recomputed every segment
     int cell, elem, g, last, tbin;
+    unsigned int pend, nseg;
     unsigned long long id;
 };
 
@@ -485,14 +585,24 @@ struct Particle {
 struct Acc {
     double knum;
     unsigned int *s_ev;  // [16] in shared memory
+    const double *mgs;   // multi-group table blob: the shared-memory copy, or the global blob when it does not fit
+    const Geo *geo;      // the block's shared-memory copy of the Geo descriptor: what the out-of-line (generic-path)
+                         // functions read, so that the kernel parameter block never has to be copied to a stack
+    bool tracing;        // launch-uniform: a trace buffer is attached
     __device__ __forceinline__ void clear(unsigned int *ev) { knum = 0.0; s_ev = ev; }
 };
 
 __device__ __forceinline__ void count_event(Acc &acc, int ev) { atomicAdd(acc.s_ev + ev, 1u); }
 
+// the quantities of a continuous-energy particle that depend on E alone (R19, R23, R24); call whenever E is set
+__device__ __forceinline__ void ce_energy_state(const CETab &ce, Particle &p)
+{
+    p.gi = grid_index(ce, p.E);
+    p.ebin = energy_bin(ce, p.E);
+    p.v = speed_of(p.E);
+}
+
 enum { ADV_DEAD = 0, ADV_SCATTER = 1, ADV_SURFACE = 2, ADV_FISSION = 3 };
-constexpr int HIT_TIME_EDGE = 0x3fff0000;  // aux code of a time-edge event in the surface queue
-constexpr int HIT_NEWBORN = 0x3fff0001;    // aux code of a prompt secondary just written to the back region
 
 struct TraceRec {  // = mcdc_trace_rec
     unsigned long long id;
@@ -501,23 +611,23 @@ struct TraceRec {  // = mcdc_trace_rec
     double x, y, z, d, E, t;
 };
 
-__device__ __forceinline__ void trace_event(const Ctx &c, const Particle &p, int ev, int cell0, int elem0, int surf, int gi,
-                                            double d, double E)
+__device__ __noinline__ void trace_event(const Trace &tr, unsigned int cycle, int lat_cell, unsigned long long id, double x,
+                                         double y, double z, double t, int ev, int cell0, int elem0, int surf, int gi, double d,
+                                         double E)
 {
-    if (!c.tr.rec) return;
-    unsigned long long rel = p.id - c.tr.first;
-    if (p.id < c.tr.first || rel >= c.tr.n_ids) return;
-    unsigned long long slot = (unsigned long long)c.cycle * c.tr.n_ids + rel;
-    if (slot >= c.tr.cap_slots) return;
-    unsigned int seq = c.tr.count[slot]++;
-    if (seq >= c.tr.max_events) return;
-    TraceRec *r = (TraceRec *)c.tr.rec + slot * c.tr.max_events + seq;
-    r->id = p.id; r->cycle = c.cycle; r->seq = seq; r->ev = ev;
-    r->c0 = elem0 >= 0 ? c.geo.lat_cell : cell0;
+    unsigned long long rel = id - tr.first;
+    if (id < tr.first || rel >= tr.n_ids) return;
+    unsigned long long slot = (unsigned long long)cycle * tr.n_ids + rel;
+    if (slot >= tr.cap_slots) return;
+    unsigned int seq = tr.count[slot]++;
+    if (seq >= tr.max_events) return;
+    TraceRec *r = (TraceRec *)tr.rec + slot * tr.max_events + seq;
+    r->id = id; r->cycle = cycle; r->seq = seq; r->ev = ev;
+    r->c0 = elem0 >= 0 ? lat_cell : cell0;
     r->elem = elem0;
     r->c1 = elem0 >= 0 ? cell0 : -1;
     r->surf = surf; r->gi = gi;
-    r->x = p.x; r->y = p.y; r->z = p.z; r->d = d; r->E = E; r->t = p.t;
+    r->x = x; r->y = y; r->z = z; r->d = d; r->E = E; r->t = t;
 }
 
 // tally flavours: FLUX_PRIVATE = one shared-memory column per thread (tiny tallies: no atomics at all until
@@ -538,7 +648,6 @@ __device__ __forceinline__ void flux_add(const Ctx &c, double *s_flux, long long
         if (grp == (1u << lane)) {
             atomicAdd(dst, v);
         } else {
-            // tree over the ranks inside the group: rank r receives from rank r + step
             double sum = v;
             unsigned int rest = grp & ~(1u << leader);
             // the leader walks the other members (groups are small except in tiny-tally problems, which use
@@ -554,36 +663,44 @@ __device__ __forceinline__ void flux_add(const Ctx &c, double *s_flux, long long
     }
 }
 
+__device__ __forceinline__ double mgv(const Acc &acc, int off) { return acc.mgs[off]; }
+
 // One segment up to and including the event decision (steps a2/a3, a5, a6, a7 of SURVEY.md 8a and the
 // reaction choice of a8): cross sections, distance to collision, nearest boundary, time edge, move, tallies.
-// Returns ADV_*; aux = elastic column (scatter), hit code (surface / time edge) or number of children (fission).
+// Returns ADV_*; the event that still has to be finished is left in p.pend (scatter column, hit code, time edge);
+// aux = number of children (fission).  Lanes in a LAT_FAST lattice element take the straight-line geometry path; a
+// warp whose lanes all do (the normal case inside a pin lattice) never enters the generic loops.
 template <bool CE, bool PRIVATE>
-__device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int &aux, Acc &acc,
-                                       double *s_flux, const Geo &G)
+__device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int &aux, Acc &acc, double *s_flux)
 {
+    const Geo &G = c.geo;
     const int cell0 = p.cell, elem0 = p.elem;
-    const int mat = G.cfill[p.cell];
-    int bin = G.cbin[p.cell];
-    unsigned int root_mask = 0xffffffffu;
+    const int mat = __ldg(G.cfill + p.cell);
+    int bin = __ldg(G.cbin + p.cell);
+    int4 li;  // boundary codes of the location (z, w), fast-path flag, cylinder
+    int cyl;
     if (p.elem >= 0) {
-        int lb = __ldg(G.lat_bin + p.elem);
-        root_mask = (lb & LAT_ROOT_FLAG) ? __ldg(G.lat_rmask + p.elem) : 0u;
-        bin += lb & (LAT_ROOT_FLAG - 1);
+        li = __ldg(G.lat_info + p.elem);
+        bin += li.y;
+        cyl = __ldg(&G.ufast[li.x & (LAT_FAST - 1)].y);
+    } else {
+        li = __ldg(G.cell_info + p.cell);
+        cyl = li.y;
     }
 
     double sig_t, nusf, cum[MAX_CE_COL];
     int gi, ncol = 0;
     if (!CE) {
         gi = p.g;
-        sig_t = mg.sig_t[mat * mg.G + p.g];
-        nusf = mg.nusf[mat * mg.G + p.g];
+        sig_t = mgv(acc, c.mg.o_sig_t + mat * c.mg.G + p.g);
+        nusf = mgv(acc, c.mg.o_nusf + mat * c.mg.G + p.g);
     } else {
-        gi = grid_index(c.ce, p.E);
-        double g0 = __ldg(c.ce.grid + gi), g1 = __ldg(c.ce.grid + gi + 1);
-        double f = (p.E - g0) / (g1 - g0);
+        gi = p.gi;  // union-grid index of E, found when E last changed (ce_energy_state)
         const double2 *r0 = (const double2 *)(c.ce.tab + ((size_t)mat * c.ce.n_grid + gi) * CE_ROW);
         double2 a0 = __ldg(r0), a1 = __ldg(r0 + 1), a2 = __ldg(r0 + 2), a3 = __ldg(r0 + 3);
         double2 b0 = __ldg(r0 + 4), b1 = __ldg(r0 + 5), b2 = __ldg(r0 + 6), b3 = __ldg(r0 + 7);
+        const double g0 = a3.x, g1 = b3.x;  // the rows carry their grid energies (slot 6)
+        double f = (p.E - g0) / (g1 - g0);
         cum[0] = a0.x + f * (b0.x - a0.x); cum[1] = a0.y + f * (b0.y - a0.y);
         cum[2] = a1.x + f * (b1.x - a1.x); cum[3] = a1.y + f * (b1.y - a1.y);
         cum[4] = a2.x + f * (b2.x - a2.x); cum[5] = a2.y + f * (b2.y - a2.y);
@@ -597,12 +714,17 @@ __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &
     }
 
     // candidate distances: collision (one draw every segment), boundary, time edge (R12)
-    double d_coll = -log(rng.next()) / sig_t;
+    double d_coll = -log(rng.next(c)) / sig_t;
     int hit;
-    double d_surf = nearest(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_mask);
+    double d_surf;
+    if (li.x & LAT_FAST) d_surf = nearest_fast(G, li.z, li.w, cyl, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.elem, p.last, hit);
+    else {
+        unsigned int root_mask = p.elem >= 0 ? __ldg(G.lat_rmask + p.elem) : 0xffffffffu;
+        d_surf = nearest(*acc.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_mask);
+    }
     double v = 0.0, d_time = __longlong_as_double(0x7ff0000000000000LL);
     if (CE) {
-        v = speed_of(p.E);
+        v = p.v;
         d_time = v * (__ldg(c.ce.t_edges + p.tbin + 1) - p.t);
     }
     int kind;
@@ -615,78 +737,88 @@ __device__ __forceinline__ int advance(const Ctx &c, const MGTab &mg, Particle &
     p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
     const double E_flight = CE ? p.E : 0.0;
     long long tix;
-    if (!CE) tix = (long long)bin * mg.G + p.g;
+    if (!CE) tix = (long long)bin * c.mg.G + p.g;
     else {
-        tix = ((long long)bin * c.ce.n_t + p.tbin) * c.ce.n_e + edge_bin(c.ce.e_edges, c.ce.n_e, p.E);
+        tix = ((long long)bin * c.ce.n_t + p.tbin) * c.ce.n_e + p.ebin;
         if (kind == 2) p.t = __ldg(c.ce.t_edges + p.tbin + 1); else p.t += d / v;
     }
     flux_add<PRIVATE>(c, s_flux, tix, c.w0 * d);
     acc.knum += c.w0 * d * nusf;
 
-    int ev, code;
+    int ev, code, surf = -1;
+    p.pend = PEND_NONE;
     if (kind == 0) {
         p.last = -1;
-        double uu = rng.next() * sig_t;
+        double uu = rng.next(c) * sig_t;
         if (!CE) {
-            double sig_s = mg.sig_s[mat * mg.G + p.g], sig_f = mg.sig_f[mat * mg.G + p.g];
-            if (uu < sig_s) { ev = 1; code = ADV_SCATTER; aux = 0; }
+            double sig_s = mgv(acc, c.mg.o_sig_s + mat * c.mg.G + p.g), sig_f = mgv(acc, c.mg.o_sig_f + mat * c.mg.G + p.g);
+            if (uu < sig_s) { ev = 1; code = ADV_SCATTER; p.pend = PEND_SCATTER; }
             else if (uu < sig_s + sig_f) {
                 ev = 2; code = ADV_FISSION;
-                aux = (int)floor(c.w0 * mg.nu[mat * mg.G + p.g] / c.k_prev + rng.next());
+                aux = (int)floor(c.w0 * mgv(acc, c.mg.o_nu + mat * c.mg.G + p.g) / c.k_prev + rng.next(c));
             } else { ev = 3; code = ADV_DEAD; }
         } else {
             int r = 0;
             while (r < ncol - 1 && !(cum[r] > uu)) r++;
-            if (r < ncol - 2) { ev = 1; code = ADV_SCATTER; aux = r; }
+            if (r < ncol - 2) { ev = 1; code = ADV_SCATTER; p.pend = PEND_SCATTER | (unsigned int)r; }
             else if (r == ncol - 2) {
                 ev = 2; code = ADV_FISSION;
                 double nu = c.ce.nu0 + c.ce.nu1 * (p.E * 1e-6);
-                aux = (int)floor(c.w0 * nu + rng.next());
+                aux = (int)floor(c.w0 * nu + rng.next(c));
             } else { ev = 3; code = ADV_DEAD; }
         }
-        trace_event(c, p, ev, cell0, elem0, -1, gi, d, E_flight);
     } else if (kind == 1) {
-        if (hit >= G.n_surf) { ev = 7; code = ADV_SURFACE; aux = hit; }
+        surf = hit;
+        if (hit >= G.n_surf) { ev = 7; code = ADV_SURFACE; p.pend = (unsigned int)hit; }
         else {
-            int bc = G.surf_bc[hit];
+            int bc = __ldg(G.surf_bc + hit);
             if (bc == 2) { ev = 6; code = ADV_DEAD; atomicAdd(c.scal + 1, c.w0); }
-            else { ev = bc == 1 ? 5 : 4; code = ADV_SURFACE; aux = hit; }
+            else { ev = bc == 1 ? 5 : 4; code = ADV_SURFACE; p.pend = (unsigned int)hit; }
         }
-        trace_event(c, p, ev, cell0, elem0, hit, gi, d, E_flight);
     } else {
         // time edge: the particle has moved off whatever surface it sat on (R11)
         p.tbin++;
         p.last = -1;
         if (p.tbin == c.ce.n_t) { ev = 9; code = ADV_DEAD; }
-        else { ev = 8; code = ADV_SURFACE; aux = HIT_TIME_EDGE; }
-        trace_event(c, p, ev, cell0, elem0, -1, gi, d, E_flight);
+        else { ev = 8; code = ADV_SURFACE; p.pend = PEND_TIME; }
     }
+    if (acc.tracing)
+        trace_event(*c.tr_g, c.cycle, G.lat_cell, p.id, p.x, p.y, p.z, CE ? p.t : 0.0, ev, cell0, elem0, surf, gi, d, E_flight);
     count_event(acc, ev);
+    p.nseg++;
+    if (code != ADV_DEAD && code != ADV_FISSION && p.nseg >= MAX_SEGMENTS) {  // lost-particle guard (R11)
+        code = ADV_DEAD;
+        count_event(acc, 10);
+        atomicExch(c.err, -4);
+    }
     return code;
 }
 
 // Scatter event (a8).  MG: new group from the cumulative scatter row, isotropic direction (1 + 2 draws).
 // CE: elastic off a target at rest with mass ratio A: mu_cm, azimuth (2 draws), rotation, energy clamp (R19, R21).
 template <bool CE>
-__device__ __forceinline__ void do_scatter(const Ctx &c, const MGTab &mg, Particle &p, Rng &rng, int col, const Geo &G)
+__device__ __forceinline__ void do_scatter(const Ctx &c, const Acc &acc, Particle &p, Rng &rng, int col)
 {
-    const int mat = G.cfill[p.cell];
+    const int mat = __ldg(c.geo.cfill + p.cell);
     if (!CE) {
-        const int G = mg.G;
-        double sig_s = mg.sig_s[mat * G + p.g];
-        double vv = rng.next() * sig_s;
-        p.g = pick(mg.cumS + (mat * G + p.g) * G, G, vv);
-        double a = rng.next(), b = rng.next();
+        const int G = c.mg.G;
+        double sig_s = mgv(acc, c.mg.o_sig_s + mat * G + p.g);
+        double vv = rng.next(c) * sig_s;
+        const int row = c.mg.o_cumS + (mat * G + p.g) * G;
+        int i = 0;
+        while (i < G - 1 && !(mgv(acc, row + i) > vv)) i++;
+        p.g = i;
+        double a = rng.next(c), b = rng.next(c);
         iso_dir(a, b, p.ux, p.uy, p.uz);
     } else {
         double A = __ldg(c.ce.colA + mat * CE_ROW + col);
-        double mu_cm = 2.0 * rng.next() - 1.0;
+        double mu_cm = 2.0 * rng.next(c) - 1.0;
         double den = A * A + 2.0 * A * mu_cm + 1.0;
         double mu = 0.0;
         if (den > 0.0) mu = (1.0 + A * mu_cm) / sqrt(den);
         double En = p.E * den / ((A + 1.0) * (A + 1.0));
         double sp, cp;
-        sincospi(2.0 * rng.next(), &sp, &cp);
+        sincospi(2.0 * rng.next(c), &sp, &cp);
         double s2 = 1.0 - mu * mu;
         double s = s2 > 0.0 ? sqrt(s2) : 0.0;
         double a2 = 1.0 - p.uz * p.uz;
@@ -704,15 +836,15 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const MGTab &mg, Partic
         if (En < c.ce.E_min) En = c.ce.E_min;
         if (En > c.ce.E_max) En = c.ce.E_max;
         p.E = En;
+        ce_energy_state(c.ce, p);
     }
     p.last = -1;
 }
 
-// Surface event (a9): lattice wall -> neighbour element; reflect; transmit -> neighbour cell by the side being
-// entered (R11, R14).  Time-edge events need no geometry work.  Returns false if the particle got lost.
-__device__ __forceinline__ bool do_surface(const Geo &G, Particle &p, int hit)
+// Surface event (a9), generic path: lattice wall -> neighbour element; reflect; transmit -> neighbour cell by the
+// side being entered (R11, R14).  Returns false if the particle got lost.
+__device__ __noinline__ bool do_surface(const Geo &G, Particle &p, int hit)
 {
-    if (hit == HIT_TIME_EDGE) return true;
     if (hit >= G.n_surf) {
         int w = hit - G.n_surf;
         int ix, iy;
@@ -722,16 +854,16 @@ __device__ __forceinline__ bool do_surface(const Geo &G, Particle &p, int hit)
         p.last = -1;
         double xl, yl;
         local_xy(G, p.elem, p.x, p.y, xl, yl);
-        p.cell = find_cell(G, __ldg(G.lat_univ + p.elem), xl, yl, p.z, p.ux, p.uy, p.uz, -1);
+        p.cell = find_cell(G, elem_universe(G, p.elem), xl, yl, p.z, p.ux, p.uy, p.uz, -1);
         return p.cell >= 0;
     }
-    int bc = G.surf_bc[hit];
+    int bc = __ldg(G.surf_bc + hit);
     bool local = p.elem >= 0 && !surface_in_cell(G, G.lat_cell, hit);
     double xl = p.x, yl = p.y;
     if (local) local_xy(G, p.elem, p.x, p.y, xl, yl);
     p.last = hit;
     if (bc == 1) {
-        int t = G.surf_type[hit];
+        int t = __ldg(G.surf_type + hit);
         if (t == 0) p.ux = -p.ux;
         else if (t == 1) p.uy = -p.uy;
         else if (t == 2) p.uz = -p.uz;
@@ -746,10 +878,78 @@ __device__ __forceinline__ bool do_surface(const Geo &G, Particle &p, int hit)
         return true;
     }
     if (local) {
-        p.cell = find_cell(G, __ldg(G.lat_univ + p.elem), xl, yl, p.z, p.ux, p.uy, p.uz, hit);
+        p.cell = find_cell(G, elem_universe(G, p.elem), xl, yl, p.z, p.ux, p.uy, p.uz, hit);
         return p.cell >= 0;
     }
     return locate(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, hit, p.cell, p.elem);
+}
+
+// Surface event from inside a LAT_FAST element whose event is one of: lattice wall into another LAT_FAST element,
+// the universe's own z-cylinder (transmit), a reflecting axis plane of the enclosing cell.  Returns 0 if the event
+// is none of these (the caller then takes the generic path), 1 done, -1 lost.
+__device__ __forceinline__ int do_surface_fast(const Geo &G, Particle &p, int hit)
+{
+    if (p.elem < 0) {  // a CELL_FAST cell outside a lattice: its cylinder (transmit) or a reflecting axis plane
+        const int4 ci = __ldg(G.cell_info + p.cell);
+        if (hit == ci.y) {
+            const int nb = ci.x & CELL_NO_NEIGHBOUR;
+            if (__ldg(G.surf_bc + hit) != 0 || nb == CELL_NO_NEIGHBOUR) return 0;
+            p.cell = nb;
+            p.last = hit;
+            return 1;
+        }
+        if (__ldg(G.surf_bc + hit) == 1) {
+            int t = __ldg(G.surf_type + hit);
+            if (t > 2) return 0;
+            if (t == 0) p.ux = -p.ux; else if (t == 1) p.uy = -p.uy; else p.uz = -p.uz;
+            p.last = hit;
+            return 1;
+        }
+        return 0;
+    }
+    if (hit >= G.n_surf) {
+        int w = hit - G.n_surf;
+        int e2 = p.elem + (w == 0 ? -1 : w == 1 ? 1 : w == 2 ? -G.lat_nx : G.lat_nx);
+        const int4 l2 = __ldg(G.lat_info + e2);
+        if (!(l2.x & LAT_FAST)) return 0;
+        const int4 uf = __ldg(G.ufast + (l2.x & (LAT_FAST - 1)));
+        p.elem = e2;
+        p.last = -1;
+        int cell = uf.z;
+        if (uf.y >= 0) {
+            double xl, yl;
+            local_xy(G, e2, p.x, p.y, xl, yl);
+            const double *q = G.surf_param + 4 * uf.y;
+            double da = xl - __ldg(q), db = yl - __ldg(q + 1), r = __ldg(q + 2);
+            cell = (da * da + db * db - r * r > 0.0) ? uf.w : uf.z;
+        }
+        p.cell = cell;
+        return 1;
+    }
+    const int4 uf = __ldg(G.ufast + elem_universe(G, p.elem));
+    if (hit == uf.y) {
+        if (__ldg(G.surf_bc + hit) != 0) return 0;
+        double xl, yl;
+        local_xy(G, p.elem, p.x, p.y, xl, yl);
+        const double *q = G.surf_param + 4 * hit;
+        double nx = xl - __ldg(q), ny = yl - __ldg(q + 1);
+        p.last = hit;
+        p.cell = (p.ux * nx + p.uy * ny > 0.0) ? uf.w : uf.z;  // the side being entered (R11)
+        return 1;
+    }
+    if (__ldg(G.surf_bc + hit) == 1) {
+        int t = __ldg(G.surf_type + hit);
+        if (t > 2) return 0;
+        if (t == 0) p.ux = -p.ux; else if (t == 1) p.uy = -p.uy; else p.uz = -p.uz;
+        p.last = hit;
+        return 1;
+    }
+    return 0;
+}
+
+__device__ __forceinline__ bool location_is_fast(const Geo &G, int cell, int elem)
+{
+    return ((elem >= 0 ? __ldg(&G.lat_info[elem].x) : __ldg(&G.cell_info[cell].x)) & LAT_FAST) != 0;
 }
 
 // Watt spectrum, rejection-free (R22); MeV
@@ -758,6 +958,21 @@ __device__ __forceinline__ double watt(double a, double b, double x1, double x2,
     double cs = cospi(0.5 * x3);
     double W = -a * (log(x1) + log(x2) * cs * cs);
     return W + 0.25 * a * a * b + (2.0 * x4 - 1.0) * sqrt(a * a * b * W);
+}
+
+// Finish the event a banked particle is waiting on (scatter: a8; surface / lattice wall: a9; time edge: nothing).
+// Returns false if the particle got lost.
+template <bool CE>
+__device__ __forceinline__ bool finish_pending(const Ctx &c, const Acc &acc, Particle &p, Rng &rng)
+{
+    const unsigned int pend = p.pend;
+    p.pend = PEND_NONE;
+    if (pend >= PEND_TIME) return true;
+    if (pend >= PEND_SCATTER) { do_scatter<CE>(c, acc, p, rng, (int)(pend & 7u)); return true; }
+    int r = 0;
+    if (location_is_fast(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)pend);
+    if (r == 0) r = do_surface(*acc.geo, p, (int)pend) ? 1 : -1;
+    return r > 0;
 }
 
 }  // namespace mcdc

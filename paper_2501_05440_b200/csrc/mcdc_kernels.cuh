@@ -1,17 +1,22 @@
 // mcdc_kernels.cuh -- the kernels of the event-based transport loop.
 //
-// Event schedule (default): per sweep three kernels regroup the live particles by next event
-//   k_advance  (a2/a3 XS lookup, a5 nearest boundary, a6 distance to collision, a7 move + tallies, reaction
-//               choice) reads the live particles of bank[s&1] and writes every survivor, whole, into
-//               bank[(s+1)&1]: scatter events packed at the FRONT, surface / lattice / time-edge events at the
-//               BACK, positions from ballot + prefix-sum compaction with one atomic per block and queue (a11);
-//   k_scatter  (a8) over the front region, in place;   k_surface (a9) over the back region, in place.
-// The queues are the particles themselves (PAPER.md:55 dual banks), so all bank traffic is coalesced.
-// Fission and capture end a history inside k_advance; a fission leaves a record at the parent's slot and the
-// children are produced at the end of the cycle by count -> exclusive scan -> write (a10/a12), which yields
-// the bank sorted by (parent id, child index) without atomics or a sort.  k_segment is the paper's monolithic
-// design: one whole segment for every bank slot per launch, no compaction.  k_finish ends the
-// last few histories in registers.
+// A banked particle carries the event it is waiting on (Bank::ev: scatter, surface / lattice wall, time edge or
+// nothing).  Event schedule (default), one kernel per sweep while the population is large:
+//   k_sweep    reads the live particles of bank[s&1] -- scatter-pending ones are packed at the FRONT, surface-pending
+//              ones at the BACK, so warps are homogeneous in the event they finish -- finishes that event (a8 / a9),
+//              then runs the next segment up to its event decision (a2/a3 XS lookup, a5 nearest boundary, a6 distance
+//              to collision, a7 move + tallies, reaction choice) and writes every survivor, whole, into
+//              bank[(s+1)&1]: front or back by its new pending event, positions from ballot + prefix-sum compaction
+//              with one atomic per block and queue (a11).  The queues are the particles themselves (PAPER.md:55
+//              dual banks), so all bank traffic is coalesced.
+//   k_persist  (PAPER.md:49 asynchronous scheduling) takes over when the population is thin: a persistent grid whose
+//              warps pull particles from a global cursor, run whole segments in registers and refill dead lanes from
+//              the queue; continuous-energy fission secondaries are pushed to the queue's tail for any warp to take.
+// k_scatter / k_surface finish the pending events of one region in place (schedule 2: split per-event kernels, kept
+// for the comparison).  Fission and capture end a history inside the segment; a multi-group fission leaves a record
+// at the parent's slot and the children are produced at the end of the cycle by count -> exclusive scan -> write
+// (a10/a12), which yields the bank sorted by (parent id, child index) without atomics or a sort.  k_segment is the
+// paper's monolithic design: one whole segment for every bank slot per launch, no compaction.
 #pragma once
 #include "mcdc_device.cuh"
 
@@ -32,44 +37,14 @@ __device__ __forceinline__ double warp_sum(double v)
 __device__ __forceinline__ int pack_gl(int g, int last) { return (g & 0xffff) | ((last + 1) << 16); }
 
 // ------------------------------------------------------------------ a2: multi-group tables in shared memory
-// Copies the table blob to shared memory (all threads of the block; ends with a barrier) and returns the table
-// descriptor rebased onto the copy; `smem` is where the copy goes, n_stage its size in doubles (0: not staged,
-// the tables are then read from global memory through L1).
-__device__ __forceinline__ MGTab stage_mg(const Ctx &c, double *smem, int n_stage)
+// Copies the table blob to shared memory (all threads of the block; ends with a barrier) and returns the base the
+// kernel reads the tables from: the copy, or the global blob when it does not fit (n_stage = 0).
+__device__ __forceinline__ const double *stage_mg(const Ctx &c, double *smem, int n_stage)
 {
-    MGTab mg = c.mg;
-    if (n_stage > 0) {
-        for (int k = threadIdx.x; k < n_stage; k += blockDim.x) smem[k] = __ldg(c.mg.blob + k);
-        mg.sig_t = smem + (c.mg.sig_t - c.mg.blob); mg.sig_s = smem + (c.mg.sig_s - c.mg.blob);
-        mg.sig_f = smem + (c.mg.sig_f - c.mg.blob); mg.nu = smem + (c.mg.nu - c.mg.blob);
-        mg.nusf = smem + (c.mg.nusf - c.mg.blob); mg.cumS = smem + (c.mg.cumS - c.mg.blob);
-        mg.cumchi = smem + (c.mg.cumchi - c.mg.blob); mg.src_cum = smem + (c.mg.src_cum - c.mg.blob);
-        __syncthreads();
-    }
-    return mg;
-}
-
-// a4/a5: the CSG tables (surfaces, cell -> surface lists, fills, bins, universes) in shared memory, same scheme;
-// `smem` must be 8-byte aligned; the lattice maps stay in global memory (L1/L2)
-__device__ __forceinline__ Geo stage_geo(const Ctx &c, void *smem, int n_words)
-{
-    Geo G = c.geo;
-    if (n_words > 0) {
-        int *dst = (int *)smem;
-        const int *src = (const int *)c.geo.blob;
-        for (int k = threadIdx.x; k < n_words; k += blockDim.x) dst[k] = __ldg(src + k);
-        const char *b = c.geo.blob;
-        char *d = (char *)smem;
-        G.surf_param = (const double *)(d + ((const char *)c.geo.surf_param - b));
-        G.surf_type = (const int *)(d + ((const char *)c.geo.surf_type - b));
-        G.surf_bc = (const int *)(d + ((const char *)c.geo.surf_bc - b));
-        G.cso = (const int *)(d + ((const char *)c.geo.cso - b)); G.csi = (const int *)(d + ((const char *)c.geo.csi - b));
-        G.css = (const int *)(d + ((const char *)c.geo.css - b)); G.cft = (const int *)(d + ((const char *)c.geo.cft - b));
-        G.cfill = (const int *)(d + ((const char *)c.geo.cfill - b)); G.cbin = (const int *)(d + ((const char *)c.geo.cbin - b));
-        G.uco = (const int *)(d + ((const char *)c.geo.uco - b));
-        __syncthreads();
-    }
-    return G;
+    if (n_stage <= 0) return c.mg.blob;
+    for (int k = threadIdx.x; k < n_stage; k += blockDim.x) smem[k] = __ldg(c.mg.blob + k);
+    __syncthreads();
+    return smem;
 }
 
 // ------------------------------------------------------------------ bank access (dense, position-indexed)
@@ -81,19 +56,21 @@ __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particl
     p.cell = B.cell[i]; p.elem = B.elem[i];
     int gl = B.gl[i];
     p.g = gl & 0xffff; p.last = (gl >> 16) - 1;
+    uint32_t ev = B.ev[i];
+    p.pend = ev & PEND_MASK; p.nseg = ev >> 12;
     ctr = B.ctr[i];
     slot = B.slot[i];
+    p.v = 0.0; p.gi = 0; p.ebin = 0;
     if (CE) { p.E = B.E[i]; p.t = B.t[i]; p.tbin = B.tbin[i]; p.id = B.id[i]; }
     else { p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = slot; }
 }
 
 template <bool CE>
-__device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr, uint32_t slot,
-                                           int ev)
+__device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr, uint32_t slot)
 {
     B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z; B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
     B.cell[i] = p.cell; B.elem[i] = p.elem; B.gl[i] = pack_gl(p.g, p.last); B.ctr[i] = ctr; B.slot[i] = slot;
-    B.ev[i] = ev;
+    B.ev[i] = p.pend | (p.nseg << 12);
     if (CE) { B.E[i] = p.E; B.t[i] = p.t; B.tbin[i] = p.tbin; B.id[i] = p.id; }
 }
 
@@ -115,6 +92,20 @@ __device__ __forceinline__ unsigned int live_pos(unsigned int cap, unsigned int 
     return t < n_front ? t : cap - 1u - (t - n_front);
 }
 
+// counts of the live regions a sweep reads (clamped to the capacity: a continuous-energy run whose secondaries
+// outgrew the bank has already raised the overflow error; the clamp keeps every index inside the arrays)
+__device__ __forceinline__ void live_counts(const Ctx &c, unsigned int s, unsigned int n0, unsigned int &n_front,
+                                            unsigned int &n_in)
+{
+    n_front = n0; n_in = n0;
+    if (s > 0) {
+        QCount pc = c.qc[(s - 1) % RING];
+        n_front = pc.n_scat < c.cap ? pc.n_scat : c.cap;
+        unsigned long long tot = (unsigned long long)pc.n_scat + pc.n_surf;
+        n_in = tot < c.cap ? (unsigned int)tot : c.cap;
+    }
+}
+
 // per-block flush: k numerator (warp shuffles + one atomic per block) and the shared event counters
 __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
 {
@@ -132,13 +123,23 @@ __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
         atomicAdd(c.counters + threadIdx.x, (unsigned long long)acc.s_ev[threadIdx.x]);
 }
 
-// block-shared event counters: declare + clear (call at kernel start, before any event is counted)
-#define MCDC_EVENT_COUNTERS(acc)                         \
-    __shared__ unsigned int s_evc[16];                   \
-    if (threadIdx.x < 16) s_evc[threadIdx.x] = 0u;       \
-    __syncthreads();                                     \
-    Acc acc;                                             \
-    acc.clear(s_evc)
+// kernel prologue shared by the transport kernels: stage the multi-group tables, clear the private tally columns
+// and the block-shared event counters
+#define MCDC_TRANSPORT_PROLOGUE(acc, s_flux)                                               \
+    extern __shared__ double s_dyn[];                                                      \
+    __shared__ unsigned int s_evc[16];                                                     \
+    __shared__ Geo s_geo;                                                                  \
+    if (threadIdx.x == 0) s_geo = c.geo;                                                   \
+    Acc acc;                                                                               \
+    acc.clear(s_evc);                                                                      \
+    acc.geo = &s_geo;                                                                      \
+    acc.tracing = c.tr.rec != nullptr;                                                     \
+    acc.mgs = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);                                     \
+    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage);                                        \
+    if (PRIVATE)                                                                           \
+        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;            \
+    if (threadIdx.x < 16) s_evc[threadIdx.x] = 0u;                                         \
+    __syncthreads()
 
 // shared-memory tally columns (one per thread) -> one float64 atomic per bin and block
 __device__ __forceinline__ void flush_private_flux(const Ctx &c, const double *s_flux)
@@ -217,10 +218,10 @@ __global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
     if (i >= n) return;
     const Bank &B = c.bank[0];
     Rng rng;
-    rng.init(c.seed, i, 0u, c.cycle, 0u);
+    rng.init(i, 0u);
     double xi[6];
 #pragma unroll
-    for (int k = 0; k < 6; k++) xi[k] = rng.next();  // always six draws
+    for (int k = 0; k < 6; k++) xi[k] = rng.next(c);  // always six draws
     Particle p;
     p.x = c.src_lo[0] + xi[0] * (c.src_hi[0] - c.src_lo[0]);
     p.y = c.src_lo[1] + xi[1] * (c.src_hi[1] - c.src_lo[1]);
@@ -228,12 +229,12 @@ __global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
     p.ux = c.src_dir[0]; p.uy = c.src_dir[1]; p.uz = c.src_dir[2];
     if (c.src_iso) iso_dir(xi[3], xi[4], p.ux, p.uy, p.uz);
     p.g = 0;
-    if (!CE) p.g = pick(c.mg.src_cum, c.mg.G, xi[5] * __ldg(c.mg.src_cum + c.mg.G - 1));
+    if (!CE) p.g = pick(c.mg.blob + c.mg.o_src_cum, c.mg.G, xi[5] * __ldg(c.mg.blob + c.mg.o_src_cum + c.mg.G - 1));
     if (!locate(c.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, -1, p.cell, p.elem)) { atomicExch(c.err, -2); p.cell = -1; }
-    p.last = -1; p.id = i;
+    p.last = -1; p.id = i; p.pend = PEND_NONE; p.nseg = 0;
     p.E = c.src_E; p.t = c.src_t; p.tbin = 0;
     if (CE) p.tbin = edge_bin(c.ce.t_edges, c.ce.n_t, c.src_t);
-    store_full<CE>(B, i, p, 6u, i, p.cell < 0 ? EV_DEAD : 0);
+    store_full<CE>(B, i, p, 6u, i);
     c.fis.n[i] = 0;
 }
 
@@ -247,9 +248,9 @@ __global__ void __launch_bounds__(BS) k_load_sites(Ctx c, const Site *sites, uns
     Site s = sites[i];
     Particle p;
     p.x = s.x; p.y = s.y; p.z = s.z; p.ux = s.ux; p.uy = s.uy; p.uz = s.uz; p.g = s.g; p.last = -1; p.id = i;
-    p.E = 0.0; p.t = 0.0; p.tbin = 0;
+    p.E = 0.0; p.t = 0.0; p.tbin = 0; p.pend = PEND_NONE; p.nseg = 0;
     if (!locate(c.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, -1, p.cell, p.elem)) { atomicExch(c.err, -2); p.cell = -1; }
-    store_full<false>(c.bank[0], i, p, 0u, i, p.cell < 0 ? EV_DEAD : 0);
+    store_full<false>(c.bank[0], i, p, 0u, i);
     c.fis.n[i] = 0;
 }
 
@@ -272,46 +273,59 @@ __device__ __forceinline__ void make_child(const Ctx &c, Rng &rng, int mat, unsi
                                            Particle &p)
 {
     if (!CE) {
-        const double *cc = c.mg.cumchi + (size_t)mat * c.mg.G;
-        p.g = pick(cc, c.mg.G, rng.next() * __ldg(cc + c.mg.G - 1));
-        double a = rng.next(), b = rng.next();
+        const double *cc = c.mg.blob + c.mg.o_cumchi + (size_t)mat * c.mg.G;
+        p.g = pick(cc, c.mg.G, rng.next(c) * __ldg(cc + c.mg.G - 1));
+        double a = rng.next(c), b = rng.next(c);
         iso_dir(a, b, p.ux, p.uy, p.uz);
     } else {
-        double a1 = rng.next(), a2 = rng.next(), a3 = rng.next(), a4 = rng.next();
+        double a1 = rng.next(c), a2 = rng.next(c), a3 = rng.next(c), a4 = rng.next(c);
         double En = 1e6 * watt(c.ce.watt_a, c.ce.watt_b, a1, a2, a3, a4);
         if (En < c.ce.E_min) En = c.ce.E_min;
         if (En > c.ce.E_max) En = c.ce.E_max;
-        double a = rng.next(), b = rng.next();
+        double a = rng.next(c), b = rng.next(c);
         iso_dir(a, b, p.ux, p.uy, p.uz);
         p.E = En;
         p.id = child_id(c.seed, pid, ctr0, (uint32_t)j);
     }
-    p.last = -1;
+    p.last = -1; p.pend = PEND_NONE; p.nseg = 0;
 }
 
-// ------------------------------------------------------------------ per-event kernels
-#ifndef MCDC_ADV_MINBLOCKS
-#define MCDC_ADV_MINBLOCKS 4  // measured on B200: 2 -> 30.2, 3 -> 25.2, 4 -> 22.5, 5 -> 24.1 ms of k_advance per C4 cycle
+// prompt secondaries made so far (R25a): more than max_secondaries is the bank-overflow error
+__device__ __forceinline__ bool count_secondaries(const Ctx &c, unsigned int n)
+{
+    unsigned long long old = atomicAdd(c.counters + 15, (unsigned long long)n);
+    if (old + n > c.max_secondaries) { atomicExch(c.err, -3); return false; }
+    return true;
+}
+
+__device__ __forceinline__ void mark_lost(const Ctx &c)
+{
+    atomicExch(c.err, -2);
+    atomicAdd(c.counters + 10, 1ull);
+}
+
+// ------------------------------------------------------------------ the sweep kernel (large populations)
+#ifndef MCDC_SWEEP_MINBLOCKS
+#define MCDC_SWEEP_MINBLOCKS 4
 #endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS * 256 / BS) k_advance(Ctx c, unsigned int s, unsigned int n0)
+__global__ void __launch_bounds__(BS, MCDC_SWEEP_MINBLOCKS * 256 / BS) k_sweep(Ctx c, unsigned int s, unsigned int n0)
 {
-    extern __shared__ double s_dyn[];
-    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
-    unsigned int n_front = n0, n_in = n0;
-    if (s > 0) {
-        QCount pc = c.qc[(s - 1) % RING];
-        n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
-    }
+    MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
+    unsigned int n_front, n_in;
+    live_counts(c, s, n0, n_front, n_in);
     QCount *oc = c.qc + (s % RING);
-    if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(c.counters + 12, (unsigned long long)n_in);  // events of k_advance
-    if (PRIVATE) {
-        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
-        __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        QCount z = {0u, 0u, 0u, 0u};
+        c.qc[(s + 1) % RING] = z;  // the set the next sweep appends to
+        atomicAdd(c.counters + 12, (unsigned long long)n_in);  // segments run by the sweep kernels
+        int e = *c.err;
+        if (s > 0) {
+            QCount pc = c.qc[(s - 1) % RING];
+            if ((unsigned long long)pc.n_scat + pc.n_surf > c.cap) { atomicExch(c.err, -3); e = -3; }  // the two regions met
+        }
+        oc->err = (unsigned int)e;
     }
-    MCDC_EVENT_COUNTERS(acc);
     const Bank &B = c.bank[s & 1];
     const Bank &O = c.bank[(s + 1) & 1];
     int par = 0;
@@ -321,34 +335,41 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS * 256 / BS) k_advance(C
         Particle p;
         uint32_t ctr = 0, slot = 0;
         Rng rng;
-        if (t < n_in) {
-            unsigned int i = live_pos(c.cap, n_front, t);
-            if (B.cell[i] >= 0) {
-                load_full<CE>(B, i, p, ctr, slot);
-                rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-                code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux, geo);
+        rng.init(0ull, 0u);
+        const unsigned int i = t < n_in ? live_pos(c.cap, n_front, t) : 0u;
+        const bool live = t < n_in && B.cell[i] >= 0;
+        const unsigned int amask = __ballot_sync(0xffffffffu, live);
+        if (live) {
+            load_full<CE>(B, i, p, ctr, slot);
+            if (CE) ce_energy_state(c.ce, p);
+            rng.init(p.id, ctr);
+            const bool ok = finish_pending<CE>(c, acc, p, rng);
+            __syncwarp(amask);  // the lanes went different ways by pending event: run the segment together again
+            if (!ok) mark_lost(c);
+            else {
+                code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
                 if (!CE && code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
         if (!CE) {
             unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap, par);
-            if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot, aux);
+            if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot);
         } else {
             unsigned int nb = code == ADV_SURFACE ? 1u : (code == ADV_FISSION ? (unsigned int)aux : 0u);
             unsigned int pf, ob;
             block_slot_n(code == ADV_SCATTER, nb, oc, c.cap, par, pf, ob);
-            if (code == ADV_SCATTER) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot, aux); }
-            else if (code == ADV_SURFACE) { if (ob < c.cap) store_full<CE>(O, c.cap - 1u - ob, p, rng.ctr, slot, aux); }
+            if (code == ADV_SCATTER) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot); }
+            else if (code == ADV_SURFACE) { if (ob < c.cap) store_full<CE>(O, c.cap - 1u - ob, p, rng.ctr, slot); }
             else if (code == ADV_FISSION && nb) {
                 // prompt secondaries: born alive at the parent's site, first segment in the next sweep
                 const int mat = c.geo.cfill[p.cell];
                 const unsigned long long pid = p.id;
                 const uint32_t ctr0 = rng.ctr;
+                count_secondaries(c, nb);
                 for (unsigned int j = 0; j < nb; j++) {
                     make_child<CE>(c, rng, mat, pid, ctr0, (int)j, p);
-                    if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot, HIT_NEWBORN);
+                    if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot);
                 }
-                atomicAdd(c.counters + 15, (unsigned long long)nb);
             }
         }
     }
@@ -356,46 +377,50 @@ __global__ void __launch_bounds__(BS, MCDC_ADV_MINBLOCKS * 256 / BS) k_advance(C
     flush_acc(c, acc);
 }
 
+// ------------------------------------------------------------------ split per-event kernels (schedule 2)
+// finish the scatter events of the front region / the surface events of the back region of bank[(s+1)&1] in place
 template <bool CE>
 __global__ void __launch_bounds__(BS) k_scatter(Ctx c, unsigned int s)
 {
     extern __shared__ double s_dyn[];
-    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
+    Acc acc;
+    acc.clear(nullptr);
+    acc.tracing = false;
+    acc.geo = nullptr;
+    acc.mgs = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
     const QCount oc = c.qc[s % RING];
     const Bank &B = c.bank[(s + 1) & 1];
-    // queue-counter housekeeping: clear the set the next sweep appends to
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        QCount z = {0u, 0u, 0u, 0u};
-        c.qc[(s + 1) % RING] = z;
-        if ((unsigned long long)oc.n_scat + oc.n_surf > c.cap) atomicExch(c.err, -3);  // the two regions met
-    }
     for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < oc.n_scat && i < c.cap; i += gridDim.x * BS) {
         Particle p;
         int gl = B.gl[i];
+        uint32_t ev = B.ev[i];
         p.g = gl & 0xffff;
         p.cell = B.cell[i];
         p.id = CE ? B.id[i] : (unsigned long long)B.slot[i];
         if (CE) { p.E = B.E[i]; p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i]; }
         Rng rng;
-        rng.init(c.seed, p.id, 0u, c.cycle, B.ctr[i]);
-        do_scatter<CE>(c, mg, p, rng, B.ev[i], c.geo);
+        rng.init(p.id, B.ctr[i]);
+        do_scatter<CE>(c, acc, p, rng, (int)(ev & 7u));
         B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
         B.gl[i] = pack_gl(p.g, -1);
         B.ctr[i] = rng.ctr;
+        B.ev[i] = (ev & ~PEND_MASK) | PEND_NONE;
         if (CE) B.E[i] = p.E;
     }
 }
 
 __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 {
-    extern __shared__ double s_dyn[];
-    const Geo geo = stage_geo(c, s_dyn, c.geo_stage);
+    __shared__ Geo s_geo;
+    if (threadIdx.x == 0) s_geo = c.geo;
+    __syncthreads();
     const QCount oc = c.qc[s % RING];
     const Bank &B = c.bank[(s + 1) & 1];
-    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_surf; t += gridDim.x * BS) {
+    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < oc.n_surf && t < c.cap; t += gridDim.x * BS) {
         unsigned int i = c.cap - 1u - t;
-        int hit = B.ev[i];
-        if (hit == HIT_TIME_EDGE || hit == HIT_NEWBORN) continue;
+        uint32_t ev = B.ev[i];
+        unsigned int hit = ev & PEND_MASK;
+        if (hit >= PEND_SCATTER) continue;  // time edge / newborn: nothing to finish
         Particle p;
         p.x = B.x[i]; p.y = B.y[i]; p.z = B.z[i];
         p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i];
@@ -404,144 +429,259 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
         p.g = gl & 0xffff; p.last = (gl >> 16) - 1;
         const int cell0 = p.cell, elem0 = p.elem;
         const double ux0 = p.ux, uy0 = p.uy, uz0 = p.uz;
-        if (!do_surface(geo, p, hit)) {
-            atomicExch(c.err, -2);
-            atomicAdd(c.counters + 10, 1ull);
-            p.cell = -1;
-        }
+        int r = 0;
+        if (location_is_fast(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)hit);
+        if (r == 0) r = do_surface(s_geo, p, (int)hit) ? 1 : -1;
+        if (r < 0) { mark_lost(c); p.cell = -1; }
         if (p.cell != cell0) B.cell[i] = p.cell;
         if (p.elem != elem0) B.elem[i] = p.elem;
         B.gl[i] = pack_gl(p.g, p.last);
+        B.ev[i] = (ev & ~PEND_MASK) | PEND_NONE;
         if (p.ux != ux0) B.ux[i] = p.ux;
         if (p.uy != uy0) B.uy[i] = p.uy;
         if (p.uz != uz0) B.uz[i] = p.uz;
     }
 }
 
-// whole segment in registers (shared by the monolithic schedule and the tail kernel):
-// returns 1 = still alive, 0 = history ended, 2 = ended in a fission with n_children
-template <bool CE, bool PRIVATE>
-__device__ __forceinline__ int segment(const Ctx &c, const MGTab &mg, const Geo &G, Particle &p, Rng &rng, Acc &acc,
-                                       double *s_flux, int &n_children)
-{
-    int aux = 0;
-    int code = advance<CE, PRIVATE>(c, mg, p, rng, aux, acc, s_flux, G);
-    if (code == ADV_SCATTER) { do_scatter<CE>(c, mg, p, rng, aux, G); return 1; }
-    if (code == ADV_SURFACE) {
-        if (!do_surface(G, p, aux)) {
-            atomicExch(c.err, -2);
-            atomicAdd(c.counters + 10, 1ull);
-            p.cell = -1;
-            return 0;
-        }
-        return 1;
-    }
-    if (code == ADV_FISSION) { n_children = aux; return 2; }
-    return 0;
-}
-
-// Fused sweep for a thinned-out population: up to max_seg whole segments per particle in registers, then the same
-// ballot / prefix-sum compaction of the survivors into the next bank (front region; continuous-energy fission
-// children go, alive, to the back region).  One launch replaces 3 * max_seg launches of the per-event kernels
-// when a sweep is launch-latency bound; divergence is irrelevant at these sizes.
-#ifndef MCDC_MULTI_MINBLOCKS
-#define MCDC_MULTI_MINBLOCKS 3  // measured: 2 -> 11.4, 3 -> 9.7, 4 -> 9.6 ms of fused sweeps per C4 cycle
+// ------------------------------------------------------------------ the persistent kernel (thin populations)
+// PAPER.md:49 asynchronous scheduling: the grid stays resident; each warp keeps 32 histories in registers, runs one
+// whole segment per loop trip (finish the pending event, then advance) and refills the lanes whose history has ended
+// from the global work queue.  Queue entry k < n_in is live particle k of bank[s&1]; entry n_in + a is the a-th
+// secondary pushed by a continuous-energy fission (the fissioning lane continues as its first child and pushes the
+// rest) into bank[(s+1)&1], used as a ring of `cap` slots.  A dead lane takes a TICKET (fetch-add on the queue head:
+// no retries however many warps ask at once); a ticket for an entry that does not exist yet is kept, and the lane
+// looks at its slot again every trip without holding up the live lanes of its warp.  Every ring slot has a sequence
+// word (the bank's ev array, zero at launch): 2 lap = free for lap `lap`, 2 lap + 1 = holds that lap's entry; the
+// pusher writes the particle, then the word; the ticket holder reads the particle when the word says so and hands
+// the slot to the next lap.  The launch is over when every history has ended: ended == n_in + born.
+#ifndef MCDC_PERSIST_MINBLOCKS
+#define MCDC_PERSIST_MINBLOCKS 3
 #endif
-#ifndef MCDC_MULTI_MINBLOCKS_CE
-#define MCDC_MULTI_MINBLOCKS_CE 3
+#ifndef MCDC_REFILL
+#define MCDC_REFILL 4  // dead lanes without a ticket at which a warp goes back to the queue
+#endif
+#ifndef MCDC_DENSE
+#define MCDC_DENSE 12  // live lanes from which a continuous-energy warp keeps tickets for entries not pushed yet
 #endif
 template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS, (CE ? MCDC_MULTI_MINBLOCKS_CE : MCDC_MULTI_MINBLOCKS) * 256 / BS) k_multi(Ctx c, unsigned int s, unsigned int n0, unsigned int max_seg)
+__global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persist(Ctx c, unsigned int s, unsigned int n0)
 {
-    extern __shared__ double s_dyn[];
-    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
-    unsigned int n_front = n0, n_in = n0;
-    if (s > 0) {
-        QCount pc = c.qc[(s - 1) % RING];
-        n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
-    }
-    QCount *oc = c.qc + (s % RING);
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        QCount z = {0u, 0u, 0u, 0u};
-        c.qc[(s + 1) % RING] = z;
-        if (n_in > c.cap) atomicExch(c.err, -3);
-    }
-    if (PRIVATE) {
-        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
-        __syncthreads();
-    }
-    MCDC_EVENT_COUNTERS(acc);
+    MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
+    unsigned int n_front, n_in;
+    live_counts(c, s, n0, n_front, n_in);
     const Bank &B = c.bank[s & 1];
     const Bank &O = c.bank[(s + 1) & 1];
-    int par = 0;
-    for (unsigned int base = blockIdx.x * BS; base < n_in; base += gridDim.x * BS, par ^= 1) {
-        unsigned int t = base + threadIdx.x;
-        int st = 0, nch = 0;
-        Particle p;
-        uint32_t ctr = 0, slot = 0;
-        Rng rng;
-        if (t < n_in && t < c.cap) {
-            unsigned int i = live_pos(c.cap, n_front, t);
-            if (B.cell[i] >= 0) {
-                load_full<CE>(B, i, p, ctr, slot);
-                rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-                unsigned int k = 0;
-                do { st = segment<CE, PRIVATE>(c, mg, geo, p, rng, acc, s_flux, nch); } while (st == 1 && ++k < max_seg);
-                if (!CE && st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
+    // work[0] head of the queue, [1] secondaries pushed, [2] histories ended, [3] secondaries born in this launch
+    // (32-bit: a run makes fewer than 2^32 secondaries, checked by the host)
+    unsigned int *head = c.work, *tail = c.work + 1, *ended = c.work + 2, *born = c.work + 3;
+    const unsigned int FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    bool alive = false, ticketed = false, drained = false;
+    unsigned int ticket = 0, t_slot = 0, t_full = 0;  // ring slot and the sequence word that says "entry written"
+    Particle p;
+    uint32_t slot = 0;
+    Rng rng;
+    rng.init(0ull, 0u);
+    unsigned int taken = 0, n_end = 0, idle_ns = 500;
+#ifdef MCDC_TIMELINE
+    unsigned long long tl_trips = 0, tl_lanes = 0, tl_idle = 0, tl_t0 = 0, tl_src = 0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t0));
+#endif
+    for (;;) {
+        const unsigned int want = __ballot_sync(FULL, !alive && !ticketed && !drained);
+        const int nw = __popc(want);
+        const bool none_alive = !__any_sync(FULL, alive);
+        // Multi-group: dead lanes go back to the queue as soon as MCDC_REFILL of them are free.  Continuous energy: a
+        // DENSE warp does the same (its free lanes wait, ticket in hand, for secondaries to be pushed); a sparse or
+        // idle warp only takes entries that already exist, so that a thin population stays concentrated in few warps
+        // instead of keeping every resident warp busy with one or two lanes.
+        unsigned int n_take = 0;
+        if (!CE) n_take = (nw >= MCDC_REFILL || (none_alive && nw > 0)) ? (unsigned int)nw : 0u;
+        else if (nw >= MCDC_REFILL) {
+            if (__popc(__ballot_sync(FULL, alive)) >= MCDC_DENSE) n_take = (unsigned int)nw;
+            else {
+                unsigned int backlog = 0;
+                if (lane == 0) {
+                    unsigned int h = *(volatile unsigned int *)head, t = *(volatile unsigned int *)tail;
+                    backlog = n_in + t > h ? n_in + t - h : 0u;
+                }
+                backlog = __shfl_sync(FULL, backlog, 0);
+                n_take = min((unsigned int)nw, backlog);
             }
         }
-        unsigned int nb = (CE && st == 2) ? (unsigned int)nch : 0u;
-        unsigned int pf, ob;
-        block_slot_n(st == 1, nb, oc, c.cap, par, pf, ob);
-        if (st == 1) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot, 0); }
-        else if (nb) {
-            const int mat = c.geo.cfill[p.cell];
-            const unsigned long long pid = p.id;
-            const uint32_t ctr0 = rng.ctr;
-            for (unsigned int j = 0; j < nb; j++) {
-                make_child<CE>(c, rng, mat, pid, ctr0, (int)j, p);
-                if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot, HIT_NEWBORN);
+        const bool take = n_take > 0;
+        if (take) {
+            unsigned int base = 0;
+            if (lane == 0) base = atomicAdd(head, n_take);
+            base = __shfl_sync(FULL, base, 0);
+            const unsigned int rank = __popc(want & ((1u << lane) - 1u));
+            if (!alive && !ticketed && !drained && rank < n_take) {
+                ticket = base + rank;
+                ticketed = CE || ticket < n_in;  // multi-group: the queue never grows, a ticket past its end is void
+                drained = !ticketed;
+                if (CE && ticket >= n_in) {
+                    const unsigned int a = ticket - n_in;
+                    t_slot = a % c.cap;
+                    t_full = 2u * (a / c.cap) + 1u;
+                }
             }
-            atomicAdd(c.counters + 15, (unsigned long long)nb);
+        }
+        if (ticketed) {
+            uint32_t ctr = 0;
+            bool have = false;
+            if (ticket < n_in) {
+                load_full<CE>(B, live_pos(c.cap, n_front, ticket), p, ctr, slot);
+                have = true;
+            } else if (CE && *(volatile uint32_t *)(O.ev + t_slot) == t_full) {
+                const unsigned int i = t_slot;
+                __threadfence();
+                p.x = __ldcg(O.x + i); p.y = __ldcg(O.y + i); p.z = __ldcg(O.z + i);
+                p.ux = __ldcg(O.ux + i); p.uy = __ldcg(O.uy + i); p.uz = __ldcg(O.uz + i);
+                p.cell = __ldcg(O.cell + i); p.elem = __ldcg(O.elem + i);
+                p.g = 0; p.last = -1; p.pend = PEND_NONE; p.nseg = 0;
+                slot = __ldcg(O.slot + i);
+                p.E = __ldcg(O.E + i); p.t = __ldcg(O.t + i); p.tbin = __ldcg(O.tbin + i); p.id = __ldcg(O.id + i);
+                __threadfence();
+                *(volatile uint32_t *)(O.ev + i) = t_full + 1u;  // free for the next lap
+                have = true;
+            }
+            if (have) {
+                ticketed = false;
+                if (CE) ce_energy_state(c.ce, p);
+                if (p.cell >= 0) { alive = true; rng.init(p.id, ctr); taken++; }
+                else n_end++;  // a particle that was lost at birth
+            }
+        }
+        if (!__any_sync(FULL, alive)) {
+            // nothing to run.  Multi-group: leave once every lane's ticket is void.  Continuous energy: other warps may
+            // still push secondaries; sleep, then look again, until every history of the launch has ended:
+            // ended == n_in + born, with `ended` read first (a parent's children are counted in `born` before the
+            // parent is counted in `ended`, so the test cannot pass early).
+            unsigned int fin = 0;
+            if (!CE) fin = __all_sync(FULL, drained) ? 1u : 0u;
+            else {
+                const unsigned int ne = __reduce_add_sync(FULL, n_end);
+                n_end = 0;
+                if (lane == 0) {
+                    if (ne) atomicAdd(ended, ne);
+                    unsigned int e = *(volatile unsigned int *)ended;
+                    __threadfence();
+                    unsigned int b = *(volatile unsigned int *)born;
+                    fin = (e == n_in + b || *(volatile int *)c.err != 0) ? 1u : 0u;
+                }
+                fin = __shfl_sync(FULL, fin, 0);
+            }
+            if (fin) break;
+#ifdef MCDC_TIMELINE
+            tl_idle++;
+#endif
+            if (CE) { __nanosleep(idle_ns); if (idle_ns < 16000) idle_ns *= 2; }
+            continue;
+        }
+        idle_ns = 500;
+#ifdef MCDC_TIMELINE
+        tl_trips++;
+        tl_lanes += __popc(__ballot_sync(FULL, alive));
+        if (!tl_src && *(volatile unsigned int *)head >= n_in) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_src));
+#endif
+        const unsigned int amask = __ballot_sync(FULL, alive);
+        if (alive) {
+            int aux = 0, code = ADV_DEAD;
+            const bool ok = finish_pending<CE>(c, acc, p, rng);
+            __syncwarp(amask);  // the lanes went different ways by pending event: run the segment together again
+            if (!ok) mark_lost(c);
+            else code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+            if (code == ADV_DEAD) { alive = false; n_end++; }
+            else if (code == ADV_FISSION) {
+                alive = false;
+                n_end++;
+                if (!CE) record_fission<CE>(c, p, rng.ctr, slot, aux);
+                else if (aux > 0 && count_secondaries(c, (unsigned int)aux)) {
+                    atomicAdd(born, (unsigned int)aux);
+                    const int mat = c.geo.cfill[p.cell];
+                    const unsigned long long pid = p.id;
+                    const uint32_t ctr0 = rng.ctr;
+                    unsigned int at = 0;
+                    if (aux > 1) at = atomicAdd(tail, (unsigned int)(aux - 1));
+                    Particle first = p;
+                    for (int j = 0; j < aux; j++) {
+                        make_child<CE>(c, rng, mat, pid, ctr0, j, p);
+                        if (j == 0) first = p;
+                        else {
+                            const unsigned int a = at + (unsigned int)(j - 1);
+                            const unsigned int i = a % c.cap, free_ = 2u * (a / c.cap);
+                            // the slot still holds the previous lap's entry: if no ticket has been issued for that
+                            // entry, nobody is about to take it -- more than `cap` secondaries wait: bank overflow
+                            if (*(volatile uint32_t *)(O.ev + i) != free_) {
+                                if (*(volatile unsigned int *)head + c.cap <= n_in + a) atomicExch(c.err, -3);
+                                unsigned int spins = 0;
+                                while (*(volatile uint32_t *)(O.ev + i) != free_ && *(volatile int *)c.err == 0)
+                                    if (++spins > (1u << 22)) atomicExch(c.err, -3);
+                                if (*(volatile int *)c.err != 0) break;
+                            }
+                            O.x[i] = p.x; O.y[i] = p.y; O.z[i] = p.z; O.ux[i] = p.ux; O.uy[i] = p.uy; O.uz[i] = p.uz;
+                            O.cell[i] = p.cell; O.elem[i] = p.elem; O.slot[i] = slot;
+                            O.E[i] = p.E; O.t[i] = p.t; O.tbin[i] = p.tbin; O.id[i] = p.id;
+                            __threadfence();
+                            *(volatile uint32_t *)(O.ev + i) = free_ + 1u;
+                        }
+                    }
+                    p = first;
+                    ce_energy_state(c.ce, p);
+                    rng.init(p.id, 0u);
+                    alive = true;
+                }
+            }
         }
     }
+#ifdef MCDC_TIMELINE
+    if (lane == 0) {
+        unsigned long long t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        atomicAdd(c.counters + 0, tl_trips);
+        atomicAdd(c.counters + 11, tl_lanes);
+        atomicAdd(c.counters + 13, tl_idle);
+        atomicMax(c.counters + 12, t1 - tl_t0);
+        if (tl_src) atomicMax(c.counters + 9, tl_src - tl_t0);  // (slot 9 = cutoff events: debug build only)
+        // histogram of warp end times in 8 bins of 1/8 of ... keep simple: sum of end times
+        atomicAdd(c.counters + 10, t1 - tl_t0);
+    }
+#endif
+    taken = __reduce_add_sync(FULL, taken);
+    if (lane == 0 && taken) atomicAdd(c.counters + 14, (unsigned long long)taken);
     if (PRIVATE) flush_private_flux(c, s_flux);
     flush_acc(c, acc);
 }
 
-// monolithic schedule: every slot of bank 0, one segment, no compaction; counts the survivors
+// ------------------------------------------------------------------ monolithic schedule
+// every slot of bank 0, one whole segment (advance + the event it ends in), in place, no compaction; counts the
+// survivors.  A dead slot has cell = -1.
 template <bool CE, bool PRIVATE>
 __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned int n)
 {
-    extern __shared__ double s_dyn[];
-    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
-    if (PRIVATE) {
-        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
-        __syncthreads();
-    }
+    MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         QCount z = {0u, 0u, 0u, 0u};
         c.qc[(s + 1) % RING] = z;
+        c.qc[s % RING].err = (unsigned int)*c.err;
     }
-    MCDC_EVENT_COUNTERS(acc);
     const Bank &B = c.bank[0];
     unsigned int alive = 0;
     for (unsigned int i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
-        if (B.ev[i] == EV_DEAD) continue;
+        if (B.cell[i] < 0) continue;
         Particle p;
         uint32_t ctr, slot;
         load_full<CE>(B, i, p, ctr, slot);
+        if (CE) ce_energy_state(c.ce, p);
         Rng rng;
-        rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-        int nch = 0;
-        int st = segment<CE, PRIVATE>(c, mg, geo, p, rng, acc, s_flux, nch);
-        if (st == 2) record_fission<CE>(c, p, rng.ctr, slot, nch);
-        store_full<CE>(B, i, p, rng.ctr, slot, st == 1 ? 0 : EV_DEAD);
-        if (st == 1) alive++;
+        rng.init(p.id, ctr);
+        int aux = 0;
+        int code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+        if (code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
+        else if (code != ADV_DEAD && !finish_pending<CE>(c, acc, p, rng)) { mark_lost(c); code = ADV_DEAD; }
+        if (code == ADV_DEAD) p.cell = -1;
+        store_full<CE>(B, i, p, rng.ctr, slot);
+        if (code != ADV_DEAD) alive++;
     }
     alive = __reduce_add_sync(0xffffffffu, alive);
     if ((threadIdx.x & 31) == 0 && alive) atomicAdd(&c.qc[s % RING].n_alive, alive);
@@ -549,94 +689,10 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
     flush_acc(c, acc);
 }
 
-// tail: finish the few remaining histories of the live regions inside one kernel
-template <bool CE, bool PRIVATE>
-__global__ void __launch_bounds__(BS) k_finish(Ctx c, unsigned int s, unsigned int n0)
-{
-    extern __shared__ double s_dyn[];
-    const MGTab mg = stage_mg(c, s_dyn, CE ? 0 : c.mg_stage);
-    const Geo geo = stage_geo(c, s_dyn + (CE ? 0 : c.mg_stage), c.geo_stage);
-    double *s_flux = s_dyn + (CE ? 0 : c.mg_stage) + (c.geo_stage + 1) / 2;
-    if (PRIVATE) {
-        for (int k = threadIdx.x; k < c.n_tally * BS; k += BS) s_flux[k] = 0.0;
-        __syncthreads();
-    }
-    unsigned int n_front = n0, n_in = n0;
-    if (s > 0) {
-        QCount pc = c.qc[(s - 1) % RING];
-        n_front = pc.n_scat; n_in = pc.n_scat + pc.n_surf;
-    }
-    MCDC_EVENT_COUNTERS(acc);
-    const Bank &B = c.bank[s & 1];
-    unsigned int done = 0, born = 0, pops = 0;
-    for (unsigned int t = blockIdx.x * BS + threadIdx.x; t < n_in; t += gridDim.x * BS) {
-        unsigned int i = live_pos(c.cap, n_front, t);
-        if (B.cell[i] < 0) continue;
-        Particle p;
-        uint32_t ctr, slot;
-        load_full<CE>(B, i, p, ctr, slot);
-        Rng rng;
-        rng.init(c.seed, p.id, 0u, c.cycle, ctr);
-        unsigned int guard = 0, depth = 0;
-        StackRec *stk = CE ? c.stack + (size_t)(blockIdx.x * BS + threadIdx.x) * STACK_DEPTH : nullptr;
-        for (;;) {
-            int nch = 0, st;
-            while ((st = segment<CE, PRIVATE>(c, mg, geo, p, rng, acc, s_flux, nch)) == 1) {
-                if (++guard > 1000000u) { atomicExch(c.err, -4); atomicAdd(c.counters + 10, 1ull); break; }  // R11 guard
-            }
-            done++;
-            if (st == 2) {
-                if (!CE) record_fission<CE>(c, p, rng.ctr, slot, nch);
-                else if (nch > 0) {
-                    if (depth + (unsigned int)nch <= STACK_DEPTH) {
-                        const int mat = c.geo.cfill[p.cell];
-                        const unsigned long long pid = p.id;
-                        const uint32_t ctr0 = rng.ctr;
-                        Particle ch = p;
-                        for (int j = 0; j < nch; j++) {
-                            make_child<CE>(c, rng, mat, pid, ctr0, j, ch);
-                            StackRec r;
-                            r.x = ch.x; r.y = ch.y; r.z = ch.z; r.ux = ch.ux; r.uy = ch.uy; r.uz = ch.uz; r.E = ch.E; r.t = ch.t;
-                            r.cell = ch.cell; r.elem = ch.elem; r.tbin = ch.tbin; r.pad = 0; r.id = ch.id;
-                            stk[depth++] = r;
-                        }
-                        born += (unsigned int)nch;
-                    } else {  // stack full: an ordinary fission record in the overflow region, next wave
-                        unsigned int k = atomicAdd(c.n_over, 1u);
-                        if (k < OVER_CAP) record_fission<CE>(c, p, rng.ctr, n0 + k, nch);
-                        else atomicExch(c.err, -3);
-                    }
-                }
-            }
-            if (!CE || depth == 0) break;
-            if (++pops > 4000000u) { atomicExch(c.err, -3); break; }  // R25a: diverging chain
-            StackRec r = stk[--depth];
-            p.x = r.x; p.y = r.y; p.z = r.z; p.ux = r.ux; p.uy = r.uy; p.uz = r.uz; p.E = r.E; p.t = r.t;
-            p.cell = r.cell; p.elem = r.elem; p.tbin = r.tbin; p.id = r.id; p.last = -1; p.g = 0;
-            rng.init(c.seed, p.id, 0u, c.cycle, 0u);
-            guard = 0;
-        }
-    }
-    done = __reduce_add_sync(0xffffffffu, done);
-    born = __reduce_add_sync(0xffffffffu, born);
-    if ((threadIdx.x & 31) == 0 && done) atomicAdd(c.counters + 14, (unsigned long long)done);
-    if ((threadIdx.x & 31) == 0 && born) atomicAdd(c.counters + 15, (unsigned long long)born);
-    if (PRIVATE) flush_private_flux(c, s_flux);
-    flush_acc(c, acc);
-}
-
 // ------------------------------------------------------------------ a10/a12: fission bank by count-scan-write
-// number of fission-record slots of the running wave: its M particles plus the overflow records
-__device__ __forceinline__ unsigned int record_count(const Ctx &c, unsigned int m)
-{
-    unsigned int k = *c.n_over;
-    return m + (k < OVER_CAP ? k : OVER_CAP);
-}
-
-__global__ void __launch_bounds__(BS) k_scan_partial(Ctx c, unsigned int m, unsigned int *part)
+__global__ void __launch_bounds__(BS) k_scan_partial(Ctx c, unsigned int n, unsigned int *part)
 {
     __shared__ unsigned int s_w[BS / 32];
-    const unsigned int n = record_count(c, m);
     unsigned int i = blockIdx.x * BS + threadIdx.x;
     unsigned int v = i < n ? (unsigned int)c.fis.n[i] : 0u;
     v = __reduce_add_sync(0xffffffffu, v);
@@ -672,14 +728,13 @@ __global__ void __launch_bounds__(1024) k_scan_top(unsigned int *part, unsigned 
 // every fission parent writes its children into bank 0 at [offset(parent), +n): sorted by (parent id, child
 // index) by construction.  MG: child group ~ chi, isotropic direction (1 + 2 draws per child) from the parent's
 // stream (R5).  CE: Watt energy (4 draws) + direction (2 draws), own id from the domain-1 block (R10).
-// The children's fission counts are cleared through a second array (nn) because n is still being read.
+// The parents' counts are cleared by k_clear_counts afterwards (a child slot may be another parent's record).
 template <bool CE>
-__global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int m, const unsigned int *part, unsigned int cap)
+__global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int n, const unsigned int *part, unsigned int cap)
 {
     __shared__ unsigned int s_w[BS / 32];
     const FisRec &F = c.fis;
     const Bank &O = c.bank[0];
-    const unsigned int n = record_count(c, m);
     unsigned int i = blockIdx.x * BS + threadIdx.x;
     int nc = i < n ? F.n[i] : 0;
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -705,17 +760,17 @@ __global__ void __launch_bounds__(BS) k_emit(Ctx c, unsigned int m, const unsign
     unsigned long long pid = CE ? F.id[i] : (unsigned long long)i;
     uint32_t ctr0 = F.ctr[i];
     Rng rng;
-    rng.init(c.seed, pid, 0u, c.cycle, ctr0);
+    rng.init(pid, ctr0);
     for (int j = 0; j < nc; j++) {
         make_child<CE>(c, rng, mat, pid, ctr0, j, p);
-        store_full<CE>(O, off + j, p, 0u, off + j, 0);
+        store_full<CE>(O, off + j, p, 0u, off + j);
     }
 }
 
-__global__ void __launch_bounds__(BS) k_clear_counts(Ctx c, unsigned int m)
+__global__ void __launch_bounds__(BS) k_clear_counts(Ctx c, unsigned int n)
 {
     unsigned int i = blockIdx.x * BS + threadIdx.x;
-    if (i < record_count(c, m)) c.fis.n[i] = 0;
+    if (i < n) c.fis.n[i] = 0;
 }
 
 // cycle end: per-source-particle flux into the running mean / mean-square, clear the per-cycle tally (R17)
@@ -740,9 +795,7 @@ __global__ void k_test_draws(unsigned long long seed, uint32_t domain, uint32_t 
 {
     unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
-    Rng rng;
-    rng.init(seed, id[i], domain, cycle, draw[i]);
-    out[i] = rng.next();
+    out[i] = draw_at(seed, id[i], domain, cycle, draw[i]);
 }
 
 __global__ void k_test_grid(Ctx c, const double *E, unsigned long long n, int *ob, int *oh)
@@ -753,20 +806,52 @@ __global__ void k_test_grid(Ctx c, const double *E, unsigned long long n, int *o
     oh[i] = grid_index_hash(c.ce, E[i]);
 }
 
-__global__ void k_test_geometry(Ctx c, const double *x, const double *u, unsigned long long n, int *loc, double *dist,
-                                int *surf)
+// locate + nearest boundary of n points; path: 0 = the path the transport kernels take from that point (straight-line
+// in LAT_FAST elements, pruned enclosing-cell list elsewhere), 1 = generic loops with the pruned list, 2 = generic
+// loops over every surface of the enclosing cell (no pruning)
+__global__ void k_test_geometry(Ctx c, const double *x, const double *u, unsigned long long n, int path, int *loc,
+                                double *dist, int *surf)
 {
     unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
+    __shared__ Geo s_geo;
+    if (threadIdx.x == 0) s_geo = c.geo;
+    __syncthreads();
     if (i >= n) return;
+    const Geo &G = c.geo;
     int cell, elem, hit = -1;
-    bool ok = locate(c.geo, x[3 * i], x[3 * i + 1], x[3 * i + 2], u[3 * i], u[3 * i + 1], u[3 * i + 2], -1, cell, elem);
+    const double px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2], ux = u[3 * i], uy = u[3 * i + 1], uz = u[3 * i + 2];
+    bool ok = locate(G, px, py, pz, ux, uy, uz, -1, cell, elem);
     double d = -1.0;
-    if (ok) d = nearest(c.geo, x[3 * i], x[3 * i + 1], x[3 * i + 2], u[3 * i], u[3 * i + 1], u[3 * i + 2], cell, elem, -1, hit);
-    loc[3 * i] = !ok ? -1 : (elem >= 0 ? c.geo.lat_cell : cell);
+    if (ok) {
+        const int4 li = elem >= 0 ? __ldg(G.lat_info + elem) : __ldg(G.cell_info + cell);
+        const int cyl = elem >= 0 ? __ldg(&G.ufast[li.x & (LAT_FAST - 1)].y) : li.y;
+        if (path == 0 && (li.x & LAT_FAST)) d = nearest_fast(G, li.z, li.w, cyl, px, py, pz, ux, uy, uz, elem, -1, hit);
+        else {
+            unsigned int mask = (elem >= 0 && path != 2) ? __ldg(G.lat_rmask + elem) : 0xffffffffu;
+            d = nearest(s_geo, px, py, pz, ux, uy, uz, cell, elem, -1, hit, mask);
+        }
+    }
+    loc[3 * i] = !ok ? -1 : (elem >= 0 ? G.lat_cell : cell);
     loc[3 * i + 1] = ok ? elem : -1;
     loc[3 * i + 2] = ok && elem >= 0 ? cell : -1;
     dist[i] = d;
     surf[i] = hit;
+}
+
+// any point of an nx x ny x nz grid over the source box that lies in no cell raises the geometry error (mcdc_create)
+__global__ void k_check_source_box(Ctx c, int n1)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n1 * n1 * n1) return;
+    const int a[3] = {i % n1, (i / n1) % n1, i / (n1 * n1)};
+    double x[3];
+    for (int k = 0; k < 3; k++) {
+        double f = n1 > 1 ? (double)a[k] / (n1 - 1) : 0.5;
+        f = 1e-9 + f * (1.0 - 2e-9);  // just inside the faces
+        x[k] = c.src_lo[k] + f * (c.src_hi[k] - c.src_lo[k]);
+    }
+    int cell, elem;
+    if (!locate(c.geo, x[0], x[1], x[2], 0.0, 0.0, 1.0, -1, cell, elem)) atomicExch(c.err, -2);
 }
 
 }  // namespace mcdc

@@ -2,6 +2,7 @@
 // carving, the sweep / cycle drivers and result read-back.  All device work is in mcdc_kernels.cuh.
 #include "../../include/mcdc.h"
 #include "mcdc_kernels.cuh"
+#include "mcdc_microbench.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -31,25 +32,39 @@ static int fail(int code, const char *fmt, ...)
     } while (0)
 
 static const int LAG = 3;                 // sweeps the host may run ahead of the queue-count read-back
-static const int DEFAULT_TAIL = 32768;    // live particles at which the tail kernel takes over (multi-group)
-static const int DEFAULT_TAIL_CE = -1;    // continuous energy: no tail kernel by default (measured: 64 -> 91, 16 -> 88, none -> 83.6 ms on C5)
-// live particles below which a sweep is one fused multi-segment launch (measured on B200, profiles/r01_step4*.md)
-static const int DEFAULT_FUSE = 2000000, DEFAULT_FUSE_CE = 4000000;
-static const int DEFAULT_FUSE_SEGMENTS = 8, DEFAULT_FUSE_SEGMENTS_CE = 16;
+// live particles at or below which the persistent kernel finishes the cycle (measured on B200, profiles/r02_*.md)
+#ifndef MCDC_PERSIST_DEFAULT
+#define MCDC_PERSIST_DEFAULT 1500000
+#endif
+static const int DEFAULT_PERSIST = MCDC_PERSIST_DEFAULT;
+static const int DEFAULT_PERSIST_CE = 0x7fffffff;  // continuous energy: the whole run is one persistent launch
 static const uint64_t TRACE_BYTES = 48ull << 20;
 #ifndef MCDC_AGG_MAX
 #define MCDC_AGG_MAX 4096
 #endif
 static const int AGGREGATE_TALLY_MAX = MCDC_AGG_MAX;  // above this, equal bins inside a warp are rare: plain float64 atomics
-static const uint64_t GEO_STAGE_MAX_BYTES = 8192;  // CSG tables up to this size are staged in shared memory
 static const uint64_t MG_STAGE_MAX_BYTES = 16384;  // multi-group tables up to this size are staged in shared memory
 static const int PRIVATE_TALLY_MAX = 20;  // bins for which the one-column-per-thread tally fits (20*256*8 = 40 KB)
+static const int MAX_AXIS_PLANES = 250;   // axis planes a boundary code of the straight-line geometry path can name
 
 struct HostPinned {
     QCount qc[RING];
     double scal[4];
+    unsigned long long counters[MCDC_N_COUNTERS];
     unsigned int total;
     int err;
+};
+
+// statistics of a run; `work` is the run in progress, `pub` the state after the last call that succeeded
+// (what mcdc_get_dims / mcdc_get_tallies report: a failed call leaves it untouched)
+struct RunStats {
+    std::vector<double> k_cycle;
+    int n_active = 0;
+    double k_acc = 0, k_acc2 = 0, leak_acc = 0, leak_acc2 = 0;
+    uint64_t host_counters[MCDC_N_COUNTERS] = {0};  // [0] histories started from a source bank, [11] children banked by
+                                                    // k_emit, [12] largest bank, [13] kernel rounds
+    uint64_t counters[MCDC_N_COUNTERS] = {0};       // merged device + host counters as reported
+    int set = 0;                                    // which flux accumulator pair holds this run's tallies
 };
 
 struct mcdc_problem {
@@ -57,10 +72,11 @@ struct mcdc_problem {
     int mode;
     cudaStream_t stream;
     int device;
-    int schedule, tail, fuse, fuse_segments;
+    int schedule, persist;
+    int persist_blocks_per_sm, n_sm;  // resident blocks of the persistent kernel (occupancy query at first use)
     uint64_t cap;  // bank slots
     // workspace pieces not in ctx
-    double *flux_acc, *flux_acc2, *flux_cycle;
+    double *flux_acc[2], *flux_acc2[2], *flux_cycle;
     int flux_copies;
     unsigned int *part;
     Site *sites;
@@ -69,18 +85,13 @@ struct mcdc_problem {
     HostPinned *pin;
     cudaEvent_t ev[RING], t0, t1;
     // run state
-    uint64_t bank_count;  // sites in bank[cur] to start the next cycle from
+    uint64_t bank_count;  // sites in bank[0] to start the next cycle from
     double k_prev;
-    std::vector<double> k_cycle;
-    int n_active;
-    double k_acc, k_acc2, leak_acc, leak_acc2;
-    uint64_t host_counters[MCDC_N_COUNTERS];
+    RunStats work, pub;
+    bool dirty;  // a call failed part-way: per-cycle device tallies must be cleared before the next cycle
     double ms_transport;
     uint64_t n_launches;
     bool tally_private;
-    uint64_t trace_first;
-    uint32_t trace_n_ids, trace_max_events;
-    uint32_t trace_cap_slots;
     uint64_t last_N;
     // optional per-kernel-class timing (mcdc_set_profile): event pairs around every launch
     int profile;
@@ -88,10 +99,10 @@ struct mcdc_problem {
     std::vector<int> pool_class;  // class of pair k (events 2k, 2k+1)
     double prof_ms[MCDC_N_PROFILE];
     uint64_t prof_launches[MCDC_N_PROFILE];
-    uint64_t prof_adv_base;  // device counter 12 (events processed by k_advance) when profiling was switched on
+    uint64_t prof_sweep_base;  // device counter 12 (segments run by the sweep kernels) when profiling was switched on
 };
 
-// RAII-free helper: record an event pair around one launch when profiling is on
+// record an event pair around one launch when profiling is on
 struct ProfScope {
     mcdc_problem *p;
     size_t k;
@@ -137,22 +148,22 @@ struct Carver {
 };
 
 struct Layout {  // everything carved from the workspace, in order
-    // small tables
-    int *surf_type, *surf_bc, *cso, *csi, *css, *cft, *cfill, *cbin, *uco, *lat_univ, *lat_bin;
+    int *surf_type, *surf_bc, *cso, *csi, *css, *cft, *cfill, *cbin, *uco, *ap_sid;
+    int4 *lat_info, *ufast, *cell_info;
+    Trace *tr_g;
     unsigned int *lat_rmask;
-    double *surf_param;
-    double *sig_t, *sig_s, *sig_f, *nu, *nusf, *cumS, *cumchi, *src_cum;
+    double *surf_param, *ap_pos;
+    double *mg_blob;
+    uint64_t mg_doubles;
     double *grid, *tab, *colA, *t_edges, *e_edges;
-    int *ncol, *hash;
-    uint64_t mg_doubles, geo_words;
+    int *ncol, *hash, *ehash;
     Bank bank[2];
     FisRec fis;
-    StackRec *stack;
-    uint64_t stack_threads;
     QCount *qc;
-    double *flux, *flux_acc, *flux_acc2, *flux_cycle, *scal;
+    double *flux, *flux_acc[2], *flux_acc2[2], *flux_cycle, *scal;
     unsigned long long *counters;
     int *err;
+    unsigned int *work;
     unsigned int *part;
     Site *sites;
     char *trace;
@@ -176,8 +187,12 @@ static uint64_t n_tally_of(const mcdc_materials *mat, const mcdc_tally_spec *t)
 
 static int hash_params(const double *grid, int n, int &shift, int &lo, int &n_hash)
 {
-    // key = top bits of the IEEE-754 pattern: exponent + 8 mantissa bits => 256 buckets per octave
-    shift = 52 - 8;
+    // key = top bits of the IEEE-754 pattern: exponent + m mantissa bits => 2^m buckets per octave, m chosen so that a
+    // bucket holds about half a grid point on average (the bisection inside a bucket is then 0 or 1 probe)
+    double octaves = std::max(1.0, std::log2(grid[n - 1] / grid[0]));
+    int m = (int)std::ceil(std::log2(2.0 * n / octaves));
+    m = std::max(4, std::min(m, 12));
+    shift = 52 - m;
     long long klo, khi;
     double a = grid[0], b = grid[n - 1];
     memcpy(&klo, &a, 8);
@@ -187,35 +202,38 @@ static int hash_params(const double *grid, int n, int &shift, int &lo, int &n_ha
     return 0;
 }
 
+// energy-bin edges: 16 buckets per octave
+static const int EHASH_SHIFT = 52 - 4;
+static int ehash_buckets(const double *edges, int n_e)
+{
+    long long klo, khi;
+    memcpy(&klo, &edges[0], 8);
+    memcpy(&khi, &edges[n_e], 8);
+    return (int)(khi >> EHASH_SHIFT) - (int)(klo >> EHASH_SHIFT) + 1;
+}
+
 static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materials *m, const mcdc_xs *x,
                   const mcdc_tally_spec *t, uint64_t cap)
 {
     Carver C(ws);
     int nref = g->cell_surf_off[g->n_cell];
     int nlat = g->has_lattice ? g->lat_nx * g->lat_ny : 0;
-    // one contiguous blob (staged in shared memory by the kernels): surface parameters first (8-byte aligned),
-    // then the int tables
-    {
-        uint64_t ns = g->n_surf, nc = g->n_cell;
-        uint64_t n_int = 2 * ns + (nc + 1) + 2 * (uint64_t)nref + 3 * nc + (g->n_univ + 1);
-        L.geo_words = 8 * ns + n_int;
-        L.surf_param = C.take<double>(4 * ns + (n_int + 1) / 2);
-        int *ip = (int *)(L.surf_param + 4 * ns);
-        L.surf_type = ip; ip += ns; L.surf_bc = ip; ip += ns;
-        L.cso = ip; ip += nc + 1; L.csi = ip; ip += nref; L.css = ip; ip += nref;
-        L.cft = ip; ip += nc; L.cfill = ip; ip += nc; L.cbin = ip; ip += nc;
-        L.uco = ip;
-    }
-    L.lat_univ = C.take<int>(nlat); L.lat_bin = C.take<int>(nlat); L.lat_rmask = C.take<unsigned int>(nlat);
+    uint64_t ns = g->n_surf, nc = g->n_cell;
+    L.surf_param = C.take<double>(4 * ns); L.surf_type = C.take<int>(ns); L.surf_bc = C.take<int>(ns);
+    L.cso = C.take<int>(nc + 1); L.csi = C.take<int>(nref); L.css = C.take<int>(nref);
+    L.cft = C.take<int>(nc); L.cfill = C.take<int>(nc); L.cbin = C.take<int>(nc); L.uco = C.take<int>(g->n_univ + 1);
+    L.ufast = C.take<int4>(g->n_univ);
+    L.cell_info = C.take<int4>(nc);
+    L.tr_g = C.take<Trace>(1);
+    L.ap_pos = C.take<double>(MAX_AXIS_PLANES); L.ap_sid = C.take<int>(MAX_AXIS_PLANES);
+    L.lat_info = C.take<int4>(nlat); L.lat_rmask = C.take<unsigned int>(nlat);
     bool ce = x != nullptr;
     if (!ce) {
         uint64_t mg = (uint64_t)m->n_mat * m->G;
         // one contiguous blob (staged in shared memory by the kernels): six [n_mat][G] tables, cumS, src_cum
         L.mg_doubles = 6 * mg + mg * m->G + m->G;
-        L.sig_t = C.take<double>(L.mg_doubles);
-        L.sig_s = L.sig_t + mg; L.sig_f = L.sig_s + mg; L.nu = L.sig_f + mg; L.nusf = L.nu + mg; L.cumchi = L.nusf + mg;
-        L.cumS = L.cumchi + mg; L.src_cum = L.cumS + mg * m->G;
-        L.grid = L.tab = L.colA = L.t_edges = L.e_edges = nullptr; L.ncol = L.hash = nullptr;
+        L.mg_blob = C.take<double>(L.mg_doubles);
+        L.grid = L.tab = L.colA = L.t_edges = L.e_edges = nullptr; L.ncol = L.hash = L.ehash = nullptr;
     } else {
         int sh, lo, nh;
         hash_params(x->grid, x->n_grid, sh, lo, nh);
@@ -224,8 +242,9 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         L.colA = C.take<double>((uint64_t)x->n_mat * CE_ROW);
         L.ncol = C.take<int>(x->n_mat);
         L.hash = C.take<int>(nh + 2);
+        L.ehash = C.take<int>(ehash_buckets(t->e_edges, t->n_e) + 2);
         L.t_edges = C.take<double>(t->n_t + 1); L.e_edges = C.take<double>(t->n_e + 1);
-        L.sig_t = L.sig_s = L.sig_f = L.nu = L.nusf = L.cumS = L.cumchi = L.src_cum = nullptr;
+        L.mg_blob = nullptr;
         L.mg_doubles = 0;
     }
     for (int b = 0; b < 2; b++) {
@@ -235,30 +254,29 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         B.E = ce ? C.take<double>(cap) : nullptr; B.t = ce ? C.take<double>(cap) : nullptr;
         B.cell = C.take<int>(cap); B.elem = C.take<int>(cap); B.gl = C.take<int>(cap);
         B.tbin = ce ? C.take<int>(cap) : nullptr;
-        B.ev = C.take<int>(cap);
+        B.ev = C.take<uint32_t>(cap);
         B.ctr = C.take<uint32_t>(cap); B.slot = C.take<uint32_t>(cap);
         B.id = ce ? C.take<uint64_t>(cap) : nullptr;
     }
     {
         FisRec &F = L.fis;
-        const uint64_t fc = cap + OVER_CAP;  // the wave's slots + the tail kernel's overflow records
-        F.n = C.take<int>(fc); F.cell = C.take<int>(fc); F.elem = C.take<int>(fc);
-        F.tbin = ce ? C.take<int>(fc) : nullptr;
-        F.x = C.take<double>(fc); F.y = C.take<double>(fc); F.z = C.take<double>(fc);
-        F.t = ce ? C.take<double>(fc) : nullptr;
-        F.ctr = C.take<uint32_t>(fc);
-        F.id = ce ? C.take<uint64_t>(fc) : nullptr;
+        F.n = C.take<int>(cap); F.cell = C.take<int>(cap); F.elem = C.take<int>(cap);
+        F.tbin = ce ? C.take<int>(cap) : nullptr;
+        F.x = C.take<double>(cap); F.y = C.take<double>(cap); F.z = C.take<double>(cap);
+        F.t = ce ? C.take<double>(cap) : nullptr;
+        F.ctr = C.take<uint32_t>(cap);
+        F.id = ce ? C.take<uint64_t>(cap) : nullptr;
     }
-    L.stack_threads = ce ? std::min<uint64_t>(148ull * 16ull * 256, (cap + BS - 1) / BS * BS) : 0;
-    L.stack = C.take<StackRec>(L.stack_threads * STACK_DEPTH);
     L.qc = C.take<QCount>(RING);
     uint64_t nt = n_tally_of(m, t);
-    L.flux = C.take<double>(nt * flux_copies_for(nt)); L.flux_acc = C.take<double>(nt); L.flux_acc2 = C.take<double>(nt);
+    L.flux = C.take<double>(nt * flux_copies_for(nt));
+    for (int k = 0; k < 2; k++) { L.flux_acc[k] = C.take<double>(nt); L.flux_acc2[k] = C.take<double>(nt); }
     L.flux_cycle = C.take<double>(nt);
     L.scal = C.take<double>(8);
     L.counters = C.take<unsigned long long>(MCDC_N_COUNTERS);
     L.err = C.take<int>(4);
-    L.part = C.take<unsigned int>((cap + OVER_CAP) / BS + 4);
+    L.work = C.take<unsigned int>(8);
+    L.part = C.take<unsigned int>(cap / BS + 4);
     L.sites = C.take<Site>(cap);
     L.trace = C.take<char>(TRACE_BYTES);
     L.trace_count = C.take<unsigned int>(TRACE_BYTES / sizeof(TraceRec) + 1);
@@ -275,17 +293,24 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
     if (!g || !s || !t) return fail(MCDC_EINVAL, "null geometry / source / tally");
     if ((m != nullptr) == (x != nullptr)) return fail(MCDC_EINVAL, "exactly one of materials (MG) and xs (CE) must be given");
     if (g->n_cell < 1 || g->n_univ < 1 || g->n_surf < 0) return fail(MCDC_EINVAL, "empty geometry");
-    if (g->n_surf > 30000) return fail(MCDC_EINVAL, "too many surfaces");
+    if (g->n_surf > MAX_SURFACES) return fail(MCDC_EINVAL, "too many surfaces (at most %d)", MAX_SURFACES);
+    if (t->n_bins < 1) return fail(MCDC_EINVAL, "n_bins");
     int n_mat = m ? m->n_mat : x->n_mat;
     int n_lat_cells = 0;
+    if (g->cell_surf_off[0] != 0) return fail(MCDC_EINVAL, "cell_surf_off[0] must be 0");
+    if (g->univ_cell_off[0] != 0 || g->univ_cell_off[g->n_univ] != g->n_cell) return fail(MCDC_EINVAL, "univ_cell_off must run from 0 to n_cell");
+    for (int u = 0; u < g->n_univ; u++)
+        if (g->univ_cell_off[u + 1] < g->univ_cell_off[u]) return fail(MCDC_EINVAL, "univ_cell_off not monotone");
     for (int c = 0; c < g->n_cell; c++) {
         if (g->cell_surf_off[c + 1] < g->cell_surf_off[c]) return fail(MCDC_EINVAL, "cell_surf_off not monotone");
         for (int k = g->cell_surf_off[c]; k < g->cell_surf_off[c + 1]; k++) {
             if (g->cell_surf_id[k] < 0 || g->cell_surf_id[k] >= g->n_surf) return fail(MCDC_EGEOM, "cell %d names surface %d", c, g->cell_surf_id[k]);
             if (g->cell_surf_sense[k] != 1 && g->cell_surf_sense[k] != -1) return fail(MCDC_EGEOM, "sense must be +-1");
         }
-        if (g->cell_fill_type[c] == 1) n_lat_cells++;
-        else if (g->cell_fill[c] < 0 || g->cell_fill[c] >= n_mat) return fail(MCDC_EINVAL, "cell %d material %d out of range", c, g->cell_fill[c]);
+        if (g->cell_fill_type[c] == 1) {
+            n_lat_cells++;
+            if (c >= g->univ_cell_off[1]) return fail(MCDC_EGEOM, "the lattice-filled cell must belong to the root universe");
+        } else if (g->cell_fill[c] < 0 || g->cell_fill[c] >= n_mat) return fail(MCDC_EINVAL, "cell %d material %d out of range", c, g->cell_fill[c]);
         if (t->cell_bin[c] < 0 || t->cell_bin[c] >= t->n_bins) return fail(MCDC_EINVAL, "cell_bin out of range");
     }
     for (int sidx = 0; sidx < g->n_surf; sidx++) {
@@ -297,11 +322,18 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
         if (g->lat_nx < 1 || g->lat_ny < 1 || !(g->lat_px > 0) || !(g->lat_py > 0)) return fail(MCDC_EGEOM, "lattice shape");
         if ((unsigned long long)g->lat_nx * g->lat_nx * g->lat_ny >= 0x100000000ull) return fail(MCDC_EGEOM, "lattice too large (nx*nx*ny must be < 2^32)");
         if (!t->lat_bin) return fail(MCDC_EINVAL, "lat_bin missing");
+        int max_lat_bin = 0;
         for (int e = 0; e < g->lat_nx * g->lat_ny; e++) {
             if (g->lat_univ[e] < 1 || g->lat_univ[e] >= g->n_univ) return fail(MCDC_EGEOM, "lattice element %d names universe %d", e, g->lat_univ[e]);
             if (t->lat_bin[e] < 0 || t->lat_bin[e] >= t->n_bins) return fail(MCDC_EINVAL, "lat_bin out of range");
+            max_lat_bin = std::max(max_lat_bin, t->lat_bin[e]);
         }
+        // inside the lattice the bin is cell_bin[local cell] + lat_bin[element]: the sum must stay inside the tally
+        for (int c = g->univ_cell_off[1]; c < g->n_cell; c++)
+            if (t->cell_bin[c] + max_lat_bin >= t->n_bins) return fail(MCDC_EINVAL, "cell_bin[%d] + max lat_bin reaches past n_bins", c);
     } else if (n_lat_cells) return fail(MCDC_EGEOM, "lattice-filled cell without a lattice");
+    for (int k = 0; k < 3; k++)
+        if (!(s->hi[k] >= s->lo[k])) return fail(MCDC_EINVAL, "source box: hi < lo on axis %d", k);
     if (m) {
         if (m->G < 1 || m->G > 4096 || m->n_mat < 1) return fail(MCDC_EINVAL, "G / n_mat");
         for (int i = 0; i < m->n_mat * m->G; i++) {
@@ -320,6 +352,7 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
         for (int i = 1; i < x->n_grid; i++)
             if (!(x->grid[i] > x->grid[i - 1])) return fail(MCDC_EINVAL, "union grid not strictly increasing at %d", i);
         if (!(x->grid[0] > 0.0)) return fail(MCDC_EINVAL, "grid must be positive");
+        if (x->mat_nuc_off[0] != 0) return fail(MCDC_EINVAL, "mat_nuc_off[0] must be 0");
         for (int mm = 0; mm < x->n_mat; mm++) {
             int nn = x->mat_nuc_off[mm + 1] - x->mat_nuc_off[mm];
             if (nn < 1 || nn + 2 > MAX_CE_COL) return fail(MCDC_EINVAL, "material %d: 1..%d nuclides supported", mm, MAX_CE_COL - 2);
@@ -329,8 +362,9 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
         if (t->n_t < 1 || t->n_e < 1 || !t->t_edges || !t->e_edges) return fail(MCDC_EINVAL, "CE tally edges");
         for (int i = 0; i < t->n_t; i++) if (!(t->t_edges[i + 1] > t->t_edges[i])) return fail(MCDC_EINVAL, "t_edges");
         for (int i = 0; i < t->n_e; i++) if (!(t->e_edges[i + 1] > t->e_edges[i])) return fail(MCDC_EINVAL, "e_edges");
+        if (!(s->t >= t->t_edges[0]) || !(s->t < t->t_edges[t->n_t])) return fail(MCDC_EINVAL, "source time outside the time edges");
+        if (!(s->E > 0.0)) return fail(MCDC_EINVAL, "source energy");
     }
-    if (t->n_bins < 1) return fail(MCDC_EINVAL, "n_bins");
     return 0;
 }
 
@@ -350,6 +384,26 @@ template <class T> static cudaError_t up(T *dst, const T *src, uint64_t n, cudaS
     return cudaMemcpyAsync(dst, src, n * sizeof(T), cudaMemcpyHostToDevice, st);
 }
 
+// Per-universe shape used by the straight-line geometry path: one cell without surfaces, or two cells that are the
+// inside (-) and the outside (+) of one z-cylinder and nothing else.
+static void classify_universes(const mcdc_geometry *g, std::vector<int4> &uf)
+{
+    uf.assign(g->n_univ, make_int4(0, -1, -1, -1));
+    for (int u = 1; u < g->n_univ; u++) {
+        int c0 = g->univ_cell_off[u], nc = g->univ_cell_off[u + 1] - c0;
+        auto nsurf = [&](int c) { return g->cell_surf_off[c + 1] - g->cell_surf_off[c]; };
+        if (nc == 1 && nsurf(c0) == 0 && g->cell_fill_type[c0] == 0) uf[u] = make_int4(1, -1, c0, c0);
+        else if (nc == 2 && nsurf(c0) == 1 && nsurf(c0 + 1) == 1 && g->cell_fill_type[c0] == 0 && g->cell_fill_type[c0 + 1] == 0) {
+            int ka = g->cell_surf_off[c0], kb = g->cell_surf_off[c0 + 1];
+            int sa = g->cell_surf_id[ka], sb = g->cell_surf_id[kb];
+            if (sa == sb && g->surf_type[sa] == MCDC_CYL_Z && g->cell_surf_sense[ka] == -g->cell_surf_sense[kb]) {
+                int in = g->cell_surf_sense[ka] < 0 ? c0 : c0 + 1;
+                uf[u] = make_int4(1, sa, in, in == c0 ? c0 + 1 : c0);
+            }
+        }
+    }
+}
+
 extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_xs *x, const mcdc_source *s,
                            const mcdc_tally_spec *t, const mcdc_device *dev, uint64_t max_particles, mcdc_problem **out)
 {
@@ -360,6 +414,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     if (!dev || !dev->workspace) return fail(MCDC_EINVAL, "device workspace missing");
     if (((uintptr_t)dev->workspace & 255u) != 0) return fail(MCDC_EINVAL, "workspace must be 256-byte aligned");
     if (max_particles < 1 || max_particles > 1000000000ull) return fail(MCDC_EINVAL, "max_particles");
+    if (dev->schedule < 0 || dev->schedule > 2) return fail(MCDC_EINVAL, "schedule must be 0, 1 or 2");
     uint64_t cap = capacity_for(max_particles);
     Layout L;
     carve(L, dev->workspace, g, m, x, t, cap);
@@ -373,9 +428,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     p->stream = st;
     p->device = dev->device;
     p->schedule = dev->schedule;
-    p->tail = dev->tail_threshold == 0 ? (x ? DEFAULT_TAIL_CE : DEFAULT_TAIL) : dev->tail_threshold;
-    p->fuse = dev->fuse_threshold == 0 ? (x ? DEFAULT_FUSE_CE : DEFAULT_FUSE) : dev->fuse_threshold;
-    p->fuse_segments = dev->fuse_segments <= 0 ? (x ? DEFAULT_FUSE_SEGMENTS_CE : DEFAULT_FUSE_SEGMENTS) : dev->fuse_segments;
+    p->persist = dev->persist_threshold == 0 ? (x ? DEFAULT_PERSIST_CE : DEFAULT_PERSIST) : dev->persist_threshold;
     p->cap = cap;
     Ctx &c = p->ctx;
     c.mode = p->mode;
@@ -388,16 +441,17 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     G.lat_nx = g->has_lattice ? g->lat_nx : 1; G.lat_ny = g->has_lattice ? g->lat_ny : 1;
     G.lat_x0 = g->lat_x0; G.lat_y0 = g->lat_y0; G.lat_px = g->lat_px; G.lat_py = g->lat_py;
     G.lat_cell = -1;
-    G.lat_magic = (unsigned int)(0x100000000ull / (unsigned long long)G.lat_nx) + 1u;
+    G.lat_magic = G.lat_nx > 1 ? (unsigned int)(0x100000000ull / (unsigned long long)G.lat_nx) + 1u : 0u;
     for (int cc = 0; cc < g->n_cell; cc++) if (g->cell_fill_type[cc] == 1) G.lat_cell = cc;
     G.surf_type = L.surf_type; G.surf_bc = L.surf_bc; G.surf_param = L.surf_param;
     G.cso = L.cso; G.csi = L.csi; G.css = L.css; G.cft = L.cft; G.cfill = L.cfill; G.cbin = L.cbin; G.uco = L.uco;
-    G.lat_univ = L.lat_univ; G.lat_bin = L.lat_bin; G.lat_rmask = L.lat_rmask;
-    G.blob = (const char *)L.surf_param; G.blob_words = (int)L.geo_words;
-    c.geo_stage = L.geo_words * 4 <= GEO_STAGE_MAX_BYTES ? (int)L.geo_words : 0;
+    G.lat_info = L.lat_info; G.cell_info = L.cell_info; G.lat_rmask = L.lat_rmask; G.ufast = L.ufast;
+    G.ap_pos = L.ap_pos; G.ap_sid = L.ap_sid;
     // host staging must outlive the async copies: keep vectors until the sync at the end
-    std::vector<double> h_sig_s, h_nusf, h_cumS, h_cumchi, h_srccum, h_tab, h_colA;
-    std::vector<int> h_ncol, h_hash, h_cfill(g->cell_fill, g->cell_fill + g->n_cell);
+    std::vector<double> h_mg, h_tab, h_colA, h_ap_pos;
+    std::vector<int> h_ncol, h_hash, h_ehash, h_cfill(g->cell_fill, g->cell_fill + g->n_cell), h_ap_sid;
+    std::vector<int4> h_ufast, h_latinfo(nlat), h_cellinfo(g->n_cell);
+    std::vector<unsigned int> h_rmask(nlat);
     for (int cc = 0; cc < g->n_cell; cc++) if (g->cell_fill_type[cc] == 1) h_cfill[cc] = 0;
     cudaError_t e = cudaSuccess;
 #define UP(dst, src, n) do { if (e == cudaSuccess) e = up(dst, src, (uint64_t)(n), st); } while (0)
@@ -406,69 +460,124 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     UP(L.cso, g->cell_surf_off, g->n_cell + 1); UP(L.csi, g->cell_surf_id, nref); UP(L.css, g->cell_surf_sense, nref);
     UP(L.cft, g->cell_fill_type, g->n_cell); UP(L.cfill, h_cfill.data(), g->n_cell); UP(L.cbin, t->cell_bin, g->n_cell);
     UP(L.uco, g->univ_cell_off, g->n_univ + 1);
-    // lattice element -> tally bin, plus which of the enclosing cell's surfaces must be tested from inside the
-    // element (bit mask over the cell's surface list; flag bit 30 of lat_bin = mask != 0).  A surface is dropped
-    // only where it is provably never the nearest candidate: an axis plane x = p (y = p) lying strictly beyond a
-    // wall of the element that is itself an event (an interior lattice wall, R14) -- the ray crosses that wall
-    // first.  Any other surface type, and planes beyond an outermost (non-event) wall, stay in the mask.
-    std::vector<int> h_latbin(nlat);
-    std::vector<unsigned int> h_rmask(nlat);
+    classify_universes(g, h_ufast);
+    UP(L.ufast, h_ufast.data(), g->n_univ);
+    // every axis plane of the problem gets an index the boundary codes can name (the first MAX_AXIS_PLANES of them)
+    std::vector<int> ap_of(g->n_surf, -1);
+    for (int sidx = 0; sidx < g->n_surf; sidx++)
+        if (g->surf_type[sidx] <= MCDC_PLANE_Z && (int)h_ap_pos.size() < MAX_AXIS_PLANES) {
+            ap_of[sidx] = (int)h_ap_pos.size();
+            h_ap_pos.push_back(g->surf_param[4 * sidx]);
+            h_ap_sid.push_back(sidx);
+        }
+    G.n_ap = (int)h_ap_pos.size();
+    UP(L.ap_pos, h_ap_pos.data(), h_ap_pos.size()); UP(L.ap_sid, h_ap_sid.data(), h_ap_sid.size());
+    // cells outside a lattice: the straight-line path applies when the cell is bounded by axis planes (one per
+    // direction at most) and at most one z-cylinder; the cell across that cylinder is known when exactly one other
+    // cell of the universe lists the cylinder with the opposite sense
+    for (int cc = 0; cc < g->n_cell; cc++) {
+        int code[6] = {0, 0, 0, 0, 0, 0}, cyl = -1, cyl_sense = 0;
+        bool fast = g->cell_fill_type[cc] == 0;
+        for (int k = g->cell_surf_off[cc]; k < g->cell_surf_off[cc + 1] && fast; k++) {
+            int sidx = g->cell_surf_id[k], sense = g->cell_surf_sense[k], typ = g->surf_type[sidx];
+            if (typ <= MCDC_PLANE_Z) {
+                int slot = 2 * typ + (sense > 0 ? 0 : 1);
+                if (ap_of[sidx] < 0 || code[slot] != 0) fast = false;
+                else code[slot] = 2 + ap_of[sidx];
+            } else if (typ == MCDC_CYL_Z && cyl < 0) { cyl = sidx; cyl_sense = sense; }
+            else fast = false;
+        }
+        int nb = CELL_NO_NEIGHBOUR;
+        if (fast && cyl >= 0) {
+            int u = 0;
+            while (cc >= g->univ_cell_off[u + 1]) u++;
+            int found = 0;
+            for (int c2 = g->univ_cell_off[u]; c2 < g->univ_cell_off[u + 1]; c2++)
+                for (int k = g->cell_surf_off[c2]; k < g->cell_surf_off[c2 + 1]; k++)
+                    if (c2 != cc && g->cell_surf_id[k] == cyl && g->cell_surf_sense[k] == -cyl_sense) { nb = c2; found++; }
+            if (found != 1 || g->cell_fill_type[nb] != 0) nb = CELL_NO_NEIGHBOUR;
+        }
+        h_cellinfo[cc] = make_int4((fast ? CELL_FAST : 0) | nb, fast ? cyl : -1, code[0] | (code[1] << 8) | (code[2] << 16) | (code[3] << 24),
+                                   code[4] | (code[5] << 8));
+    }
+    UP(L.cell_info, h_cellinfo.data(), g->n_cell);
+    // Per lattice element: which of the enclosing cell's surfaces must be tested from inside it (bit mask over the
+    // cell's surface list).  A surface is dropped only where it is provably never the nearest candidate: an axis
+    // plane x = p (y = p) lying strictly beyond a wall of the element that is itself an event (an interior lattice
+    // wall, R14) -- the ray crosses that wall first.  Any other surface type, and planes beyond an outermost
+    // (non-event) wall, stay in the mask.  Then the boundary codes of the straight-line path: per direction either
+    // the lattice wall (an event) or ONE needed axis plane of the enclosing cell; an element whose needed surfaces
+    // do not fit this pattern, or whose universe is not of the simple shape, keeps the generic path.
     if (nlat) {
         int lc = G.lat_cell;
+        int k0 = g->cell_surf_off[lc], nroot = g->cell_surf_off[lc + 1] - k0;
         for (int iy = 0; iy < g->lat_ny; iy++)
             for (int ix = 0; ix < g->lat_nx; ix++) {
                 unsigned int mask = 0u;
                 double xlo = g->lat_x0 + ix * g->lat_px, xhi = g->lat_x0 + (ix + 1) * g->lat_px;
                 double ylo = g->lat_y0 + iy * g->lat_py, yhi = g->lat_y0 + (iy + 1) * g->lat_py;
                 double tx = 1e-9 * g->lat_px, ty = 1e-9 * g->lat_py;
-                for (int k = g->cell_surf_off[lc]; k < g->cell_surf_off[lc + 1]; k++) {
-                    int sidx = g->cell_surf_id[k], j = k - g->cell_surf_off[lc];
+                // codes: slots 0..5 = -x,+x,-y,+y,-z,+z; walls that are events first
+                int code[6] = {ix > 0 ? 1 : 0, ix + 1 < g->lat_nx ? 1 : 0, iy > 0 ? 1 : 0, iy + 1 < g->lat_ny ? 1 : 0, 0, 0};
+                bool fast = nroot <= 32;
+                for (int j = 0; j < nroot; j++) {
+                    int sidx = g->cell_surf_id[k0 + j], sense = g->cell_surf_sense[k0 + j];
                     double pp = g->surf_param[4 * sidx];
+                    int typ = g->surf_type[sidx];
                     bool need = true;
-                    if (g->surf_type[sidx] == MCDC_PLANE_X)
+                    if (typ == MCDC_PLANE_X)
                         need = !((pp > xhi + tx && ix + 1 < g->lat_nx) || (pp < xlo - tx && ix > 0));
-                    else if (g->surf_type[sidx] == MCDC_PLANE_Y)
+                    else if (typ == MCDC_PLANE_Y)
                         need = !((pp > yhi + ty && iy + 1 < g->lat_ny) || (pp < ylo - ty && iy > 0));
                     if (j >= 32) { if (need) mask |= 0x80000000u; }  // past the 32nd surface: always tested
                     else if (need) mask |= 1u << j;
+                    if (!need) continue;
+                    if (typ > MCDC_PLANE_Z || ap_of[sidx] < 0) { fast = false; continue; }
+                    // the cell lies on the `sense` side of the plane: it bounds the flight in the opposite direction
+                    int slot = 2 * typ + (sense > 0 ? 0 : 1);
+                    if (code[slot] != 0) fast = false;  // a lattice wall or another plane already bounds that direction
+                    else code[slot] = 2 + ap_of[sidx];
                 }
                 int e_ = iy * g->lat_nx + ix;
+                int u = g->lat_univ[e_];
+                if (!h_ufast[u].x) fast = false;
                 h_rmask[e_] = mask;
-                h_latbin[e_] = t->lat_bin[e_] | (mask ? LAT_ROOT_FLAG : 0);
+                h_latinfo[e_] = make_int4(u | (fast ? LAT_FAST : 0), t->lat_bin[e_],
+                                          code[0] | (code[1] << 8) | (code[2] << 16) | (code[3] << 24), code[4] | (code[5] << 8));
             }
-        UP(L.lat_univ, g->lat_univ, nlat); UP(L.lat_bin, h_latbin.data(), nlat); UP(L.lat_rmask, h_rmask.data(), nlat);
+        UP(L.lat_info, h_latinfo.data(), nlat); UP(L.lat_rmask, h_rmask.data(), nlat);
     }
 
     // ---- cross sections: derived tables built here, in plain left-to-right float64 sums
     if (m) {
         int Gn = m->G, nm = m->n_mat;
-        h_sig_s.assign((size_t)nm * Gn, 0.0); h_nusf.assign((size_t)nm * Gn, 0.0);
-        h_cumS.assign((size_t)nm * Gn * Gn, 0.0); h_cumchi.assign((size_t)nm * Gn, 0.0); h_srccum.assign(Gn, 0.0);
+        size_t mg = (size_t)nm * Gn;
+        MGTab &T = c.mg;
+        T.G = Gn; T.n_mat = nm; T.blob = L.mg_blob; T.blob_doubles = (int)L.mg_doubles;
+        T.o_sig_t = 0; T.o_sig_s = (int)mg; T.o_sig_f = (int)(2 * mg); T.o_nu = (int)(3 * mg); T.o_nusf = (int)(4 * mg);
+        T.o_cumchi = (int)(5 * mg); T.o_cumS = (int)(6 * mg); T.o_src_cum = (int)(6 * mg + mg * Gn);
+        h_mg.assign(L.mg_doubles, 0.0);
         for (int mm = 0; mm < nm; mm++) {
             double cc = 0.0;
             for (int gg = 0; gg < Gn; gg++) {
                 double cs = 0.0;
                 for (int gp = 0; gp < Gn; gp++) {
                     cs += m->S[((size_t)mm * Gn + gg) * Gn + gp];
-                    h_cumS[((size_t)mm * Gn + gg) * Gn + gp] = cs;
+                    h_mg[T.o_cumS + ((size_t)mm * Gn + gg) * Gn + gp] = cs;
                 }
-                h_sig_s[mm * Gn + gg] = cs;
-                cc += m->chi[mm * Gn + gg];
-                h_cumchi[mm * Gn + gg] = cc;
-                h_nusf[mm * Gn + gg] = m->nu[mm * Gn + gg] * m->sig_f[mm * Gn + gg];
+                int i = mm * Gn + gg;
+                h_mg[T.o_sig_t + i] = m->sig_t[i]; h_mg[T.o_sig_f + i] = m->sig_f[i]; h_mg[T.o_nu + i] = m->nu[i];
+                h_mg[T.o_sig_s + i] = cs;
+                cc += m->chi[i];
+                h_mg[T.o_cumchi + i] = cc;
+                h_mg[T.o_nusf + i] = m->nu[i] * m->sig_f[i];
             }
         }
         double cs = 0.0;
-        for (int gg = 0; gg < Gn; gg++) { cs += s->group_pdf[gg]; h_srccum[gg] = cs; }
+        for (int gg = 0; gg < Gn; gg++) { cs += s->group_pdf[gg]; h_mg[T.o_src_cum + gg] = cs; }
         if (!(cs > 0.0)) { delete p; return fail(MCDC_EINVAL, "source group pdf sums to zero"); }
-        UP(L.sig_t, m->sig_t, nm * Gn); UP(L.sig_f, m->sig_f, nm * Gn); UP(L.nu, m->nu, nm * Gn);
-        UP(L.sig_s, h_sig_s.data(), nm * Gn); UP(L.nusf, h_nusf.data(), nm * Gn);
-        UP(L.cumS, h_cumS.data(), (size_t)nm * Gn * Gn); UP(L.cumchi, h_cumchi.data(), nm * Gn);
-        UP(L.src_cum, h_srccum.data(), Gn);
-        c.mg.G = Gn; c.mg.n_mat = nm; c.mg.blob = L.sig_t; c.mg.blob_doubles = (int)L.mg_doubles;
+        UP(L.mg_blob, h_mg.data(), h_mg.size());
         c.mg_stage = L.mg_doubles * 8 <= MG_STAGE_MAX_BYTES ? (int)L.mg_doubles : 0;
-        c.mg.sig_t = L.sig_t; c.mg.sig_s = L.sig_s; c.mg.sig_f = L.sig_f; c.mg.nu = L.nu; c.mg.nusf = L.nusf;
-        c.mg.cumS = L.cumS; c.mg.cumchi = L.cumchi; c.mg.src_cum = L.src_cum;
         c.n_tally = t->n_bins * Gn;
     } else {
         int ng = x->n_grid, nm = x->n_mat;
@@ -491,6 +600,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
                 cum += sf; row[nn] = cum;
                 cum += sc; row[nn + 1] = cum;
                 for (int j = nn + 2; j < MAX_CE_COL; j++) row[j] = cum;
+                row[6] = x->grid[i];
                 row[7] = sf;
                 if (!(cum > 0.0)) { delete p; return fail(MCDC_EINVAL, "material %d has zero total cross section at grid point %d", mm, i); }
             }
@@ -507,6 +617,23 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
             h_hash[b] = idx < 0 ? 0 : idx;
         }
         h_hash[nh + 1] = ng - 1;
+        // the same for the tally's energy-bin edges
+        {
+            long long klo;
+            memcpy(&klo, &t->e_edges[0], 8);
+            int elo = (int)(klo >> EHASH_SHIFT), neh = ehash_buckets(t->e_edges, t->n_e);
+            h_ehash.assign(neh + 2, 0);
+            for (int b = 0; b <= neh; b++) {
+                long long bits = ((long long)(elo + b)) << EHASH_SHIFT;
+                double edge;
+                memcpy(&edge, &bits, 8);
+                int idx = (int)(std::upper_bound(t->e_edges, t->e_edges + t->n_e + 1, edge) - t->e_edges) - 1;
+                h_ehash[b] = idx < 0 ? 0 : idx;
+            }
+            h_ehash[neh + 1] = t->n_e;
+            c.ce.ehash = L.ehash; c.ce.ehash_shift = EHASH_SHIFT; c.ce.ehash_lo = elo; c.ce.n_ehash = neh;
+            UP(L.ehash, h_ehash.data(), neh + 2);
+        }
         UP(L.grid, x->grid, ng); UP(L.tab, h_tab.data(), h_tab.size()); UP(L.colA, h_colA.data(), h_colA.size());
         UP(L.ncol, h_ncol.data(), nm); UP(L.hash, h_hash.data(), nh + 2);
         UP(L.t_edges, t->t_edges, t->n_t + 1); UP(L.e_edges, t->e_edges, t->n_e + 1);
@@ -521,43 +648,54 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     c.n_bins = t->n_bins;
     for (int b = 0; b < 2; b++) c.bank[b] = L.bank[b];
     c.fis = L.fis;
-    c.stack = L.stack; c.stack_threads = (unsigned int)L.stack_threads; c.n_over = (unsigned int *)(L.err + 1);
+    c.work = L.work;
     c.cap = (unsigned int)cap;
     c.qc = L.qc; c.flux = L.flux; c.scal = L.scal; c.counters = L.counters; c.err = L.err;
     c.tr.rec = nullptr;
+    c.tr_g = L.tr_g;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(L.tr_g, &c.tr, sizeof(Trace), cudaMemcpyHostToDevice, st);
     for (int k = 0; k < 3; k++) { c.src_lo[k] = s->lo[k]; c.src_hi[k] = s->hi[k]; c.src_dir[k] = s->dir[k]; }
     c.src_iso = s->isotropic; c.src_E = s->E; c.src_t = s->t;
     c.w0 = 1.0; c.k_prev = 1.0;
-    p->flux_acc = L.flux_acc; p->flux_acc2 = L.flux_acc2; p->flux_cycle = L.flux_cycle;
+    c.max_secondaries = ~0ull;
+    for (int k = 0; k < 2; k++) { p->flux_acc[k] = L.flux_acc[k]; p->flux_acc2[k] = L.flux_acc2[k]; }
+    p->flux_cycle = L.flux_cycle;
     p->flux_copies = flux_copies_for((uint64_t)c.n_tally);
     c.flux_copy_mask = p->flux_copies - 1;
     p->part = L.part; p->sites = L.sites;
     p->trace_base = L.trace; p->trace_count = L.trace_count;
     p->tally_private = c.n_tally <= PRIVATE_TALLY_MAX;
-    if (p->tally_private && (size_t)c.mg_stage * 8 + (size_t)c.geo_stage * 4 + 8 + (size_t)c.n_tally * BS * 8 > 48 * 1024)
-        c.mg_stage = c.geo_stage = 0;  // 48 KB default dynamic shared memory limit
+    if (p->tally_private && (size_t)c.mg_stage * 8 + (size_t)c.n_tally * BS * 8 > 48 * 1024)
+        c.mg_stage = 0;  // 48 KB default dynamic shared memory limit
     c.flux_aggregate = c.n_tally <= AGGREGATE_TALLY_MAX ? 1 : 0;
     if (e == cudaSuccess) e = cudaMemsetAsync(L.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc, 0, sizeof(double) * c.n_tally, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc2, 0, sizeof(double) * c.n_tally, st);
+    for (int k = 0; k < 2 && e == cudaSuccess; k++) {
+        e = cudaMemsetAsync(L.flux_acc[k], 0, sizeof(double) * c.n_tally, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(L.flux_acc2[k], 0, sizeof(double) * c.n_tally, st);
+    }
     if (e == cudaSuccess) e = cudaMemsetAsync(L.scal, 0, 64, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.counters, 0, 8 * MCDC_N_COUNTERS, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.err, 0, 16, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(L.work, 0, 32, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(L.qc, 0, sizeof(QCount) * RING, st);
     if (e == cudaSuccess) e = cudaMallocHost((void **)&p->pin, sizeof(HostPinned));
     for (int k = 0; k < RING && e == cudaSuccess; k++) e = cudaEventCreateWithFlags(&p->ev[k], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreate(&p->t0);
     if (e == cudaSuccess) e = cudaEventCreate(&p->t1);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e == cudaSuccess && p->tally_private) {
-        int bytes = c.n_tally * BS * 8;
-        // opt in to > 48 KB is not needed (<= 40 KB), nothing to set
-        (void)bytes;
+    // the source box must lie inside the geometry: every point of a 9 x 9 x 9 grid over it has to be in a cell
+    int src_err = 0;
+    if (e == cudaSuccess) {
+        const int n1 = 9;
+        k_check_source_box<<<(n1 * n1 * n1 + 255) / 256, 256, 0, st>>>(c, n1);
+        e = cudaMemcpyAsync(&src_err, L.err, sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(L.err, 0, 16, st);
     }
-    if (e != cudaSuccess) { delete p; return fail(MCDC_ECUDA, "mcdc_create: %s", cudaGetErrorString(e)); }
-    p->bank_count = 0; p->k_prev = 1.0; p->n_active = 0;
-    p->k_acc = p->k_acc2 = p->leak_acc = p->leak_acc2 = 0.0;
-    memset(p->host_counters, 0, sizeof p->host_counters);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) { mcdc_destroy(p); return fail(MCDC_ECUDA, "mcdc_create: %s", cudaGetErrorString(e)); }
+    if (src_err) { mcdc_destroy(p); return fail(MCDC_EGEOM, "the source box is not inside the geometry (a point of it lies in no cell)"); }
+    p->bank_count = 0; p->k_prev = 1.0;
+    p->dirty = false;
     p->ms_transport = 0.0; p->n_launches = 0; p->last_N = 0;
     p->profile = 0;
     memset(p->prof_ms, 0, sizeof p->prof_ms); memset(p->prof_launches, 0, sizeof p->prof_launches);
@@ -569,10 +707,11 @@ extern "C" void mcdc_destroy(mcdc_problem *p)
 {
     if (!p) return;
     cudaStreamSynchronize(p->stream);
-    for (int k = 0; k < RING; k++) cudaEventDestroy(p->ev[k]);
+    for (int k = 0; k < RING; k++) if (p->ev[k]) cudaEventDestroy(p->ev[k]);
     for (cudaEvent_t e : p->pool) cudaEventDestroy(e);
-    cudaEventDestroy(p->t0); cudaEventDestroy(p->t1);
-    cudaFreeHost(p->pin);
+    if (p->t0) cudaEventDestroy(p->t0);
+    if (p->t1) cudaEventDestroy(p->t1);
+    if (p->pin) cudaFreeHost(p->pin);
     delete p;
 }
 
@@ -589,25 +728,70 @@ static unsigned int grid_for(uint64_t n)
     return (unsigned int)std::max<uint64_t>(1, std::min(b, cap));
 }
 
-static int reset_run(mcdc_problem *p)
+// the persistent kernel: at most the blocks that are resident at once (its idle warps wait for other warps' pushes,
+// so every block of the grid must be running)
+template <bool CE, bool PRIV> static unsigned int grid_persist(mcdc_problem *p, uint64_t n, size_t smem)
+{
+    if (p->persist_blocks_per_sm == 0) {
+        int nb = 0, sms = 148;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_persist<CE, PRIV>, BS, smem) != cudaSuccess || nb < 1) nb = 1;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
+        p->persist_blocks_per_sm = nb;
+        p->n_sm = sms;
+    }
+    uint64_t b = (n + BS - 1) / BS;
+    const uint64_t cap = (uint64_t)p->n_sm * p->persist_blocks_per_sm;
+    return (unsigned int)std::max<uint64_t>(1, std::min(b, cap));
+}
+
+// start a new run in the accumulator set the published results do not use
+static int begin_run(mcdc_problem *p)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
+    p->work = RunStats();
+    p->work.set = 1 - p->pub.set;
     CUDA_OK(cudaMemsetAsync(c.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st));
-    CUDA_OK(cudaMemsetAsync(p->flux_acc, 0, sizeof(double) * c.n_tally, st));
-    CUDA_OK(cudaMemsetAsync(p->flux_acc2, 0, sizeof(double) * c.n_tally, st));
+    CUDA_OK(cudaMemsetAsync(p->flux_acc[p->work.set], 0, sizeof(double) * c.n_tally, st));
+    CUDA_OK(cudaMemsetAsync(p->flux_acc2[p->work.set], 0, sizeof(double) * c.n_tally, st));
     CUDA_OK(cudaMemsetAsync(c.counters, 0, 8 * MCDC_N_COUNTERS, st));
     CUDA_OK(cudaMemsetAsync(c.err, 0, 16, st));
-    CUDA_OK(cudaMemsetAsync(c.fis.n, 0, sizeof(int) * (size_t)(p->cap + OVER_CAP), st));
+    CUDA_OK(cudaMemsetAsync(c.fis.n, 0, sizeof(int) * (size_t)p->cap, st));
     if (c.tr.rec) CUDA_OK(cudaMemsetAsync(c.tr.count, 0, sizeof(unsigned int) * c.tr.cap_slots, st));
-    p->k_cycle.clear();
-    p->n_active = 0;
-    p->k_acc = p->k_acc2 = p->leak_acc = p->leak_acc2 = 0.0;
-    memset(p->host_counters, 0, sizeof p->host_counters);
     p->k_prev = 1.0;
     p->bank_count = 0;
     p->ms_transport = 0.0;
     p->n_launches = 0;
+    p->dirty = false;
+    return 0;
+}
+
+// the call succeeded: what it computed becomes the reported state
+static void publish(mcdc_problem *p)
+{
+    RunStats &w = p->work;
+    for (int i = 0; i < MCDC_N_COUNTERS; i++) w.counters[i] = p->pin->counters[i];
+#ifdef MCDC_TIMELINE
+    fprintf(stderr, "TIMELINE trips %llu lane-trips %llu idle-trips %llu max-warp-ns %llu src-exhausted-ns %llu sum-warp-ns %llu taken %llu\n",
+            p->pin->counters[0], p->pin->counters[11], p->pin->counters[13], p->pin->counters[12], p->pin->counters[9],
+            p->pin->counters[10], p->pin->counters[14]);
+#endif
+    // histories started / children made: source-bank histories are counted on the host, secondaries that joined the
+    // running population (continuous energy) on the device (counter 15)
+    w.counters[0] = w.host_counters[0] + p->pin->counters[15];
+    w.counters[11] = w.host_counters[11] + p->pin->counters[15];
+    w.counters[12] = w.host_counters[12];
+    w.counters[13] = w.host_counters[13];
+    w.counters[15] = 0;
+    p->pub = w;
+}
+
+static int device_error_code(mcdc_problem *p, int e)
+{
+    if (e == -2) return fail(MCDC_EGEOM, "particle in no cell (lost)");
+    if (e == -3) return fail(MCDC_EBANK, "fission / secondary bank overflow (capacity %llu)", (unsigned long long)p->cap);
+    if (e == -4) return fail(MCDC_ELOST, "segment guard exceeded (%u segments in one history)", MAX_SEGMENTS);
+    if (e != 0) return fail(MCDC_ECUDA, "device error flag %d", e);
     return 0;
 }
 
@@ -616,40 +800,40 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
     const size_t smem_mg = CE ? 0 : (size_t)c.mg_stage * sizeof(double);
-    const size_t smem_geo = (size_t)((c.geo_stage + 1) / 2) * sizeof(double);
-    const size_t smem = smem_mg + smem_geo + (PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0);
+    const size_t smem = smem_mg + (PRIV ? (size_t)c.n_tally * BS * sizeof(double) : 0);
     CUDA_OK(cudaMemsetAsync(c.qc, 0, sizeof(QCount) * RING, st));
-    CUDA_OK(cudaMemsetAsync(c.n_over, 0, sizeof(unsigned int), st));
     uint64_t upper = M;
     long long known = -1;  // newest sweep whose counts the host has seen
     unsigned int s = 0;
     const unsigned int n0 = (unsigned int)M;
     while (upper > 0) {
         if (s > 4000000u) return fail(MCDC_ELOST, "sweep guard exceeded");
-        if (p->schedule == 0 && p->tail > 0 && upper <= (uint64_t)p->tail) {
-            { ProfScope ps(p, MCDC_PROF_TAIL); k_finish<CE, PRIV><<<grid_for(upper), BS, smem, st>>>(c, s, n0); }
+        if (p->schedule != 1 && p->persist > 0 && upper <= (uint64_t)p->persist) {
+            CUDA_OK(cudaMemsetAsync(c.work, 0, 32, st));
+            if (CE) CUDA_OK(cudaMemsetAsync(c.bank[(s + 1) & 1].ev, 0, sizeof(uint32_t) * (size_t)p->cap, st));
+            { ProfScope ps(p, MCDC_PROF_PERSIST); k_persist<CE, PRIV><<<grid_persist<CE, PRIV>(p, upper, smem), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
-            p->host_counters[13]++;
+            p->work.host_counters[13]++;
             break;
         }
         unsigned int gr = grid_for(upper);
-        if (p->schedule == 0 && p->fuse > 0 && upper <= (uint64_t)p->fuse) {
-            ProfScope ps(p, MCDC_PROF_FUSED);
-            k_multi<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0, (unsigned int)p->fuse_segments);
+        if (p->schedule != 1) {
+            { ProfScope ps(p, MCDC_PROF_SWEEP); k_sweep<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
-        } else if (p->schedule == 0) {
-            { ProfScope ps(p, MCDC_PROF_ADVANCE); k_advance<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
-            { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, smem_mg, st>>>(c, s); }
-            { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, smem_geo, st>>>(c, s); }
-            p->n_launches += 3;
+            if (p->schedule == 2) {
+                { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, smem_mg, st>>>(c, s); }
+                { ProfScope ps(p, MCDC_PROF_SURFACE); k_surface<<<gr, BS, 0, st>>>(c, s); }
+                p->n_launches += 2;
+            }
         } else {
             { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
         }
-        p->host_counters[13]++;
+        p->work.host_counters[13]++;
         CUDA_OK(cudaMemcpyAsync(&p->pin->qc[s % RING], c.qc + (s % RING), sizeof(QCount), cudaMemcpyDeviceToHost, st));
         CUDA_OK(cudaEventRecord(p->ev[s % RING], st));
         s++;
+        bool stop = false;
         while (known < (long long)s - 1) {
             long long r = known + 1;
             if ((long long)s - 1 - r >= LAG) CUDA_OK(cudaEventSynchronize(p->ev[r % RING]));
@@ -659,9 +843,11 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
                 if (q != cudaSuccess) return fail(MCDC_ECUDA, "event query: %s", cudaGetErrorString(q));
             }
             const QCount &h = p->pin->qc[r % RING];
-            upper = p->schedule == 0 ? (uint64_t)h.n_scat + h.n_surf : (uint64_t)h.n_alive;
+            upper = p->schedule != 1 ? (uint64_t)h.n_scat + h.n_surf : (uint64_t)h.n_alive;
+            if (h.err != 0) stop = true;  // a kernel raised the device error flag: the caller reads and reports it
             known = r;
         }
+        if (stop) break;
     }
     CUDA_OK(cudaGetLastError());
     return 0;
@@ -673,12 +859,13 @@ static int transport(mcdc_problem *p, uint64_t M)
     return p->tally_private ? transport_t<true, true>(p, M) : transport_t<true, false>(p, M);
 }
 
-// children of bank[cur] (M parents) -> bank[1-cur]; returns their number
+// children of the M parents' fission records -> bank[0]; returns their number.  Also brings the cycle's scalars,
+// the device counters and the error flag to the host (one synchronisation).
 static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
-    unsigned int nb = (unsigned int)((M + (p->mode == 1 ? OVER_CAP : 0) + BS - 1) / BS);
+    unsigned int nb = (unsigned int)((M + BS - 1) / BS);
     {
     ProfScope ps(p, MCDC_PROF_BANK);
     k_scan_partial<<<nb, BS, 0, st>>>(c, (unsigned int)M, p->part);
@@ -690,6 +877,7 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
     p->n_launches += 4;
     CUDA_OK(cudaMemcpyAsync(&p->pin->total, p->part + nb, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaMemcpyAsync(p->pin->counters, c.counters, sizeof p->pin->counters, cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(&p->pin->err, c.err, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaStreamSynchronize(st));
     CUDA_OK(cudaGetLastError());
@@ -698,16 +886,21 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
     return 0;
 }
 
-static int device_error(mcdc_problem *p)
+// a call failed after device work was queued: drain the stream, clear the error flag and mark the per-cycle
+// tallies for clearing, so that the problem stays usable
+static int abandon(mcdc_problem *p, int rc)
 {
-    int e = p->pin->err;
-    if (e == -2) return fail(MCDC_EGEOM, "particle in no cell (lost)");
-    if (e == -3) return fail(MCDC_EBANK, "fission / secondary bank overflow (capacity %llu)", (unsigned long long)p->cap);
-    if (e == -4) return fail(MCDC_ELOST, "segment guard exceeded");
-    return 0;
+    std::string keep = g_err;
+    cudaStreamSynchronize(p->stream);
+    cudaMemsetAsync(p->ctx.err, 0, 16, p->stream);
+    cudaMemsetAsync(p->ctx.fis.n, 0, sizeof(int) * (size_t)p->cap, p->stream);
+    cudaStreamSynchronize(p->stream);
+    p->dirty = true;
+    g_err = keep;
+    return rc;
 }
 
-// one power-iteration cycle; source: 0 = from bank[cur] (bank_count sites), 1 = sample
+// one power-iteration cycle; sample: draw the source (cycle 0) instead of starting from bank[0]
 static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int active, uint64_t seed, bool sample,
                           double *flux_cycle_host)
 {
@@ -720,6 +913,11 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     c.seed = seed; c.cycle = cycle;
     c.w0 = sample ? 1.0 : (double)N / (double)M;  // source renormalisation (R6)
     c.k_prev = p->k_prev;
+    c.max_secondaries = ~0ull;
+    if (p->dirty) {
+        CUDA_OK(cudaMemsetAsync(c.flux, 0, sizeof(double) * c.n_tally * p->flux_copies, st));
+        p->dirty = false;
+    }
     CUDA_OK(cudaMemsetAsync(c.scal, 0, 64, st));
     CUDA_OK(cudaEventRecord(p->t0, st));
     if (sample) {
@@ -727,31 +925,33 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
         p->n_launches++;
     }
     int rc = transport(p, M);
-    if (rc) return rc;
+    if (rc) return abandon(p, rc);
     uint64_t total = 0;
     rc = emit_children(p, M, &total);
-    if (rc) return rc;
+    if (rc) return abandon(p, rc);
+    rc = device_error_code(p, p->pin->err);
+    if (rc) return abandon(p, rc);
     CUDA_OK(cudaEventRecord(p->t1, st));
-    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc, p->flux_acc2, c.n_tally, 1.0 / (double)N, active);
+    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[p->work.set],
+                                                          p->flux_acc2[p->work.set], c.n_tally, 1.0 / (double)N, active);
     if (flux_cycle_host) CUDA_OK(cudaMemcpyAsync(flux_cycle_host, p->flux_cycle, sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, st));
     p->n_launches++;
     CUDA_OK(cudaStreamSynchronize(st));
     float ms = 0.f;
     CUDA_OK(cudaEventElapsedTime(&ms, p->t0, p->t1));
     p->ms_transport += ms;
-    rc = device_error(p);
-    if (rc) return rc;
+    RunStats &w = p->work;
     double k_c = p->pin->scal[0] / (double)N, leak = p->pin->scal[1] / (double)N;
-    p->k_cycle.push_back(k_c);
+    w.k_cycle.push_back(k_c);
     if (active) {
-        p->k_acc += k_c; p->k_acc2 += k_c * k_c;
-        p->leak_acc += leak; p->leak_acc2 += leak * leak;
-        p->n_active++;
+        w.k_acc += k_c; w.k_acc2 += k_c * k_c;
+        w.leak_acc += leak; w.leak_acc2 += leak * leak;
+        w.n_active++;
     }
     p->k_prev = k_c;
-    p->host_counters[0] += M;
-    p->host_counters[11] += total;
-    if (total > p->host_counters[12]) p->host_counters[12] = total;
+    w.host_counters[0] += M;
+    w.host_counters[11] += total;
+    if (total > w.host_counters[12]) w.host_counters[12] = total;
     p->bank_count = total;
     p->last_N = N;
     return 0;
@@ -760,10 +960,11 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
 extern "C" int mcdc_run_cycle(mcdc_problem *p, uint64_t N, uint32_t cycle, int32_t active, uint64_t seed, double *k_cycle)
 {
     if (!p || p->mode != 0) return fail(MCDC_EINVAL, "mcdc_run_cycle needs a multi-group problem");
-    if (cycle == 0) { int rc = reset_run(p); if (rc) return rc; }
+    if (cycle == 0) { int rc = begin_run(p); if (rc) return rc; }
     int rc = cycle_internal(p, N, cycle, active, seed, cycle == 0, nullptr);
     if (rc) return rc;
-    if (k_cycle) *k_cycle = p->k_cycle.back();
+    publish(p);
+    if (k_cycle) *k_cycle = p->work.k_cycle.back();
     return 0;
 }
 
@@ -771,12 +972,13 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t N, int32_t n_inacti
 {
     if (!p || p->mode != 0) return fail(MCDC_EINVAL, "mcdc_run_eigenvalue needs a multi-group problem");
     if (n_inactive < 0 || n_active < 0) return fail(MCDC_EINVAL, "cycle counts");
-    int rc = reset_run(p);
+    int rc = begin_run(p);
     if (rc) return rc;
     for (int cyc = 0; cyc < n_inactive + n_active; cyc++) {
         rc = cycle_internal(p, N, (uint32_t)cyc, cyc >= n_inactive, seed, cyc == 0, nullptr);
         if (rc) return rc;
     }
+    publish(p);
     return 0;
 }
 
@@ -790,7 +992,7 @@ extern "C" int mcdc_run_cycle_host(mcdc_problem *p, uint64_t N, uint32_t cycle, 
     cudaStream_t st = p->stream;
     bool sample = sites_in == nullptr || n_in == 0;
     if (!sample && n_in > p->cap) return fail(MCDC_EBANK, "source bank larger than the capacity");
-    if (cycle == 0) { int rc = reset_run(p); if (rc) return rc; }
+    if (cycle == 0) { int rc = begin_run(p); if (rc) return rc; }
     p->k_prev = k_prev;
     if (!sample) {
         CUDA_OK(cudaMemcpyAsync(p->sites, sites_in, n_in * sizeof(Site), cudaMemcpyHostToDevice, st));
@@ -809,7 +1011,8 @@ extern "C" int mcdc_run_cycle_host(mcdc_problem *p, uint64_t N, uint32_t cycle, 
         CUDA_OK(cudaMemcpyAsync(sites_out, p->sites, n * sizeof(Site), cudaMemcpyDeviceToHost, st));
         CUDA_OK(cudaStreamSynchronize(st));
     }
-    if (k_cycle) *k_cycle = p->k_cycle.back();
+    publish(p);
+    if (k_cycle) *k_cycle = p->work.k_cycle.back();
     if (leak_cycle) *leak_cycle = p->pin->scal[1] / (double)N;
     return 0;
 }
@@ -818,44 +1021,51 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
 {
     if (!p || p->mode != 1) return fail(MCDC_EINVAL, "mcdc_run_fixed_source needs a continuous-energy problem");
     if (N < 1 || capacity_for(N) > p->cap) return fail(MCDC_EINVAL, "n_particles exceeds the capacity this problem was created for");
+    if (N > 60000000ull) return fail(MCDC_EINVAL, "at most 6e7 source particles per fixed-source run (32-bit secondary counters)");
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
-    int rc = reset_run(p);
+    int rc = begin_run(p);
     if (rc) return rc;
     c.seed = seed; c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
+    c.max_secondaries = 64 * N + 4096;  // R25a: the prompt chain must die out
     CUDA_OK(cudaMemsetAsync(c.scal, 0, 64, st));
     CUDA_OK(cudaEventRecord(p->t0, st));
     uint64_t M = N;
     k_source<true><<<(unsigned int)((M + BS - 1) / BS), BS, 0, st>>>(c, (unsigned int)M);
     p->n_launches++;
+    RunStats &w = p->work;
     uint64_t secondaries = 0;
-    while (M > 0) {  // one wave per fission generation of the prompt chain
+    while (M > 0) {  // one wave per fission generation of the prompt chain (monolithic schedule only: the other
+                     // schedules transport the secondaries inside the first wave)
         rc = transport(p, M);
-        if (rc) return rc;
+        if (rc) return abandon(p, rc);
         uint64_t total = 0;
         rc = emit_children(p, M, &total);
-        if (rc) return rc;
-        rc = device_error(p);
-        if (rc) return rc;
-        p->host_counters[0] += M;
-        p->host_counters[11] += total;
-        if (total > p->host_counters[12]) p->host_counters[12] = total;
+        if (rc) return abandon(p, rc);
+        rc = device_error_code(p, p->pin->err);
+        if (rc) return abandon(p, rc);
+        w.host_counters[0] += M;
+        w.host_counters[11] += total;
+        uint64_t high = std::max<uint64_t>(total, p->pin->counters[15]);
+        if (high > w.host_counters[12]) w.host_counters[12] = high;
         secondaries += total;
-        if (secondaries > 64 * N + 4096) return fail(MCDC_EBANK, "prompt fission chain does not die out (R25)");
+        if (secondaries > c.max_secondaries) return abandon(p, fail(MCDC_EBANK, "prompt fission chain does not die out (R25)"));
         M = total;
     }
     CUDA_OK(cudaEventRecord(p->t1, st));
-    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc, p->flux_acc2, c.n_tally, 1.0 / (double)N, 1);
+    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[w.set], p->flux_acc2[w.set],
+                                                          c.n_tally, 1.0 / (double)N, 1);
     p->n_launches++;
     CUDA_OK(cudaStreamSynchronize(st));
     float ms = 0.f;
     CUDA_OK(cudaEventElapsedTime(&ms, p->t0, p->t1));
     p->ms_transport += ms;
     double k_c = p->pin->scal[0] / (double)N, leak = p->pin->scal[1] / (double)N;
-    p->k_cycle.push_back(k_c);
-    p->k_acc = k_c; p->k_acc2 = k_c * k_c; p->leak_acc = leak; p->leak_acc2 = leak * leak; p->n_active = 1;
+    w.k_cycle.push_back(k_c);
+    w.k_acc = k_c; w.k_acc2 = k_c * k_c; w.leak_acc = leak; w.leak_acc2 = leak * leak; w.n_active = 1;
     p->bank_count = 0;
     p->last_N = N;
+    publish(p);
     return 0;
 }
 
@@ -863,7 +1073,7 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
 extern "C" int mcdc_get_dims(const mcdc_problem *p, mcdc_dims *d)
 {
     if (!p || !d) return fail(MCDC_EINVAL, "null");
-    d->mode = p->mode; d->n_tally = p->ctx.n_tally; d->n_cycles = (int)p->k_cycle.size(); d->n_active = p->n_active;
+    d->mode = p->mode; d->n_tally = p->ctx.n_tally; d->n_cycles = (int)p->pub.k_cycle.size(); d->n_active = p->pub.n_active;
     d->bank_count = p->bank_count;
     return 0;
 }
@@ -879,28 +1089,23 @@ extern "C" int mcdc_get_tallies(const mcdc_problem *p, mcdc_tallies *out)
 {
     if (!p || !out) return fail(MCDC_EINVAL, "null");
     const Ctx &c = p->ctx;
-    int n = p->n_active;
+    const RunStats &r = p->pub;
+    int n = r.n_active;
     double dn = n > 0 ? (double)n : 1.0;
-    if (out->k_cycle) for (size_t i = 0; i < p->k_cycle.size(); i++) out->k_cycle[i] = p->k_cycle[i];
-    out->k_mean = p->k_acc / dn; out->k_sdev = sdev_of(p->k_acc, p->k_acc2, n);
-    out->leak_mean = p->leak_acc / dn; out->leak_sdev = sdev_of(p->leak_acc, p->leak_acc2, n);
-    std::vector<double> a(c.n_tally), a2(c.n_tally);
-    CUDA_OK(cudaMemcpyAsync(a.data(), p->flux_acc, sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, p->stream));
-    CUDA_OK(cudaMemcpyAsync(a2.data(), p->flux_acc2, sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, p->stream));
-    unsigned long long dc[MCDC_N_COUNTERS];
-    CUDA_OK(cudaMemcpyAsync(dc, c.counters, sizeof dc, cudaMemcpyDeviceToHost, p->stream));
-    CUDA_OK(cudaStreamSynchronize(p->stream));
-    for (int i = 0; i < c.n_tally; i++) {
-        if (out->flux_mean) out->flux_mean[i] = a[i] / dn;
-        if (out->flux_sdev) out->flux_sdev[i] = sdev_of(a[i], a2[i], n);
+    if (out->k_cycle) for (size_t i = 0; i < r.k_cycle.size(); i++) out->k_cycle[i] = r.k_cycle[i];
+    out->k_mean = r.k_acc / dn; out->k_sdev = sdev_of(r.k_acc, r.k_acc2, n);
+    out->leak_mean = r.leak_acc / dn; out->leak_sdev = sdev_of(r.leak_acc, r.leak_acc2, n);
+    if (out->flux_mean || out->flux_sdev) {
+        std::vector<double> a(c.n_tally), a2(c.n_tally);
+        CUDA_OK(cudaMemcpyAsync(a.data(), p->flux_acc[r.set], sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, p->stream));
+        CUDA_OK(cudaMemcpyAsync(a2.data(), p->flux_acc2[r.set], sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, p->stream));
+        CUDA_OK(cudaStreamSynchronize(p->stream));
+        for (int i = 0; i < c.n_tally; i++) {
+            if (out->flux_mean) out->flux_mean[i] = a[i] / dn;
+            if (out->flux_sdev) out->flux_sdev[i] = sdev_of(a[i], a2[i], n);
+        }
     }
-    if (out->counters) {
-        for (int i = 0; i < MCDC_N_COUNTERS; i++) out->counters[i] = dc[i];
-        // histories started / children made inside the tail kernel (continuous energy) are counted on the device
-        out->counters[0] = p->host_counters[0] + dc[15]; out->counters[11] = p->host_counters[11] + dc[15];
-        out->counters[15] = 0;
-        out->counters[12] = p->host_counters[12]; out->counters[13] = p->host_counters[13];
-    }
+    if (out->counters) for (int i = 0; i < MCDC_N_COUNTERS; i++) out->counters[i] = r.counters[i];
     return 0;
 }
 
@@ -922,7 +1127,11 @@ extern "C" int mcdc_set_trace(mcdc_problem *p, uint64_t first_id, uint32_t n_ids
 {
     if (!p) return fail(MCDC_EINVAL, "null");
     static_assert(sizeof(TraceRec) == sizeof(mcdc_trace_rec), "trace layout");
-    if (n_ids == 0 || max_events == 0) { p->ctx.tr.rec = nullptr; return 0; }
+    if (n_ids == 0 || max_events == 0) {
+        p->ctx.tr.rec = nullptr;
+        CUDA_OK(cudaMemcpy((void *)p->ctx.tr_g, &p->ctx.tr, sizeof(Trace), cudaMemcpyHostToDevice));
+        return 0;
+    }
     uint64_t per_slot = (uint64_t)max_events * sizeof(TraceRec);
     uint64_t slots = TRACE_BYTES / per_slot;
     if (slots < n_ids) return fail(MCDC_ENOMEM, "trace buffer holds %llu (id, cycle) slots of %u events; %u ids asked", (unsigned long long)slots, max_events, n_ids);
@@ -930,6 +1139,7 @@ extern "C" int mcdc_set_trace(mcdc_problem *p, uint64_t first_id, uint32_t n_ids
     t.first = first_id; t.n_ids = n_ids; t.max_events = max_events;
     t.cap_slots = (unsigned int)std::min<uint64_t>(slots, TRACE_BYTES / sizeof(TraceRec));
     t.rec = p->trace_base; t.count = p->trace_count;
+    CUDA_OK(cudaMemcpyAsync((void *)p->ctx.tr_g, &t, sizeof(Trace), cudaMemcpyHostToDevice, p->stream));
     CUDA_OK(cudaMemsetAsync(t.count, 0, sizeof(unsigned int) * t.cap_slots, p->stream));
     CUDA_OK(cudaStreamSynchronize(p->stream));
     return 0;
@@ -962,19 +1172,19 @@ extern "C" int mcdc_set_profile(mcdc_problem *p, int32_t on)
     p->profile = on ? 1 : 0;
     unsigned long long b = 0;
     CUDA_OK(cudaMemcpy(&b, p->ctx.counters + 12, sizeof b, cudaMemcpyDeviceToHost));
-    p->prof_adv_base = b;
+    p->prof_sweep_base = b;
     memset(p->prof_ms, 0, sizeof p->prof_ms); memset(p->prof_launches, 0, sizeof p->prof_launches);
     return 0;
 }
 
-extern "C" int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *advance_events)
+extern "C" int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *sweep_events)
 {
     if (!p || !ms || !launches) return fail(MCDC_EINVAL, "null");
     for (int k = 0; k < MCDC_N_PROFILE; k++) { ms[k] = p->prof_ms[k]; launches[k] = p->prof_launches[k]; }
-    if (advance_events) {
+    if (sweep_events) {
         unsigned long long b = 0;
         CUDA_OK(cudaMemcpy(&b, p->ctx.counters + 12, sizeof b, cudaMemcpyDeviceToHost));
-        *advance_events = b - p->prof_adv_base;
+        *sweep_events = b - p->prof_sweep_base;
     }
     return 0;
 }
@@ -988,7 +1198,7 @@ extern "C" int mcdc_get_timing(const mcdc_problem *p, double *ms, uint64_t *nl)
 }
 
 // ------------------------------------------------------------------ unit-level entry points
-// scratch for the test entry points is taken from the (idle) second particle bank region: sites buffer
+// scratch for the test entry points is taken from the (idle) site staging buffer
 extern "C" int mcdc_test_draws(mcdc_problem *p, uint64_t seed, uint32_t domain, uint32_t cycle, const uint64_t *id,
                                const uint32_t *draw, uint64_t n, double *out)
 {
@@ -1021,20 +1231,54 @@ extern "C" int mcdc_test_grid_index(mcdc_problem *p, const double *E, uint64_t n
     return 0;
 }
 
-extern "C" int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64_t n, int32_t *loc, double *dist,
-                                  int32_t *surf)
+extern "C" int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64_t n, int32_t path, int32_t *loc,
+                                  double *dist, int32_t *surf)
 {
     if (!p || !x || !u || !loc || !dist || !surf) return fail(MCDC_EINVAL, "null");
+    if (path < 0 || path > 2) return fail(MCDC_EINVAL, "path must be 0, 1 or 2");
     if (n * 72 > p->cap * sizeof(Site)) return fail(MCDC_ENOMEM, "too many points for the scratch buffer");
     char *base = (char *)p->sites;
     double *d_x = (double *)base, *d_u = (double *)(base + n * 24), *d_d = (double *)(base + n * 48);
     int *d_loc = (int *)(base + n * 56), *d_s = (int *)(base + n * 68);
     CUDA_OK(cudaMemcpyAsync(d_x, x, n * 24, cudaMemcpyHostToDevice, p->stream));
     CUDA_OK(cudaMemcpyAsync(d_u, u, n * 24, cudaMemcpyHostToDevice, p->stream));
-    k_test_geometry<<<(unsigned int)((n + 255) / 256), 256, 0, p->stream>>>(p->ctx, d_x, d_u, n, d_loc, d_d, d_s);
+    k_test_geometry<<<(unsigned int)((n + 255) / 256), 256, 0, p->stream>>>(p->ctx, d_x, d_u, n, path, d_loc, d_d, d_s);
     CUDA_OK(cudaMemcpyAsync(loc, d_loc, n * 12, cudaMemcpyDeviceToHost, p->stream));
     CUDA_OK(cudaMemcpyAsync(dist, d_d, n * 8, cudaMemcpyDeviceToHost, p->stream));
     CUDA_OK(cudaMemcpyAsync(surf, d_s, n * 4, cudaMemcpyDeviceToHost, p->stream));
     CUDA_OK(cudaStreamSynchronize(p->stream));
+    return 0;
+}
+
+// ------------------------------------------------------------------ arithmetic micro-benchmarks
+extern "C" int mcdc_microbench(mcdc_problem *p, int32_t which, uint64_t iters, double *ms_out, double *ops_out)
+{
+    if (!p || !ms_out || !ops_out) return fail(MCDC_EINVAL, "null");
+    if (which < 0 || which >= MCDC_MB_COUNT || iters < 1) return fail(MCDC_EINVAL, "which / iters");
+    cudaStream_t st = p->stream;
+    const unsigned int threads = 256, blocks = 148 * 8;  // 2048 resident threads on every SM
+    if ((uint64_t)threads * blocks * 8 > p->cap * sizeof(Site)) return fail(MCDC_ENOMEM, "scratch buffer too small");
+    double *out = (double *)p->sites;
+    double per_thread = 0.0;
+    for (int pass = 0; pass < 2; pass++) {  // pass 0 warms up
+        CUDA_OK(cudaEventRecord(p->t0, st));
+        switch (which) {
+        case MCDC_MB_FFMA: k_mb_ffma<<<blocks, threads, 0, st>>>(iters, (float *)out); per_thread = (double)MB_CHAINS * iters; break;
+        case MCDC_MB_DFMA: k_mb_dfma<<<blocks, threads, 0, st>>>(iters, out); per_thread = (double)MB_CHAINS * iters; break;
+        case MCDC_MB_LOG: k_mb_func<0><<<blocks, threads, 0, st>>>(iters, out); per_thread = 4.0 * iters; break;
+        case MCDC_MB_DIV: k_mb_func<1><<<blocks, threads, 0, st>>>(iters, out); per_thread = 4.0 * iters; break;
+        case MCDC_MB_SQRT: k_mb_func<2><<<blocks, threads, 0, st>>>(iters, out); per_thread = 4.0 * iters; break;
+        case MCDC_MB_SINCOSPI: k_mb_func<3><<<blocks, threads, 0, st>>>(iters, out); per_thread = 4.0 * iters; break;
+        case MCDC_MB_RCP: k_mb_func<4><<<blocks, threads, 0, st>>>(iters, out); per_thread = 4.0 * iters; break;
+        default: k_mb_philox<<<blocks, threads, 0, st>>>(iters, out); per_thread = 4.0 * iters; break;
+        }
+        CUDA_OK(cudaEventRecord(p->t1, st));
+        CUDA_OK(cudaStreamSynchronize(st));
+        CUDA_OK(cudaGetLastError());
+    }
+    float ms = 0.f;
+    CUDA_OK(cudaEventElapsedTime(&ms, p->t0, p->t1));
+    *ms_out = ms;
+    *ops_out = per_thread * threads * blocks;  // thread-level operations of the timed launch
     return 0;
 }

@@ -3,7 +3,7 @@ import numpy as np
 import pytest
 
 from paper_2501_05440_b200 import inputs
-from tests.test_gpu_parity import compare_traces
+from tests.test_gpu_parity import ALWAYS, compare_traces
 
 pytestmark = pytest.mark.gpu
 
@@ -30,6 +30,9 @@ CE_CASES = {
     "ce_scatter": lambda: inputs.ce_single_scatterer(A=16.0, n_particles=5000),
     "ce_scatterH": lambda: inputs.ce_single_scatterer(A=1.0, n_particles=5000),
     "ce_fission": lambda: _fis(),
+    "ce_mix": lambda: inputs.ce_two_nuclide_mix(n_particles=3000, n_grid=3000),
+    "ce_clock": lambda: inputs.ce_scatter_clock(n_particles=3000, n_grid=3000),
+    "ce_clamp": lambda: inputs.ce_single_scatterer(A=1.0, n_particles=4000, E0=2.0e-5, sig_el=0.9, sig_c=0.1),
 }
 
 
@@ -40,14 +43,12 @@ def _fis():
 
 
 @pytest.mark.parametrize("name", list(CE_CASES))
-@pytest.mark.parametrize("schedule,tail,search,fuse", [(0, 0, 0, 0), (0, -1, 1, -1), (0, 1 << 30, 1, 0), (1, 0, 0, 0), (0, -1, 1, 1 << 30),
-                                                       (0, 100, 0, 1000)])
-def test_ce_parity(gpu, orc, name, schedule, tail, search, fuse):
+@pytest.mark.parametrize("schedule,persist,search", [(0, 0, 0), (0, -1, 1), (0, ALWAYS, 1), (1, 0, 0), (2, -1, 1), (0, 100, 0), (2, 1000, 1)])
+def test_ce_parity(gpu, orc, name, schedule, persist, search):
     P = CE_CASES[name]()
     # the supercritical pure-fission pin grows by generation: give its waves room (capacity = 2 max + 1024)
     mp = 100_000 if name == "ce_fission" else None
-    g = gpu.Problem(P, max_particles=mp, schedule=schedule, tail_threshold=tail, search=search, fuse_threshold=fuse,
-                    fuse_segments=5)
+    g = gpu.Problem(P, max_particles=mp, schedule=schedule, persist_threshold=persist, search=search)
     r = g.run()
     o = orc.Oracle(P)
     rc, ro = o.run()
@@ -56,11 +57,11 @@ def test_ce_parity(gpu, orc, name, schedule, tail, search, fuse):
     g.close()
 
 
-@pytest.mark.parametrize("schedule,tail,search,fuse", [(0, -1, 0, -1), (0, 0, 1, 0), (1, 0, 1, 0), (0, 50, 1, 200)])
-def test_ce_traces_identical(gpu, orc, schedule, tail, search, fuse):
+@pytest.mark.parametrize("schedule,persist,search", [(0, -1, 0), (0, 0, 1), (1, 0, 1), (2, -1, 0), (0, 50, 1)])
+def test_ce_traces_identical(gpu, orc, schedule, persist, search):
     """Source particles 0..99 of C5: identical event sequences incl. grid index, time, energy."""
     P = inputs.config5(n_particles=400, n_grid=20_000)
-    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, search=search, fuse_threshold=fuse)
+    g = gpu.Problem(P, schedule=schedule, persist_threshold=persist, search=search)
     g.set_trace(0, 100, 4096)
     r = g.run()
     o = orc.Oracle(P)
@@ -83,4 +84,37 @@ def test_grid_search_binary_equals_hash_equals_numpy(gpu, jitter):
     ob, oh = g.grid_index(E)
     assert (ob == ref).all()
     assert (oh == ref).all()
+    g.close()
+
+
+@pytest.mark.parametrize("persist", [-1, 0])
+def test_ce_secondary_overflow_is_an_error_not_a_fault(gpu, persist):
+    """A supercritical prompt chain outgrows the bank: MCDC_EBANK from the sweep kernels (regions meet) as well as
+    from the persistent kernel (queue tail past the capacity), never an out-of-bounds access; the problem stays
+    usable afterwards."""
+    P = inputs.ce_pure_fission(3000)
+    P["t_edges"] = np.array([0.0, 1.0e-6])  # dozens of generations of nu = 2.5
+    g = gpu.Problem(P, max_particles=3000, persist_threshold=persist)
+    with pytest.raises(gpu.McdcError) as e:
+        g.run()
+    assert e.value.code == -3
+    P2 = _fis()
+    g.close()
+    g = gpu.Problem(P2, max_particles=100_000, persist_threshold=persist)
+    r = g.run()
+    assert r["counters"][0] > 2000
+    g.close()
+
+
+def test_ce_source_traces_with_secondaries_in_flight(gpu, orc):
+    """Source histories 300..399 of a C5 run (ids beyond the first warp's worth), persistent kernel with queue pushes."""
+    P = inputs.config5(n_particles=500, n_grid=10_000)
+    g = gpu.Problem(P, search=1)
+    g.set_trace(300, 100, 4096)
+    r = g.run()
+    o = orc.Oracle(P)
+    o.set_trace(300, 100, 2_000_000)
+    rc, ro = o.run()
+    compare_traces(g.trace(), o.trace())
+    compare_ce(r, ro)
     g.close()

@@ -12,6 +12,7 @@ from paper_2501_05440_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
+ALWAYS = 0x7FFFFFFF  # persist_threshold: the persistent kernel from the first segment on
 DISCRETE = ["id", "cycle", "seq", "ev", "c0", "elem", "c1", "surf", "gi"]
 FLOATS = ["x", "y", "z", "d", "E", "t"]
 
@@ -33,7 +34,7 @@ def compare_results(r, ro, rtol=1e-9):
     assert (r["counters"][:12] == ro["counters"][:12]).all(), (r["counters"], ro["counters"])
 
 
-def compare_traces(tg, to):
+def compare_traces(tg, to, atol=1e-11):
     assert len(tg) == len(to) and len(to) > 0
     kg = np.lexsort((tg["seq"], tg["id"], tg["cycle"]))
     ko = np.lexsort((to["seq"], to["id"], to["cycle"]))
@@ -41,7 +42,14 @@ def compare_traces(tg, to):
     for f in DISCRETE:
         assert (tg[f] == to[f]).all(), f
     for f in FLOATS:
-        assert np.allclose(tg[f], to[f], rtol=1e-9, atol=1e-11), f
+        assert np.allclose(tg[f], to[f], rtol=1e-9, atol=atol), f
+
+
+def float_atol(name):
+    """Absolute tolerance on positions.  Specular reflection off a CURVED wall amplifies the last-bit differences
+    between the two implementations (FMA contraction, libm) along near-tangent multi-bounce paths: measured worst
+    case 1.2e-9 cm after dozens of bounces; tallies and k still agree to 1e-9 relative."""
+    return 1e-7 if name.startswith("mirror") else 1e-11
 
 
 CASES = {
@@ -52,18 +60,28 @@ CASES = {
     "C4small": lambda: inputs.config4(n_particles=3001, n_inactive=1, n_active=2, n_asm=1, n_pin=3, n_refl=1),
     "mixed": lambda: inputs.mixed_surfaces(n_particles=4000),
     "C4_3d": lambda: inputs.config4(n_particles=4000, n_inactive=1, n_active=2, n_asm=1, n_pin=4, n_refl=1, height=6.0),
+    "lat1x6": lambda: inputs.rect_lattice(1, 6),
+    "lat5x1": lambda: inputs.rect_lattice(5, 1),
+    "lat3x5": lambda: inputs.rect_lattice(3, 5),
+    "mirror_sphere": lambda: inputs.curved_mirror("sphere", n_particles=3000, n_inactive=1, n_active=2),
+    "mirror_cyl_z": lambda: inputs.curved_mirror("cyl_z", n_particles=3000, n_inactive=1, n_active=2),
+    "mirror_cyl_x": lambda: inputs.curved_mirror("cyl_x", n_particles=3000, n_inactive=1, n_active=2),
     "slab": lambda: inputs.slab_beam(n_particles=5000),
     "sphere": lambda: inputs.sphere_absorber(n_particles=5000),
 }
 
 
+SCHEDULES = [(0, 0), (0, -1), (0, ALWAYS), (1, 0), (2, -1), (0, 300), (2, 700)]
+
+
 @pytest.mark.parametrize("name", list(CASES))
-@pytest.mark.parametrize("schedule,tail,fuse", [(0, 0, 0), (0, -1, -1), (0, 1 << 30, 0), (1, 0, 0), (0, -1, 1 << 30), (0, 300, 2000)])
-def test_mg_parity(gpu, orc, name, schedule, tail, fuse):
-    """Default schedule, pure per-event kernels (no tail, no fused sweeps), tail-only (histories in registers),
-    the monolithic schedule, fused sweeps only, and a mix of all three stages all reproduce the oracle."""
+@pytest.mark.parametrize("schedule,persist", SCHEDULES)
+def test_mg_parity(gpu, orc, name, schedule, persist):
+    """Default schedule, event sweeps only (no persistent kernel), the persistent kernel alone (whole histories in
+    registers, lanes refilled from the queue), the monolithic schedule, split per-event kernels, and sweeps handing
+    over to the persistent kernel part-way all reproduce the oracle."""
     P = CASES[name]()
-    g = gpu.Problem(P, schedule=schedule, tail_threshold=tail, fuse_threshold=fuse, fuse_segments=3)
+    g = gpu.Problem(P, schedule=schedule, persist_threshold=persist)
     r = g.run()
     o = orc.Oracle(P)
     rc, ro = o.run()
@@ -73,23 +91,24 @@ def test_mg_parity(gpu, orc, name, schedule, tail, fuse):
     assert len(bg) == len(bo)
     assert (bg["g"] == bo["g"]).all()
     for f in ("x", "y", "z", "ux", "uy", "uz"):
-        assert np.allclose(bg[f], bo[f], rtol=1e-9, atol=1e-11), f
+        assert np.allclose(bg[f], bo[f], rtol=1e-9, atol=float_atol(name)), f
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d"])
-@pytest.mark.parametrize("schedule,tail,fuse", [(0, -1, -1), (0, 0, 0), (1, 0, 0), (0, 100, 500)])
-def test_mg_traces_identical(gpu, orc, name, schedule, tail, fuse):
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d", "lat1x6", "lat3x5", "mirror_sphere",
+                                  "mirror_cyl_x"])
+@pytest.mark.parametrize("schedule,persist", [(0, -1), (0, 0), (1, 0), (2, -1), (0, 100)])
+def test_mg_traces_identical(gpu, orc, name, schedule, persist):
     """100 particles x 2 cycles: identical per-particle event sequences (SURVEY.md 8d parity protocol 1)."""
     P = CASES[name]()
     N = 1000
-    g = gpu.Problem(P, max_particles=N, schedule=schedule, tail_threshold=tail, fuse_threshold=fuse)
+    g = gpu.Problem(P, max_particles=N, schedule=schedule, persist_threshold=persist)
     g.set_trace(0, 100, 1024)
     r = g.run(n_particles=N, n_inactive=0, n_active=2)
     o = orc.Oracle(P)
     o.set_trace(0, 100, 400000)
     rc, ro = o.run(n_particles=N, n_inactive=0, n_active=2)
-    compare_traces(g.trace(), o.trace())
+    compare_traces(g.trace(), o.trace(), atol=float_atol(name))
     compare_results(r, ro)
     g.close()
 
@@ -141,23 +160,54 @@ def test_rng_bit_exact(gpu, orc):
     g.close()
 
 
-def test_geometry_unit_parity(gpu, orc):
-    P = inputs.config4(n_particles=1000)
+@pytest.mark.parametrize("height", [None, 3.0])
+def test_geometry_unit_parity(gpu, orc, height):
+    P = inputs.config4(n_particles=1000, height=height)
     g = gpu.Problem(P, max_particles=20000)
     o = orc.Oracle(P)
     rng = np.random.default_rng(5)
     n = 4000
     side = 51 * 1.26
-    x = np.column_stack([rng.uniform(0, side, n), rng.uniform(0, side, n), rng.uniform(-1, 1, n)])
+    x = np.column_stack([rng.uniform(0, side, n), rng.uniform(0, side, n), rng.uniform(0, 1, n) * (height or 1.0)])
+    x[: n // 4, 0] = rng.uniform(0, 1.26, n // 4)           # edge elements: the enclosing cell's planes matter there
+    x[n // 4: n // 2, 1] = rng.uniform(50 * 1.26, side, n // 4)
     mu, phi = rng.uniform(-1, 1, n), rng.uniform(0, 2 * np.pi, n)
     s = np.sqrt(1 - mu * mu)
     u = np.column_stack([s * np.cos(phi), s * np.sin(phi), mu])
-    loc, dist, surf = g.geometry(x, u)
+    # all three device paths: straight-line / pruned list as the kernels choose, generic loops with the pruned list of
+    # the enclosing cell's surfaces, generic loops over every surface
+    res = [g.geometry(x, u, path=k) for k in (0, 1, 2)]
     for i in range(n):
         rc, lo = o.locate(x[i], u[i])
-        assert rc == 0 and tuple(lo) == tuple(loc[i])
         d, sh = o.distance(x[i], u[i], lo)
-        assert sh == surf[i] and dist[i] == pytest.approx(d, rel=1e-13)
+        for loc, dist, surf in res:
+            assert rc == 0 and tuple(lo) == tuple(loc[i])
+            assert sh == surf[i] and dist[i] == pytest.approx(d, rel=1e-13)
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5"])
+def test_geometry_unit_parity_plain_cells(gpu, orc, name):
+    """Cells outside a lattice (box, pin cell: straight-line path; mixed surfaces: generic loops) and a small lattice:
+    locate + nearest boundary of random points, every device path against the oracle."""
+    P = CASES[name]()
+    g = gpu.Problem(P, max_particles=20000)
+    o = orc.Oracle(P)
+    rng = np.random.default_rng(11)
+    n = 3000
+    lo, hi = np.array(P["src_lo"], float), np.array(P["src_hi"], float)
+    hi = np.where(hi > lo, hi, lo + 1.0)
+    x = lo + rng.uniform(0, 1, (n, 3)) * (hi - lo)
+    mu, phi = rng.uniform(-1, 1, n), rng.uniform(0, 2 * np.pi, n)
+    sq = np.sqrt(1 - mu * mu)
+    u = np.column_stack([sq * np.cos(phi), sq * np.sin(phi), mu])
+    res = [g.geometry(x, u, path=k) for k in (0, 1, 2)]
+    for i in range(n):
+        rc, lo_ = o.locate(x[i], u[i])
+        d, sh = o.distance(x[i], u[i], lo_)
+        for loc, dist, surf in res:
+            assert rc == 0 and tuple(lo_) == tuple(loc[i])
+            assert sh == surf[i] and (dist[i] == pytest.approx(d, rel=1e-12) or (np.isinf(d) and np.isinf(dist[i])))
     g.close()
 
 
@@ -183,20 +233,68 @@ def test_empty_and_error_paths(gpu):
     g2.close()
 
 
-def test_bank_overflow_and_lost_particle_errors(gpu):
-    """R6: more than 2N fission sites is MCDC_EBANK; a source point in no cell is MCDC_EGEOM; both leave the
-    problem usable for a later valid run."""
-    P = inputs.config1(n_particles=2000, n_inactive=0, n_active=2)
-    P["mg_nu"] = P["mg_nu"] * 4.0  # k_inf = 5.2: the first cycle banks about 5 N sites
+def test_bank_overflow_and_lost_particle_errors(gpu, orc):
+    """R6: more than 2N fission sites is MCDC_EBANK and leaves the problem usable; a source box that is not inside
+    the geometry is MCDC_EGEOM at create; a failed run leaves the last successful run's results readable."""
+    P = inputs.config1(n_particles=2000, n_inactive=1, n_active=2)
     g = gpu.Problem(P)
+    good = g.run()
+    # cycle 0 of a new run samples 2000 source particles as before; then feed a cycle more particles than it can bank
+    with pytest.raises(gpu.McdcError) as e:
+        g.run(n_particles=5000)  # exceeds the capacity the problem was created for: refused before any device work
+    assert e.value.code == -1
+    after = g.results()
+    assert (after["k_cycle"] == good["k_cycle"]).all() and (after["flux_mean"] == good["flux_mean"]).all()
+    g.close()
+    P2 = inputs.config1(n_particles=2000, n_inactive=0, n_active=2)
+    P2["mg_nu"] = P2["mg_nu"] * 4.0  # k_inf = 5.2: the first cycle banks about 5 N sites
+    g = gpu.Problem(P2)
     with pytest.raises(gpu.McdcError) as e:
         g.run()
     assert e.value.code == -3
+    assert g.dims().n_cycles == 0  # nothing was published
+    r = g.run(n_particles=300, n_inactive=0, n_active=1)  # 300 x 5.2 sites fit: the problem is still usable
+    assert r["counters"][0] == 300 and len(r["k_cycle"]) == 1
+    with pytest.raises(gpu.McdcError):
+        g.run()
+    again = g.results()  # the failed run did not touch what the last good one published
+    assert (again["k_cycle"] == r["k_cycle"]).all() and (again["flux_mean"] == r["flux_mean"]).all()
+    assert (again["counters"] == r["counters"]).all()
     g.close()
     P = inputs.config1(n_particles=500, n_inactive=0, n_active=1)
     P["src_hi"] = np.array([1.5, 1.0, 1.0])  # a third of the source box lies outside the cube
-    g = gpu.Problem(P)
+    with pytest.raises(gpu.McdcError) as e:
+        gpu.Problem(P)
+    assert e.value.code == -2
+
+
+def test_segment_guard(gpu, orc):
+    """R11: a history that never ends (pure scatterer in a reflecting box) is cut at 10^6 segments with MCDC_ELOST;
+    the oracle reports the same error and the same number of events."""
+    P = inputs.config1(n_particles=3, n_inactive=0, n_active=1)
+    P["mg_S"] = P["mg_sig_t"].reshape(1, 1, 1).copy()  # Sigma_s = Sigma_t: nothing absorbs
+    P["mg_sig_f"] = P["mg_sig_f"] * 0.0
+    o = orc.Oracle(P)
+    rc, ro = o.run()
+    assert rc == -4 and ro["counters"][10] == 3
+    g = gpu.Problem(P, persist_threshold=ALWAYS)
     with pytest.raises(gpu.McdcError) as e:
         g.run()
-    assert e.value.code == -2
+    assert e.value.code == -4
     g.close()
+
+
+def test_validation_errors(gpu):
+    P = inputs.rect_lattice(3, 2)
+    bad = dict(P)
+    bad["cell_bin"] = P["cell_bin"].copy()
+    bad["cell_bin"][1:] = 1  # cell_bin + max lat_bin reaches n_bins
+    with pytest.raises(gpu.McdcError) as e:
+        gpu.Problem(bad)
+    assert e.value.code == -1
+    bad = dict(P)
+    bad["univ_cell_off"] = P["univ_cell_off"].copy()
+    bad["univ_cell_off"][-1] += 1
+    with pytest.raises(gpu.McdcError) as e:
+        gpu.Problem(bad)
+    assert e.value.code == -1
