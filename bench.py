@@ -29,11 +29,10 @@ if ROOT not in sys.path:
 
 METRIC = "active particle histories/sec"
 UNIT = "histories/s"
-B_ALG_MG = 176.0      # algorithmic bytes per MG event, whole event (SURVEY.md 8d; DESIGN.md 6)
-B_ADV_MG = 112.0      # part of it moved by k_advance
-B_ALG_CE = 374.0
-B_ADV_CE = 310.0
+B_ALG_MG = 176.0      # algorithmic bytes per MG event, whole event (SURVEY.md 8d; DESIGN.md 5)
+B_ALG_CE = 374.0      # per CE event
 FALLBACK_HBM_GBS = 6650.0
+N_SM, N_SMSP = 148, 4  # B200: issue slots per second = N_SM * N_SMSP * SM clock (one warp instruction per slot)
 
 
 def peaks():
@@ -89,6 +88,43 @@ class ClockSampler:
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def ncu_counts():
+    """Per-event instruction and DRAM-traffic figures of the dominant kernels, measured by ncu on this build (they are
+    properties of the build and the workload, not of a timing); profiles/r02_counts.md names the captures."""
+    out = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_counts.csv")) as f:
+            rows = [l.strip().split(",") for l in f if l.strip()]
+        for r in rows[1:]:
+            ev = float(r[1])
+            out[r[0]] = {"warp_inst_per_event": float(r[2]) / ev, "dram_bytes_per_event": (float(r[3]) + float(r[4])) / ev,
+                         "source": "ncu --set full, profiles/r02_counts.md"}
+    except Exception:
+        pass
+    return out
+
+
+def alu_roofline(g, key, events_per_sec, clocks_mhz):
+    """The path is bound by instruction issue / dependent latency, not by HBM: report the issue-slot roofline beside
+    the HBM one.  peak = measured FFMA issue rate of this GPU (library micro-benchmark, warp instructions/s);
+    achieved = warp instructions per event (ncu, this build) x events/s."""
+    cnt = ncu_counts().get(key, {})
+    try:
+        ffma = g.microbench("ffma", 20000) / 32.0   # warp instructions per second
+        dfma = g.microbench("dfma", 20000)
+    except Exception:
+        return None
+    wipe = cnt.get("warp_inst_per_event")
+    out = {"bound": "alu", "unit": "warp-inst/s", "peak": ffma, "peak_source": "measured: mcdc_microbench FFMA issue rate",
+           "nominal_peak": N_SM * N_SMSP * (clocks_mhz or 1965.0) * 1e6, "dfma_per_sec_measured": dfma,
+           "warp_inst_per_event": wipe, "thread_inst_per_event": cnt.get("thread_inst_per_event"),
+           "counts_source": cnt.get("source")}
+    if wipe:
+        out["achieved"] = wipe * events_per_sec
+        out["frac"] = out["achieved"] / ffma
+    return out
 
 
 def max_over_ranks(x: float, world: int, device=None) -> float:
@@ -148,7 +184,8 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "C4 2-D quarter core, 7 groups (bounded sample)", "particles_per_cycle": n},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "host_cores_available": os.cpu_count()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -213,29 +250,32 @@ def run_ours(args):
     g.set_profile(False)
     ca = g.results()["counters"]
     ev_prof = events_of(ca) - events_of(cb)
-    adv = prof["sweep"]
     peak, peak_src = peaks()
     tot_ms = sum(v["ms"] for v in prof.values())
+    # the dominant kernel: the persistent kernel (default schedule: the whole cycle), else the sweep kernel
+    ev_sweep = prof["sweep"].get("events", 0)
+    dom = "persist" if prof["persist"]["ms"] >= prof["sweep"]["ms"] else "sweep"
+    ev_dom = ev_prof - ev_sweep if dom == "persist" else ev_sweep
+    kd = prof[dom]
+    cnt = ncu_counts().get("k_persist_mg" if dom == "persist" else "k_sweep_mg", {})
     roof = None
-    if adv["launches"]:
-        ev_adv = adv["events"]  # live particles the k_advance launches processed (device counter)
-        bytes_per_launch = B_ADV_MG * ev_adv / adv["launches"]
-        dur = adv["ms"] * 1e-3 / adv["launches"]
+    if kd["launches"]:
+        bytes_per_launch = B_ALG_MG * ev_dom / kd["launches"]
+        dur = kd["ms"] * 1e-3 / kd["launches"]
         ach = bytes_per_launch / dur / 1e9
-        roof = {"bound": "hbm", "kernel": "k_sweep<MG>", "achieved": ach, "peak": peak, "unit": "GB/s",
-                "frac": ach / peak, "traffic": None, "peak_source": peak_src,
-                "bytes_per_event": B_ADV_MG, "events_per_launch": ev_adv / adv["launches"],
-                "share_of_events": ev_adv / max(ev_prof, 1),
-                "avg_launch_ms": 1e3 * dur, "share_of_step": adv["ms"] / tot_ms if tot_ms else None,
+        roof = {"bound": "hbm", "kernel": f"k_{dom}<MG>", "achieved": ach, "peak": peak, "unit": "GB/s",
+                "frac": ach / peak, "peak_source": peak_src, "bytes_per_event": B_ALG_MG,
+                "events_per_launch": ev_dom / kd["launches"], "share_of_events": ev_dom / max(ev_prof, 1),
+                "avg_launch_ms": 1e3 * dur, "share_of_step": kd["ms"] / tot_ms if tot_ms else None,
+                "traffic": (cnt["dram_bytes_per_event"] * ev_dom / kd["launches"]) if "dram_bytes_per_event" in cnt else None,
+                "traffic_source": cnt.get("source"),
                 "whole_event": {"bytes_per_event": B_ALG_MG, "achieved": ev_per_s / world * B_ALG_MG / 1e9,
                                 "frac": ev_per_s / world * B_ALG_MG / 1e9 / peak},
-                "kernel_ms": {k: round(v["ms"] / n_prof, 3) for k, v in prof.items() if v["launches"]}}
-        tr = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tr):
-            try:
-                roof["traffic"] = json.load(open(tr))["k_advance_bytes_per_event"] * ev_adv / adv["launches"]
-            except Exception:
-                pass
+                "kernel_ms": {k: round(v["ms"] / n_prof, 3) for k, v in prof.items() if v["launches"]},
+                "note": "the persistent kernel keeps particle state in registers: the algorithmic bytes of SURVEY.md 8d "
+                        "(state read + written every event) are mostly never moved; DRAM traffic is far below them"}
+        roof["alu"] = alu_roofline(g, "k_persist_mg" if dom == "persist" else "k_sweep_mg", ev_per_s / world,
+                                   (clocks or {}).get("sm_mhz"))
 
     # ---- end to end through the host-buffer C-ABI call: source bank H2D, fission bank + flux D2H every step
     cap = 2 * N + 1024
@@ -266,7 +306,8 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config][0],
                    "particles_per_cycle": N, "step": "one power-iteration cycle", "parallelism": "replicas only",
-                   "l2": "particle bank (>1.2 GB) larger than L2" if N >= 2_000_000 else "bank fits in L2 (small configuration)", "schedule": "event sweeps over dense queues regrouped by next event; persistent asynchronous kernel below the library's live-particle threshold",
+                   "l2": "particle bank (>1.2 GB) larger than L2" if N >= 2_000_000 else "bank fits in L2 (small configuration)", "schedule": ("persistent asynchronous kernel: one launch per cycle, warps refill dead lanes from a ticket queue (library default)"
+                                if args.persist == 0 and args.schedule == 0 else f"schedule {args.schedule}, persist_threshold {args.persist}"),
                    "k_mean": res["k_mean"]},
         "events_per_sec": ev_per_s, "events_per_history": events / max(tracks, 1),
         "roofline": roof, "e2e": e2e, "gpu_launches": int(nl1 - nl0), "clocks": clocks,
@@ -282,11 +323,22 @@ def run_ours(args):
         o.n_cycles = 1 + args.ref_cycles
         cnt = o.results()["counters"]
         dtc = max(tt - tw, 1e-9)
+        ncore = os.cpu_count() or 1
+        nm = 4 * n  # the all-core run gets a four times larger sample of the same workload
+        Pm = inputs.config4(n_particles=nm, n_inactive=1, n_active=args.ref_cycles)
+        om = oracle.Oracle(Pm)
+        t0 = time.perf_counter(); om.L.orc_run_eigenvalue_mt(om.h, nm, 1, 0, 1, ncore); twm = time.perf_counter() - t0
+        t0 = time.perf_counter(); om.L.orc_run_eigenvalue_mt(om.h, nm, 1, args.ref_cycles, 1, ncore); ttm = time.perf_counter() - t0
         out["cpu_baseline"] = {"value": args.ref_cycles * n / dtc, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": f"C4 at {n} particles/cycle, {args.ref_cycles} active cycles after 1 (full: 1e7/cycle)",
-                               "events_per_sec": events_of(cnt) / tt, "host_cores_available": os.cpu_count()}
+                               "events_per_sec": events_of(cnt) / tt, "host_cores_available": ncore,
+                               "all_cores": {"value": args.ref_cycles * nm / max(ttm - twm, 1e-9), "unit": UNIT, "cores": ncore,
+                                             "kind": "oracle (OpenMP over particles, tallies joined in thread order)",
+                                             "sample": f"C4 at {nm} particles/cycle, {args.ref_cycles} active cycles after 1"}}
         # PAPER.md:118-120 Eq. (1): CPU cores one GPU is worth = (cores x CPU time) / (GPUs x GPU time) on the same work
         out["core_equivalency_eq1"] = value / world / (out["cpu_baseline"]["value"] / out["cpu_baseline"]["cores"])
+        ac = out["cpu_baseline"]["all_cores"]
+        out["core_equivalency_eq1_all_cores"] = value / world / (ac["value"] / ac["cores"])
 
     if rank == 0 and args.ce:
         out["secondary"] = bench_ce(binding, inputs, args, peak)
@@ -317,15 +369,24 @@ def bench_ce(binding, inputs, args, peak):
     g.run()
     prof = g.profile()
     g.set_profile(False)
+    ev_sweep = prof["sweep"].get("events", 0)
+    dom = "persist" if prof["persist"]["ms"] >= prof["sweep"]["ms"] else "sweep"
+    kd = prof[dom]
+    ev_dom = ev - ev_sweep if dom == "persist" else ev_sweep
+    cnt = ncu_counts().get("k_persist_ce" if dom == "persist" else "k_sweep_ce", {})
+    ach = B_ALG_CE * ev_dom / (kd["ms"] * 1e-3) / 1e9 if kd["ms"] else None
+    ev_per_s = ev / (best * 1e-3)
+    roof = {"bound": "hbm", "kernel": f"k_{dom}<CE>", "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak if ach else None, "bytes_per_event": B_ALG_CE,
+            "events_per_launch": ev_dom / max(kd["launches"], 1), "avg_launch_ms": kd["ms"] / max(kd["launches"], 1),
+            "traffic": (cnt["dram_bytes_per_event"] * ev_dom / max(kd["launches"], 1)) if "dram_bytes_per_event" in cnt else None,
+            "traffic_source": cnt.get("source"),
+            "whole_event": {"bytes_per_event": B_ALG_CE, "frac": ev_per_s * B_ALG_CE / 1e9 / peak}}
+    roof["alu"] = alu_roofline(g, "k_persist_ce" if dom == "persist" else "k_sweep_ce", ev_per_s, None)
     g.close()
-    adv = prof["sweep"]
-    ach = B_ADV_CE * adv["events"] / (adv["ms"] * 1e-3) / 1e9 if adv["ms"] else None
     return {"workload": "C5: continuous-energy time-dependent pin cell", "source_particles": args.ce_particles,
             "histories_per_sec": args.ce_particles / (best * 1e-3), "tracks": int(r["counters"][0]),
-            "events_per_sec": ev / (best * 1e-3), "ms": best,
-            "roofline": {"bound": "hbm", "kernel": "k_sweep<CE>", "achieved": ach, "peak": peak, "unit": "GB/s",
-                         "frac": ach / peak if ach else None, "bytes_per_event": B_ADV_CE,
-                         "whole_event": {"bytes_per_event": B_ALG_CE, "frac": ev / (best * 1e-3) * B_ALG_CE / 1e9 / peak}},
+            "events_per_sec": ev_per_s, "ms": best, "roofline": roof,
             "kernel_ms": {k: round(v["ms"], 3) for k, v in prof.items() if v["launches"]}}
 
 

@@ -758,8 +758,10 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
                 aux = (int)floor(c.w0 * mgv(acc, c.mg.o_nu + mat * c.mg.G + p.g) / c.k_prev + rng.next(c));
             } else { ev = 3; code = ADV_DEAD; }
         } else {
-            int r = 0;
-            while (r < ncol - 1 && !(cum[r] > uu)) r++;
+            int r = ncol - 1;  // first column whose cumulative value exceeds uu (static indices: cum stays in registers)
+#pragma unroll
+            for (int j = MAX_CE_COL - 2; j >= 0; j--)
+                if (j < ncol - 1 && cum[j] > uu) r = j;
             if (r < ncol - 2) { ev = 1; code = ADV_SCATTER; p.pend = PEND_SCATTER | (unsigned int)r; }
             else if (r == ncol - 2) {
                 ev = 2; code = ADV_FISSION;

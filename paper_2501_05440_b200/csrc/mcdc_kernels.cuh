@@ -483,10 +483,6 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
     Rng rng;
     rng.init(0ull, 0u);
     unsigned int taken = 0, n_end = 0, idle_ns = 500;
-#ifdef MCDC_TIMELINE
-    unsigned long long tl_trips = 0, tl_lanes = 0, tl_idle = 0, tl_t0 = 0, tl_src = 0;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t0));
-#endif
     for (;;) {
         const unsigned int want = __ballot_sync(FULL, !alive && !ticketed && !drained);
         const int nw = __popc(want);
@@ -572,18 +568,10 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
                 fin = __shfl_sync(FULL, fin, 0);
             }
             if (fin) break;
-#ifdef MCDC_TIMELINE
-            tl_idle++;
-#endif
             if (CE) { __nanosleep(idle_ns); if (idle_ns < 16000) idle_ns *= 2; }
             continue;
         }
         idle_ns = 500;
-#ifdef MCDC_TIMELINE
-        tl_trips++;
-        tl_lanes += __popc(__ballot_sync(FULL, alive));
-        if (!tl_src && *(volatile unsigned int *)head >= n_in) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_src));
-#endif
         const unsigned int amask = __ballot_sync(FULL, alive);
         if (alive) {
             int aux = 0, code = ADV_DEAD;
@@ -634,19 +622,6 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
             }
         }
     }
-#ifdef MCDC_TIMELINE
-    if (lane == 0) {
-        unsigned long long t1;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-        atomicAdd(c.counters + 0, tl_trips);
-        atomicAdd(c.counters + 11, tl_lanes);
-        atomicAdd(c.counters + 13, tl_idle);
-        atomicMax(c.counters + 12, t1 - tl_t0);
-        if (tl_src) atomicMax(c.counters + 9, tl_src - tl_t0);  // (slot 9 = cutoff events: debug build only)
-        // histogram of warp end times in 8 bins of 1/8 of ... keep simple: sum of end times
-        atomicAdd(c.counters + 10, t1 - tl_t0);
-    }
-#endif
     taken = __reduce_add_sync(FULL, taken);
     if (lane == 0 && taken) atomicAdd(c.counters + 14, (unsigned long long)taken);
     if (PRIVATE) flush_private_flux(c, s_flux);

@@ -32,12 +32,14 @@ static int fail(int code, const char *fmt, ...)
     } while (0)
 
 static const int LAG = 3;                 // sweeps the host may run ahead of the queue-count read-back
-// live particles at or below which the persistent kernel finishes the cycle (measured on B200, profiles/r02_*.md)
+// live particles at or below which the persistent kernel takes over from the event sweeps.  Measured on B200
+// (profiles/r02_schedules.md, ms per C4 cycle): 1.5e6 -> 36.1, 4e6 -> 33.7, 6e6 -> 32.3, 9e6 -> 30.5, always -> 29.2:
+// the default is "always" -- a cycle (a whole fixed-source run) is ONE persistent launch.
 #ifndef MCDC_PERSIST_DEFAULT
-#define MCDC_PERSIST_DEFAULT 1500000
+#define MCDC_PERSIST_DEFAULT 0x7fffffff
 #endif
 static const int DEFAULT_PERSIST = MCDC_PERSIST_DEFAULT;
-static const int DEFAULT_PERSIST_CE = 0x7fffffff;  // continuous energy: the whole run is one persistent launch
+static const int DEFAULT_PERSIST_CE = 0x7fffffff;
 static const uint64_t TRACE_BYTES = 48ull << 20;
 #ifndef MCDC_AGG_MAX
 #define MCDC_AGG_MAX 4096
@@ -771,11 +773,6 @@ static void publish(mcdc_problem *p)
 {
     RunStats &w = p->work;
     for (int i = 0; i < MCDC_N_COUNTERS; i++) w.counters[i] = p->pin->counters[i];
-#ifdef MCDC_TIMELINE
-    fprintf(stderr, "TIMELINE trips %llu lane-trips %llu idle-trips %llu max-warp-ns %llu src-exhausted-ns %llu sum-warp-ns %llu taken %llu\n",
-            p->pin->counters[0], p->pin->counters[11], p->pin->counters[13], p->pin->counters[12], p->pin->counters[9],
-            p->pin->counters[10], p->pin->counters[14]);
-#endif
     // histories started / children made: source-bank histories are counted on the host, secondaries that joined the
     // running population (continuous energy) on the device (counter 15)
     w.counters[0] = w.host_counters[0] + p->pin->counters[15];
