@@ -43,6 +43,7 @@ class OrcInput(C.Structure):
         ("n_t", C.c_int32), ("t_edges", _dp), ("n_e", C.c_int32), ("e_edges", _dp),
         ("src_lo", C.c_double * 3), ("src_hi", C.c_double * 3), ("src_iso", C.c_int32),
         ("src_dir", C.c_double * 3), ("src_group_pdf", _dp), ("src_E", C.c_double), ("src_t", C.c_double),
+        ("kT", C.c_double), ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double),
     ]
 
 
@@ -81,6 +82,9 @@ def lib():
         L.orc_get_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
         L.orc_get_bank.restype = C.c_uint64
         L.orc_get_bank.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+        L.orc_get_balance.argtypes = [C.c_void_p, _dp]
+        L.orc_free_gas.argtypes = [C.c_double, _dp, C.c_double, C.c_double, C.c_uint64, C.c_uint64, C.c_uint32,
+                                   C.POINTER(C.c_uint32), _dp, _dp]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.orc_draw.restype = C.c_double
         L.orc_draw.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32]
@@ -165,6 +169,10 @@ class Oracle:
         inp.src_iso = int(P["src_iso"])
         inp.src_dir = (C.c_double * 3)(*P["src_dir"])
         inp.src_t = P.get("src_t", 0.0)
+        inp.kT = float(P.get("kT", 0.0))
+        inp.implicit_capture = int(P.get("implicit_capture", 0))
+        inp.w_roulette = float(P.get("w_roulette", 0.25))
+        inp.w_survive = float(P.get("w_survive", 1.0))
         self.L = lib()
         self.h = self.L.orc_create(C.byref(inp))
         self.n_tally = self.L.orc_n_tally(self.h)
@@ -217,6 +225,12 @@ class Oracle:
                                     cnt.ctypes.data_as(C.POINTER(C.c_uint64)))
         return dict(rc=rc, k_cycle=kc[: self.n_cycles], k_mean=sc[0].value, k_sdev=sc[1].value, flux_mean=fm,
                     flux_sdev=fs, leak_mean=sc[2].value, leak_sdev=sc[3].value, counters=cnt)
+
+    def balance(self):
+        """Weight balance of the last run: dict(source, absorbed, leaked, cutoff, roulette_loss, roulette_gain)."""
+        out = np.zeros(6)
+        self.L.orc_get_balance(self.h, out.ctypes.data_as(_dp))
+        return dict(zip(("source", "absorbed", "leaked", "cutoff", "roulette_loss", "roulette_gain"), out))
 
     def trace(self):
         n = self.L.orc_get_trace(self.h, None, 0)
@@ -280,6 +294,16 @@ def elastic(E, u, A, a, b):
     e = C.c_double()
     lib().orc_elastic(E, u.ctypes.data_as(_dp), A, a, b, C.byref(e), o.ctypes.data_as(_dp))
     return e.value, o
+
+
+def free_gas(E, u, A, kT, seed, pid, cycle=0, ctr=0):
+    """One free-gas collision drawn from stream (seed, pid, 0, cycle) starting at draw ctr: (E', u', draws used)."""
+    u = _d(u)
+    o = np.zeros(3)
+    e = C.c_double()
+    c = C.c_uint32(ctr)
+    lib().orc_free_gas(E, u.ctypes.data_as(_dp), A, kT, seed, pid, cycle, C.byref(c), C.byref(e), o.ctypes.data_as(_dp))
+    return e.value, o, c.value - ctr
 
 
 def watt(a, b, x1, x2, x3, x4):

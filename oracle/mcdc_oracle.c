@@ -16,6 +16,8 @@
 #define C_LIGHT 2.99792458e10    /* cm/s (R23) */
 #define MN_C2_EV 939.56542052e6  /* neutron rest energy, eV (R23) */
 #define MAX_SEGMENTS 1000000u    /* lost-particle guard (R11) */
+#define SQRT_PI 1.7724538509055159
+#define FREE_GAS_LIMIT 400.0     /* free gas below 400 kT, target at rest above (R35) */
 
 typedef struct {
     double x, y, z, ux, uy, uz, w, E, t;
@@ -38,6 +40,7 @@ struct orc_problem {
     int fixed;
     /* per-cycle tallies */
     double *flux_c, k_num, leak_c;
+    double balance[6]; /* see orc_get_balance */
     /* accumulated results */
     int n_cycles, n_active_done;
     double *k_cycle, *flux_acc, *flux_acc2, leak_acc, leak_acc2, k_acc, k_acc2;
@@ -163,6 +166,70 @@ void orc_elastic(double E, const double u[3], double A, double xi_mu, double xi_
     u_out[0] = o[0] / nrm;
     u_out[1] = o[1] / nrm;
     u_out[2] = o[2] / nrm;
+}
+
+/* rotate unit vector u by polar cosine mu and azimuth phi (R21 formula) */
+static void rotate(const double u[3], double mu, double phi, double o[3])
+{
+    double cp = cos(phi), sp = sin(phi);
+    double s2 = 1.0 - mu * mu;
+    double s = s2 > 0.0 ? sqrt(s2) : 0.0;
+    double a2 = 1.0 - u[2] * u[2];
+    if (a2 < 1e-10) {
+        o[0] = s * cp; o[1] = s * sp; o[2] = u[2] > 0.0 ? mu : -mu;
+    } else {
+        double r = sqrt(a2);
+        o[0] = mu * u[0] + s * (u[0] * u[2] * cp - u[1] * sp) / r;
+        o[1] = mu * u[1] + s * (u[1] * u[2] * cp + u[0] * sp) / r;
+        o[2] = mu * u[2] - s * r * cp;
+    }
+    double nrm = sqrt(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]);
+    o[0] /= nrm; o[1] /= nrm; o[2] /= nrm;
+}
+
+/* Free-gas elastic scattering with a constant cross section ("free-gas scattering model with constant
+ * cross-sections"; R35).  Velocities in units where speed = sqrt(E).  The target speed x (in units of sqrt(kT/A))
+ * and the cosine mu between target and neutron are drawn from p(x, mu) ~ |v_n - v_T| x^2 exp(-x^2) by the classic
+ * two-branch scheme: with probability alpha = 1 / (1 + sqrt(pi) y / 2), y = sqrt(A E / kT), x^2 = -ln(xi1 xi2);
+ * otherwise x^2 = -ln xi1 - ln xi2 cos^2(pi xi4 / 2); mu = 2 xi - 1; accepted with probability
+ * sqrt(y^2 + x^2 - 2 x y mu) / (x + y).  Draws per trial, in order: xi1, xi2, branch, [xi4], mu, accept.  Then the
+ * target direction (azimuth 2 pi xi around the neutron's), and an isotropic direction of the relative velocity in
+ * the centre-of-mass frame (2 draws). */
+void orc_free_gas(double E, const double u[3], double A, double kT, uint64_t seed, uint64_t id, uint32_t cycle, uint32_t *ctr,
+                  double *E_out, double u_out[3])
+{
+    double y = sqrt(A * E / kT);
+    double alpha = 1.0 / (1.0 + SQRT_PI * y / 2.0);
+    double x2, x, mu;
+    for (;;) {
+        double r1 = orc_draw(seed, id, 0u, cycle, (*ctr)++), r2 = orc_draw(seed, id, 0u, cycle, (*ctr)++);
+        if (orc_draw(seed, id, 0u, cycle, (*ctr)++) < alpha) x2 = -log(r1 * r2);
+        else {
+            double c = cos(HALF_PI * orc_draw(seed, id, 0u, cycle, (*ctr)++));
+            x2 = -log(r1) - log(r2) * c * c;
+        }
+        x = sqrt(x2);
+        mu = 2.0 * orc_draw(seed, id, 0u, cycle, (*ctr)++) - 1.0;
+        double acc = sqrt(y * y + x2 - 2.0 * x * y * mu) / (x + y);
+        if (orc_draw(seed, id, 0u, cycle, (*ctr)++) < acc) break;
+    }
+    double ut[3];
+    rotate(u, mu, TWO_PI * orc_draw(seed, id, 0u, cycle, (*ctr)++), ut);
+    double sn = sqrt(E), st = x * sqrt(kT / A);
+    double vn[3], vc[3], vr[3], o[3];
+    for (int k = 0; k < 3; k++) {
+        vn[k] = sn * u[k];
+        vc[k] = (vn[k] + A * st * ut[k]) / (A + 1.0);
+        vr[k] = vn[k] - vc[k];
+    }
+    double s = sqrt(vr[0] * vr[0] + vr[1] * vr[1] + vr[2] * vr[2]);
+    double a = orc_draw(seed, id, 0u, cycle, (*ctr)++), b = orc_draw(seed, id, 0u, cycle, (*ctr)++);
+    orc_iso_dir(a, b, o);
+    double v[3] = {vc[0] + s * o[0], vc[1] + s * o[1], vc[2] + s * o[2]};
+    double e = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    double nv = sqrt(e);
+    *E_out = e;
+    u_out[0] = v[0] / nv; u_out[1] = v[1] / nv; u_out[2] = v[2] / nv;
 }
 
 /* ------------------------------------------------------------------ geometry (R11-R14) */
@@ -579,6 +646,7 @@ static void transport(orc_problem *p, particle *q)
     const orc_input *in = &p->in;
     double xs[64];
     p->counters[0]++;
+    p->balance[0] += q->w;
     while (q->alive) {
         double x[3] = {q->x, q->y, q->z}, u[3] = {q->ux, q->uy, q->uz};
         int32_t loc[3] = {q->c0, q->elem, q->c1};
@@ -626,17 +694,36 @@ static void transport(orc_problem *p, particle *q)
         int ev;
         if (kind == 0) {
             q->last_surf = -1;
-            double uu = draw(p, q) * sig_t;
+            /* reaction choice.  Analog (R3): xi Sigma_t against [scatter, fission, capture].  Implicit capture (R36):
+             * the weight loses its capture share, w <- w (Sigma_t - Sigma_c) / Sigma_t, and xi (Sigma_t - Sigma_c) is
+             * compared against [scatter, fission]; a scattered particle whose weight fell below w_roulette plays
+             * roulette (one more draw): it survives with probability w / w_survive at weight w_survive. */
+            const int implicit = in->implicit_capture;
+            int rouletted = 0;
             if (in->mode == 0) {
                 int G = in->G;
                 double sig_s = p->sig_s[mat * G + q->g], sig_f = in->sig_f[mat * G + q->g];
+                double total = sig_t;
+                if (implicit) {
+                    total = sig_s + sig_f;
+                    double wn = q->w * (total / sig_t);
+                    p->balance[1] += q->w - wn;
+                    q->w = wn;
+                }
+                double uu = draw(p, q) * total;
                 if (uu < sig_s) {
                     ev = ORC_EV_SCATTER;
-                    double vv = draw(p, q) * sig_s;
-                    int32_t gp = pick(p->cumS + ((size_t)mat * G + q->g) * G, G, vv);
-                    double xi1 = draw(p, q), xi2 = draw(p, q), o[3];
-                    orc_iso_dir(xi1, xi2, o);
-                    q->g = gp; q->ux = o[0]; q->uy = o[1]; q->uz = o[2];
+                    if (implicit && q->w < in->w_roulette) {
+                        if (draw(p, q) * in->w_survive < q->w) { p->balance[5] += in->w_survive - q->w; q->w = in->w_survive; }
+                        else { p->balance[4] += q->w; rouletted = 1; ev = ORC_EV_CAPTURE; q->alive = 0; }
+                    }
+                    if (!rouletted) {
+                        double vv = draw(p, q) * sig_s;
+                        int32_t gp = pick(p->cumS + ((size_t)mat * G + q->g) * G, G, vv);
+                        double xi1 = draw(p, q), xi2 = draw(p, q), o[3];
+                        orc_iso_dir(xi1, xi2, o);
+                        q->g = gp; q->ux = o[0]; q->uy = o[1]; q->uz = o[2];
+                    }
                 } else if (uu < sig_s + sig_f) {
                     ev = ORC_EV_FISSION;
                     int n = (int)floor(q->w * in->nu[mat * G + q->g] / p->k_prev + draw(p, q));
@@ -648,21 +735,44 @@ static void transport(orc_problem *p, particle *q)
                         bank_site(p, q, o, gj);
                         p->counters[11]++;
                     }
+                    p->balance[1] += q->w;
                     q->alive = 0;
                 } else {
                     ev = ORC_EV_CAPTURE;
+                    p->balance[1] += q->w;
                     q->alive = 0;
                 }
             } else {
-                int32_t r = pick(xs + 1, ncol, uu);
+                double total = sig_t;
+                int32_t nsel = ncol;
+                if (implicit) {
+                    total = xs[ncol - 1]; /* cumulative value before the capture column */
+                    nsel = ncol - 1;
+                    double wn = q->w * (total / sig_t);
+                    p->balance[1] += q->w - wn;
+                    q->w = wn;
+                }
+                double uu = draw(p, q) * total;
+                int32_t r = pick(xs + 1, nsel, uu);
                 if (r < ncol - 2) { /* elastic off nuclide r of this material */
                     ev = ORC_EV_SCATTER;
-                    double A = in->nuc_A[in->mat_nuc_id[in->mat_nuc_off[mat] + r]];
-                    double xi1 = draw(p, q), xi2 = draw(p, q), En, o[3];
-                    orc_elastic(q->E, u, A, xi1, xi2, &En, o);
-                    if (En < in->grid[0]) En = in->grid[0];
-                    if (En > in->grid[in->n_grid - 1]) En = in->grid[in->n_grid - 1];
-                    q->E = En; q->ux = o[0]; q->uy = o[1]; q->uz = o[2];
+                    if (implicit && q->w < in->w_roulette) {
+                        if (draw(p, q) * in->w_survive < q->w) { p->balance[5] += in->w_survive - q->w; q->w = in->w_survive; }
+                        else { p->balance[4] += q->w; rouletted = 1; ev = ORC_EV_CAPTURE; q->alive = 0; }
+                    }
+                    if (!rouletted) {
+                        double A = in->nuc_A[in->mat_nuc_id[in->mat_nuc_off[mat] + r]];
+                        double En, o[3];
+                        if (in->kT > 0.0 && q->E < FREE_GAS_LIMIT * in->kT)
+                            orc_free_gas(q->E, u, A, in->kT, p->seed, q->id, p->cycle, &q->ctr, &En, o);
+                        else {
+                            double xi1 = draw(p, q), xi2 = draw(p, q);
+                            orc_elastic(q->E, u, A, xi1, xi2, &En, o);
+                        }
+                        if (En < in->grid[0]) En = in->grid[0];
+                        if (En > in->grid[in->n_grid - 1]) En = in->grid[in->n_grid - 1];
+                        q->E = En; q->ux = o[0]; q->uy = o[1]; q->uz = o[2];
+                    }
                 } else if (r == ncol - 2) {
                     ev = ORC_EV_FISSION;
                     double nu = in->nu0 + in->nu1 * (q->E * 1e-6);
@@ -682,9 +792,11 @@ static void transport(orc_problem *p, particle *q)
                         push_secondary(p, &c);
                         p->counters[11]++;
                     }
+                    p->balance[1] += q->w;
                     q->alive = 0;
                 } else {
                     ev = ORC_EV_CAPTURE;
+                    p->balance[1] += q->w;
                     q->alive = 0;
                 }
             }
@@ -709,6 +821,7 @@ static void transport(orc_problem *p, particle *q)
                 if (bc == 2) {
                     ev = ORC_EV_LEAK;
                     p->leak_c += q->w;
+                    p->balance[2] += q->w;
                     q->alive = 0;
                 } else if (bc == 1) {
                     ev = ORC_EV_REFLECT;
@@ -733,7 +846,7 @@ static void transport(orc_problem *p, particle *q)
         } else {
             q->tbin++;
             q->last_surf = -1; /* R11: the particle has moved off the surface it sat on */
-            if (q->tbin == in->n_t) { ev = ORC_EV_CUTOFF; q->alive = 0; } else ev = ORC_EV_TIME_EDGE;
+            if (q->tbin == in->n_t) { ev = ORC_EV_CUTOFF; p->balance[3] += q->w; q->alive = 0; } else ev = ORC_EV_TIME_EDGE;
             trace(p, q, ev, loc[0], loc[1], loc[2], -1, gi, d, E_flight);
         }
         p->counters[ev]++;
@@ -811,6 +924,7 @@ static void reset_results(orc_problem *p, int n_cycles)
     memset(p->flux_acc2, 0, (size_t)nt * sizeof(double));
     memset(p->counters, 0, sizeof(p->counters));
     p->leak_acc = p->leak_acc2 = p->k_acc = p->k_acc2 = 0.0;
+    memset(p->balance, 0, sizeof(p->balance));
     p->n_cycles = p->n_active_done = 0;
     p->error = 0; p->tr_count = 0;
 }
@@ -890,6 +1004,7 @@ int orc_run_eigenvalue_mt(orc_problem *p, uint64_t N, int n_inactive, int n_acti
             memset(q->flux_c, 0, (size_t)nt * sizeof(double));
             memset(q->counters, 0, sizeof(q->counters));
             q->k_num = 0.0; q->leak_c = 0.0; q->n_newbank = 0; q->error = 0;
+            memset(q->balance, 0, sizeof(q->balance));
             uint64_t lo = M * (uint64_t)t / (uint64_t)n_threads, hi = M * (uint64_t)(t + 1) / (uint64_t)n_threads;
             for (uint64_t i = lo; i < hi; i++) {
                 particle pt;
@@ -909,6 +1024,7 @@ int orc_run_eigenvalue_mt(orc_problem *p, uint64_t N, int n_inactive, int n_acti
         for (int t = 0; t < n_threads; t++) { /* join in thread order */
             for (int64_t i = 0; i < nt; i++) p->flux_c[i] += th[t].flux_c[i];
             p->k_num += th[t].k_num; p->leak_c += th[t].leak_c;
+            for (int k = 0; k < 6; k++) p->balance[k] += th[t].balance[k];
             for (int k = 0; k < ORC_N_COUNTERS; k++) p->counters[k] += th[t].counters[k];
             if (th[t].error && !p->error) p->error = th[t].error;
             if (p->n_newbank + th[t].n_newbank > p->cap_bank) { p->error = -3; th[t].n_newbank = p->cap_bank - p->n_newbank; }
@@ -975,6 +1091,11 @@ int orc_get_results(const orc_problem *p, double *k_cycle, double *k_mean, doubl
     }
     memcpy(counters, p->counters, sizeof(p->counters));
     return p->error;
+}
+
+void orc_get_balance(const orc_problem *p, double out[6])
+{
+    for (int k = 0; k < 6; k++) out[k] = p->balance[k];
 }
 
 uint64_t orc_get_trace(const orc_problem *p, orc_trace_rec *out, uint64_t max)

@@ -63,6 +63,11 @@ typedef struct {
     double src_dir[3];
     const double *src_group_pdf; /* [G] */
     double src_E, src_t;
+    /* free-gas thermal scattering (R35): temperature kT in eV, 0 = target at rest */
+    double kT;
+    /* implicit capture / survival biasing with weight roulette (R36) */
+    int32_t implicit_capture;
+    double w_roulette, w_survive;
 } orc_input;
 
 typedef struct {
@@ -96,6 +101,14 @@ int orc_run_fixed_source(orc_problem *p, uint64_t n_particles, uint64_t seed);
 int64_t orc_n_tally(const orc_problem *p);
 int orc_get_results(const orc_problem *p, double *k_cycle, double *k_mean, double *k_sdev, double *flux_mean,
                     double *flux_sdev, double *leak_mean, double *leak_sdev, uint64_t *counters);
+/* weight balance of the last run, summed over all its cycles (not normalised): out[0] source weight started,
+ * [1] absorbed (analog capture / fission: the particle's weight; implicit capture: the weight removed at each
+ * collision), [2] leaked, [3] cut off at the last time edge, [4] killed by roulette, [5] gained by roulette survivors.
+ * Identity (to rounding): out[0] = out[1] + out[2] + out[3] + out[4] - out[5]. */
+void orc_get_balance(const orc_problem *p, double out[6]);
+/* free-gas elastic collision (R35) with the draws taken from stream (seed, id, domain 0, cycle) starting at *ctr */
+void orc_free_gas(double E, const double u[3], double A, double kT, uint64_t seed, uint64_t id, uint32_t cycle, uint32_t *ctr,
+                  double *E_out, double u_out[3]);
 uint64_t orc_get_trace(const orc_problem *p, orc_trace_rec *out, uint64_t max);
 uint64_t orc_get_bank(const orc_problem *p, orc_site *out, uint64_t max);
 
