@@ -203,6 +203,28 @@ int mcdc_run_cycle_host(mcdc_problem *p, uint64_t n_particles, uint32_t cycle, u
  * all their prompt fission secondaries, to the last time edge. */
 int mcdc_run_fixed_source(mcdc_problem *p, uint64_t n_particles, uint64_t seed);
 
+/* Physics options beyond the analog target-at-rest model ("free-gas scattering model
+ * with constant cross-sections"; R35, R36).  Takes effect from the next run call; NULL restores the defaults.
+ *   kT (eV): continuous-energy elastic collisions below 400 kT sample the target's thermal velocity (constant cross
+ *     section free gas); 0 = every target at rest.  Ignored by multi-group problems.
+ *   implicit_capture != 0: survival biasing.  Every particle carries its own weight; a collision removes the capture
+ *     share (w <- w (Sigma_t - Sigma_c) / Sigma_t) and chooses among scatter / fission; a scattered particle whose weight
+ *     fell below w_roulette survives with probability w / w_survive at weight w_survive (one extra draw).
+ *     0 <= w_roulette <= w_survive is required (w_roulette = 0: no roulette). */
+typedef struct {
+    double kT;
+    int32_t implicit_capture;
+    int32_t pad;
+    double w_roulette, w_survive;
+} mcdc_physics;
+int mcdc_set_physics(mcdc_problem *p, const mcdc_physics *phys);
+
+/* weight balance of the last successful run, summed over its cycles (not normalised): out[0] weight started (source
+ * particles and secondaries), [1] absorbed (capture, fission, and the capture share removed by implicit capture),
+ * [2] leaked, [3] cut off at the last time edge, [4] killed by roulette, [5] gained by roulette survivors.
+ * out[0] = out[1] + out[2] + out[3] + out[4] - out[5] up to rounding. */
+int mcdc_get_balance(const mcdc_problem *p, double out[6]);
+
 int mcdc_get_dims(const mcdc_problem *p, mcdc_dims *dims);
 int mcdc_get_tallies(const mcdc_problem *p, mcdc_tallies *out);
 /* current source bank (after a cycle: the sorted fission bank), at most max sites; returns the count via *n */

@@ -25,7 +25,8 @@ EV_NAMES = {1: "scatter", 2: "fission", 3: "capture", 4: "transmit", 5: "reflect
 SYMBOLS = ["mcdc_workspace_bytes", "mcdc_create", "mcdc_run_eigenvalue", "mcdc_run_cycle", "mcdc_run_cycle_host",
            "mcdc_run_fixed_source", "mcdc_get_dims", "mcdc_get_tallies", "mcdc_get_bank", "mcdc_set_trace",
            "mcdc_get_trace", "mcdc_test_draws", "mcdc_test_grid_index", "mcdc_test_geometry", "mcdc_get_timing",
-           "mcdc_set_profile", "mcdc_get_profile", "mcdc_microbench", "mcdc_destroy", "mcdc_last_error"]
+           "mcdc_set_profile", "mcdc_get_profile", "mcdc_microbench", "mcdc_destroy", "mcdc_last_error",
+           "mcdc_set_physics", "mcdc_get_balance"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -71,6 +72,11 @@ class Device(C.Structure):
     _fields_ = [("workspace", C.c_void_p), ("workspace_bytes", C.c_uint64), ("stream", C.c_void_p),
                 ("device", C.c_int32), ("schedule", C.c_int32), ("persist_threshold", C.c_int32),
                 ("reserved", C.c_int32 * 3)]
+
+
+class Physics(C.Structure):
+    _fields_ = [("kT", C.c_double), ("implicit_capture", C.c_int32), ("pad", C.c_int32), ("w_roulette", C.c_double),
+                ("w_survive", C.c_double)]
 
 
 class Dims(C.Structure):
@@ -137,6 +143,8 @@ def load_library():
     L.mcdc_set_profile.argtypes = [vp, i32]
     L.mcdc_get_profile.argtypes = [vp, _dp, P(u64), P(u64)]
     L.mcdc_microbench.argtypes = [vp, i32, u64, _dp, _dp]
+    L.mcdc_set_physics.argtypes = [vp, P(Physics)]
+    L.mcdc_get_balance.argtypes = [vp, _dp]
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -237,6 +245,8 @@ class Problem:
         self._check(self.L.mcdc_create(C.byref(g), mp, xp, C.byref(s), C.byref(t), C.byref(d), self.max_particles, C.byref(h)))
         self.h = h
         self.workspace_bytes = nbytes.value
+        if P.get("kT", 0.0) or P.get("implicit_capture", 0):
+            self.set_physics(P.get("kT", 0.0), P.get("implicit_capture", 0), P.get("w_roulette", 0.25), P.get("w_survive", 1.0))
         dims = self.dims()
         self.n_tally = dims.n_tally
 
@@ -259,6 +269,16 @@ class Problem:
         d = Dims()
         self._check(self.L.mcdc_get_dims(self.h, C.byref(d)))
         return d
+
+    def set_physics(self, kT=0.0, implicit_capture=0, w_roulette=0.25, w_survive=1.0):
+        ph = Physics(float(kT), int(implicit_capture), 0, float(w_roulette), float(w_survive))
+        self._check(self.L.mcdc_set_physics(self.h, C.byref(ph)))
+
+    def balance(self):
+        """Weight balance of the last run: dict(source, absorbed, leaked, cutoff, roulette_loss, roulette_gain)."""
+        out = np.zeros(6)
+        self._check(self.L.mcdc_get_balance(self.h, out.ctypes.data_as(_dp)))
+        return dict(zip(("source", "absorbed", "leaked", "cutoff", "roulette_loss", "roulette_gain"), out))
 
     # ---- runs
     def run(self, n_particles=None, n_inactive=None, n_active=None, seed=None):

@@ -74,6 +74,7 @@ struct CETab {
 // slot = index of the particle inside its cycle / wave (= its id in eigenvalue mode, R6).
 struct Bank {
     double *x, *y, *z, *ux, *uy, *uz, *E, *t;
+    double *w;  // statistical weight (implicit capture, R36); the analog path never touches it (R2: w = w0)
     int *cell, *elem, *gl, *tbin;
     uint32_t *ev, *ctr, *slot;
     uint64_t *id;
@@ -123,6 +124,10 @@ struct Ctx {
     unsigned long long seed;
     unsigned int cycle;
     double w0, k_prev;
+    // options set by mcdc_set_physics: free-gas thermal scattering below 400 kT (R35; kT in eV, 0 = target at rest),
+    // implicit capture with weight roulette (R36)
+    double kT, w_roulette, w_survive;
+    int implicit;
     int src_iso;
     double src_lo[3], src_hi[3], src_dir[3], src_E, src_t;
 };
@@ -151,6 +156,8 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 // consecutive draws cost one Philox evaluation; seed and cycle are launch constants read from the Ctx at use.
 // (A buffer of the segment's 5 draws filled at one code site was measured: 3 instead of ~5 Philox evaluations per
 // warp and segment, but 8 more live registers and the selects to read it: 31.0 instead of 29.9 ms per C4 cycle.)
+// (One out-of-line copy of the ten rounds called from every draw site -- 5 % less code -- was measured as well:
+// 31.5 instead of 29.8 ms per C4 cycle, C5 unchanged; profiles/r02_experiments.md.)
 struct Rng {
     unsigned long long id;
     uint32_t ctr, blk;
@@ -572,6 +579,7 @@ __device__ __forceinline__ bool surface_in_cell(const Geo &G, int c, int s)
 // ------------------------------------------------------------------ particle in registers
 struct Particle {
     double x, y, z, ux, uy, uz, E, t;
+    double w;       // statistical weight (read and written only by the weighted kernels, R36)
     double v;       // continuous energy: speed, union-grid index and tally energy bin of E (they change only when E
     int gi, ebin;   // does: at birth and in a scatter), kept with the particle instead of recomputed every segment
     int cell, elem, g, last, tbin;
@@ -584,12 +592,13 @@ struct Particle {
 // of the registers, which is what limits the occupancy of the latency-bound transport kernels.
 struct Acc {
     double knum;
+    double wabs;         // weight absorbed (weighted kernels only: capture share removed at collisions, fission, capture)
     unsigned int *s_ev;  // [16] in shared memory
     const double *mgs;   // multi-group table blob: the shared-memory copy, or the global blob when it does not fit
     const Geo *geo;      // the block's shared-memory copy of the Geo descriptor: what the out-of-line (generic-path)
                          // functions read, so that the kernel parameter block never has to be copied to a stack
     bool tracing;        // launch-uniform: a trace buffer is attached
-    __device__ __forceinline__ void clear(unsigned int *ev) { knum = 0.0; s_ev = ev; }
+    __device__ __forceinline__ void clear(unsigned int *ev) { knum = 0.0; wabs = 0.0; s_ev = ev; }
 };
 
 __device__ __forceinline__ void count_event(Acc &acc, int ev) { atomicAdd(acc.s_ev + ev, 1u); }
@@ -670,7 +679,11 @@ __device__ __forceinline__ double mgv(const Acc &acc, int off) { return acc.mgs[
 // Returns ADV_*; the event that still has to be finished is left in p.pend (scatter column, hit code, time edge);
 // aux = number of children (fission).  Lanes in a LAT_FAST lattice element take the straight-line geometry path; a
 // warp whose lanes all do (the normal case inside a pin lattice) never enters the generic loops.
-template <bool CE, bool PRIVATE>
+// W: the weighted variant (implicit capture with roulette, R36): the particle carries its own weight p.w, every
+// collision removes the capture share, the reaction is chosen among scatter / fission, and a scattered particle whose
+// weight fell below w_roulette plays roulette (one draw).  W = false is the analog path (R2): weight = the launch
+// constant w0, p.w is never read.
+template <bool CE, bool PRIVATE, bool W>
 __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int &aux, Acc &acc, double *s_flux)
 {
     const Geo &G = c.geo;
@@ -742,46 +755,74 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         tix = ((long long)bin * c.ce.n_t + p.tbin) * c.ce.n_e + p.ebin;
         if (kind == 2) p.t = __ldg(c.ce.t_edges + p.tbin + 1); else p.t += d / v;
     }
-    flux_add<PRIVATE>(c, s_flux, tix, c.w0 * d);
-    acc.knum += c.w0 * d * nusf;
+    const double w = W ? p.w : c.w0;
+    flux_add<PRIVATE>(c, s_flux, tix, w * d);
+    acc.knum += w * d * nusf;
 
     int ev, code, surf = -1;
     p.pend = PEND_NONE;
     if (kind == 0) {
         p.last = -1;
-        double uu = rng.next(c) * sig_t;
         if (!CE) {
             double sig_s = mgv(acc, c.mg.o_sig_s + mat * c.mg.G + p.g), sig_f = mgv(acc, c.mg.o_sig_f + mat * c.mg.G + p.g);
+            double total = sig_t;
+            if (W) {  // the weight loses its capture share; the reaction is chosen among scatter / fission
+                total = sig_s + sig_f;
+                const double wn = p.w * (total / sig_t);
+                acc.wabs += p.w - wn;
+                p.w = wn;
+            }
+            double uu = rng.next(c) * total;
             if (uu < sig_s) { ev = 1; code = ADV_SCATTER; p.pend = PEND_SCATTER; }
             else if (uu < sig_s + sig_f) {
                 ev = 2; code = ADV_FISSION;
-                aux = (int)floor(c.w0 * mgv(acc, c.mg.o_nu + mat * c.mg.G + p.g) / c.k_prev + rng.next(c));
+                aux = (int)floor((W ? p.w : c.w0) * mgv(acc, c.mg.o_nu + mat * c.mg.G + p.g) / c.k_prev + rng.next(c));
             } else { ev = 3; code = ADV_DEAD; }
         } else {
-            int r = ncol - 1;  // first column whose cumulative value exceeds uu (static indices: cum stays in registers)
+            const int nsel = W ? ncol - 1 : ncol;  // columns the reaction is chosen from (implicit capture: all but capture)
+            double total = sig_t;
+            if (W) {
+                total = cum[0];
+#pragma unroll
+                for (int j = 1; j < MAX_CE_COL; j++)
+                    if (j == nsel - 1) total = cum[j];
+                const double wn = p.w * (total / sig_t);
+                acc.wabs += p.w - wn;
+                p.w = wn;
+            }
+            double uu = rng.next(c) * total;
+            int r = nsel - 1;  // first column whose cumulative value exceeds uu (static indices: cum stays in registers)
 #pragma unroll
             for (int j = MAX_CE_COL - 2; j >= 0; j--)
-                if (j < ncol - 1 && cum[j] > uu) r = j;
+                if (j < nsel - 1 && cum[j] > uu) r = j;
             if (r < ncol - 2) { ev = 1; code = ADV_SCATTER; p.pend = PEND_SCATTER | (unsigned int)r; }
             else if (r == ncol - 2) {
                 ev = 2; code = ADV_FISSION;
                 double nu = c.ce.nu0 + c.ce.nu1 * (p.E * 1e-6);
-                aux = (int)floor(c.w0 * nu + rng.next(c));
+                aux = (int)floor((W ? p.w : c.w0) * nu + rng.next(c));
             } else { ev = 3; code = ADV_DEAD; }
+        }
+        if (W) {
+            if (code == ADV_SCATTER) {
+                if (p.w < c.w_roulette) {  // roulette (one draw): survive at w_survive with probability w / w_survive
+                    if (rng.next(c) * c.w_survive < p.w) { atomicAdd(c.scal + 5, c.w_survive - p.w); p.w = c.w_survive; }
+                    else { atomicAdd(c.scal + 4, p.w); ev = 3; code = ADV_DEAD; p.pend = PEND_NONE; }
+                }
+            } else acc.wabs += p.w;  // fission / capture end the history with its whole weight
         }
     } else if (kind == 1) {
         surf = hit;
         if (hit >= G.n_surf) { ev = 7; code = ADV_SURFACE; p.pend = (unsigned int)hit; }
         else {
             int bc = __ldg(G.surf_bc + hit);
-            if (bc == 2) { ev = 6; code = ADV_DEAD; atomicAdd(c.scal + 1, c.w0); }
+            if (bc == 2) { ev = 6; code = ADV_DEAD; atomicAdd(c.scal + 1, w); }
             else { ev = bc == 1 ? 5 : 4; code = ADV_SURFACE; p.pend = (unsigned int)hit; }
         }
     } else {
         // time edge: the particle has moved off whatever surface it sat on (R11)
         p.tbin++;
         p.last = -1;
-        if (p.tbin == c.ce.n_t) { ev = 9; code = ADV_DEAD; }
+        if (p.tbin == c.ce.n_t) { ev = 9; code = ADV_DEAD; if (W) atomicAdd(c.scal + 3, w); }
         else { ev = 8; code = ADV_SURFACE; p.pend = PEND_TIME; }
     }
     if (acc.tracing)
@@ -794,6 +835,70 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         atomicExch(c.err, -4);
     }
     return code;
+}
+
+// rotate the unit vector (ux, uy, uz) by polar cosine mu and azimuth (sp, cp = sin, cos), then renormalise (R21)
+__device__ __forceinline__ void rotate_dir(double ux, double uy, double uz, double mu, double sp, double cp, double &ox,
+                                           double &oy, double &oz)
+{
+    double s2 = 1.0 - mu * mu;
+    double s = s2 > 0.0 ? sqrt(s2) : 0.0;
+    double a2 = 1.0 - uz * uz;
+    if (a2 < 1e-10) {
+        ox = s * cp; oy = s * sp; oz = uz > 0.0 ? mu : -mu;
+    } else {
+        double r = sqrt(a2);
+        ox = mu * ux + s * (ux * uz * cp - uy * sp) / r;
+        oy = mu * uy + s * (uy * uz * cp + ux * sp) / r;
+        oz = mu * uz - s * r * cp;
+    }
+    double nrm = sqrt(ox * ox + oy * oy + oz * oz);
+    ox /= nrm; oy /= nrm; oz /= nrm;
+}
+
+// Free-gas elastic scattering with a constant cross section (R35), speeds in units of sqrt(eV).
+// Target speed x (units of sqrt(kT/A)) and cosine mu between target and neutron from |v_n - v_T| x^2 exp(-x^2):
+// with probability 1 / (1 + sqrt(pi) y / 2), y = sqrt(A E / kT): x^2 = -ln(xi1 xi2), else x^2 = -ln xi1 - ln xi2
+// cos^2(pi xi4 / 2); mu = 2 xi - 1; accepted with probability sqrt(y^2 + x^2 - 2 x y mu) / (x + y).  Draws per trial,
+// in order: xi1, xi2, branch, [xi4], mu, accept.  Then the target's azimuth around the neutron's direction (1 draw)
+// and an isotropic direction of the relative velocity in the centre-of-mass frame (2 draws).
+// Out of line (thermal collisions only): takes the stream by value, returns the new draw counter; out = E', u'.
+__device__ __noinline__ uint32_t free_gas(unsigned long long seed, uint32_t cycle, unsigned long long id, uint32_t ctr, double A,
+                                          double kT, double E, double ux, double uy, double uz, double *out)
+{
+    const double y = sqrt(A * E / kT);
+    const double alpha = 1.0 / (1.0 + 1.7724538509055159 * y / 2.0);
+    double x2, x, mu;
+    for (;;) {
+        const double r1 = draw_at(seed, id, 0u, cycle, ctr), r2 = draw_at(seed, id, 0u, cycle, ctr + 1u);
+        ctr += 3u;
+        if (draw_at(seed, id, 0u, cycle, ctr - 1u) < alpha) x2 = -log(r1 * r2);
+        else {
+            const double cs = cospi(0.5 * draw_at(seed, id, 0u, cycle, ctr++));
+            x2 = -log(r1) - log(r2) * cs * cs;
+        }
+        x = sqrt(x2);
+        mu = 2.0 * draw_at(seed, id, 0u, cycle, ctr++) - 1.0;
+        const double accept = sqrt(y * y + x2 - 2.0 * x * y * mu) / (x + y);
+        if (draw_at(seed, id, 0u, cycle, ctr++) < accept) break;
+    }
+    double sp, cp, tx, ty, tz;
+    sincospi(2.0 * draw_at(seed, id, 0u, cycle, ctr++), &sp, &cp);
+    rotate_dir(ux, uy, uz, mu, sp, cp, tx, ty, tz);
+    const double sn = sqrt(E), st = x * sqrt(kT / A);
+    const double vnx = sn * ux, vny = sn * uy, vnz = sn * uz;
+    const double vcx = (vnx + A * st * tx) / (A + 1.0), vcy = (vny + A * st * ty) / (A + 1.0), vcz = (vnz + A * st * tz) / (A + 1.0);
+    const double rx = vnx - vcx, ry = vny - vcy, rz = vnz - vcz;
+    const double sr = sqrt(rx * rx + ry * ry + rz * rz);
+    double ox, oy, oz;
+    const double a = draw_at(seed, id, 0u, cycle, ctr), b = draw_at(seed, id, 0u, cycle, ctr + 1u);
+    ctr += 2u;
+    iso_dir(a, b, ox, oy, oz);
+    const double vx = vcx + sr * ox, vy = vcy + sr * oy, vz = vcz + sr * oz;
+    const double e = vx * vx + vy * vy + vz * vz;
+    const double nv = sqrt(e);
+    out[0] = e; out[1] = vx / nv; out[2] = vy / nv; out[3] = vz / nv;
+    return ctr;
 }
 
 // Scatter event (a8).  MG: new group from the cumulative scatter row, isotropic direction (1 + 2 draws).
@@ -814,27 +919,24 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const Acc &acc, Particl
         iso_dir(a, b, p.ux, p.uy, p.uz);
     } else {
         double A = __ldg(c.ce.colA + mat * CE_ROW + col);
-        double mu_cm = 2.0 * rng.next(c) - 1.0;
-        double den = A * A + 2.0 * A * mu_cm + 1.0;
-        double mu = 0.0;
-        if (den > 0.0) mu = (1.0 + A * mu_cm) / sqrt(den);
-        double En = p.E * den / ((A + 1.0) * (A + 1.0));
-        double sp, cp;
-        sincospi(2.0 * rng.next(c), &sp, &cp);
-        double s2 = 1.0 - mu * mu;
-        double s = s2 > 0.0 ? sqrt(s2) : 0.0;
-        double a2 = 1.0 - p.uz * p.uz;
-        double ox, oy, oz;
-        if (a2 < 1e-10) {
-            ox = s * cp; oy = s * sp; oz = p.uz > 0.0 ? mu : -mu;
+        double En;
+        if (c.kT > 0.0 && p.E < 400.0 * c.kT) {  // free gas below 400 kT, target at rest above (R35)
+            double o[4];
+            const uint32_t ctr = free_gas(c.seed, c.cycle, rng.id, rng.ctr, A, c.kT, p.E, p.ux, p.uy, p.uz, o);
+            rng.init(rng.id, ctr);
+            En = o[0]; p.ux = o[1]; p.uy = o[2]; p.uz = o[3];
         } else {
-            double r = sqrt(a2);
-            ox = mu * p.ux + s * (p.ux * p.uz * cp - p.uy * sp) / r;
-            oy = mu * p.uy + s * (p.uy * p.uz * cp + p.ux * sp) / r;
-            oz = mu * p.uz - s * r * cp;
+            double mu_cm = 2.0 * rng.next(c) - 1.0;
+            double den = A * A + 2.0 * A * mu_cm + 1.0;
+            double mu = 0.0;
+            if (den > 0.0) mu = (1.0 + A * mu_cm) / sqrt(den);
+            En = p.E * den / ((A + 1.0) * (A + 1.0));
+            double sp, cp;
+            sincospi(2.0 * rng.next(c), &sp, &cp);
+            double ox, oy, oz;
+            rotate_dir(p.ux, p.uy, p.uz, mu, sp, cp, ox, oy, oz);
+            p.ux = ox; p.uy = oy; p.uz = oz;
         }
-        double nrm = sqrt(ox * ox + oy * oy + oz * oz);
-        p.ux = ox / nrm; p.uy = oy / nrm; p.uz = oz / nrm;
         if (En < c.ce.E_min) En = c.ce.E_min;
         if (En > c.ce.E_max) En = c.ce.E_max;
         p.E = En;

@@ -48,8 +48,11 @@ __device__ __forceinline__ const double *stage_mg(const Ctx &c, double *smem, in
 }
 
 // ------------------------------------------------------------------ bank access (dense, position-indexed)
-template <bool CE>
-__device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr, uint32_t &slot)
+// W (weighted kernels): a particle that has not run a segment yet starts with the launch weight w0 (source
+// renormalisation, R6; secondaries of a fixed-source run: 1), later its own banked weight
+template <bool CE, bool W = false>
+__device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr, uint32_t &slot,
+                                          double w0 = 1.0)
 {
     p.x = B.x[i]; p.y = B.y[i]; p.z = B.z[i];
     p.ux = B.ux[i]; p.uy = B.uy[i]; p.uz = B.uz[i];
@@ -63,15 +66,18 @@ __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particl
     p.v = 0.0; p.gi = 0; p.ebin = 0;
     if (CE) { p.E = B.E[i]; p.t = B.t[i]; p.tbin = B.tbin[i]; p.id = B.id[i]; }
     else { p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = slot; }
+    p.w = w0;
+    if (W && p.nseg != 0) p.w = B.w[i];
 }
 
-template <bool CE>
+template <bool CE, bool W = false>
 __device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr, uint32_t slot)
 {
     B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z; B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
     B.cell[i] = p.cell; B.elem[i] = p.elem; B.gl[i] = pack_gl(p.g, p.last); B.ctr[i] = ctr; B.slot[i] = slot;
     B.ev[i] = p.pend | (p.nseg << 12);
     if (CE) { B.E[i] = p.E; B.t[i] = p.t; B.tbin[i] = p.tbin; B.id[i] = p.id; }
+    if (W) B.w[i] = p.w;
 }
 
 // a fission ends the history: leave what k_emit needs at the parent's slot
@@ -107,6 +113,7 @@ __device__ __forceinline__ void live_counts(const Ctx &c, unsigned int s, unsign
 }
 
 // per-block flush: k numerator (warp shuffles + one atomic per block) and the shared event counters
+template <bool W = false>
 __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
 {
     __shared__ double s_k[BS / 32];
@@ -118,6 +125,10 @@ __device__ __forceinline__ void flush_acc(const Ctx &c, const Acc &acc)
         double ks = 0.0;
         for (int i = 0; i < BS / 32; i++) ks += s_k[i];
         if (ks != 0.0) atomicAdd(c.scal + 0, ks);
+    }
+    if (W) {  // absorbed weight (scal[2]); one atomic per warp
+        double a = warp_sum(acc.wabs);
+        if (lane == 0 && a != 0.0) atomicAdd(c.scal + 2, a);
     }
     if (threadIdx.x >= 1 && threadIdx.x < 11 && acc.s_ev[threadIdx.x])
         atomicAdd(c.counters + threadIdx.x, (unsigned long long)acc.s_ev[threadIdx.x]);
@@ -308,7 +319,7 @@ __device__ __forceinline__ void mark_lost(const Ctx &c)
 #ifndef MCDC_SWEEP_MINBLOCKS
 #define MCDC_SWEEP_MINBLOCKS 4
 #endif
-template <bool CE, bool PRIVATE>
+template <bool CE, bool PRIVATE, bool W>
 __global__ void __launch_bounds__(BS, MCDC_SWEEP_MINBLOCKS * 256 / BS) k_sweep(Ctx c, unsigned int s, unsigned int n0)
 {
     MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
@@ -340,26 +351,26 @@ __global__ void __launch_bounds__(BS, MCDC_SWEEP_MINBLOCKS * 256 / BS) k_sweep(C
         const bool live = t < n_in && B.cell[i] >= 0;
         const unsigned int amask = __ballot_sync(0xffffffffu, live);
         if (live) {
-            load_full<CE>(B, i, p, ctr, slot);
+            load_full<CE, W>(B, i, p, ctr, slot, c.w0);
             if (CE) ce_energy_state(c.ce, p);
             rng.init(p.id, ctr);
             const bool ok = finish_pending<CE>(c, acc, p, rng);
             __syncwarp(amask);  // the lanes went different ways by pending event: run the segment together again
             if (!ok) mark_lost(c);
             else {
-                code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+                code = advance<CE, PRIVATE, W>(c, p, rng, aux, acc, s_flux);
                 if (!CE && code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
         if (!CE) {
             unsigned int o = block_slot(code == ADV_SCATTER, code == ADV_SURFACE, oc, c.cap, par);
-            if (code != ADV_DEAD) store_full<CE>(O, o, p, rng.ctr, slot);
+            if (code != ADV_DEAD) store_full<CE, W>(O, o, p, rng.ctr, slot);
         } else {
             unsigned int nb = code == ADV_SURFACE ? 1u : (code == ADV_FISSION ? (unsigned int)aux : 0u);
             unsigned int pf, ob;
             block_slot_n(code == ADV_SCATTER, nb, oc, c.cap, par, pf, ob);
-            if (code == ADV_SCATTER) { if (pf < c.cap) store_full<CE>(O, pf, p, rng.ctr, slot); }
-            else if (code == ADV_SURFACE) { if (ob < c.cap) store_full<CE>(O, c.cap - 1u - ob, p, rng.ctr, slot); }
+            if (code == ADV_SCATTER) { if (pf < c.cap) store_full<CE, W>(O, pf, p, rng.ctr, slot); }
+            else if (code == ADV_SURFACE) { if (ob < c.cap) store_full<CE, W>(O, c.cap - 1u - ob, p, rng.ctr, slot); }
             else if (code == ADV_FISSION && nb) {
                 // prompt secondaries: born alive at the parent's site, first segment in the next sweep
                 const int mat = c.geo.cfill[p.cell];
@@ -368,13 +379,13 @@ __global__ void __launch_bounds__(BS, MCDC_SWEEP_MINBLOCKS * 256 / BS) k_sweep(C
                 count_secondaries(c, nb);
                 for (unsigned int j = 0; j < nb; j++) {
                     make_child<CE>(c, rng, mat, pid, ctr0, (int)j, p);
-                    if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot);
+                    if (ob + j < c.cap) store_full<CE>(O, c.cap - 1u - (ob + j), p, 0u, slot);  // nseg = 0: weight w0
                 }
             }
         }
     }
     if (PRIVATE) flush_private_flux(c, s_flux);
-    flush_acc(c, acc);
+    flush_acc<W>(c, acc);
 }
 
 // ------------------------------------------------------------------ split per-event kernels (schedule 2)
@@ -463,7 +474,7 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 #ifndef MCDC_DENSE
 #define MCDC_DENSE 12  // live lanes from which a continuous-energy warp keeps tickets for entries not pushed yet
 #endif
-template <bool CE, bool PRIVATE>
+template <bool CE, bool PRIVATE, bool W>
 __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persist(Ctx c, unsigned int s, unsigned int n0)
 {
     MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
@@ -526,7 +537,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
             uint32_t ctr = 0;
             bool have = false;
             if (ticket < n_in) {
-                load_full<CE>(B, live_pos(c.cap, n_front, ticket), p, ctr, slot);
+                load_full<CE, W>(B, live_pos(c.cap, n_front, ticket), p, ctr, slot, c.w0);
                 have = true;
             } else if (CE && *(volatile uint32_t *)(O.ev + t_slot) == t_full) {
                 const unsigned int i = t_slot;
@@ -535,6 +546,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
                 p.ux = __ldcg(O.ux + i); p.uy = __ldcg(O.uy + i); p.uz = __ldcg(O.uz + i);
                 p.cell = __ldcg(O.cell + i); p.elem = __ldcg(O.elem + i);
                 p.g = 0; p.last = -1; p.pend = PEND_NONE; p.nseg = 0;
+                p.w = c.w0;
                 slot = __ldcg(O.slot + i);
                 p.E = __ldcg(O.E + i); p.t = __ldcg(O.t + i); p.tbin = __ldcg(O.tbin + i); p.id = __ldcg(O.id + i);
                 __threadfence();
@@ -578,7 +590,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
             const bool ok = finish_pending<CE>(c, acc, p, rng);
             __syncwarp(amask);  // the lanes went different ways by pending event: run the segment together again
             if (!ok) mark_lost(c);
-            else code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+            else code = advance<CE, PRIVATE, W>(c, p, rng, aux, acc, s_flux);
             if (code == ADV_DEAD) { alive = false; n_end++; }
             else if (code == ADV_FISSION) {
                 alive = false;
@@ -615,6 +627,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
                         }
                     }
                     p = first;
+                    p.w = c.w0;
                     ce_energy_state(c.ce, p);
                     rng.init(p.id, 0u);
                     alive = true;
@@ -625,13 +638,13 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
     taken = __reduce_add_sync(FULL, taken);
     if (lane == 0 && taken) atomicAdd(c.counters + 14, (unsigned long long)taken);
     if (PRIVATE) flush_private_flux(c, s_flux);
-    flush_acc(c, acc);
+    flush_acc<W>(c, acc);
 }
 
 // ------------------------------------------------------------------ monolithic schedule
 // every slot of bank 0, one whole segment (advance + the event it ends in), in place, no compaction; counts the
 // survivors.  A dead slot has cell = -1.
-template <bool CE, bool PRIVATE>
+template <bool CE, bool PRIVATE, bool W>
 __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned int n)
 {
     MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
@@ -646,22 +659,22 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         if (B.cell[i] < 0) continue;
         Particle p;
         uint32_t ctr, slot;
-        load_full<CE>(B, i, p, ctr, slot);
+        load_full<CE, W>(B, i, p, ctr, slot, c.w0);
         if (CE) ce_energy_state(c.ce, p);
         Rng rng;
         rng.init(p.id, ctr);
         int aux = 0;
-        int code = advance<CE, PRIVATE>(c, p, rng, aux, acc, s_flux);
+        int code = advance<CE, PRIVATE, W>(c, p, rng, aux, acc, s_flux);
         if (code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
         else if (code != ADV_DEAD && !finish_pending<CE>(c, acc, p, rng)) { mark_lost(c); code = ADV_DEAD; }
         if (code == ADV_DEAD) p.cell = -1;
-        store_full<CE>(B, i, p, rng.ctr, slot);
+        store_full<CE, W>(B, i, p, rng.ctr, slot);
         if (code != ADV_DEAD) alive++;
     }
     alive = __reduce_add_sync(0xffffffffu, alive);
     if ((threadIdx.x & 31) == 0 && alive) atomicAdd(&c.qc[s % RING].n_alive, alive);
     if (PRIVATE) flush_private_flux(c, s_flux);
-    flush_acc(c, acc);
+    flush_acc<W>(c, acc);
 }
 
 // ------------------------------------------------------------------ a10/a12: fission bank by count-scan-write

@@ -51,7 +51,7 @@ static const int MAX_AXIS_PLANES = 250;   // axis planes a boundary code of the 
 
 struct HostPinned {
     QCount qc[RING];
-    double scal[4];
+    double scal[8];
     unsigned long long counters[MCDC_N_COUNTERS];
     unsigned int total;
     int err;
@@ -67,6 +67,7 @@ struct RunStats {
                                                     // k_emit, [12] largest bank, [13] kernel rounds
     uint64_t counters[MCDC_N_COUNTERS] = {0};       // merged device + host counters as reported
     int set = 0;                                    // which flux accumulator pair holds this run's tallies
+    double balance[6] = {0, 0, 0, 0, 0, 0};         // weight balance summed over the run's cycles (mcdc_get_balance)
 };
 
 struct mcdc_problem {
@@ -253,6 +254,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         Bank &B = L.bank[b];
         B.x = C.take<double>(cap); B.y = C.take<double>(cap); B.z = C.take<double>(cap);
         B.ux = C.take<double>(cap); B.uy = C.take<double>(cap); B.uz = C.take<double>(cap);
+        B.w = C.take<double>(cap);
         B.E = ce ? C.take<double>(cap) : nullptr; B.t = ce ? C.take<double>(cap) : nullptr;
         B.cell = C.take<int>(cap); B.elem = C.take<int>(cap); B.gl = C.take<int>(cap);
         B.tbin = ce ? C.take<int>(cap) : nullptr;
@@ -732,11 +734,11 @@ static unsigned int grid_for(uint64_t n)
 
 // the persistent kernel: at most the blocks that are resident at once (its idle warps wait for other warps' pushes,
 // so every block of the grid must be running)
-template <bool CE, bool PRIV> static unsigned int grid_persist(mcdc_problem *p, uint64_t n, size_t smem)
+template <bool CE, bool PRIV, bool W> static unsigned int grid_persist(mcdc_problem *p, uint64_t n, size_t smem)
 {
     if (p->persist_blocks_per_sm == 0) {
         int nb = 0, sms = 148;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_persist<CE, PRIV>, BS, smem) != cudaSuccess || nb < 1) nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_persist<CE, PRIV, W>, BS, smem) != cudaSuccess || nb < 1) nb = 1;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
         p->persist_blocks_per_sm = nb;
         p->n_sm = sms;
@@ -792,7 +794,7 @@ static int device_error_code(mcdc_problem *p, int e)
     return 0;
 }
 
-template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M)
+template <bool CE, bool PRIV, bool W> static int transport_t(mcdc_problem *p, uint64_t M)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
@@ -808,14 +810,14 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
         if (p->schedule != 1 && p->persist > 0 && upper <= (uint64_t)p->persist) {
             CUDA_OK(cudaMemsetAsync(c.work, 0, 32, st));
             if (CE) CUDA_OK(cudaMemsetAsync(c.bank[(s + 1) & 1].ev, 0, sizeof(uint32_t) * (size_t)p->cap, st));
-            { ProfScope ps(p, MCDC_PROF_PERSIST); k_persist<CE, PRIV><<<grid_persist<CE, PRIV>(p, upper, smem), BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_PERSIST); k_persist<CE, PRIV, W><<<grid_persist<CE, PRIV, W>(p, upper, smem), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
             p->work.host_counters[13]++;
             break;
         }
         unsigned int gr = grid_for(upper);
         if (p->schedule != 1) {
-            { ProfScope ps(p, MCDC_PROF_SWEEP); k_sweep<CE, PRIV><<<gr, BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_SWEEP); k_sweep<CE, PRIV, W><<<gr, BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
             if (p->schedule == 2) {
                 { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, smem_mg, st>>>(c, s); }
@@ -823,7 +825,7 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
                 p->n_launches += 2;
             }
         } else {
-            { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV, W><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
         }
         p->work.host_counters[13]++;
@@ -852,8 +854,30 @@ template <bool CE, bool PRIV> static int transport_t(mcdc_problem *p, uint64_t M
 
 static int transport(mcdc_problem *p, uint64_t M)
 {
-    if (p->mode == 0) return p->tally_private ? transport_t<false, true>(p, M) : transport_t<false, false>(p, M);
-    return p->tally_private ? transport_t<true, true>(p, M) : transport_t<true, false>(p, M);
+    if (p->ctx.implicit) {  // weighted kernels (implicit capture, R36)
+        if (p->mode == 0) return p->tally_private ? transport_t<false, true, true>(p, M) : transport_t<false, false, true>(p, M);
+        return p->tally_private ? transport_t<true, true, true>(p, M) : transport_t<true, false, true>(p, M);
+    }
+    if (p->mode == 0) return p->tally_private ? transport_t<false, true, false>(p, M) : transport_t<false, false, false>(p, M);
+    return p->tally_private ? transport_t<true, true, false>(p, M) : transport_t<true, false, false>(p, M);
+}
+
+// Weight balance of the transport just finished (the scalars and counters are in pinned memory): source weight,
+// absorbed, leaked, cut off, roulette loss / gain.  Analog: every ended history carried w0, so the terms follow from
+// the event-counter increments; weighted: the kernels summed them (scal[2..5]).
+static void add_balance(mcdc_problem *p, double source_weight, const uint64_t *before)
+{
+    RunStats &w = p->work;
+    const double *sc = p->pin->scal;
+    const unsigned long long *cn = p->pin->counters;
+    w.balance[0] += source_weight;
+    w.balance[2] += sc[1];
+    if (p->ctx.implicit) {
+        w.balance[1] += sc[2]; w.balance[3] += sc[3]; w.balance[4] += sc[4]; w.balance[5] += sc[5];
+    } else {
+        w.balance[1] += p->ctx.w0 * (double)((cn[2] - before[2]) + (cn[3] - before[3]));
+        w.balance[3] += p->ctx.w0 * (double)(cn[9] - before[9]);
+    }
 }
 
 // children of the M parents' fission records -> bank[0]; returns their number.  Also brings the cycle's scalars,
@@ -873,7 +897,7 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
     }
     p->n_launches += 4;
     CUDA_OK(cudaMemcpyAsync(&p->pin->total, p->part + nb, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
-    CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->counters, c.counters, sizeof p->pin->counters, cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(&p->pin->err, c.err, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaStreamSynchronize(st));
@@ -921,6 +945,8 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
         k_source<false><<<(unsigned int)((M + BS - 1) / BS), BS, 0, st>>>(c, (unsigned int)M);
         p->n_launches++;
     }
+    uint64_t before[MCDC_N_COUNTERS];
+    for (int i = 0; i < MCDC_N_COUNTERS; i++) before[i] = cycle == 0 ? 0 : p->pin->counters[i];
     int rc = transport(p, M);
     if (rc) return abandon(p, rc);
     uint64_t total = 0;
@@ -928,6 +954,7 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     if (rc) return abandon(p, rc);
     rc = device_error_code(p, p->pin->err);
     if (rc) return abandon(p, rc);
+    add_balance(p, c.w0 * (double)M, before);
     CUDA_OK(cudaEventRecord(p->t1, st));
     k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[p->work.set],
                                                           p->flux_acc2[p->work.set], c.n_tally, 1.0 / (double)N, active);
@@ -1060,9 +1087,35 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
     double k_c = p->pin->scal[0] / (double)N, leak = p->pin->scal[1] / (double)N;
     w.k_cycle.push_back(k_c);
     w.k_acc = k_c; w.k_acc2 = k_c * k_c; w.leak_acc = leak; w.leak_acc2 = leak * leak; w.n_active = 1;
+    {  // the scalars and counters run over all waves of the run: one balance entry
+        const uint64_t zero[MCDC_N_COUNTERS] = {0};
+        add_balance(p, (double)(w.host_counters[0] + p->pin->counters[15]), zero);  // every track starts with weight 1
+    }
     p->bank_count = 0;
     p->last_N = N;
     publish(p);
+    return 0;
+}
+
+extern "C" int mcdc_set_physics(mcdc_problem *p, const mcdc_physics *ph)
+{
+    if (!p) return fail(MCDC_EINVAL, "null");
+    Ctx &c = p->ctx;
+    p->persist_blocks_per_sm = 0;  // the weighted kernels have their own occupancy
+    if (!ph) { c.kT = 0.0; c.implicit = 0; c.w_roulette = c.w_survive = 0.0; return 0; }
+    if (!(ph->kT >= 0.0)) return fail(MCDC_EINVAL, "kT must be >= 0");
+    if (ph->implicit_capture && !(ph->w_roulette >= 0.0 && ph->w_survive >= ph->w_roulette))
+        return fail(MCDC_EINVAL, "implicit capture needs 0 <= w_roulette <= w_survive");
+    c.kT = ph->kT;
+    c.implicit = ph->implicit_capture ? 1 : 0;
+    c.w_roulette = ph->w_roulette; c.w_survive = ph->w_survive;
+    return 0;
+}
+
+extern "C" int mcdc_get_balance(const mcdc_problem *p, double out[6])
+{
+    if (!p || !out) return fail(MCDC_EINVAL, "null");
+    for (int k = 0; k < 6; k++) out[k] = p->pub.balance[k];
     return 0;
 }
 
