@@ -34,6 +34,8 @@ class OrcInput(C.Structure):
         ("n_univ", C.c_int32), ("univ_cell_off", _ip),
         ("has_lat", C.c_int32), ("lat_x0", C.c_double), ("lat_y0", C.c_double), ("lat_px", C.c_double),
         ("lat_py", C.c_double), ("lat_nx", C.c_int32), ("lat_ny", C.c_int32), ("lat_univ", _ip), ("lat_bin", _ip),
+        ("n_lat2", C.c_int32), ("lat2_nx", _ip), ("lat2_ny", _ip), ("lat2_px", _dp), ("lat2_py", _dp), ("lat2_off", _ip),
+        ("lat2_univ", _ip), ("lat2_bin", _ip),
         ("n_bins", C.c_int32), ("n_mat", C.c_int32),
         ("G", C.c_int32), ("sig_t", _dp), ("sig_f", _dp), ("nu", _dp), ("chi", _dp), ("S", _dp),
         ("n_grid", C.c_int32), ("grid", _dp), ("n_nuc", C.c_int32), ("nuc_A", _dp),
@@ -148,6 +150,11 @@ class Oracle:
             inp.lat_x0, inp.lat_y0, inp.lat_px, inp.lat_py = lat["x0"], lat["y0"], lat["px"], lat["py"]
             inp.lat_nx, inp.lat_ny = lat["nx"], lat["ny"]
             inp.lat_univ, inp.lat_bin = ip(lat["univ"]), ip(lat["bin"])
+        inp.n_lat2 = len(P["lat2_nx"]) if "lat2_nx" in P else 0
+        if inp.n_lat2:
+            inp.lat2_nx, inp.lat2_ny, inp.lat2_off = ip(P["lat2_nx"]), ip(P["lat2_ny"]), ip(P["lat2_off"])
+            inp.lat2_px, inp.lat2_py = dp(P["lat2_px"]), dp(P["lat2_py"])
+            inp.lat2_univ, inp.lat2_bin = ip(P["lat2_univ"]), ip(P["lat2_bin"])
         inp.n_bins, inp.n_mat = P["n_bins"], P["n_mat"]
         if not ce:
             inp.G = P["G"]

@@ -292,14 +292,78 @@ static int32_t find_cell(const orc_problem *p, int32_t univ, const double x[3], 
     return -1;
 }
 
-/* element-local coordinates, recomputed from the global position every time (R14) */
-static void local_coords(const orc_problem *p, int32_t elem, const double x[3], double xl[3])
+/* Location inside lattices: `elem` packs the element of the (first-level) lattice in its low 16 bits and, inside a
+ * second-level lattice (R37), that lattice's element + 1 in the bits above; -1 = not in a lattice. */
+#define OUTER(e) ((e) & 0xffff)
+#define INNER(e) (((e) >> 16) - 1)
+
+/* coordinates centred on first-level element `outer`, recomputed from the global position every time (R14) */
+static void outer_coords(const orc_problem *p, int32_t outer, const double x[3], double xl[3])
 {
     const orc_input *in = &p->in;
-    int32_t ix = elem % in->lat_nx, iy = elem / in->lat_nx;
+    int32_t ix = outer % in->lat_nx, iy = outer / in->lat_nx;
     xl[0] = x[0] - (in->lat_x0 + (ix + 0.5) * in->lat_px);
     xl[1] = x[1] - (in->lat_y0 + (iy + 0.5) * in->lat_py);
     xl[2] = x[2];
+}
+
+/* the cell of first-level element `outer`'s universe that a second-level lattice fills (-1: none) */
+static int32_t mid_cell(const orc_problem *p, int32_t outer)
+{
+    const orc_input *in = &p->in;
+    int32_t un = in->lat_univ[outer];
+    for (int32_t c = in->univ_cell_off[un]; c < in->univ_cell_off[un + 1]; c++)
+        if (in->cell_fill_type[c] == 2) return c;
+    return -1;
+}
+
+/* lower-left corner of second-level lattice k in its universe's coordinates: centred on the origin (R37) */
+static double lat2_x0(const orc_input *in, int32_t k) { return -0.5 * (in->lat2_nx[k] * in->lat2_px[k]); }
+static double lat2_y0(const orc_input *in, int32_t k) { return -0.5 * (in->lat2_ny[k] * in->lat2_py[k]); }
+
+/* coordinates centred on element `inner` of second-level lattice k, from first-level-element coordinates xo */
+static void inner_coords(const orc_problem *p, int32_t k, int32_t inner, const double xo[3], double xl[3])
+{
+    const orc_input *in = &p->in;
+    int32_t ix = inner % in->lat2_nx[k], iy = inner / in->lat2_nx[k];
+    xl[0] = xo[0] - (lat2_x0(in, k) + (ix + 0.5) * in->lat2_px[k]);
+    xl[1] = xo[1] - (lat2_y0(in, k) + (iy + 0.5) * in->lat2_py[k]);
+    xl[2] = xo[2];
+}
+
+/* element-local coordinates of the innermost level of `elem` */
+static void local_coords(const orc_problem *p, int32_t elem, const double x[3], double xl[3])
+{
+    double xo[3];
+    outer_coords(p, OUTER(elem), x, xo);
+    if (INNER(elem) >= 0) inner_coords(p, p->in.cell_fill[mid_cell(p, OUTER(elem))], INNER(elem), xo, xl);
+    else { xl[0] = xo[0]; xl[1] = xo[1]; xl[2] = xo[2]; }
+}
+
+/* cell of first-level element `outer` that holds the point xo (first-level-element coordinates), descending into a
+ * second-level lattice where a cell is filled by one: *elem = packed location, returns the material cell or -1.  The
+ * second-level element index is found by floor and CLAMPED to the lattice's range (R37): the enclosing cell has
+ * already established that the point is inside the lattice, and a point on the lattice's rim (a particle that has just
+ * crossed a first-level wall) must not fall off it by a rounding error. */
+static int32_t descend(const orc_problem *p, int32_t outer, const double xo[3], const double u[3], int32_t last_surf,
+                       int32_t *elem)
+{
+    const orc_input *in = &p->in;
+    *elem = outer;
+    int32_t c = find_cell(p, in->lat_univ[outer], xo, u, last_surf);
+    if (c < 0 || in->cell_fill_type[c] != 2) return c;
+    int32_t k = in->cell_fill[c];
+    int32_t ix = (int32_t)floor((xo[0] - lat2_x0(in, k)) / in->lat2_px[k]);
+    int32_t iy = (int32_t)floor((xo[1] - lat2_y0(in, k)) / in->lat2_py[k]);
+    if (ix < 0) ix = 0;
+    if (iy < 0) iy = 0;
+    if (ix > in->lat2_nx[k] - 1) ix = in->lat2_nx[k] - 1;
+    if (iy > in->lat2_ny[k] - 1) iy = in->lat2_ny[k] - 1;
+    int32_t inner = iy * in->lat2_nx[k] + ix;
+    double xl[3];
+    inner_coords(p, k, inner, xo, xl);
+    *elem = outer | ((inner + 1) << 16);
+    return find_cell(p, in->lat2_univ[in->lat2_off[k] + inner], xl, u, last_surf);
 }
 
 int orc_locate(const orc_problem *p, const double x[3], const double u[3], int32_t last_surf, int32_t loc[3])
@@ -312,10 +376,9 @@ int orc_locate(const orc_problem *p, const double x[3], const double u[3], int32
         int32_t ix = (int32_t)floor((x[0] - in->lat_x0) / in->lat_px);
         int32_t iy = (int32_t)floor((x[1] - in->lat_y0) / in->lat_py);
         if (ix < 0 || iy < 0 || ix >= in->lat_nx || iy >= in->lat_ny) return -1;
-        loc[1] = iy * in->lat_nx + ix;
-        double xl[3];
-        local_coords(p, loc[1], x, xl);
-        loc[2] = find_cell(p, in->lat_univ[loc[1]], xl, u, last_surf);
+        double xo[3];
+        outer_coords(p, iy * in->lat_nx + ix, x, xo);
+        loc[2] = descend(p, iy * in->lat_nx + ix, xo, u, last_surf, &loc[1]);
         if (loc[2] < 0) return -1;
     }
     return 0;
@@ -364,8 +427,9 @@ static double surf_distance(const orc_problem *p, int32_t s, const double x[3], 
     return d > 0.0 ? d : INFINITY;
 }
 
-/* nearest boundary of the current location; candidates in the order: root-cell surfaces, local-cell
- * surfaces, lattice walls (-x,+x,-y,+y); ties keep the first (R12, R14) */
+/* nearest boundary of the current location; candidates in the order: root-cell surfaces, [surfaces of the cell a
+ * second-level lattice fills,] local-cell surfaces, [second-level lattice walls (-x,+x,-y,+y), codes n_surf+4..7,]
+ * first-level lattice walls (-x,+x,-y,+y), codes n_surf+0..3; ties keep the first (R12, R14, R37) */
 double orc_distance(const orc_problem *p, const double x[3], const double u[3], const int32_t loc[3],
                     int32_t last_surf, int32_t *surf)
 {
@@ -378,14 +442,44 @@ double orc_distance(const orc_problem *p, const double x[3], const double u[3], 
         if (d < best) { best = d; *surf = s; }
     }
     if (loc[1] >= 0) {
-        double xl[3];
+        double xl[3], xo[3];
+        outer_coords(p, OUTER(loc[1]), x, xo);
         local_coords(p, loc[1], x, xl);
+        if (INNER(loc[1]) >= 0) {
+            int32_t mid = mid_cell(p, OUTER(loc[1]));
+            for (int32_t k = in->cell_surf_off[mid]; k < in->cell_surf_off[mid + 1]; k++) {
+                int32_t s = in->cell_surf_id[k];
+                double d = surf_distance(p, s, xo, u, s == last_surf);
+                if (d < best) { best = d; *surf = s; }
+            }
+        }
         for (int32_t k = in->cell_surf_off[loc[2]]; k < in->cell_surf_off[loc[2] + 1]; k++) {
             int32_t s = in->cell_surf_id[k];
             double d = surf_distance(p, s, xl, u, s == last_surf);
             if (d < best) { best = d; *surf = s; }
         }
-        int32_t ix = loc[1] % in->lat_nx, iy = loc[1] / in->lat_nx;
+        if (INNER(loc[1]) >= 0) {
+            /* second-level walls, in first-level-element coordinates: only the wall ahead, never the outermost ones */
+            int32_t k2 = in->cell_fill[mid_cell(p, OUTER(loc[1]))];
+            int32_t jx = INNER(loc[1]) % in->lat2_nx[k2], jy = INNER(loc[1]) / in->lat2_nx[k2];
+            if (u[0] < 0.0 && jx > 0) {
+                double d = (lat2_x0(in, k2) + jx * in->lat2_px[k2] - xo[0]) / u[0];
+                if (d > 0.0 && d < best) { best = d; *surf = in->n_surf + 4; }
+            }
+            if (u[0] > 0.0 && jx + 1 < in->lat2_nx[k2]) {
+                double d = (lat2_x0(in, k2) + (jx + 1) * in->lat2_px[k2] - xo[0]) / u[0];
+                if (d > 0.0 && d < best) { best = d; *surf = in->n_surf + 5; }
+            }
+            if (u[1] < 0.0 && jy > 0) {
+                double d = (lat2_y0(in, k2) + jy * in->lat2_py[k2] - xo[1]) / u[1];
+                if (d > 0.0 && d < best) { best = d; *surf = in->n_surf + 6; }
+            }
+            if (u[1] > 0.0 && jy + 1 < in->lat2_ny[k2]) {
+                double d = (lat2_y0(in, k2) + (jy + 1) * in->lat2_py[k2] - xo[1]) / u[1];
+                if (d > 0.0 && d < best) { best = d; *surf = in->n_surf + 7; }
+            }
+        }
+        int32_t ix = OUTER(loc[1]) % in->lat_nx, iy = OUTER(loc[1]) / in->lat_nx;
         /* only the wall ahead on each axis; the lattice's outermost walls are never events */
         if (u[0] < 0.0 && ix > 0) {
             double d = (in->lat_x0 + ix * in->lat_px - x[0]) / u[0];
@@ -512,6 +606,15 @@ orc_problem *orc_create(const orc_input *in)
     if (in->has_lat) {
         DUP(lat_univ, in->lat_nx * in->lat_ny, int32_t);
         DUP(lat_bin, in->lat_nx * in->lat_ny, int32_t);
+    }
+    if (in->n_lat2 > 0) {
+        DUP(lat2_nx, in->n_lat2, int32_t);
+        DUP(lat2_ny, in->n_lat2, int32_t);
+        DUP(lat2_px, in->n_lat2, double);
+        DUP(lat2_py, in->n_lat2, double);
+        DUP(lat2_off, in->n_lat2 + 1, int32_t);
+        DUP(lat2_univ, in->lat2_off[in->n_lat2], int32_t);
+        DUP(lat2_bin, in->lat2_off[in->n_lat2], int32_t);
     }
     int64_t n_tally;
     if (in->mode == 0) {
@@ -651,7 +754,9 @@ static void transport(orc_problem *p, particle *q)
         double x[3] = {q->x, q->y, q->z}, u[3] = {q->ux, q->uy, q->uz};
         int32_t loc[3] = {q->c0, q->elem, q->c1};
         int32_t mat = loc[1] >= 0 ? in->cell_fill[loc[2]] : in->cell_fill[loc[0]];
-        int32_t bin = loc[1] >= 0 ? in->lat_bin[loc[1]] + in->cell_bin[loc[2]] : in->cell_bin[loc[0]];
+        int32_t bin = loc[1] >= 0 ? in->lat_bin[OUTER(loc[1])] + in->cell_bin[loc[2]] : in->cell_bin[loc[0]];
+        if (loc[1] >= 0 && INNER(loc[1]) >= 0)
+            bin += in->lat2_bin[in->lat2_off[in->cell_fill[mid_cell(p, OUTER(loc[1]))]] + INNER(loc[1])];
         /* cross sections */
         double sig_t, nusf;
         int32_t gi, ncol = 0;
@@ -802,22 +907,38 @@ static void transport(orc_problem *p, particle *q)
             }
             trace(p, q, ev, loc[0], loc[1], loc[2], -1, gi, d, E_flight);
         } else if (kind == 1) {
-            if (hit >= in->n_surf) { /* lattice wall: step to the neighbour element (R14) */
+            if (hit >= in->n_surf + 4) { /* second-level lattice wall: step to the neighbour element (R37) */
                 ev = ORC_EV_LATTICE;
-                int w = hit - in->n_surf;
-                int32_t ix = loc[1] % in->lat_nx, iy = loc[1] / in->lat_nx;
-                if (w == 0) ix--; else if (w == 1) ix++; else if (w == 2) iy--; else iy++;
-                q->elem = iy * in->lat_nx + ix;
+                int w = hit - in->n_surf - 4;
+                int32_t k2 = in->cell_fill[mid_cell(p, OUTER(loc[1]))];
+                int32_t jx = INNER(loc[1]) % in->lat2_nx[k2], jy = INNER(loc[1]) / in->lat2_nx[k2];
+                if (w == 0) jx--; else if (w == 1) jx++; else if (w == 2) jy--; else jy++;
+                int32_t inner = jy * in->lat2_nx[k2] + jx;
+                q->elem = OUTER(loc[1]) | ((inner + 1) << 16);
                 q->last_surf = -1;
                 double xn[3] = {q->x, q->y, q->z}, xl[3];
                 local_coords(p, q->elem, xn, xl);
-                q->c1 = find_cell(p, in->lat_univ[q->elem], xl, u, -1);
+                q->c1 = find_cell(p, in->lat2_univ[in->lat2_off[k2] + inner], xl, u, -1);
+                if (q->c1 < 0) { ev = ORC_EV_LOST; q->alive = 0; p->error = -2; }
+            } else if (hit >= in->n_surf) { /* lattice wall: step to the neighbour element (R14) */
+                ev = ORC_EV_LATTICE;
+                int w = hit - in->n_surf;
+                int32_t ix = OUTER(loc[1]) % in->lat_nx, iy = OUTER(loc[1]) / in->lat_nx;
+                if (w == 0) ix--; else if (w == 1) ix++; else if (w == 2) iy--; else iy++;
+                q->last_surf = -1;
+                double xn[3] = {q->x, q->y, q->z}, xo[3];
+                outer_coords(p, iy * in->lat_nx + ix, xn, xo);
+                q->c1 = descend(p, iy * in->lat_nx + ix, xo, u, -1, &q->elem);
                 if (q->c1 < 0) { ev = ORC_EV_LOST; q->alive = 0; p->error = -2; }
             } else {
                 int bc = in->surf_bc[hit];
-                int local = !surface_in_cell(p, loc[0], hit); /* the surface belongs to the local cell */
+                /* whose surface is it: the root cell's (global coordinates), the cell's that the second-level lattice
+                 * fills (first-level-element coordinates), or the local cell's (innermost coordinates) */
+                int local = !surface_in_cell(p, loc[0], hit);
+                int midlevel = local && loc[1] >= 0 && INNER(loc[1]) >= 0 && surface_in_cell(p, mid_cell(p, OUTER(loc[1])), hit);
                 double xn[3] = {q->x, q->y, q->z}, xl[3];
-                if (local) local_coords(p, loc[1], xn, xl);
+                if (midlevel) outer_coords(p, OUTER(loc[1]), xn, xl);
+                else if (local) local_coords(p, loc[1], xn, xl);
                 if (bc == 2) {
                     ev = ORC_EV_LEAK;
                     p->leak_c += q->w;
@@ -833,7 +954,14 @@ static void transport(orc_problem *p, particle *q)
                     ev = ORC_EV_TRANSMIT;
                     q->last_surf = hit;
                     if (local) {
-                        q->c1 = find_cell(p, in->lat_univ[loc[1]], xl, u, hit);
+                        if (!midlevel && INNER(loc[1]) >= 0) { /* inside the same second-level element */
+                            int32_t k2 = in->cell_fill[mid_cell(p, OUTER(loc[1]))];
+                            q->c1 = find_cell(p, in->lat2_univ[in->lat2_off[k2] + INNER(loc[1])], xl, u, hit);
+                        } else { /* inside the same first-level element: its universe, descending where a lattice fills */
+                            double xo[3];
+                            outer_coords(p, OUTER(loc[1]), xn, xo);
+                            q->c1 = descend(p, OUTER(loc[1]), xo, u, hit, &q->elem);
+                        }
                         if (q->c1 < 0) { ev = ORC_EV_LOST; q->alive = 0; p->error = -2; }
                     } else {
                         int32_t nl[3];

@@ -38,6 +38,15 @@ typedef struct {
     double lat_x0, lat_y0, lat_px, lat_py;
     int32_t lat_nx, lat_ny;
     const int32_t *lat_univ, *lat_bin; /* [ny][nx] */
+    /* second-level lattices (R37; "fully 3D C5G7": assemblies are lattices of pin lattices): a cell of a
+     * lattice element's universe with cell_fill_type 2 is filled by inner lattice k = cell_fill, nx[k] x ny[k] elements
+     * of pitch px[k], py[k], centred on the origin of that universe's coordinates; the universes and tally-bin offsets
+     * of its elements are lat2_univ / lat2_bin [lat2_off[k] + iy nx[k] + ix].  At most one such cell per universe. */
+    int32_t n_lat2;
+    const int32_t *lat2_nx, *lat2_ny;
+    const double *lat2_px, *lat2_py;
+    const int32_t *lat2_off; /* [n_lat2+1] */
+    const int32_t *lat2_univ, *lat2_bin;
     int32_t n_bins;
     int32_t n_mat;
     /* multi-group */

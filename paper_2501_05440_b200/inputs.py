@@ -14,10 +14,14 @@ geometry (SURVEY.md 8b/8c rules 11-16; "constructive solid geometry 
                         CYL_Z: (x0,y0,r,-) (CYL_X: (y0,z0,r), CYL_Y: (x0,z0,r)); SPHERE: (x0,y0,z0,r)
   surf_bc    i32[ns]    0 TRANSMIT, 1 REFLECT, 2 VACUUM
   cell_surf_off i32[nc+1], cell_surf_id i32[], cell_surf_sense i32[] (+1: f>0, -1: f<0)
-  cell_fill_type i32[nc] 0 material, 1 lattice;  cell_fill i32[nc] material id (or 0 for the lattice)
+  cell_fill_type i32[nc] 0 material, 1 lattice, 2 second-level lattice;  cell_fill i32[nc] material id (0 for the
+                        lattice; the second-level lattice's index)
   cell_bin   i32[nc]    spatial tally bin of the cell (added to the lattice element's bin)
   univ_cell_off i32[nu+1]  cells are sorted by universe; universe 0 is the root
   lat        None | dict(x0,y0,px,py,nx,ny, univ i32[ny,nx], bin i32[ny,nx])
+  lat2_nx, lat2_ny i32[n2], lat2_px, lat2_py f64[n2], lat2_off i32[n2+1], lat2_univ, lat2_bin i32[]  (optional)
+                        second-level lattices: lattice k fills a cell (fill type 2) of a first-level element's
+                        universe, centred on that universe's origin; element (ix,iy) is entry lat2_off[k]+iy*nx+ix
   n_bins     number of spatial tally bins
 physics
   mode 'mg': G, n_mat, mg_sig_t/mg_sig_c/mg_sig_f/mg_nu/mg_chi f64[nm,G], mg_S f64[nm,G,G] (row = from)
@@ -53,10 +57,23 @@ class _Geom:
         self.sb.append(bc)
         return len(self.st) - 1
 
-    def cell(self, univ, region, fill, bin_=0, lattice=False):
-        self.cells.append((univ, list(region), 1 if lattice else 0, fill, bin_))
+    def cell(self, univ, region, fill, bin_=0, lattice=False, lattice2=False):
+        self.cells.append((univ, list(region), 2 if lattice2 else (1 if lattice else 0), fill, bin_))
 
-    def finish(self, lat=None, n_bins=1):
+    def finish(self, lat=None, n_bins=1, lat2=None):
+        """lat2: list of dict(nx, ny, px, py, univ i32[ny,nx], bin i32[ny,nx]) -- the second-level lattices."""
+        out = self._finish(lat, n_bins)
+        if lat2:
+            out["lat2_nx"] = np.array([L["nx"] for L in lat2], np.int32)
+            out["lat2_ny"] = np.array([L["ny"] for L in lat2], np.int32)
+            out["lat2_px"] = np.array([L["px"] for L in lat2], np.float64)
+            out["lat2_py"] = np.array([L["py"] for L in lat2], np.float64)
+            out["lat2_off"] = np.concatenate([[0], np.cumsum([L["nx"] * L["ny"] for L in lat2])]).astype(np.int32)
+            out["lat2_univ"] = np.concatenate([np.asarray(L["univ"], np.int32).ravel() for L in lat2])
+            out["lat2_bin"] = np.concatenate([np.asarray(L["bin"], np.int32).ravel() for L in lat2])
+        return out
+
+    def _finish(self, lat=None, n_bins=1):
         cells = sorted(enumerate(self.cells), key=lambda t: (t[1][0], t[0]))
         nu = max(c[1][0] for c in cells) + 1
         off, sid, sse, ft, fl, cb = [0], [], [], [], [], []
@@ -258,6 +275,121 @@ def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_refl
     return g.finish(lat=lat, n_bins=nfuel * nfuel + 1)
 
 
+def geom_quarter_core_2l(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl_asm=1, all_reflect=False, height=None,
+                         reflector_lattice=True):
+    """The quarter core of geom_quarter_core as a TWO-LEVEL lattice (the paper's multi-group benchmark
+    is a core of assemblies of pins): a first-level (n_asm + n_refl_asm)^2 lattice of assemblies of pitch n_pin * pitch;
+    every assembly universe is one cell without surfaces filled by a second-level n_pin x n_pin pin lattice.  Same pin
+    map, materials and per-pin tally bins as the flat geometry with n_refl = n_refl_asm * n_pin, so both describe the
+    same physical problem.  Universes 1..7 as there; 8, 9 = the two fuel assembly types, 10 = reflector assembly
+    (reflector_lattice=False: reflector assemblies are one moderator cell with no inner walls)."""
+    g = _Geom()
+    na = n_asm + n_refl_asm
+    nfuel = n_asm * n_pin
+    ap = n_pin * pitch
+    side = na * ap
+    outer = REFLECT if all_reflect else VACUUM
+    x0 = g.surf(PLANE_X, [0.0], REFLECT)
+    x1 = g.surf(PLANE_X, [side], outer)
+    y0 = g.surf(PLANE_Y, [0.0], REFLECT)
+    y1 = g.surf(PLANE_Y, [side], outer)
+    cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
+    root = [(x0, +1), (x1, -1), (y0, +1), (y1, -1)]
+    if height is not None:
+        z0 = g.surf(PLANE_Z, [0.0], REFLECT)
+        z1 = g.surf(PLANE_Z, [float(height)], outer)
+        root += [(z0, +1), (z1, -1)]
+    g.cell(0, root, 0, lattice=True)
+    for u in range(1, 7):
+        g.cell(u, [(cy, -1)], u - 1)
+        g.cell(u, [(cy, +1)], 6)
+    g.cell(7, [], 6)
+    g.cell(8, [], 0, lattice2=True)
+    g.cell(9, [], 1, lattice2=True)
+    if reflector_lattice:
+        g.cell(10, [], 2, lattice2=True)
+    else:
+        g.cell(10, [], 6)
+    tubes = set(tube_positions()) if n_pin == 17 else set()
+    inner = []
+    for kind in (0, 1):
+        un = np.zeros((n_pin, n_pin), np.int32)
+        for py in range(n_pin):
+            for px in range(n_pin):
+                edge = min(px, py, n_pin - 1 - px, n_pin - 1 - py)
+                if (px, py) in tubes:
+                    u = 6
+                elif kind == 0:
+                    u = 1 if edge < 2 else (2 if edge < 5 else 3)
+                else:
+                    u = 4 if edge < 3 else 5
+                un[py, px] = u
+        bins = (np.arange(n_pin)[:, None] * nfuel + np.arange(n_pin)[None, :]).astype(np.int32)
+        inner.append(dict(nx=n_pin, ny=n_pin, px=float(pitch), py=float(pitch), univ=un, bin=bins))
+    if reflector_lattice:
+        inner.append(dict(nx=n_pin, ny=n_pin, px=float(pitch), py=float(pitch), univ=np.full((n_pin, n_pin), 7, np.int32),
+                          bin=np.zeros((n_pin, n_pin), np.int32)))
+    univ = np.full((na, na), 10, np.int32)
+    bins = np.full((na, na), nfuel * nfuel, np.int32)
+    for ay in range(n_asm):
+        for ax in range(n_asm):
+            univ[ay, ax] = 8 if (ax + ay) % 2 == 0 else 9
+            bins[ay, ax] = ay * n_pin * nfuel + ax * n_pin
+    lat = dict(x0=0.0, y0=0.0, px=float(ap), py=float(ap), nx=na, ny=na, univ=univ, bin=bins)
+    return g.finish(lat=lat, n_bins=nfuel * nfuel + 1, lat2=inner)
+
+
+def geom_assembly_gap(n_asm=2, n_pin=3, pitch=1.26, r=0.54, gap=0.2):
+    """Two-level lattice whose assembly universe has structure of its own: the pin lattice fills a square cell
+    |x|, |y| < n_pin * pitch / 2 (four planes in assembly coordinates) and a moderator gap of width `gap` surrounds it
+    (four conjunctive cells).  n_asm x n_asm assemblies; x = 0, y = 0 reflect, the far faces are vacuum.  Materials:
+    0 fuel, 1 moderator.  One tally bin per pin plus one gap bin per assembly."""
+    g = _Geom()
+    h = 0.5 * n_pin * pitch
+    ap = 2.0 * (h + gap)
+    side = n_asm * ap
+    x0 = g.surf(PLANE_X, [0.0], REFLECT)
+    x1 = g.surf(PLANE_X, [side], VACUUM)
+    y0 = g.surf(PLANE_Y, [0.0], REFLECT)
+    y1 = g.surf(PLANE_Y, [side], VACUUM)
+    cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
+    xl = g.surf(PLANE_X, [-h], TRANSMIT)
+    xh = g.surf(PLANE_X, [h], TRANSMIT)
+    yl = g.surf(PLANE_Y, [-h], TRANSMIT)
+    yh = g.surf(PLANE_Y, [h], TRANSMIT)
+    g.cell(0, [(x0, +1), (x1, -1), (y0, +1), (y1, -1)], 0, lattice=True)
+    g.cell(1, [(cy, -1)], 0)
+    g.cell(1, [(cy, +1)], 1)
+    g.cell(2, [], 1)
+    npp = n_pin * n_pin
+    # assembly universe 3: the lattice cell first, then the four gap cells (bin offset npp = the assembly's gap bin)
+    g.cell(3, [(xl, +1), (xh, -1), (yl, +1), (yh, -1)], 0, lattice2=True)
+    g.cell(3, [(xl, -1)], 1, bin_=npp)
+    g.cell(3, [(xh, +1)], 1, bin_=npp)
+    g.cell(3, [(xl, +1), (xh, -1), (yl, -1)], 1, bin_=npp)
+    g.cell(3, [(xl, +1), (xh, -1), (yh, +1)], 1, bin_=npp)
+    un = np.array([[1 if (ix + iy) % 3 else 2 for ix in range(n_pin)] for iy in range(n_pin)], np.int32)
+    inner = [dict(nx=n_pin, ny=n_pin, px=float(pitch), py=float(pitch), univ=un,
+                  bin=np.arange(npp, dtype=np.int32).reshape(n_pin, n_pin))]
+    univ = np.full((n_asm, n_asm), 3, np.int32)
+    bins = (np.arange(n_asm * n_asm, dtype=np.int32) * (npp + 1)).reshape(n_asm, n_asm)
+    lat = dict(x0=0.0, y0=0.0, px=float(ap), py=float(ap), nx=n_asm, ny=n_asm, univ=univ, bin=bins)
+    return g.finish(lat=lat, n_bins=n_asm * n_asm * (npp + 1), lat2=inner)
+
+
+def assembly_gap(n_asm=2, n_pin=3, n_particles=4000, n_inactive=1, n_active=2, seed=43, G=3, gap=0.2):
+    """Two synthetic 3-group materials in geom_assembly_gap; eigenvalue run."""
+    rng = np.random.default_rng(7)
+    mats = [mg_fuel(rng, G, 1.5), mg_moderator(rng, G)]
+    P = geom_assembly_gap(n_asm, n_pin, gap=gap)
+    P.update(_mg_pack(mats))
+    side = n_asm * (n_pin * 1.26 + 2 * gap)
+    P.update(_src([0, 0, 0], [side, side, 0], G=G, pdf=mats[0]["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "asm_gap"
+    return P
+
+
 def geom_rect_lattice(nx, ny, pitch=1.26, r=0.54, x_hi=VACUUM, y_hi=REFLECT):
     """nx x ny pin lattice filling the box [0, nx p] x [0, ny p] (parity geometry for non-square and one-column /
     one-row lattices): universes 1 = fuel pin (material 0 in a cylinder, 1 outside), 2 = moderator only, in a
@@ -409,16 +541,23 @@ def config3(n_particles=1_000_000, n_inactive=20, n_active=80, seed=1, same_mate
 
 
 def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform=False,
-            n_asm=2, n_pin=17, n_refl=17, G=7, height=None):
+            n_asm=2, n_pin=17, n_refl=17, G=7, height=None, two_level=False, reflector_lattice=True):
     """C4: 2-D quarter core stand-in for the paper's C5G7 workload: 7 synthetic
-    materials from seed 4.  uniform=True: all materials identical + all faces reflecting (pin)."""
+    materials from seed 4.  uniform=True: all materials identical + all faces reflecting (pin).
+    two_level=True: the same core described as a lattice of assemblies of pin lattices (n_refl must be a
+    multiple of n_pin)."""
     rng = np.random.default_rng(4)
     mats = [mg_fuel(rng, G, kt) for kt in (1.05, 1.15, 1.25)]
     mats += [mg_fuel(rng, G, kt, thermal_boost=1.5) for kt in (1.10, 1.20)]
     mats += [mg_moderator(rng, G), mg_moderator(rng, G)]
     if uniform:
         mats = [mg_fuel(np.random.default_rng(2), G, 1.2)] * 7
-    P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform, height=height)
+    if two_level:
+        assert n_refl % n_pin == 0
+        P = geom_quarter_core_2l(n_asm=n_asm, n_pin=n_pin, n_refl_asm=n_refl // n_pin, all_reflect=uniform, height=height,
+                                 reflector_lattice=reflector_lattice)
+    else:
+        P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform, height=height)
     P.update(_mg_pack(mats))
     side = n_asm * n_pin * 1.26
     P.update(_src([0, 0, 0], [side, side, 0.9 * height if height else 0], G=G, pdf=mats[0]["chi"]))

@@ -106,6 +106,22 @@ class World:
             self.nx, self.ny = int(L["nx"]), int(L["ny"])
             self.x0, self.y0, self.px, self.py = float(L["x0"]), float(L["y0"]), float(L["px"]), float(L["py"])
             self.univ = [[int(v) for v in row] for row in L["univ"]]
+        # second-level lattices: (nx, ny, px, py, x0, y0, universes[iy][ix], bins[iy][ix]), centred on the origin of the
+        # universe whose cell (fill type 2) they fill
+        self.lat2 = []
+        for k in range(len(P.get("lat2_nx", []))):
+            nx, ny = int(P["lat2_nx"][k]), int(P["lat2_ny"][k])
+            px, py, o = float(P["lat2_px"][k]), float(P["lat2_py"][k]), int(P["lat2_off"][k])
+            un = [[int(P["lat2_univ"][o + iy * nx + ix]) for ix in range(nx)] for iy in range(ny)]
+            bn = [[int(P["lat2_bin"][o + iy * nx + ix]) for ix in range(nx)] for iy in range(ny)]
+            self.lat2.append((nx, ny, px, py, -0.5 * nx * px, -0.5 * ny * py, un, bn))
+
+    def _lat2_of(self, univ):
+        """(cell, lattice) of the second-level lattice that fills a cell of `univ`, or None."""
+        for c in range(self.uoff[univ], self.uoff[univ + 1]):
+            if int(self.P["cell_fill_type"][c]) == 2:
+                return c, self.lat2[int(self.P["cell_fill"][c])]
+        return None
 
     def _in_cell(self, c, x):
         P = self.P
@@ -131,7 +147,18 @@ class World:
             return None
         xl = [x[0] - (self.x0 + (ix + 0.5) * self.px), x[1] - (self.y0 + (iy + 0.5) * self.py), x[2]]
         c1 = self._cell_in(self.univ[iy][ix], xl)
-        return None if c1 < 0 else (c0, iy * self.nx + ix, c1)
+        if c1 < 0:
+            return None
+        elem = iy * self.nx + ix
+        if int(self.P["cell_fill_type"][c1]) == 2:  # a lattice of its own fills this cell of the element's universe
+            nx, ny, px, py, x0, y0, un, _ = self.lat2[int(self.P["cell_fill"][c1])]
+            jx, jy = math.floor((xl[0] - x0) / px), math.floor((xl[1] - y0) / py)
+            if not (0 <= jx < nx and 0 <= jy < ny):
+                return None
+            x2 = [xl[0] - (x0 + (jx + 0.5) * px), xl[1] - (y0 + (jy + 0.5) * py), xl[2]]
+            c2 = self._cell_in(un[jy][jx], x2)
+            return None if c2 < 0 else (c0, elem | ((jy * nx + jx + 1) << 16), c2)
+        return (c0, elem, c1)
 
     def material(self, loc):
         return int(self.P["cell_fill"][loc[2] if loc[1] >= 0 else loc[0]])
@@ -139,7 +166,11 @@ class World:
     def spatial_bin(self, loc):
         b = int(self.P["cell_bin"][loc[2] if loc[1] >= 0 else loc[0]])
         if loc[1] >= 0:
-            b += int(self.lat["bin"].ravel()[loc[1]])
+            outer, inner = loc[1] & 0xFFFF, (loc[1] >> 16) - 1
+            b += int(self.lat["bin"].ravel()[outer])
+            if inner >= 0:
+                nx, _, _, _, _, _, _, bn = self._lat2_of(self.univ[outer // self.nx][outer % self.nx])[1]
+                b += bn[inner // nx][inner % nx]
         return b
 
     def candidates(self, x, u):
@@ -166,6 +197,26 @@ class World:
                     xl = [x[0] - (self.x0 + (ix + 0.5) * self.px), x[1] - (self.y0 + (iy + 0.5) * self.py), x[2]]
                     for s in surfs:
                         out += [(d, 0, s) for d in _roots(self.st[s], self.sq[s], xl, u) if d > 1e-9]
+                    l2 = self._lat2_of(un)
+                    if l2 is None:
+                        continue
+                    # second level: every grid line of the inner lattice (wall codes n_surf + 4..7) and the surfaces of
+                    # every inner element's universe, moved to that element's centre
+                    nx2, ny2, px2, py2, x02, y02, un2, _ = l2[1]
+                    for ax, (o, p, n) in enumerate(((x02, px2, nx2), (y02, py2, ny2))):
+                        if u[ax] != 0:
+                            for k in range(n + 1):
+                                d = (o + k * p - xl[ax]) / u[ax]
+                                if d > 1e-9:
+                                    out.append((d, 1, self.ns + 4 + 2 * ax + (1 if u[ax] > 0 else 0)))
+                    for jy in range(ny2):
+                        for jx in range(nx2):
+                            uu = un2[jy][jx]
+                            surfs2 = {int(P["cell_surf_id"][k]) for c in range(self.uoff[uu], self.uoff[uu + 1])
+                                      for k in range(P["cell_surf_off"][c], P["cell_surf_off"][c + 1])}
+                            x2 = [xl[0] - (x02 + (jx + 0.5) * px2), xl[1] - (y02 + (jy + 0.5) * py2), xl[2]]
+                            for s in surfs2:
+                                out += [(d, 0, s) for d in _roots(self.st[s], self.sq[s], x2, u) if d > 1e-9]
         return sorted(out)
 
     def next_event(self, x, u):
@@ -190,13 +241,16 @@ class World:
                 continue
             for c in real:
                 return here, c[0], c[2]
-            return here, group[0][0], group[0][2]
+            # grid lines only: where a first-level line and the rim of a second-level lattice coincide, the first-level
+            # wall is the event (a lattice's outermost lines never are, R14 / R37)
+            first = min(group, key=lambda c: c[2])
+            return here, first[0], first[2]
         return here, math.inf, -1
 
     def reflect(self, s, x, u, loc):
         xl = list(x)
         if loc[1] >= 0 and not self._surface_of_root(s):
-            ix, iy = loc[1] % self.nx, loc[1] // self.nx
+            ix, iy = (loc[1] & 0xFFFF) % self.nx, (loc[1] & 0xFFFF) // self.nx
             xl = [x[0] - (self.x0 + (ix + 0.5) * self.px), x[1] - (self.y0 + (iy + 0.5) * self.py), x[2]]
         n = _normal(self.st[s], self.sq[s], xl)
         dot = sum(u[i] * n[i] for i in range(3))
