@@ -46,6 +46,8 @@ class OrcInput(C.Structure):
         ("src_lo", C.c_double * 3), ("src_hi", C.c_double * 3), ("src_iso", C.c_int32),
         ("src_dir", C.c_double * 3), ("src_group_pdf", _dp), ("src_E", C.c_double), ("src_t", C.c_double),
         ("kT", C.c_double), ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double),
+        ("td", C.c_int32), ("n_dgroup", C.c_int32), ("speed", _dp), ("nu_d", _dp), ("decay", _dp), ("chi_d", _dp),
+        ("census_target", C.c_int64),
     ]
 
 
@@ -77,6 +79,10 @@ def lib():
         L.orc_run_eigenvalue.argtypes = [C.c_void_p, C.c_uint64, C.c_int, C.c_int, C.c_uint64]
         L.orc_run_eigenvalue_mt.argtypes = [C.c_void_p, C.c_uint64, C.c_int, C.c_int, C.c_uint64, C.c_int]
         L.orc_run_fixed_source.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
+        L.orc_run_td.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
+        L.orc_get_census.argtypes = [C.c_void_p, C.POINTER(C.c_uint64), _dp, C.c_int]
+        L.orc_comb.restype = C.c_double
+        L.orc_comb.argtypes = [_dp, C.c_uint64, C.c_uint64, C.c_double, C.POINTER(C.c_uint32)]
         L.orc_n_tally.restype = C.c_int64
         L.orc_n_tally.argtypes = [C.c_void_p]
         L.orc_get_results.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp, _dp, _dp, C.POINTER(C.c_uint64)]
@@ -180,6 +186,13 @@ class Oracle:
         inp.implicit_capture = int(P.get("implicit_capture", 0))
         inp.w_roulette = float(P.get("w_roulette", 0.25))
         inp.w_survive = float(P.get("w_survive", 1.0))
+        td = P.get("td")
+        inp.td = 1 if td else 0
+        if td:  # time-dependent multi-group: speeds, delayed-neutron data, time edges, census population target
+            inp.n_dgroup = int(td["J"])
+            inp.speed, inp.nu_d, inp.decay, inp.chi_d = dp(td["speed"]), dp(td["nu_d"]), dp(td["decay"]), dp(td["chi_d"])
+            inp.census_target = int(td.get("census_target", 0))
+            inp.n_t, inp.t_edges = len(P["t_edges"]) - 1, dp(P["t_edges"])
         self.L = lib()
         self.h = self.L.orc_create(C.byref(inp))
         self.n_tally = self.L.orc_n_tally(self.h)
@@ -217,6 +230,9 @@ class Oracle:
         if r["kind"] == "eigen":
             rc = self.L.orc_run_eigenvalue(self.h, N, ni, na, sd)
             self.n_cycles = ni + na
+        elif r["kind"] == "td":
+            rc = self.L.orc_run_td(self.h, N, sd)
+            self.n_cycles = 1
         else:
             rc = self.L.orc_run_fixed_source(self.h, N, sd)
             self.n_cycles = 1
@@ -238,6 +254,13 @@ class Oracle:
         out = np.zeros(6)
         self.L.orc_get_balance(self.h, out.ctypes.data_as(_dp))
         return dict(zip(("source", "absorbed", "leaked", "cutoff", "roulette_loss", "roulette_gain"), out))
+
+    def census(self):
+        """Population entering each census interval of the last time-dependent multi-group run:
+        (particles before the comb, after it, weight before, weight after) per interval."""
+        cnt, w = np.zeros(128, np.uint64), np.zeros(128)
+        n = self.L.orc_get_census(self.h, cnt.ctypes.data_as(C.POINTER(C.c_uint64)), w.ctypes.data_as(_dp), 64)
+        return [(int(cnt[2 * k]), int(cnt[2 * k + 1]), float(w[2 * k]), float(w[2 * k + 1])) for k in range(n)]
 
     def trace(self):
         n = self.L.orc_get_trace(self.h, None, 0)
@@ -319,3 +342,11 @@ def watt(a, b, x1, x2, x3, x4):
 
 def speed(E):
     return lib().orc_speed(E)
+
+
+def comb(w, n_teeth, xi):
+    """The population-control comb on plain arrays (orc_comb): copies per particle and the tooth spacing."""
+    w = _d(w)
+    copies = np.zeros(len(w), np.uint32)
+    delta = lib().orc_comb(w.ctypes.data_as(_dp), len(w), int(n_teeth), float(xi), copies.ctypes.data_as(C.POINTER(C.c_uint32)))
+    return copies, delta

@@ -22,6 +22,7 @@
 typedef struct {
     double x, y, z, ux, uy, uz, w, E, t;
     int32_t g, c0, elem, c1, last_surf, tbin, alive;
+    int32_t resumed; /* taken from a census bank: already counted as a started track */
     uint32_t ctr, nseg;
     uint64_t id;
 } particle;
@@ -50,6 +51,14 @@ struct orc_problem {
     uint64_t n_bank, n_newbank, cap_bank;
     particle *stack;
     uint64_t n_stack, cap_stack;
+    /* time-dependent multi-group (R38-R40): delayed-spectrum / yield tables, the census banks (one per interval) */
+    double *cumchi_d, *cum_nu;
+    int census_stop;
+    particle **cbank;
+    uint64_t *n_cbank, *cap_cbank;
+    uint64_t census_counts[2 * 64];
+    double census_weights[2 * 64];
+    int n_census;
     /* trace */
     uint64_t tr_first, tr_n, tr_max, tr_count;
     orc_trace_rec *trace;
@@ -292,10 +301,10 @@ static int32_t find_cell(const orc_problem *p, int32_t univ, const double x[3], 
     return -1;
 }
 
-/* Location inside lattices: `elem` packs the element of the (first-level) lattice in its low 16 bits and, inside a
+/* Location inside lattices: `elem` packs the element of the (first-level) lattice in its low 20 bits and, inside a
  * second-level lattice (R37), that lattice's element + 1 in the bits above; -1 = not in a lattice. */
-#define OUTER(e) ((e) & 0xffff)
-#define INNER(e) (((e) >> 16) - 1)
+#define OUTER(e) ((e) & 0xfffff)
+#define INNER(e) (((e) >> 20) - 1)
 
 /* coordinates centred on first-level element `outer`, recomputed from the global position every time (R14) */
 static void outer_coords(const orc_problem *p, int32_t outer, const double x[3], double xl[3])
@@ -362,7 +371,7 @@ static int32_t descend(const orc_problem *p, int32_t outer, const double xo[3], 
     int32_t inner = iy * in->lat2_nx[k] + ix;
     double xl[3];
     inner_coords(p, k, inner, xo, xl);
-    *elem = outer | ((inner + 1) << 16);
+    *elem = outer | ((inner + 1) << 20);
     return find_cell(p, in->lat2_univ[in->lat2_off[k] + inner], xl, u, last_surf);
 }
 
@@ -647,6 +656,31 @@ orc_problem *orc_create(const orc_input *in)
         double cs = 0.0;
         for (int g = 0; g < G; g++) { cs += in->src_group_pdf[g]; p->src_cum[g] = cs; }
         n_tally = (int64_t)in->n_bins * G;
+        if (in->td) {
+            int J = in->n_dgroup;
+            DUP(speed, G, double);
+            DUP(nu_d, (size_t)nm * J * G, double);
+            DUP(decay, (size_t)nm * J, double);
+            DUP(chi_d, (size_t)nm * J * G, double);
+            DUP(t_edges, in->n_t + 1, double);
+            p->cumchi_d = (double *)calloc((size_t)nm * J * G + 1, sizeof(double));
+            p->cum_nu = (double *)calloc((size_t)nm * G * (J + 1), sizeof(double));
+            for (int m = 0; m < nm; m++) {
+                for (int j = 0; j < J; j++) {
+                    double cc = 0.0;
+                    for (int g = 0; g < G; g++) { cc += in->chi_d[((size_t)m * J + j) * G + g]; p->cumchi_d[((size_t)m * J + j) * G + g] = cc; }
+                }
+                for (int g = 0; g < G; g++) { /* cumulative yields [prompt, +delayed 1, ..., +delayed J] */
+                    double cn = in->nu[m * G + g];
+                    p->cum_nu[((size_t)m * G + g) * (J + 1)] = cn;
+                    for (int j = 0; j < J; j++) { cn += in->nu_d[((size_t)m * J + j) * G + g]; p->cum_nu[((size_t)m * G + g) * (J + 1) + 1 + j] = cn; }
+                }
+            }
+            n_tally = (int64_t)in->n_bins * in->n_t * G;
+            p->cbank = (particle **)calloc((size_t)in->n_t + 1, sizeof(particle *));
+            p->n_cbank = (uint64_t *)calloc((size_t)in->n_t + 1, sizeof(uint64_t));
+            p->cap_cbank = (uint64_t *)calloc((size_t)in->n_t + 1, sizeof(uint64_t));
+        }
     } else {
         int nm = in->n_mat, ng = in->n_grid;
         DUP(grid, ng, double);
@@ -702,7 +736,8 @@ void orc_destroy(orc_problem *p)
 
 int64_t orc_n_tally(const orc_problem *p)
 {
-    return p->in.mode == 0 ? (int64_t)p->in.n_bins * p->in.G : (int64_t)p->in.n_bins * p->in.n_t * p->in.n_e;
+    if (p->in.mode == 0) return p->in.td ? (int64_t)p->in.n_bins * p->in.n_t * p->in.G : (int64_t)p->in.n_bins * p->in.G;
+    return (int64_t)p->in.n_bins * p->in.n_t * p->in.n_e;
 }
 
 int orc_set_trace(orc_problem *p, uint64_t first_id, uint64_t n_ids, uint64_t max_records)
@@ -736,6 +771,16 @@ static void push_secondary(orc_problem *p, const particle *c)
     p->stack[p->n_stack++] = *c;
 }
 
+/* a particle that waits for census interval k (it reached the time edge, or it is a delayed neutron born there) */
+static void push_census(orc_problem *p, int k, const particle *c)
+{
+    if (p->n_cbank[k] == p->cap_cbank[k]) {
+        p->cap_cbank[k] = p->cap_cbank[k] ? 2 * p->cap_cbank[k] : 1024;
+        p->cbank[k] = (particle *)realloc(p->cbank[k], p->cap_cbank[k] * sizeof(particle));
+    }
+    p->cbank[k][p->n_cbank[k]++] = *c;
+}
+
 static void bank_site(orc_problem *p, const particle *q, const double u[3], int32_t g)
 {
     if (p->n_newbank == p->cap_bank) { p->error = -3; return; } /* bank overflow (R6) */
@@ -748,8 +793,8 @@ static void transport(orc_problem *p, particle *q)
 {
     const orc_input *in = &p->in;
     double xs[64];
-    p->counters[0]++;
-    p->balance[0] += q->w;
+    const int timed = in->mode == 1 || in->td; /* the particle carries a clock: time edges are candidate events */
+    if (!q->resumed) { p->counters[0]++; p->balance[0] += q->w; }
     while (q->alive) {
         double x[3] = {q->x, q->y, q->z}, u[3] = {q->ux, q->uy, q->uz};
         int32_t loc[3] = {q->c0, q->elem, q->c1};
@@ -776,8 +821,8 @@ static void transport(orc_problem *p, particle *q)
         int32_t hit;
         double d_surf = orc_distance(p, x, u, loc, q->last_surf, &hit);
         double v = 0.0, d_time = INFINITY;
-        if (in->mode == 1) {
-            v = orc_speed(q->E);
+        if (timed) {
+            v = in->mode == 1 ? orc_speed(q->E) : in->speed[q->g]; /* R23 / the group's speed (R38) */
             d_time = v * (in->t_edges[q->tbin + 1] - q->t);
         }
         int kind; /* 0 collision, 1 surface, 2 time edge (R12) */
@@ -789,11 +834,9 @@ static void transport(orc_problem *p, particle *q)
         q->x += d * u[0]; q->y += d * u[1]; q->z += d * u[2];
         double E_flight = q->E;
         int64_t tix;
-        if (in->mode == 0) tix = (int64_t)bin * in->G + q->g;
-        else {
-            tix = ((int64_t)bin * in->n_t + q->tbin) * in->n_e + edge_bin(in->e_edges, in->n_e, q->E);
-            if (kind == 2) q->t = in->t_edges[q->tbin + 1]; else q->t += d / v;
-        }
+        if (in->mode == 0) tix = in->td ? ((int64_t)bin * in->n_t + q->tbin) * in->G + q->g : (int64_t)bin * in->G + q->g;
+        else tix = ((int64_t)bin * in->n_t + q->tbin) * in->n_e + edge_bin(in->e_edges, in->n_e, q->E);
+        if (timed) { if (kind == 2) q->t = in->t_edges[q->tbin + 1]; else q->t += d / v; }
         p->flux_c[tix] += q->w * d;
         p->k_num += q->w * d * nusf;
         int ev;
@@ -829,6 +872,37 @@ static void transport(orc_problem *p, particle *q)
                         orc_iso_dir(xi1, xi2, o);
                         q->g = gp; q->ux = o[0]; q->uy = o[1]; q->uz = o[2];
                     }
+                } else if (uu < sig_s + sig_f && in->td) {
+                    /* time-dependent fixed source (R39): nu = prompt yield + delayed yields; n = floor(nu + xi)
+                     * children of the parent's weight; per child: type (prompt / precursor group j) by xi nu against
+                     * the cumulative yields, group from the type's spectrum, emission time t (prompt) or
+                     * t - ln(xi) / lambda_j (delayed), isotropic direction; own stream (R10).  A delayed neutron
+                     * emitted after the last time edge is never born (its draws are consumed all the same). */
+                    ev = ORC_EV_FISSION;
+                    int J = in->n_dgroup;
+                    const double *cn = p->cum_nu + ((size_t)mat * G + q->g) * (J + 1);
+                    double nu_tot = cn[J];
+                    int n = (int)floor(nu_tot + draw(p, q));
+                    uint32_t ctr_birth = q->ctr;
+                    for (int j = 0; j < n; j++) {
+                        int32_t typ = pick(cn, J + 1, draw(p, q) * nu_tot); /* 0 prompt, 1 + precursor group */
+                        const double *cc = typ == 0 ? p->cumchi + (size_t)mat * G : p->cumchi_d + ((size_t)mat * J + typ - 1) * G;
+                        int32_t gj = pick(cc, G, draw(p, q) * cc[G - 1]);
+                        double tj = q->t;
+                        if (typ > 0) tj = q->t - log(draw(p, q)) / in->decay[mat * J + typ - 1];
+                        double xi1 = draw(p, q), xi2 = draw(p, q), o[3];
+                        orc_iso_dir(xi1, xi2, o);
+                        if (!(tj < in->t_edges[in->n_t])) continue;
+                        particle c = *q; /* same position, cell and weight as the parent */
+                        c.ux = o[0]; c.uy = o[1]; c.uz = o[2]; c.g = gj; c.t = tj;
+                        c.tbin = edge_bin(in->t_edges, in->n_t, tj);
+                        c.id = orc_child_id(p->seed, q->id, ctr_birth, (uint32_t)j);
+                        c.ctr = 0; c.nseg = 0; c.last_surf = -1; c.alive = 1; c.resumed = 0;
+                        if (c.tbin == q->tbin) push_secondary(p, &c); else push_census(p, c.tbin, &c);
+                        p->counters[11]++;
+                    }
+                    p->balance[1] += q->w;
+                    q->alive = 0;
                 } else if (uu < sig_s + sig_f) {
                     ev = ORC_EV_FISSION;
                     int n = (int)floor(q->w * in->nu[mat * G + q->g] / p->k_prev + draw(p, q));
@@ -914,7 +988,7 @@ static void transport(orc_problem *p, particle *q)
                 int32_t jx = INNER(loc[1]) % in->lat2_nx[k2], jy = INNER(loc[1]) / in->lat2_nx[k2];
                 if (w == 0) jx--; else if (w == 1) jx++; else if (w == 2) jy--; else jy++;
                 int32_t inner = jy * in->lat2_nx[k2] + jx;
-                q->elem = OUTER(loc[1]) | ((inner + 1) << 16);
+                q->elem = OUTER(loc[1]) | ((inner + 1) << 20);
                 q->last_surf = -1;
                 double xn[3] = {q->x, q->y, q->z}, xl[3];
                 local_coords(p, q->elem, xn, xl);
@@ -976,6 +1050,13 @@ static void transport(orc_problem *p, particle *q)
             q->last_surf = -1; /* R11: the particle has moved off the surface it sat on */
             if (q->tbin == in->n_t) { ev = ORC_EV_CUTOFF; p->balance[3] += q->w; q->alive = 0; } else ev = ORC_EV_TIME_EDGE;
             trace(p, q, ev, loc[0], loc[1], loc[2], -1, gi, d, E_flight);
+            if (ev == ORC_EV_TIME_EDGE && p->census_stop) { /* the census: the particle waits in the next interval's bank */
+                p->counters[ev]++;
+                q->nseg++;
+                q->resumed = 1;
+                push_census(p, q->tbin, q);
+                return;
+            }
         }
         p->counters[ev]++;
         q->nseg++;
@@ -1005,6 +1086,7 @@ static int sample_source(orc_problem *p, particle *q)
     if (in->mode == 0) {
         q->g = pick(p->src_cum, in->G, xi[5] * p->src_cum[in->G - 1]);
         q->E = 0.0; q->t = 0.0; q->tbin = 0;
+        if (in->td) { q->t = in->src_t; q->tbin = edge_bin(in->t_edges, in->n_t, q->t); }
     } else {
         q->g = 0; q->E = in->src_E; q->t = in->src_t;
         q->tbin = edge_bin(in->t_edges, in->n_t, q->t);
@@ -1196,6 +1278,118 @@ int orc_run_fixed_source(orc_problem *p, uint64_t N, uint64_t seed)
     if (p->error == -3) return p->error;
     accumulate_cycle(p, N, 1);
     return p->error;
+}
+
+/* Population control at a census by combing (R40): the M particles of the bank in bank order (sorted by id), weights
+ * w_i, running sums C_i; N teeth at (xi + j) W / N; a particle gets one copy per tooth in [C_{i-1}, C_i), each of
+ * weight W / N: the total weight is conserved exactly and the population becomes exactly N. */
+double orc_comb(const double *w, uint64_t M, uint64_t N, double xi, uint32_t *copies)
+{
+    double W = 0.0;
+    for (uint64_t i = 0; i < M; i++) W += w[i];
+    double delta = W / (double)N, off = xi * delta, C = 0.0;
+    uint64_t j = 0;
+    for (uint64_t i = 0; i < M; i++) {
+        double hi = C + w[i];
+        copies[i] = 0;
+        while (j < N && off + (double)j * delta < hi) { copies[i]++; j++; }
+        C = hi;
+    }
+    if (M > 0) { copies[M - 1] += (uint32_t)(N - j); } /* a last tooth lost to rounding stays with the last particle */
+    return delta;
+}
+
+static int cmp_particle_id(const void *a, const void *b)
+{
+    uint64_t x = ((const particle *)a)->id, y = ((const particle *)b)->id;
+    return x < y ? -1 : (x > y ? 1 : 0);
+}
+
+/* Time-dependent multi-group fixed source (R38-R40), census interval by census interval: the particles of interval k
+ * are the source particles born in it, the survivors of interval k-1 and the delayed neutrons emitted in it; sorted by
+ * id, combed to census_target particles if population control is on (k > first interval), then each followed to its
+ * death or to the next time edge, its same-interval secondaries depth-first. */
+int orc_run_td(orc_problem *p, uint64_t N, uint64_t seed)
+{
+    const orc_input *in = &p->in;
+    if (in->mode != 0 || !in->td) return -1;
+    int64_t nt = orc_n_tally(p);
+    reset_results(p, 1);
+    p->seed = seed; p->fixed = 1; p->k_prev = 1.0; p->cycle = 0;
+    memset(p->flux_c, 0, (size_t)nt * sizeof(double));
+    p->k_num = 0.0; p->leak_c = 0.0; p->n_stack = 0;
+    p->census_stop = 1;
+    p->n_census = 0;
+    for (int k = 0; k <= in->n_t; k++) p->n_cbank[k] = 0;
+    int first = edge_bin(in->t_edges, in->n_t, in->src_t);
+    for (uint64_t i = 0; i < N; i++) { /* the source particles wait for their interval like everybody else */
+        particle q;
+        memset(&q, 0, sizeof q);
+        q.id = i; q.w = 1.0;
+        sample_source(p, &q);
+        place(p, &q);
+        if (q.alive) push_census(p, q.tbin, &q); else p->counters[0]++;
+    }
+    for (int k = first; k < in->n_t && p->error != -3; k++) {
+        uint64_t M = p->n_cbank[k];
+        particle *B = p->cbank[k];
+        qsort(B, (size_t)M, sizeof(particle), cmp_particle_id);
+        double W = 0.0;
+        for (uint64_t i = 0; i < M; i++) W += B[i].w;
+        if (p->n_census < 64) { p->census_counts[2 * p->n_census] = M; p->census_weights[2 * p->n_census] = W; }
+        particle *run = B;
+        uint64_t n_run = M;
+        if (in->census_target > 0 && k > first && M > 0) {
+            uint64_t T = (uint64_t)in->census_target;
+            double *w = (double *)malloc((size_t)M * sizeof(double));
+            uint32_t *copies = (uint32_t *)malloc((size_t)M * sizeof(uint32_t));
+            for (uint64_t i = 0; i < M; i++) w[i] = B[i].w;
+            double xi = orc_draw(seed, (uint64_t)k, 3u, 0u, 0u); /* the comb's own stream: domain 3, id = interval */
+            double delta = orc_comb(w, M, T, xi, copies);
+            run = (particle *)malloc((size_t)T * sizeof(particle));
+            n_run = 0;
+            for (uint64_t i = 0; i < M; i++)
+                for (uint32_t c = 0; c < copies[i]; c++) {
+                    particle q = B[i];
+                    q.w = delta;
+                    /* every copy is a new track with a stream of its own: id from the domain-2 block
+                     * (parent id, interval, copy index) */
+                    uint32_t ctr[4] = {(uint32_t)B[i].id, (uint32_t)(B[i].id >> 32), (2u << 24) | (uint32_t)k, c};
+                    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+                    uint32_t o[4];
+                    orc_philox4x32_10(ctr, key, o);
+                    q.id = ((uint64_t)o[1] << 32) | o[0];
+                    q.ctr = 0; q.nseg = 0; q.resumed = 1;
+                    run[n_run++] = q;
+                }
+            free(w); free(copies);
+            W = delta * (double)n_run;
+        }
+        if (p->n_census < 64) { p->census_counts[2 * p->n_census + 1] = n_run; p->census_weights[2 * p->n_census + 1] = W; p->n_census++; }
+        for (uint64_t i = 0; i < n_run; i++) {
+            particle q = run[i];
+            transport(p, &q);
+            while (p->n_stack > 0) {
+                /* R25a with population control: the comb re-seeds every interval with census_target particles */
+                if (p->counters[11] > 64 * (N + (uint64_t)in->census_target * (uint64_t)in->n_t) + 4096) { p->error = -3; p->n_stack = 0; break; }
+                particle c = p->stack[--p->n_stack];
+                transport(p, &c);
+            }
+            if (p->error == -3) break;
+        }
+        if (run != B) free(run);
+    }
+    p->census_stop = 0;
+    if (p->error == -3) return p->error;
+    accumulate_cycle(p, N, 1);
+    return p->error;
+}
+
+int orc_get_census(const orc_problem *p, uint64_t *counts, double *weights, int max_intervals)
+{
+    int n = p->n_census < max_intervals ? p->n_census : max_intervals;
+    for (int i = 0; i < 2 * n; i++) { counts[i] = p->census_counts[i]; weights[i] = p->census_weights[i]; }
+    return n;
 }
 
 int orc_get_results(const orc_problem *p, double *k_cycle, double *k_mean, double *k_sdev, double *flux_mean,

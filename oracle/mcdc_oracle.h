@@ -77,6 +77,15 @@ typedef struct {
     /* implicit capture / survival biasing with weight roulette (R36) */
     int32_t implicit_capture;
     double w_roulette, w_survive;
+    /* time-dependent multi-group with delayed-neutron precursors and census population control (R38-R40;
+     * PAPER.md:31 "fully dynamic simulations"): td != 0 switches it on for a multi-group problem.  speed[G] cm/s;
+     * n_dgroup precursor groups per material: nu_d[n_mat][n_dgroup][G] delayed yields (nu above = the prompt yield),
+     * decay[n_mat][n_dgroup] 1/s, chi_d[n_mat][n_dgroup][G] emission spectra; time edges t_edges[n_t+1] above (every
+     * edge is a census); census_target > 0: the population entering each census interval but the first is combed to
+     * that many particles. */
+    int32_t td, n_dgroup;
+    const double *speed, *nu_d, *decay, *chi_d;
+    int64_t census_target;
 } orc_input;
 
 typedef struct {
@@ -106,6 +115,14 @@ int orc_run_eigenvalue(orc_problem *p, uint64_t n_particles, int n_inactive, int
 /* all-core timing variant (bench.py cpu_baseline): n_threads contiguous id ranges, joined in thread order */
 int orc_run_eigenvalue_mt(orc_problem *p, uint64_t n_particles, int n_inactive, int n_active, uint64_t seed, int n_threads);
 int orc_run_fixed_source(orc_problem *p, uint64_t n_particles, uint64_t seed);
+/* time-dependent multi-group fixed source (td != 0), census interval by census interval (R38-R40) */
+int orc_run_td(orc_problem *p, uint64_t n_particles, uint64_t seed);
+/* population entering each census interval of the last orc_run_td: out[2k] = particles before, out[2k+1] after the
+ * comb (equal without population control); weights[2k], [2k+1] = their total weights; returns the number of intervals */
+int orc_get_census(const orc_problem *p, uint64_t *counts, double *weights, int max_intervals);
+/* the comb itself (R40) on plain arrays: M weights in bank order, N teeth, offset draw xi in (0,1): copies[i] = number
+ * of teeth that fall on particle i; returns the tooth spacing */
+double orc_comb(const double *w, uint64_t M, uint64_t N, double xi, uint32_t *copies);
 /* results; arrays sized by the caller: k_cycle[n_cycles], flux_*[n_tally], counters[ORC_N_COUNTERS] */
 int64_t orc_n_tally(const orc_problem *p);
 int orc_get_results(const orc_problem *p, double *k_cycle, double *k_mean, double *k_sdev, double *flux_mean,

@@ -29,10 +29,13 @@ physics
              mat_nuc_off i32[nm+1], mat_nuc_id i32[], mat_nuc_dens f64[] (1/(b cm)),
              nu0, nu1 (nu = nu0 + nu1*E[MeV]), watt_a [MeV], watt_b [1/MeV],
              t_edges f64[nt+1] (s), e_edges f64[ne+1] (eV)
+  td (optional, mode 'mg'): time-dependent multi-group with delayed neutrons (run kind 'td'; tally flux[bin][time bin][g]):
+             dict(speed f64[G] cm/s, J precursor groups, nu_d f64[nm,J,G] delayed yields (mg_nu = prompt yield),
+             decay f64[nm,J] 1/s, chi_d f64[nm,J,G], census_target (0 = no population control)); t_edges f64[nt+1]
 source
   src_lo, src_hi f64[3]; src_iso (1/0); src_dir f64[3]; src_group_pdf f64[G] | src_E (eV); src_t (s)
 run
-  run: dict(kind 'eigen'|'fixed', n_particles, n_inactive, n_active, seed)
+  run: dict(kind 'eigen'|'fixed'|'td', n_particles, n_inactive, n_active, seed)
 """
 from __future__ import annotations
 
@@ -563,6 +566,49 @@ def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform
     P.update(_src([0, 0, 0], [side, side, 0.9 * height if height else 0], G=G, pdf=mats[0]["chi"]))
     P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
     P["name"] = "C4"
+    return P
+
+
+# --------------------------------------------------------------------------- time-dependent multi-group
+def td_infinite(n_particles=20_000, seed=47, G=1, J=1, t_end=4.0e-3, n_t=8, census_target=0, geom="cube"):
+    """Infinite homogeneous medium (reflecting unit cube) with delayed neutrons, a pulse of neutrons at t = 0:
+    the kinetics problem whose expected flux per time bin is a linear ODE solution (tests integrate it).
+    G = 1, J = 1: Sigma_t 1.0, Sigma_s 0.5, Sigma_f 0.2, prompt yield 2.3, delayed yield 0.15 (k = 0.98, prompt
+    k = 0.92), decay 500 /s, speed 1e5 cm/s.  G = 2, J = 2: a fast and a slow group with down- and up-scatter, two
+    precursor groups with different spectra.  geom 'pin': the same materials in the C3 pin cell (fuel = the medium,
+    moderator = its non-fissile twin) for the geometry-coupled parity cases."""
+    if G == 1:
+        sig_t, S, sig_f = np.array([1.0]), np.array([[0.5]]), np.array([0.2])
+        nu_p, speed = np.array([2.3]), np.array([1.0e5])
+        nu_d, decay, chi_d = np.array([[0.15]]), np.array([500.0]), np.array([[1.0]])
+        chi = np.array([1.0])
+    else:
+        assert G == 2
+        sig_t, S = np.array([0.8, 1.6]), np.array([[0.30, 0.25], [0.05, 0.95]])
+        sig_f, nu_p = np.array([0.05, 0.30]), np.array([2.5, 2.2])
+        speed = np.array([4.0e5, 1.0e5])
+        nu_d, decay = np.array([[0.10, 0.08], [0.06, 0.05]]), np.array([300.0, 2500.0])
+        chi, chi_d = np.array([0.9, 0.1]), np.array([[0.3, 0.7], [0.6, 0.4]])
+    J = nu_d.shape[0]
+    mat = dict(sig_t=sig_t, S=S, sig_f=sig_f, nu=nu_p, chi=chi, sig_c=sig_t - S.sum(1) - sig_f)
+    mats = [mat]
+    td = dict(speed=speed, J=J, nu_d=nu_d[None], decay=decay[None], chi_d=chi_d[None], census_target=int(census_target))
+    if geom == "cube":
+        P = geom_box([0, 0, 0], [1, 1, 1], REFLECT)
+        lo, hi = [0, 0, 0], [1, 1, 1]
+    else:
+        P = geom_pincell()
+        mod = dict(sig_t=sig_t * 1.3, S=S * 1.5, sig_f=sig_f * 0.0, nu=nu_p, chi=chi, sig_c=sig_t * 1.3 - (S * 1.5).sum(1))
+        mats = [mat, mod]
+        td = dict(speed=speed, J=J, nu_d=np.stack([nu_d, nu_d * 0.0]), decay=np.stack([decay, decay]),
+                  chi_d=np.stack([chi_d, chi_d]), census_target=int(census_target))
+        lo, hi = [-0.63, -0.63, 0], [0.63, 0.63, 0]
+    P.update(_mg_pack(mats))
+    P.update(_src(lo, hi, G=G, pdf=chi))
+    P["td"] = td
+    P["t_edges"] = np.linspace(0.0, t_end, n_t + 1)
+    P["run"] = dict(kind="td", n_particles=n_particles, n_inactive=0, n_active=1, seed=seed)
+    P["name"] = f"td_{geom}_G{G}"
     return P
 
 

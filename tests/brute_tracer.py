@@ -157,7 +157,7 @@ class World:
                 return None
             x2 = [xl[0] - (x0 + (jx + 0.5) * px), xl[1] - (y0 + (jy + 0.5) * py), xl[2]]
             c2 = self._cell_in(un[jy][jx], x2)
-            return None if c2 < 0 else (c0, elem | ((jy * nx + jx + 1) << 16), c2)
+            return None if c2 < 0 else (c0, elem | ((jy * nx + jx + 1) << 20), c2)
         return (c0, elem, c1)
 
     def material(self, loc):
@@ -166,7 +166,7 @@ class World:
     def spatial_bin(self, loc):
         b = int(self.P["cell_bin"][loc[2] if loc[1] >= 0 else loc[0]])
         if loc[1] >= 0:
-            outer, inner = loc[1] & 0xFFFF, (loc[1] >> 16) - 1
+            outer, inner = loc[1] & 0xFFFFF, (loc[1] >> 20) - 1
             b += int(self.lat["bin"].ravel()[outer])
             if inner >= 0:
                 nx, _, _, _, _, _, _, bn = self._lat2_of(self.univ[outer // self.nx][outer % self.nx])[1]
@@ -250,7 +250,7 @@ class World:
     def reflect(self, s, x, u, loc):
         xl = list(x)
         if loc[1] >= 0 and not self._surface_of_root(s):
-            ix, iy = (loc[1] & 0xFFFF) % self.nx, (loc[1] & 0xFFFF) // self.nx
+            ix, iy = (loc[1] & 0xFFFFF) % self.nx, (loc[1] & 0xFFFFF) // self.nx
             xl = [x[0] - (self.x0 + (ix + 0.5) * self.px), x[1] - (self.y0 + (iy + 0.5) * self.py), x[2]]
         n = _normal(self.st[s], self.sq[s], xl)
         dot = sum(u[i] * n[i] for i in range(3))

@@ -11,8 +11,8 @@ from tests.test_oracle_traces import _compare
 
 
 def _flat_elem(packed, n_outer, n_pin):
-    """flat-lattice element index of a two-level (outer | (inner + 1) << 16) location"""
-    outer, inner = packed & 0xFFFF, (packed >> 16) - 1
+    """flat-lattice element index of a two-level (outer | (inner + 1) << 20) location"""
+    outer, inner = packed & 0xFFFFF, (packed >> 20) - 1
     ax, ay = outer % n_outer, outer // n_outer
     px, py = inner % n_pin, inner // n_pin
     return (ay * n_pin + py) * (n_outer * n_pin) + ax * n_pin + px
@@ -65,7 +65,7 @@ def test_trace_two_level_vs_brute_force(orc, case):
     tr = _compare(orc, P, 50, 50)
     ns = len(P["surf_type"])
     assert ((tr["ev"] == 7) & (tr["surf"] >= ns + 4)).sum() >= 30 and ((tr["ev"] == 7) & (tr["surf"] < ns + 4)).sum() >= 5
-    assert (tr["elem"] >> 16).max() >= 1
+    assert (tr["elem"] >> 20).max() >= 1
     if case.startswith("gap"):
         mid = {5, 6, 7, 8}  # the four planes that bound the pin lattice inside the assembly
         assert np.isin(tr["surf"][tr["ev"] == 4], list(mid)).sum() >= 20
