@@ -44,12 +44,21 @@ enum { MCDC_EV_SCATTER = 1, MCDC_EV_FISSION, MCDC_EV_CAPTURE, MCDC_EV_TRANSMIT, 
  * from its work queue, [15] reserved */
 #define MCDC_N_COUNTERS 16
 
-/* CSG geometry: at most 3800 surfaces, conjunctive cells grouped by universe, one optional rectangular lattice
- * (R11-R16).  surf_param[s][4]: PLANE_X/Y/Z (p,-,-,-); PLANE (a,b,c,d): a x+b y+c z = d; CYL_Z (x0,y0,r,-)
+/* CSG geometry: at most 3800 surfaces, conjunctive cells grouped by universe, one optional rectangular lattice whose
+ * elements may themselves hold second-level lattices (R11-R16, R37).  surf_param[s][4]: PLANE_X/Y/Z (p,-,-,-); PLANE (a,b,c,d): a x+b y+c z = d; CYL_Z (x0,y0,r,-)
  * (CYL_X (y0,z0,r), CYL_Y (x0,z0,r)); SPHERE (x0,y0,z0,r).  Cells of universe u are
  * [univ_cell_off[u], univ_cell_off[u+1]); universe 0 is the root.  cell_fill_type 0: cell_fill = material
  * id; 1: the cell is filled by the lattice (at most one such cell, in the root universe).  lat_univ[iy][ix]
- * names the universe of element (ix,iy); its cells are written in element-centred coordinates. */
+ * names the universe of element (ix,iy); its cells are written in element-centred coordinates.
+ * Second-level lattices (a core of assemblies of pin lattices; R37): cell_fill_type 2 = the
+ * cell, which must belong to a universe used by lattice elements, is filled by second-level lattice k = cell_fill:
+ * lat2_nx[k] x lat2_ny[k] elements of pitch lat2_px[k], lat2_py[k], centred on the origin of that universe's
+ * coordinates; element (ix,iy) holds universe lat2_univ[lat2_off[k] + iy lat2_nx[k] + ix], whose cells (material-
+ * filled only) are written in coordinates centred on the element.  At most one such cell per universe.  The
+ * first-level lattice has at most 2^20 elements, a second-level one at most 2047.
+ * A location inside lattices is reported (traces, mcdc_test_geometry) as first-level element | (second-level element
+ * + 1) << 20; lattice-wall hit codes are n_surf + 0..3 (first level: -x,+x,-y,+y) and n_surf + 4..7 (second level).
+ * A lattice's outermost lines are never events: the enclosing cell's surfaces, or the first-level walls, bound it. */
 typedef struct {
     int32_t n_surf;
     const int32_t *surf_type;
@@ -67,13 +76,35 @@ typedef struct {
     double lat_x0, lat_y0, lat_px, lat_py;
     int32_t lat_nx, lat_ny;
     const int32_t *lat_univ; /* [lat_ny][lat_nx] */
+    int32_t n_lat2;          /* second-level lattices (0: none; the pointers below may then be NULL) */
+    const int32_t *lat2_nx, *lat2_ny;
+    const double *lat2_px, *lat2_py;
+    const int32_t *lat2_off;  /* [n_lat2+1] */
+    const int32_t *lat2_univ; /* [lat2_off[n_lat2]] */
 } mcdc_geometry;
 
+/* time-dependent multi-group data ("fully dynamic simulations"; R38-R40):
+ * speed[G] cm/s; n_dgroup delayed-neutron precursor groups per material with yields nu_d[n_mat][n_dgroup][G] (the
+ * materials' nu is then the PROMPT yield), decay constants decay[n_mat][n_dgroup] 1/s and emission spectra
+ * chi_d[n_mat][n_dgroup][G].  The time edges are mcdc_tally_spec.t_edges; every edge is a census.  census_target > 0:
+ * the population entering every census interval but the first is combed to that many particles (weight-conserving
+ * population control). */
+typedef struct {
+    const double *speed;
+    int32_t n_dgroup;
+    int32_t pad;
+    const double *nu_d, *decay, *chi_d;
+    int64_t census_target;
+} mcdc_kinetics;
+
 /* multi-group materials (R3-R5, R30): arrays [n_mat][G]; S[n_mat][G][G], row = incident group.
- * Sigma_s = row sum of S; Sigma_c = Sigma_t - Sigma_s - Sigma_f.  Pass NULL for a continuous-energy problem. */
+ * Sigma_s = row sum of S; Sigma_c = Sigma_t - Sigma_s - Sigma_f.  Pass NULL for a continuous-energy problem.
+ * kinetics != NULL makes the problem a time-dependent fixed-source one (mcdc_run_fixed_source / mcdc_run_cycle);
+ * NULL: k-eigenvalue problem. */
 typedef struct {
     int32_t n_mat, G;
     const double *sig_t, *sig_f, *nu, *chi, *S;
+    const mcdc_kinetics *kinetics;
 } mcdc_materials;
 
 /* continuous-energy data (R19-R23): union grid [n_grid] (eV, strictly increasing), microscopic elastic /
@@ -106,15 +137,17 @@ typedef struct {
 } mcdc_source;
 
 /* track-length flux tally (R17, R24): spatial bin of a particle = cell_bin[cell] (+ lat_bin[element] inside
- * the lattice); MG: flux[bin][g]; CE: flux[bin][time bin][energy bin] with explicit edges. */
+ * the lattice, + lat2_bin[lat2_off[k] + element] inside second-level lattice k); MG: flux[bin][g]; CE: flux[bin][time
+ * bin][energy bin] with explicit edges; time-dependent MG: flux[bin][time bin][g]. */
 typedef struct {
     int32_t n_bins;
     const int32_t *cell_bin; /* [n_cell] */
     const int32_t *lat_bin;  /* [lat_ny][lat_nx] or NULL */
     int32_t n_t;
-    const double *t_edges; /* [n_t+1], CE only */
+    const double *t_edges; /* [n_t+1], CE and time-dependent MG */
     int32_t n_e;
     const double *e_edges; /* [n_e+1], CE only */
+    const int32_t *lat2_bin; /* [lat2_off[n_lat2]] or NULL */
 } mcdc_tally_spec;
 
 /* device resources handed in by the caller.
@@ -187,8 +220,13 @@ int mcdc_create(const mcdc_geometry *geo, const mcdc_materials *mat, const mcdc_
  * histories; cycle 0 samples the source, later cycles start from the fission bank with weight N/M. */
 int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, int32_t n_inactive, int32_t n_active, uint64_t seed);
 
-/* one power-iteration cycle (cycle 0 resets the run and samples the source); returns the cycle's
- * track-length k.  active != 0 accumulates the flux / leakage / k statistics. */
+/* Eigenvalue problem: one power-iteration cycle (cycle 0 resets the run and samples the source); returns the cycle's
+ * track-length k.  active != 0 accumulates the flux / leakage / k statistics.
+ * Fixed-source problem (continuous energy or time-dependent multi-group): `cycle` = a census interval (time edge cycle
+ * -> cycle + 1): the interval that holds the source time resets the run and samples the source; every later call must
+ * name the next interval and starts from the census bank the previous call left (the particles that reached the time
+ * edge, and delayed neutrons emitted in that interval), sorted by particle id and, with census_target > 0, combed.
+ * Intervals called in order to the last one give the tallies of mcdc_run_fixed_source.  `active` is ignored. */
 int mcdc_run_cycle(mcdc_problem *p, uint64_t n_particles, uint32_t cycle, int32_t active, uint64_t seed,
                    double *k_cycle);
 
@@ -199,8 +237,9 @@ int mcdc_run_cycle_host(mcdc_problem *p, uint64_t n_particles, uint32_t cycle, u
                         const mcdc_site *sites_in, uint64_t n_in, mcdc_site *sites_out, uint64_t max_out,
                         uint64_t *n_out, double *flux_cycle, double *k_cycle, double *leak_cycle);
 
-/* time-dependent fixed source, continuous energy (R24, R25): n_particles source particles and
- * all their prompt fission secondaries, to the last time edge. */
+/* time-dependent fixed source (R24, R25): n_particles source particles and all their fission secondaries,
+ * to the last time edge.  Continuous energy: one persistent launch (a census is a synchronisation point only).
+ * Time-dependent multi-group: census interval by census interval (population control happens between them). */
 int mcdc_run_fixed_source(mcdc_problem *p, uint64_t n_particles, uint64_t seed);
 
 /* Physics options beyond the analog target-at-rest model ("free-gas scattering model
@@ -224,6 +263,10 @@ int mcdc_set_physics(mcdc_problem *p, const mcdc_physics *phys);
  * [2] leaked, [3] cut off at the last time edge, [4] killed by roulette, [5] gained by roulette survivors.
  * out[0] = out[1] + out[2] + out[3] + out[4] - out[5] up to rounding. */
 int mcdc_get_balance(const mcdc_problem *p, double out[6]);
+
+/* population entering each census interval of the last fixed-source run made interval by interval: counts[2k] particles
+ * before and counts[2k+1] after the comb, weights[2k], [2k+1] their total weights; *n = intervals reported (<= max) */
+int mcdc_get_census(const mcdc_problem *p, uint64_t *counts, double *weights, int32_t max, int32_t *n);
 
 int mcdc_get_dims(const mcdc_problem *p, mcdc_dims *dims);
 int mcdc_get_tallies(const mcdc_problem *p, mcdc_tallies *out);

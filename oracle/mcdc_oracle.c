@@ -898,7 +898,13 @@ static void transport(orc_problem *p, particle *q)
                         c.tbin = edge_bin(in->t_edges, in->n_t, tj);
                         c.id = orc_child_id(p->seed, q->id, ctr_birth, (uint32_t)j);
                         c.ctr = 0; c.nseg = 0; c.last_surf = -1; c.alive = 1; c.resumed = 0;
-                        if (c.tbin == q->tbin) push_secondary(p, &c); else push_census(p, c.tbin, &c);
+                        if (c.tbin == q->tbin) push_secondary(p, &c);
+                        else { /* waits for a later interval, where the comb may replace it: count the track now */
+                            c.resumed = 1;
+                            p->counters[0]++;
+                            p->balance[0] += c.w;
+                            push_census(p, c.tbin, &c);
+                        }
                         p->counters[11]++;
                     }
                     p->balance[1] += q->w;

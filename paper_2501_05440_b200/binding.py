@@ -15,7 +15,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 _SO = os.path.join(_HERE, "libmcdc_b200.so")
-_SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cuh", "mcdc_device.cuh", "mcdc_microbench.cuh")]
+_SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cuh", "mcdc_device.cuh", "mcdc_census.cuh",
+                                                   "mcdc_microbench.cuh")]
 _HDR = os.path.join(_ROOT, "include", "mcdc.h")
 
 N_COUNTERS = 16
@@ -26,7 +27,7 @@ SYMBOLS = ["mcdc_workspace_bytes", "mcdc_create", "mcdc_run_eigenvalue", "mcdc_r
            "mcdc_run_fixed_source", "mcdc_get_dims", "mcdc_get_tallies", "mcdc_get_bank", "mcdc_set_trace",
            "mcdc_get_trace", "mcdc_test_draws", "mcdc_test_grid_index", "mcdc_test_geometry", "mcdc_get_timing",
            "mcdc_set_profile", "mcdc_get_profile", "mcdc_microbench", "mcdc_destroy", "mcdc_last_error",
-           "mcdc_set_physics", "mcdc_get_balance"]
+           "mcdc_set_physics", "mcdc_get_balance", "mcdc_get_census"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -43,12 +44,19 @@ class Geometry(C.Structure):
                 ("n_cell", C.c_int32), ("cell_surf_off", _ip), ("cell_surf_id", _ip), ("cell_surf_sense", _ip),
                 ("cell_fill_type", _ip), ("cell_fill", _ip), ("n_univ", C.c_int32), ("univ_cell_off", _ip),
                 ("has_lattice", C.c_int32), ("lat_x0", C.c_double), ("lat_y0", C.c_double), ("lat_px", C.c_double),
-                ("lat_py", C.c_double), ("lat_nx", C.c_int32), ("lat_ny", C.c_int32), ("lat_univ", _ip)]
+                ("lat_py", C.c_double), ("lat_nx", C.c_int32), ("lat_ny", C.c_int32), ("lat_univ", _ip),
+                ("n_lat2", C.c_int32), ("lat2_nx", _ip), ("lat2_ny", _ip), ("lat2_px", _dp), ("lat2_py", _dp),
+                ("lat2_off", _ip), ("lat2_univ", _ip)]
+
+
+class Kinetics(C.Structure):
+    _fields_ = [("speed", _dp), ("n_dgroup", C.c_int32), ("pad", C.c_int32), ("nu_d", _dp), ("decay", _dp), ("chi_d", _dp),
+                ("census_target", C.c_int64)]
 
 
 class Materials(C.Structure):
     _fields_ = [("n_mat", C.c_int32), ("G", C.c_int32), ("sig_t", _dp), ("sig_f", _dp), ("nu", _dp), ("chi", _dp),
-                ("S", _dp)]
+                ("S", _dp), ("kinetics", C.POINTER(Kinetics))]
 
 
 class XS(C.Structure):
@@ -65,7 +73,7 @@ class Source(C.Structure):
 
 class TallySpec(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("cell_bin", _ip), ("lat_bin", _ip), ("n_t", C.c_int32), ("t_edges", _dp),
-                ("n_e", C.c_int32), ("e_edges", _dp)]
+                ("n_e", C.c_int32), ("e_edges", _dp), ("lat2_bin", _ip)]
 
 
 class Device(C.Structure):
@@ -145,6 +153,7 @@ def load_library():
     L.mcdc_microbench.argtypes = [vp, i32, u64, _dp, _dp]
     L.mcdc_set_physics.argtypes = [vp, P(Physics)]
     L.mcdc_get_balance.argtypes = [vp, _dp]
+    L.mcdc_get_census.argtypes = [vp, P(u64), _dp, i32, P(i32)]
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -206,6 +215,11 @@ class Problem:
             g.lat_x0, g.lat_y0, g.lat_px, g.lat_py = lat["x0"], lat["y0"], lat["px"], lat["py"]
             g.lat_nx, g.lat_ny, g.lat_univ = lat["nx"], lat["ny"], ip(lat["univ"])
             t.lat_bin = ip(lat["bin"])
+        if "lat2_nx" in P:
+            g.n_lat2 = len(P["lat2_nx"])
+            g.lat2_nx, g.lat2_ny, g.lat2_off = ip(P["lat2_nx"]), ip(P["lat2_ny"]), ip(P["lat2_off"])
+            g.lat2_px, g.lat2_py, g.lat2_univ = dp(P["lat2_px"]), dp(P["lat2_py"]), ip(P["lat2_univ"])
+            t.lat2_bin = ip(P["lat2_bin"])
         s = Source()
         s.lo = (C.c_double * 3)(*P["src_lo"])
         s.hi = (C.c_double * 3)(*P["src_hi"])
@@ -218,6 +232,15 @@ class Problem:
             m.n_mat, m.G = int(P["n_mat"]), int(P["G"])
             m.sig_t, m.sig_f, m.nu, m.chi, m.S = dp(P["mg_sig_t"]), dp(P["mg_sig_f"]), dp(P["mg_nu"]), dp(P["mg_chi"]), dp(P["mg_S"])
             s.group_pdf = dp(P["src_group_pdf"])
+            td = P.get("td")
+            if td:  # time-dependent multi-group: speeds, delayed-neutron data; the time edges go with the tally
+                kn = Kinetics()
+                kn.speed, kn.n_dgroup = dp(td["speed"]), int(td["J"])
+                kn.nu_d, kn.decay, kn.chi_d = dp(td["nu_d"]), dp(td["decay"]), dp(td["chi_d"])
+                kn.census_target = int(td.get("census_target", 0))
+                self._keep.append(kn)
+                m.kinetics = C.pointer(kn)
+                t.n_t, t.t_edges = len(P["t_edges"]) - 1, dp(P["t_edges"])
         else:
             x = XS()
             x.n_mat, x.n_grid, x.grid = int(P["n_mat"]), len(P["grid"]), dp(P["grid"])
@@ -280,6 +303,13 @@ class Problem:
         self._check(self.L.mcdc_get_balance(self.h, out.ctypes.data_as(_dp)))
         return dict(zip(("source", "absorbed", "leaked", "cutoff", "roulette_loss", "roulette_gain"), out))
 
+    def census(self):
+        """Population entering each census interval of the last run made interval by interval:
+        (particles before the comb, after it, weight before, weight after) per interval."""
+        cnt, w, n = np.zeros(128, np.uint64), np.zeros(128), C.c_int32()
+        self._check(self.L.mcdc_get_census(self.h, cnt.ctypes.data_as(C.POINTER(C.c_uint64)), w.ctypes.data_as(_dp), 64, C.byref(n)))
+        return [(int(cnt[2 * k]), int(cnt[2 * k + 1]), float(w[2 * k]), float(w[2 * k + 1])) for k in range(n.value)]
+
     # ---- runs
     def run(self, n_particles=None, n_inactive=None, n_active=None, seed=None):
         r = self.P["run"]
@@ -289,7 +319,7 @@ class Problem:
         sd = int(seed if seed is not None else r["seed"])
         if r["kind"] == "eigen":
             self._check(self.L.mcdc_run_eigenvalue(self.h, N, ni, na, sd))
-        else:
+        else:  # "fixed" (continuous energy) and "td" (time-dependent multi-group)
             self._check(self.L.mcdc_run_fixed_source(self.h, N, sd))
         return self.results()
 

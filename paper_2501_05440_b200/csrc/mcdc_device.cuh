@@ -43,7 +43,17 @@ struct Geo {
                             // cylinder (or -1); z = cell inside it (or the only cell); w = cell outside it
     const double *ap_pos;   // [n_ap] position of axis plane j
     const int *ap_sid;      // [n_ap] its surface id
+    // Second-level lattices (R37): lattice k fills the cell umid[u] (fill type 2, cfill = k) of universe u, centred on
+    // the origin of u's coordinates.  A location packs (first-level element | (second-level element + 1) << 20); a
+    // first-level element that holds a second-level lattice is never LAT_FAST (generic geometry path).
+    int n_lat2;
+    const int *l2_nx, *l2_ny, *l2_off, *l2_univ, *l2_bin, *umid;
+    const double *l2_px, *l2_py;
 };
+constexpr int INNER_SHIFT = 20;
+constexpr int HIT_BITS = 12;  // hit codes (surfaces, lattice walls) are below PEND_SCATTER < 2^12
+__device__ __forceinline__ int outer_of(const Geo &, int elem) { return elem & ((1 << INNER_SHIFT) - 1); }
+__device__ __forceinline__ int inner_of(const Geo &, int elem) { return (elem >> INNER_SHIFT) - 1; }
 constexpr int LAT_FAST = 1 << 30, CELL_FAST = 1 << 30, CELL_NO_NEIGHBOUR = (1 << 30) - 1;
 
 struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi running chi sums.  One contiguous
@@ -89,6 +99,14 @@ struct FisRec {
     uint64_t *id;
 };
 
+// Time-dependent multi-group (R38-R40): group speeds, cumulative fission yields [prompt, +delayed 1 .. +delayed J] per
+// (material, group), delayed emission spectra (running sums) and decay constants per (material, precursor group).
+// The time edges are CETab::t_edges / n_t for both energy treatments.
+struct TDTab {
+    int on, J;
+    const double *speed, *cum_nu, *cumchi_d, *decay;
+};
+
 struct QCount {  // one set per sweep (ring of RING)
     unsigned int n_scat, n_surf, n_alive, err;
 };
@@ -105,6 +123,9 @@ struct Ctx {
     MGTab mg;
     CETab ce;
     Bank bank[2];
+    Bank cbank;          // census bank (R40): particles that wait for a later census interval; count in work[4]
+    int census_stop;     // a particle that reaches a time edge (not the last) goes to the census bank instead of going on
+    TDTab td;
     FisRec fis;
     unsigned int cap;   // slots per bank
     int mode;           // 0 MG, 1 CE
@@ -374,6 +395,52 @@ __device__ __forceinline__ void local_xy(const Geo &G, int elem, double x, doubl
 
 __device__ __forceinline__ int elem_universe(const Geo &G, int elem) { return __ldg(&G.lat_info[elem].x) & (LAT_FAST - 1); }
 
+// second-level lattice k: lower-left corner in its universe's coordinates (centred on the origin, R37)
+__device__ __forceinline__ double l2_x0(const Geo &G, int k) { return -0.5 * (__ldg(G.l2_nx + k) * __ldg(G.l2_px + k)); }
+__device__ __forceinline__ double l2_y0(const Geo &G, int k) { return -0.5 * (__ldg(G.l2_ny + k) * __ldg(G.l2_py + k)); }
+
+// coordinates centred on element `inner` of second-level lattice k, from first-level-element coordinates (xo, yo)
+__device__ __forceinline__ void inner_xy(const Geo &G, int k, int inner, double xo, double yo, double &xl, double &yl)
+{
+    const int nx = __ldg(G.l2_nx + k);
+    const int jy = inner / nx, jx = inner - jy * nx;
+    xl = xo - (l2_x0(G, k) + (jx + 0.5) * __ldg(G.l2_px + k));
+    yl = yo - (l2_y0(G, k) + (jy + 0.5) * __ldg(G.l2_py + k));
+}
+
+// coordinates of the innermost lattice level of the packed location `elem`
+__device__ __forceinline__ void innermost_xy(const Geo &G, int elem, double x, double y, double &xl, double &yl)
+{
+    const int outer = outer_of(G, elem), inner = inner_of(G, elem);
+    local_xy(G, outer, x, y, xl, yl);
+    if (inner >= 0) {
+        const double xo = xl, yo = yl;
+        inner_xy(G, __ldg(G.cfill + __ldg(G.umid + elem_universe(G, outer))), inner, xo, yo, xl, yl);
+    }
+}
+
+// cell of first-level element `outer` that holds the point (xo, yo, z) given in that element's coordinates, descending
+// into a second-level lattice where one fills the cell; the second-level index is found by floor and clamped to the
+// lattice (R37).  elem = packed location; returns the material cell or -1.
+__device__ __forceinline__ int descend(const Geo &G, int outer, double xo, double yo, double z, double ux, double uy, double uz,
+                                       int last, int &elem)
+{
+    elem = outer;
+    int c = find_cell(G, elem_universe(G, outer), xo, yo, z, ux, uy, uz, last);
+    if (c < 0 || G.n_lat2 == 0 || __ldg(G.cft + c) != 2) return c;
+    const int k = __ldg(G.cfill + c);
+    const int nx = __ldg(G.l2_nx + k), ny = __ldg(G.l2_ny + k);
+    int jx = (int)floor((xo - l2_x0(G, k)) / __ldg(G.l2_px + k));
+    int jy = (int)floor((yo - l2_y0(G, k)) / __ldg(G.l2_py + k));
+    jx = jx < 0 ? 0 : (jx > nx - 1 ? nx - 1 : jx);
+    jy = jy < 0 ? 0 : (jy > ny - 1 ? ny - 1 : jy);
+    const int inner = jy * nx + jx;
+    double xl, yl;
+    inner_xy(G, k, inner, xo, yo, xl, yl);
+    elem = outer | ((inner + 1) << INNER_SHIFT);
+    return find_cell(G, __ldg(G.l2_univ + __ldg(G.l2_off + k) + inner), xl, yl, z, ux, uy, uz, last);
+}
+
 // full point location from the root universe.  cell = material cell (root cell, or the local cell inside
 // lattice element elem); returns false if the point is in no cell.
 __device__ __forceinline__ bool locate(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int last,
@@ -386,10 +453,9 @@ __device__ __forceinline__ bool locate(const Geo &G, double x, double y, double 
         int ix = (int)floor((x - G.lat_x0) / G.lat_px);
         int iy = (int)floor((y - G.lat_y0) / G.lat_py);
         if (ix < 0 || iy < 0 || ix >= G.lat_nx || iy >= G.lat_ny) { cell = -1; return false; }
-        elem = iy * G.lat_nx + ix;
         double xl, yl;
-        local_xy(G, elem, x, y, xl, yl);
-        cell = find_cell(G, elem_universe(G, elem), xl, yl, z, ux, uy, uz, last);
+        local_xy(G, iy * G.lat_nx + ix, x, y, xl, yl);
+        cell = descend(G, iy * G.lat_nx + ix, xl, yl, z, ux, uy, uz, last, elem);
         if (cell < 0) return false;
     }
     return true;
@@ -505,6 +571,106 @@ __device__ __noinline__ double nearest(const Geo &G, double x, double y, double 
     return best;
 }
 
+// nearest boundary of a location inside a second-level lattice (generic path only); candidate order: enclosing-cell surfaces, [surfaces of the
+// cell a second-level lattice fills,] local-cell surfaces, [second-level walls -x,+x,-y,+y,] first-level walls
+// -x,+x,-y,+y; ties keep the first (R12, R14, R37).  hit = surface id, n_surf+k for first-level wall k, n_surf+4+k
+// for second-level wall k.
+__device__ __noinline__ double nearest2(const Geo &G, double x, double y, double z, double ux, double uy, double uz, int cell,
+                                       int elem, int last, int &hit, unsigned int root_mask)
+{
+    double best = __longlong_as_double(0x7ff0000000000000LL);
+    hit = -1;
+    const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;  // +-inf when the component is zero: guarded at use
+    int c0 = elem >= 0 ? G.lat_cell : cell;
+    int k1 = __ldg(G.cso + c0 + 1);
+    if (root_mask) {
+        // candidates in list order (ties keep the first, R12): the listed bits, then anything past the 32nd surface
+        const int k0 = __ldg(G.cso + c0);
+        unsigned int m = k1 - k0 >= 32 ? root_mask : root_mask & ((1u << (k1 - k0)) - 1u);
+        while (m) {
+            int s = __ldg(G.csi + k0 + __ffs(m) - 1);
+            m &= m - 1u;
+            double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
+            if (d < best) { best = d; hit = s; }
+        }
+        for (int k = k0 + 32; k < k1; k++) {
+            int s = __ldg(G.csi + k);
+            double d = surf_distance(G, s, x, y, z, ux, uy, uz, s == last, inv_ux, inv_uy);
+            if (d < best) { best = d; hit = s; }
+        }
+    }
+    if (elem >= 0) {
+        int ix, iy;
+        const int outer = outer_of(G, elem), inner = inner_of(G, elem);
+        elem_xy(G, outer, ix, iy);
+        const double xo = x - (G.lat_x0 + (ix + 0.5) * G.lat_px);
+        const double yo = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
+        double xl = xo, yl = yo;
+        int k2 = 0;
+        if (inner >= 0) {
+            const int mid = __ldg(G.umid + elem_universe(G, outer));
+            k1 = __ldg(G.cso + mid + 1);
+            for (int k = __ldg(G.cso + mid); k < k1; k++) {
+                int s = __ldg(G.csi + k);
+                double d = surf_distance(G, s, xo, yo, z, ux, uy, uz, s == last, inv_ux, inv_uy);
+                if (d < best) { best = d; hit = s; }
+            }
+            k2 = __ldg(G.cfill + mid);
+            inner_xy(G, k2, inner, xo, yo, xl, yl);
+        }
+        k1 = __ldg(G.cso + cell + 1);
+        for (int k = __ldg(G.cso + cell); k < k1; k++) {
+            int s = __ldg(G.csi + k);
+            double d = surf_distance(G, s, xl, yl, z, ux, uy, uz, s == last, inv_ux, inv_uy);
+            if (d < best) { best = d; hit = s; }
+        }
+        if (inner >= 0) {
+            // second-level walls, in first-level-element coordinates: only the wall ahead, never the outermost ones
+            const int nx2 = __ldg(G.l2_nx + k2), ny2 = __ldg(G.l2_ny + k2);
+            const double px2 = __ldg(G.l2_px + k2), py2 = __ldg(G.l2_py + k2);
+            const int jy = inner / nx2, jx = inner - jy * nx2;
+            if (ux < 0.0 && jx > 0) {
+                double d = (l2_x0(G, k2) + jx * px2 - xo) * inv_ux;
+                if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 4; }
+            }
+            if (ux > 0.0 && jx + 1 < nx2) {
+                double d = (l2_x0(G, k2) + (jx + 1) * px2 - xo) * inv_ux;
+                if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 5; }
+            }
+            if (uy < 0.0 && jy > 0) {
+                double d = (l2_y0(G, k2) + jy * py2 - yo) * inv_uy;
+                if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 6; }
+            }
+            if (uy > 0.0 && jy + 1 < ny2) {
+                double d = (l2_y0(G, k2) + (jy + 1) * py2 - yo) * inv_uy;
+                if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 7; }
+            }
+        }
+        // only the wall ahead on each axis; the lattice's outermost walls are never events (R14)
+        if (ux < 0.0 && ix > 0) {
+            double d = (G.lat_x0 + ix * G.lat_px - x) * inv_ux;
+            if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 0; }
+        }
+        if (ux > 0.0 && ix + 1 < G.lat_nx) {
+            double d = (G.lat_x0 + (ix + 1) * G.lat_px - x) * inv_ux;
+            if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 1; }
+        }
+        if (uy < 0.0 && iy > 0) {
+            double d = (G.lat_y0 + iy * G.lat_py - y) * inv_uy;
+            if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 2; }
+        }
+        if (uy > 0.0 && iy + 1 < G.lat_ny) {
+            double d = (G.lat_y0 + (iy + 1) * G.lat_py - y) * inv_uy;
+            if (d > 0.0 && d < best) { best = d; hit = G.n_surf + 3; }
+        }
+        if (inner >= 0) {  // the second-level element's tally-bin offset rides on the hit code (R37)
+            const int off = __ldg(G.l2_bin + __ldg(G.l2_off + k2) + inner);
+            if (off) hit = (hit & ((1 << HIT_BITS) - 1)) | (off << HIT_BITS);
+        }
+    }
+    return best;
+}
+
 // Straight-line path (see Geo): per axis ONE candidate, named by the location's boundary code for the direction of
 // flight (lattice wall ahead, or an axis plane), plus at most one z-cylinder (centred on the lattice element, or in
 // global coordinates outside a lattice).  Same formulas and the same candidate order as `nearest` (planes of the
@@ -612,6 +778,10 @@ __device__ __forceinline__ void ce_energy_state(const CETab &ce, Particle &p)
 }
 
 enum { ADV_DEAD = 0, ADV_SCATTER = 1, ADV_SURFACE = 2, ADV_FISSION = 3 };
+// kernel variants beyond (CE, PRIVATE, W), template parameter X: the problem has second-level lattices (generic geometry
+// through nearest2 / do_surface2); the problem is time-dependent multi-group (clock, time edges, delayed neutrons).
+// One-level, time-independent problems compile exactly the code they had before these were added.
+enum { X_L2 = 1, X_TD = 2 };
 
 struct TraceRec {  // = mcdc_trace_rec
     unsigned long long id;
@@ -683,9 +853,13 @@ __device__ __forceinline__ double mgv(const Acc &acc, int off) { return acc.mgs[
 // collision removes the capture share, the reaction is chosen among scatter / fission, and a scattered particle whose
 // weight fell below w_roulette plays roulette (one draw).  W = false is the analog path (R2): weight = the launch
 // constant w0, p.w is never read.
-template <bool CE, bool PRIVATE, bool W>
+template <bool CE, bool PRIVATE, bool W, int X = 0>
 __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int &aux, Acc &acc, double *s_flux)
 {
+    constexpr bool L2 = (X & X_L2) != 0, TD = (X & X_TD) != 0, TIMED = CE || TD;
+    // implicit capture: what the weighted kernels are for -- except the time-dependent multi-group kernel, which is
+    // always weighted (census survivors and combed copies carry their own weights, R40) and asks the option
+    const bool IMPL = W && (TD ? c.implicit != 0 : true);
     const Geo &G = c.geo;
     const int cell0 = p.cell, elem0 = p.elem;
     const int mat = __ldg(G.cfill + p.cell);
@@ -693,7 +867,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     int4 li;  // boundary codes of the location (z, w), fast-path flag, cylinder
     int cyl;
     if (p.elem >= 0) {
-        li = __ldg(G.lat_info + p.elem);
+        li = __ldg(G.lat_info + (L2 ? outer_of(G, p.elem) : p.elem));
         bin += li.y;
         cyl = __ldg(&G.ufast[li.x & (LAT_FAST - 1)].y);
     } else {
@@ -732,12 +906,19 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     double d_surf;
     if (li.x & LAT_FAST) d_surf = nearest_fast(G, li.z, li.w, cyl, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.elem, p.last, hit);
     else {
-        unsigned int root_mask = p.elem >= 0 ? __ldg(G.lat_rmask + p.elem) : 0xffffffffu;
-        d_surf = nearest(*acc.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_mask);
+        unsigned int root_mask = p.elem >= 0 ? __ldg(G.lat_rmask + (L2 ? outer_of(G, p.elem) : p.elem)) : 0xffffffffu;
+        if (L2) {
+            d_surf = nearest2(*acc.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_mask);
+            if (hit >= (1 << HIT_BITS)) {  // inside a second-level lattice: its element's tally-bin offset rides on the hit code (R37)
+                bin += hit >> HIT_BITS;
+                hit &= (1 << HIT_BITS) - 1;
+                if (hit == (1 << HIT_BITS) - 1) hit = -1;
+            }
+        } else d_surf = nearest(*acc.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.cell, p.elem, p.last, hit, root_mask);
     }
     double v = 0.0, d_time = __longlong_as_double(0x7ff0000000000000LL);
-    if (CE) {
-        v = p.v;
+    if (TIMED) {
+        v = CE ? p.v : __ldg(c.td.speed + p.g);  // R23 / the group's speed (R38)
         d_time = v * (__ldg(c.ce.t_edges + p.tbin + 1) - p.t);
     }
     int kind;
@@ -750,11 +931,9 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
     const double E_flight = CE ? p.E : 0.0;
     long long tix;
-    if (!CE) tix = (long long)bin * c.mg.G + p.g;
-    else {
-        tix = ((long long)bin * c.ce.n_t + p.tbin) * c.ce.n_e + p.ebin;
-        if (kind == 2) p.t = __ldg(c.ce.t_edges + p.tbin + 1); else p.t += d / v;
-    }
+    if (!CE) tix = TD ? ((long long)bin * c.ce.n_t + p.tbin) * c.mg.G + p.g : (long long)bin * c.mg.G + p.g;
+    else tix = ((long long)bin * c.ce.n_t + p.tbin) * c.ce.n_e + p.ebin;
+    if (TIMED) { if (kind == 2) p.t = __ldg(c.ce.t_edges + p.tbin + 1); else p.t += d / v; }
     const double w = W ? p.w : c.w0;
     flux_add<PRIVATE>(c, s_flux, tix, w * d);
     acc.knum += w * d * nusf;
@@ -766,7 +945,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         if (!CE) {
             double sig_s = mgv(acc, c.mg.o_sig_s + mat * c.mg.G + p.g), sig_f = mgv(acc, c.mg.o_sig_f + mat * c.mg.G + p.g);
             double total = sig_t;
-            if (W) {  // the weight loses its capture share; the reaction is chosen among scatter / fission
+            if (IMPL) {  // the weight loses its capture share; the reaction is chosen among scatter / fission
                 total = sig_s + sig_f;
                 const double wn = p.w * (total / sig_t);
                 acc.wabs += p.w - wn;
@@ -776,12 +955,15 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
             if (uu < sig_s) { ev = 1; code = ADV_SCATTER; p.pend = PEND_SCATTER; }
             else if (uu < sig_s + sig_f) {
                 ev = 2; code = ADV_FISSION;
-                aux = (int)floor((W ? p.w : c.w0) * mgv(acc, c.mg.o_nu + mat * c.mg.G + p.g) / c.k_prev + rng.next(c));
+                if (TD)  // time-dependent fixed source (R39): floor(prompt + delayed yields + xi) children of the parent's weight
+                    aux = (int)floor(__ldg(c.td.cum_nu + ((size_t)mat * c.mg.G + p.g) * (c.td.J + 1) + c.td.J) + rng.next(c));
+                else
+                    aux = (int)floor((W ? p.w : c.w0) * mgv(acc, c.mg.o_nu + mat * c.mg.G + p.g) / c.k_prev + rng.next(c));
             } else { ev = 3; code = ADV_DEAD; }
         } else {
-            const int nsel = W ? ncol - 1 : ncol;  // columns the reaction is chosen from (implicit capture: all but capture)
+            const int nsel = IMPL ? ncol - 1 : ncol;  // columns the reaction is chosen from (implicit capture: all but capture)
             double total = sig_t;
-            if (W) {
+            if (IMPL) {
                 total = cum[0];
 #pragma unroll
                 for (int j = 1; j < MAX_CE_COL; j++)
@@ -804,7 +986,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         }
         if (W) {
             if (code == ADV_SCATTER) {
-                if (p.w < c.w_roulette) {  // roulette (one draw): survive at w_survive with probability w / w_survive
+                if (IMPL && p.w < c.w_roulette) {  // roulette (one draw): survive at w_survive with probability w / w_survive
                     if (rng.next(c) * c.w_survive < p.w) { atomicAdd(c.scal + 5, c.w_survive - p.w); p.w = c.w_survive; }
                     else { atomicAdd(c.scal + 4, p.w); ev = 3; code = ADV_DEAD; p.pend = PEND_NONE; }
                 }
@@ -826,7 +1008,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
         else { ev = 8; code = ADV_SURFACE; p.pend = PEND_TIME; }
     }
     if (acc.tracing)
-        trace_event(*c.tr_g, c.cycle, G.lat_cell, p.id, p.x, p.y, p.z, CE ? p.t : 0.0, ev, cell0, elem0, surf, gi, d, E_flight);
+        trace_event(*c.tr_g, c.cycle, G.lat_cell, p.id, p.x, p.y, p.z, TIMED ? p.t : 0.0, ev, cell0, elem0, surf, gi, d, E_flight);
     count_event(acc, ev);
     p.nseg++;
     if (code != ADV_DEAD && code != ADV_FISSION && p.nseg >= MAX_SEGMENTS) {  // lost-particle guard (R11)
@@ -945,6 +1127,78 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const Acc &acc, Particl
     p.last = -1;
 }
 
+// Surface event of a problem with second-level lattices (R37): the same as do_surface below, with the second-level
+// walls, the surfaces of the cell a second-level lattice fills, and the descent into a second-level lattice wherever
+// the cell found is filled by one.  Returns false if the particle got lost.
+__device__ __noinline__ bool do_surface2(const Geo &G, Particle &p, int hit)
+{
+    if (hit >= G.n_surf + 4) {  // second-level wall: neighbour element of the same second-level lattice (R37)
+        const int w = hit - G.n_surf - 4;
+        const int outer = outer_of(G, p.elem);
+        const int k2 = __ldg(G.cfill + __ldg(G.umid + elem_universe(G, outer)));
+        const int nx2 = __ldg(G.l2_nx + k2);
+        int jy = inner_of(G, p.elem) / nx2, jx = inner_of(G, p.elem) - jy * nx2;
+        if (w == 0) jx--; else if (w == 1) jx++; else if (w == 2) jy--; else jy++;
+        const int inner = jy * nx2 + jx;
+        p.elem = outer | ((inner + 1) << INNER_SHIFT);
+        p.last = -1;
+        double xl, yl;
+        innermost_xy(G, p.elem, p.x, p.y, xl, yl);
+        p.cell = find_cell(G, __ldg(G.l2_univ + __ldg(G.l2_off + k2) + inner), xl, yl, p.z, p.ux, p.uy, p.uz, -1);
+        return p.cell >= 0;
+    }
+    if (hit >= G.n_surf) {
+        int w = hit - G.n_surf;
+        int ix, iy;
+        elem_xy(G, outer_of(G, p.elem), ix, iy);
+        if (w == 0) ix--; else if (w == 1) ix++; else if (w == 2) iy--; else iy++;
+        p.last = -1;
+        double xl, yl;
+        local_xy(G, iy * G.lat_nx + ix, p.x, p.y, xl, yl);
+        p.cell = descend(G, iy * G.lat_nx + ix, xl, yl, p.z, p.ux, p.uy, p.uz, -1, p.elem);
+        return p.cell >= 0;
+    }
+    int bc = __ldg(G.surf_bc + hit);
+    // whose surface: the enclosing (root) cell's, the cell's that a second-level lattice fills (first-level-element
+    // coordinates), or the local cell's (innermost coordinates)
+    const bool local = p.elem >= 0 && !surface_in_cell(G, G.lat_cell, hit);
+    const bool inner_loc = local && inner_of(G, p.elem) >= 0;
+    const bool midlevel = inner_loc && surface_in_cell(G, __ldg(G.umid + elem_universe(G, outer_of(G, p.elem))), hit);
+    double xl = p.x, yl = p.y;
+    if (midlevel) local_xy(G, outer_of(G, p.elem), p.x, p.y, xl, yl);
+    else if (local) innermost_xy(G, p.elem, p.x, p.y, xl, yl);
+    p.last = hit;
+    if (bc == 1) {
+        int t = __ldg(G.surf_type + hit);
+        if (t == 0) p.ux = -p.ux;
+        else if (t == 1) p.uy = -p.uy;
+        else if (t == 2) p.uz = -p.uz;
+        else {
+            double nx, ny, nz;
+            surf_normal(G, hit, xl, yl, p.z, nx, ny, nz);
+            double nn = sqrt(nx * nx + ny * ny + nz * nz);
+            nx /= nn; ny /= nn; nz /= nn;
+            double dot = p.ux * nx + p.uy * ny + p.uz * nz;
+            p.ux -= 2.0 * dot * nx; p.uy -= 2.0 * dot * ny; p.uz -= 2.0 * dot * nz;
+        }
+        return true;
+    }
+    if (local) {
+        if (inner_loc && !midlevel) {  // inside the same second-level element
+            const int outer = outer_of(G, p.elem);
+            const int k2 = __ldg(G.cfill + __ldg(G.umid + elem_universe(G, outer)));
+            p.cell = find_cell(G, __ldg(G.l2_univ + __ldg(G.l2_off + k2) + inner_of(G, p.elem)), xl, yl, p.z, p.ux, p.uy, p.uz, hit);
+        } else {  // inside the same first-level element: its universe, descending where a lattice fills the cell
+            const int outer = outer_of(G, p.elem);
+            double xo, yo;
+            local_xy(G, outer, p.x, p.y, xo, yo);
+            p.cell = descend(G, outer, xo, yo, p.z, p.ux, p.uy, p.uz, hit, p.elem);
+        }
+        return p.cell >= 0;
+    }
+    return locate(G, p.x, p.y, p.z, p.ux, p.uy, p.uz, hit, p.cell, p.elem);
+}
+
 // Surface event (a9), generic path: lattice wall -> neighbour element; reflect; transmit -> neighbour cell by the
 // side being entered (R11, R14).  Returns false if the particle got lost.
 __device__ __noinline__ bool do_surface(const Geo &G, Particle &p, int hit)
@@ -1051,9 +1305,10 @@ __device__ __forceinline__ int do_surface_fast(const Geo &G, Particle &p, int hi
     return 0;
 }
 
+template <bool L2 = true>
 __device__ __forceinline__ bool location_is_fast(const Geo &G, int cell, int elem)
 {
-    return ((elem >= 0 ? __ldg(&G.lat_info[elem].x) : __ldg(&G.cell_info[cell].x)) & LAT_FAST) != 0;
+    return ((elem >= 0 ? __ldg(&G.lat_info[L2 ? outer_of(G, elem) : elem].x) : __ldg(&G.cell_info[cell].x)) & LAT_FAST) != 0;
 }
 
 // Watt spectrum, rejection-free (R22); MeV
@@ -1066,16 +1321,17 @@ __device__ __forceinline__ double watt(double a, double b, double x1, double x2,
 
 // Finish the event a banked particle is waiting on (scatter: a8; surface / lattice wall: a9; time edge: nothing).
 // Returns false if the particle got lost.
-template <bool CE>
+template <bool CE, int X = 0>
 __device__ __forceinline__ bool finish_pending(const Ctx &c, const Acc &acc, Particle &p, Rng &rng)
 {
+    constexpr bool L2 = (X & X_L2) != 0;
     const unsigned int pend = p.pend;
     p.pend = PEND_NONE;
     if (pend >= PEND_TIME) return true;
     if (pend >= PEND_SCATTER) { do_scatter<CE>(c, acc, p, rng, (int)(pend & 7u)); return true; }
     int r = 0;
-    if (location_is_fast(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)pend);
-    if (r == 0) r = do_surface(*acc.geo, p, (int)pend) ? 1 : -1;
+    if (location_is_fast<L2>(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)pend);
+    if (r == 0) r = (L2 ? do_surface2(*acc.geo, p, (int)pend) : do_surface(*acc.geo, p, (int)pend)) ? 1 : -1;
     return r > 0;
 }
 

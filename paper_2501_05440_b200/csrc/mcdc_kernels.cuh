@@ -50,7 +50,9 @@ __device__ __forceinline__ const double *stage_mg(const Ctx &c, double *smem, in
 // ------------------------------------------------------------------ bank access (dense, position-indexed)
 // W (weighted kernels): a particle that has not run a segment yet starts with the launch weight w0 (source
 // renormalisation, R6; secondaries of a fixed-source run: 1), later its own banked weight
-template <bool CE, bool W = false>
+// TD (time-dependent multi-group): the clock, time bin and 64-bit id are banked as for continuous energy, and the
+// weight is always the banked one (census survivors and combed copies carry their own, R40).
+template <bool CE, bool W = false, bool TD = false>
 __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particle &p, uint32_t &ctr, uint32_t &slot,
                                           double w0 = 1.0)
 {
@@ -65,18 +67,20 @@ __device__ __forceinline__ void load_full(const Bank &B, unsigned int i, Particl
     slot = B.slot[i];
     p.v = 0.0; p.gi = 0; p.ebin = 0;
     if (CE) { p.E = B.E[i]; p.t = B.t[i]; p.tbin = B.tbin[i]; p.id = B.id[i]; }
+    else if (TD) { p.E = 0.0; p.t = B.t[i]; p.tbin = B.tbin[i]; p.id = B.id[i]; }
     else { p.E = 0.0; p.t = 0.0; p.tbin = 0; p.id = slot; }
     p.w = w0;
-    if (W && p.nseg != 0) p.w = B.w[i];
+    if (W && (TD || p.nseg != 0)) p.w = B.w[i];
 }
 
-template <bool CE, bool W = false>
+template <bool CE, bool W = false, bool TD = false>
 __device__ __forceinline__ void store_full(const Bank &B, unsigned int i, const Particle &p, uint32_t ctr, uint32_t slot)
 {
     B.x[i] = p.x; B.y[i] = p.y; B.z[i] = p.z; B.ux[i] = p.ux; B.uy[i] = p.uy; B.uz[i] = p.uz;
     B.cell[i] = p.cell; B.elem[i] = p.elem; B.gl[i] = pack_gl(p.g, p.last); B.ctr[i] = ctr; B.slot[i] = slot;
     B.ev[i] = p.pend | (p.nseg << 12);
     if (CE) { B.E[i] = p.E; B.t[i] = p.t; B.tbin[i] = p.tbin; B.id[i] = p.id; }
+    if (TD) { B.t[i] = p.t; B.tbin[i] = p.tbin; B.id[i] = p.id; }
     if (W) B.w[i] = p.w;
 }
 
@@ -222,7 +226,7 @@ __device__ __forceinline__ void block_slot_n(bool to_front, unsigned int n_back,
 }
 
 // ------------------------------------------------------------------ a1: source
-template <bool CE>
+template <bool CE, bool TD = false>
 __global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -244,8 +248,9 @@ __global__ void __launch_bounds__(BS) k_source(Ctx c, unsigned int n)
     if (!locate(c.geo, p.x, p.y, p.z, p.ux, p.uy, p.uz, -1, p.cell, p.elem)) { atomicExch(c.err, -2); p.cell = -1; }
     p.last = -1; p.id = i; p.pend = PEND_NONE; p.nseg = 0;
     p.E = c.src_E; p.t = c.src_t; p.tbin = 0;
-    if (CE) p.tbin = edge_bin(c.ce.t_edges, c.ce.n_t, c.src_t);
-    store_full<CE>(B, i, p, 6u, i);
+    if (CE || TD) p.tbin = edge_bin(c.ce.t_edges, c.ce.n_t, c.src_t);
+    p.w = 1.0;
+    store_full<CE, TD, TD>(B, i, p, 6u, i);
     c.fis.n[i] = 0;
 }
 
@@ -319,7 +324,7 @@ __device__ __forceinline__ void mark_lost(const Ctx &c)
 #ifndef MCDC_SWEEP_MINBLOCKS
 #define MCDC_SWEEP_MINBLOCKS 4
 #endif
-template <bool CE, bool PRIVATE, bool W>
+template <bool CE, bool PRIVATE, bool W, int X>
 __global__ void __launch_bounds__(BS, MCDC_SWEEP_MINBLOCKS * 256 / BS) k_sweep(Ctx c, unsigned int s, unsigned int n0)
 {
     MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
@@ -354,11 +359,11 @@ __global__ void __launch_bounds__(BS, MCDC_SWEEP_MINBLOCKS * 256 / BS) k_sweep(C
             load_full<CE, W>(B, i, p, ctr, slot, c.w0);
             if (CE) ce_energy_state(c.ce, p);
             rng.init(p.id, ctr);
-            const bool ok = finish_pending<CE>(c, acc, p, rng);
+            const bool ok = finish_pending<CE, X>(c, acc, p, rng);
             __syncwarp(amask);  // the lanes went different ways by pending event: run the segment together again
             if (!ok) mark_lost(c);
             else {
-                code = advance<CE, PRIVATE, W>(c, p, rng, aux, acc, s_flux);
+                code = advance<CE, PRIVATE, W, X>(c, p, rng, aux, acc, s_flux);
                 if (!CE && code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
             }
         }
@@ -442,7 +447,7 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
         const double ux0 = p.ux, uy0 = p.uy, uz0 = p.uz;
         int r = 0;
         if (location_is_fast(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)hit);
-        if (r == 0) r = do_surface(s_geo, p, (int)hit) ? 1 : -1;
+        if (r == 0) r = (c.geo.n_lat2 ? do_surface2(s_geo, p, (int)hit) : do_surface(s_geo, p, (int)hit)) ? 1 : -1;
         if (r < 0) { mark_lost(c); p.cell = -1; }
         if (p.cell != cell0) B.cell[i] = p.cell;
         if (p.elem != elem0) B.elem[i] = p.elem;
@@ -474,9 +479,70 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 #ifndef MCDC_DENSE
 #define MCDC_DENSE 12  // live lanes from which a continuous-energy warp keeps tickets for entries not pushed yet
 #endif
-template <bool CE, bool PRIVATE, bool W>
+// a particle that waits for a later census interval (it reached a time edge, or it is a delayed neutron that will be
+// emitted there): appended to the census bank (R40); more than `cap` of them is the bank-overflow error
+template <bool CE, bool W, bool TD>
+__device__ __forceinline__ void census_put(const Ctx &c, const Particle &p, uint32_t ctr, uint32_t slot)
+{
+    const unsigned int i = atomicAdd(c.work + 4, 1u);
+    if (i >= c.cap) { atomicExch(c.err, -3); return; }
+    store_full<CE, W, TD>(c.cbank, i, p, ctr, slot);
+}
+
+// write a secondary into entry `a` of the persistent kernel's ring (bank O) and publish it (see k_persist); returns
+// false when the run has to stop (bank overflow)
+template <bool CE, bool W, bool TD>
+__device__ __forceinline__ bool ring_put(const Ctx &c, const Bank &O, const unsigned int *head, unsigned int n_in, unsigned int a,
+                                         const Particle &p, uint32_t slot)
+{
+    const unsigned int i = a % c.cap, free_ = 2u * (a / c.cap);
+    // the slot still holds the previous lap's entry: if no ticket has been issued for that entry, nobody is about to take
+    // it -- more than `cap` secondaries wait: bank overflow
+    if (*(volatile uint32_t *)(O.ev + i) != free_) {
+        if (*(volatile const unsigned int *)head + c.cap <= n_in + a) atomicExch(c.err, -3);
+        unsigned int spins = 0;
+        while (*(volatile uint32_t *)(O.ev + i) != free_ && *(volatile int *)c.err == 0)
+            if (++spins > (1u << 22)) atomicExch(c.err, -3);
+        if (*(volatile int *)c.err != 0) return false;
+    }
+    O.x[i] = p.x; O.y[i] = p.y; O.z[i] = p.z; O.ux[i] = p.ux; O.uy[i] = p.uy; O.uz[i] = p.uz;
+    O.cell[i] = p.cell; O.elem[i] = p.elem; O.slot[i] = slot;
+    O.t[i] = p.t; O.tbin[i] = p.tbin; O.id[i] = p.id;
+    if (CE) O.E[i] = p.E;
+    if (TD) { O.gl[i] = pack_gl(p.g, -1); if (W) O.w[i] = p.w; }
+    __threadfence();
+    *(volatile uint32_t *)(O.ev + i) = free_ + 1u;
+    return true;
+}
+
+// child j of a time-dependent multi-group fission (R39): type (prompt / precursor group) by xi nu against the cumulative
+// yields, group from the type's spectrum, emission time (delayed: t - ln(xi) / lambda), isotropic direction; own id
+// (R10).  Returns false for a delayed neutron emitted after the last time edge: it is never born.
+__device__ __forceinline__ bool make_child_td(const Ctx &c, Rng &rng, int mat, int g_parent, double t_parent,
+                                              unsigned long long pid, uint32_t ctr0, int j, Particle &p)
+{
+    const int J = c.td.J, G = c.mg.G;
+    const double *cn = c.td.cum_nu + ((size_t)mat * G + g_parent) * (J + 1);
+    const int typ = pick(cn, J + 1, rng.next(c) * __ldg(cn + J));
+    const double *cc = typ == 0 ? c.mg.blob + c.mg.o_cumchi + (size_t)mat * G : c.td.cumchi_d + ((size_t)mat * J + typ - 1) * G;
+    p.g = pick(cc, G, rng.next(c) * __ldg(cc + G - 1));
+    double tj = t_parent;
+    if (typ > 0) tj = t_parent - log(rng.next(c)) / __ldg(c.td.decay + mat * J + typ - 1);
+    const double a = rng.next(c), b = rng.next(c);
+    iso_dir(a, b, p.ux, p.uy, p.uz);
+    p.last = -1; p.pend = PEND_NONE; p.nseg = 0;
+    p.id = child_id(c.seed, pid, ctr0, (uint32_t)j);
+    if (!(tj < __ldg(c.ce.t_edges + c.ce.n_t))) return false;
+    p.t = tj;
+    p.tbin = edge_bin(c.ce.t_edges, c.ce.n_t, tj);
+    return true;
+}
+
+template <bool CE, bool PRIVATE, bool W, int X>
 __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persist(Ctx c, unsigned int s, unsigned int n0)
 {
+    constexpr bool TD = (X & X_TD) != 0;
+    constexpr bool GROW = CE || TD;  // fissions put secondaries into the running population: the work queue grows
     MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
     unsigned int n_front, n_in;
     live_counts(c, s, n0, n_front, n_in);
@@ -503,7 +569,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
         // idle warp only takes entries that already exist, so that a thin population stays concentrated in few warps
         // instead of keeping every resident warp busy with one or two lanes.
         unsigned int n_take = 0;
-        if (!CE) n_take = (nw >= MCDC_REFILL || (none_alive && nw > 0)) ? (unsigned int)nw : 0u;
+        if (!GROW) n_take = (nw >= MCDC_REFILL || (none_alive && nw > 0)) ? (unsigned int)nw : 0u;
         else if (nw >= MCDC_REFILL) {
             if (__popc(__ballot_sync(FULL, alive)) >= MCDC_DENSE) n_take = (unsigned int)nw;
             else {
@@ -524,9 +590,9 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
             const unsigned int rank = __popc(want & ((1u << lane) - 1u));
             if (!alive && !ticketed && !drained && rank < n_take) {
                 ticket = base + rank;
-                ticketed = CE || ticket < n_in;  // multi-group: the queue never grows, a ticket past its end is void
+                ticketed = GROW || ticket < n_in;  // eigenvalue cycle: the queue never grows, a ticket past its end is void
                 drained = !ticketed;
-                if (CE && ticket >= n_in) {
+                if (GROW && ticket >= n_in) {
                     const unsigned int a = ticket - n_in;
                     t_slot = a % c.cap;
                     t_full = 2u * (a / c.cap) + 1u;
@@ -537,9 +603,9 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
             uint32_t ctr = 0;
             bool have = false;
             if (ticket < n_in) {
-                load_full<CE, W>(B, live_pos(c.cap, n_front, ticket), p, ctr, slot, c.w0);
+                load_full<CE, W, TD>(B, live_pos(c.cap, n_front, ticket), p, ctr, slot, c.w0);
                 have = true;
-            } else if (CE && *(volatile uint32_t *)(O.ev + t_slot) == t_full) {
+            } else if (GROW && *(volatile uint32_t *)(O.ev + t_slot) == t_full) {
                 const unsigned int i = t_slot;
                 __threadfence();
                 p.x = __ldcg(O.x + i); p.y = __ldcg(O.y + i); p.z = __ldcg(O.z + i);
@@ -548,7 +614,10 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
                 p.g = 0; p.last = -1; p.pend = PEND_NONE; p.nseg = 0;
                 p.w = c.w0;
                 slot = __ldcg(O.slot + i);
-                p.E = __ldcg(O.E + i); p.t = __ldcg(O.t + i); p.tbin = __ldcg(O.tbin + i); p.id = __ldcg(O.id + i);
+                p.E = 0.0;
+                if (CE) p.E = __ldcg(O.E + i);
+                if (TD) { p.g = __ldcg(O.gl + i) & 0xffff; if (W) p.w = __ldcg(O.w + i); }
+                p.t = __ldcg(O.t + i); p.tbin = __ldcg(O.tbin + i); p.id = __ldcg(O.id + i);
                 __threadfence();
                 *(volatile uint32_t *)(O.ev + i) = t_full + 1u;  // free for the next lap
                 have = true;
@@ -566,7 +635,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
             // ended == n_in + born, with `ended` read first (a parent's children are counted in `born` before the
             // parent is counted in `ended`, so the test cannot pass early).
             unsigned int fin = 0;
-            if (!CE) fin = __all_sync(FULL, drained) ? 1u : 0u;
+            if (!GROW) fin = __all_sync(FULL, drained) ? 1u : 0u;
             else {
                 const unsigned int ne = __reduce_add_sync(FULL, n_end);
                 n_end = 0;
@@ -580,23 +649,55 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
                 fin = __shfl_sync(FULL, fin, 0);
             }
             if (fin) break;
-            if (CE) { __nanosleep(idle_ns); if (idle_ns < 16000) idle_ns *= 2; }
+            if (GROW) { __nanosleep(idle_ns); if (idle_ns < 16000) idle_ns *= 2; }
             continue;
         }
         idle_ns = 500;
         const unsigned int amask = __ballot_sync(FULL, alive);
         if (alive) {
             int aux = 0, code = ADV_DEAD;
-            const bool ok = finish_pending<CE>(c, acc, p, rng);
+            const bool ok = finish_pending<CE, X>(c, acc, p, rng);
             __syncwarp(amask);  // the lanes went different ways by pending event: run the segment together again
             if (!ok) mark_lost(c);
-            else code = advance<CE, PRIVATE, W>(c, p, rng, aux, acc, s_flux);
+            else code = advance<CE, PRIVATE, W, X>(c, p, rng, aux, acc, s_flux);
+            if (GROW && code == ADV_SURFACE && p.pend == PEND_TIME && c.census_stop) {
+                // the census (R40): the particle waits in the census bank for the next interval
+                p.pend = PEND_NONE;
+                census_put<CE, W, TD>(c, p, rng.ctr, slot);
+                code = ADV_DEAD;
+            }
             if (code == ADV_DEAD) { alive = false; n_end++; }
             else if (code == ADV_FISSION) {
                 alive = false;
                 n_end++;
-                if (!CE) record_fission<CE>(c, p, rng.ctr, slot, aux);
-                else if (aux > 0 && count_secondaries(c, (unsigned int)aux)) {
+                if (!GROW) record_fission<CE>(c, p, rng.ctr, slot, aux);
+                else if (TD) {
+                    if (aux > 0) {
+                        // every child is counted as born first; one that is never born, or that waits for a later
+                        // interval, is counted as ended at once (the termination test stays ended == n_in + born)
+                        atomicAdd(born, (unsigned int)aux);
+                        const int mat = c.geo.cfill[p.cell], g_parent = p.g, tbin_parent = p.tbin;
+                        const double t_parent = p.t;
+                        const unsigned long long pid = p.id;
+                        const uint32_t ctr0 = rng.ctr;
+                        Particle first = p;
+                        bool have_first = false;
+                        unsigned int n_born = 0;
+                        for (int j = 0; j < aux; j++) {
+                            if (!make_child_td(c, rng, mat, g_parent, t_parent, pid, ctr0, j, p)) { n_end++; continue; }
+                            n_born++;
+                            if (p.tbin != tbin_parent) { census_put<CE, W, TD>(c, p, 0u, slot); n_end++; continue; }
+                            if (!have_first) { first = p; have_first = true; continue; }
+                            if (!ring_put<CE, W, TD>(c, O, head, n_in, atomicAdd(tail, 1u), p, slot)) break;
+                        }
+                        if (n_born) { count_secondaries(c, n_born); if (W) atomicAdd(c.scal + 6, (double)n_born * first.w); }
+                        if (have_first) {
+                            p = first;
+                            rng.init(p.id, 0u);
+                            alive = true;
+                        }
+                    }
+                } else if (aux > 0 && count_secondaries(c, (unsigned int)aux)) {
                     atomicAdd(born, (unsigned int)aux);
                     const int mat = c.geo.cfill[p.cell];
                     const unsigned long long pid = p.id;
@@ -607,24 +708,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
                     for (int j = 0; j < aux; j++) {
                         make_child<CE>(c, rng, mat, pid, ctr0, j, p);
                         if (j == 0) first = p;
-                        else {
-                            const unsigned int a = at + (unsigned int)(j - 1);
-                            const unsigned int i = a % c.cap, free_ = 2u * (a / c.cap);
-                            // the slot still holds the previous lap's entry: if no ticket has been issued for that
-                            // entry, nobody is about to take it -- more than `cap` secondaries wait: bank overflow
-                            if (*(volatile uint32_t *)(O.ev + i) != free_) {
-                                if (*(volatile unsigned int *)head + c.cap <= n_in + a) atomicExch(c.err, -3);
-                                unsigned int spins = 0;
-                                while (*(volatile uint32_t *)(O.ev + i) != free_ && *(volatile int *)c.err == 0)
-                                    if (++spins > (1u << 22)) atomicExch(c.err, -3);
-                                if (*(volatile int *)c.err != 0) break;
-                            }
-                            O.x[i] = p.x; O.y[i] = p.y; O.z[i] = p.z; O.ux[i] = p.ux; O.uy[i] = p.uy; O.uz[i] = p.uz;
-                            O.cell[i] = p.cell; O.elem[i] = p.elem; O.slot[i] = slot;
-                            O.E[i] = p.E; O.t[i] = p.t; O.tbin[i] = p.tbin; O.id[i] = p.id;
-                            __threadfence();
-                            *(volatile uint32_t *)(O.ev + i) = free_ + 1u;
-                        }
+                        else if (!ring_put<CE, W, false>(c, O, head, n_in, at + (unsigned int)(j - 1), p, slot)) break;
                     }
                     p = first;
                     p.w = c.w0;
@@ -644,7 +728,7 @@ __global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persi
 // ------------------------------------------------------------------ monolithic schedule
 // every slot of bank 0, one whole segment (advance + the event it ends in), in place, no compaction; counts the
 // survivors.  A dead slot has cell = -1.
-template <bool CE, bool PRIVATE, bool W>
+template <bool CE, bool PRIVATE, bool W, int X>
 __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned int n)
 {
     MCDC_TRANSPORT_PROLOGUE(acc, s_flux);
@@ -664,9 +748,9 @@ __global__ void __launch_bounds__(BS) k_segment(Ctx c, unsigned int s, unsigned 
         Rng rng;
         rng.init(p.id, ctr);
         int aux = 0;
-        int code = advance<CE, PRIVATE, W>(c, p, rng, aux, acc, s_flux);
+        int code = advance<CE, PRIVATE, W, X>(c, p, rng, aux, acc, s_flux);
         if (code == ADV_FISSION) { record_fission<CE>(c, p, rng.ctr, slot, aux); code = ADV_DEAD; }
-        else if (code != ADV_DEAD && !finish_pending<CE>(c, acc, p, rng)) { mark_lost(c); code = ADV_DEAD; }
+        else if (code != ADV_DEAD && !finish_pending<CE, X>(c, acc, p, rng)) { mark_lost(c); code = ADV_DEAD; }
         if (code == ADV_DEAD) p.cell = -1;
         store_full<CE, W>(B, i, p, rng.ctr, slot);
         if (code != ADV_DEAD) alive++;
@@ -811,12 +895,13 @@ __global__ void k_test_geometry(Ctx c, const double *x, const double *u, unsigne
     bool ok = locate(G, px, py, pz, ux, uy, uz, -1, cell, elem);
     double d = -1.0;
     if (ok) {
-        const int4 li = elem >= 0 ? __ldg(G.lat_info + elem) : __ldg(G.cell_info + cell);
+        const int4 li = elem >= 0 ? __ldg(G.lat_info + outer_of(G, elem)) : __ldg(G.cell_info + cell);
         const int cyl = elem >= 0 ? __ldg(&G.ufast[li.x & (LAT_FAST - 1)].y) : li.y;
         if (path == 0 && (li.x & LAT_FAST)) d = nearest_fast(G, li.z, li.w, cyl, px, py, pz, ux, uy, uz, elem, -1, hit);
         else {
-            unsigned int mask = (elem >= 0 && path != 2) ? __ldg(G.lat_rmask + elem) : 0xffffffffu;
-            d = nearest(s_geo, px, py, pz, ux, uy, uz, cell, elem, -1, hit, mask);
+            unsigned int mask = (elem >= 0 && path != 2) ? __ldg(G.lat_rmask + outer_of(G, elem)) : 0xffffffffu;
+            d = G.n_lat2 ? nearest2(s_geo, px, py, pz, ux, uy, uz, cell, elem, -1, hit, mask) : nearest(s_geo, px, py, pz, ux, uy, uz, cell, elem, -1, hit, mask);
+            if (hit >= (1 << HIT_BITS)) { hit &= (1 << HIT_BITS) - 1; if (hit == (1 << HIT_BITS) - 1) hit = -1; }
         }
     }
     loc[3 * i] = !ok ? -1 : (elem >= 0 ? G.lat_cell : cell);

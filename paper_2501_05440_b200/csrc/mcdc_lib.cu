@@ -2,6 +2,7 @@
 // carving, the sweep / cycle drivers and result read-back.  All device work is in mcdc_kernels.cuh.
 #include "../../include/mcdc.h"
 #include "mcdc_kernels.cuh"
+#include "mcdc_census.cuh"
 #include "mcdc_microbench.cuh"
 
 #include <algorithm>
@@ -51,6 +52,8 @@ static const int MAX_AXIS_PLANES = 250;   // axis planes a boundary code of the 
 
 struct HostPinned {
     QCount qc[RING];
+    unsigned int census[4];  // [0] census-bank count read back, [1] particles of the next interval, [2] count to set
+    double comb_w;           // total weight of the particles entering an interval
     double scal[8];
     unsigned long long counters[MCDC_N_COUNTERS];
     unsigned int total;
@@ -68,6 +71,9 @@ struct RunStats {
     uint64_t counters[MCDC_N_COUNTERS] = {0};       // merged device + host counters as reported
     int set = 0;                                    // which flux accumulator pair holds this run's tallies
     double balance[6] = {0, 0, 0, 0, 0, 0};         // weight balance summed over the run's cycles (mcdc_get_balance)
+    std::vector<uint64_t> census_counts;            // per census interval: particles before / after the comb
+    std::vector<double> census_weights;             // and their total weights
+    int next_interval = -1;                         // fixed source by intervals: the interval the next call must name
 };
 
 struct mcdc_problem {
@@ -78,6 +84,16 @@ struct mcdc_problem {
     int schedule, persist;
     int persist_blocks_per_sm, n_sm;  // resident blocks of the persistent kernel (occupancy query at first use)
     uint64_t cap;  // bank slots
+    // time-dependent fixed source: census banks (ping-pong), radix-sort and comb scratch
+    bool timed, td;
+    int first_interval;
+    long long census_target;
+    Bank cb[2];
+    int cb_cur;
+    unsigned long long *sort_key[2];
+    unsigned int *sort_idx[2], *sort_hist, *comb_copies, *comb_offs;
+    double *comb_w;
+    uint64_t census_n;  // particles in the current census bank
     // workspace pieces not in ctx
     double *flux_acc[2], *flux_acc2[2], *flux_cycle;
     int flux_copies;
@@ -153,6 +169,8 @@ struct Carver {
 struct Layout {  // everything carved from the workspace, in order
     int *surf_type, *surf_bc, *cso, *csi, *css, *cft, *cfill, *cbin, *uco, *ap_sid;
     int4 *lat_info, *ufast, *cell_info;
+    int *l2_nx, *l2_ny, *l2_off, *l2_univ, *l2_bin, *umid;
+    double *l2_px, *l2_py;
     Trace *tr_g;
     unsigned int *lat_rmask;
     double *surf_param, *ap_pos;
@@ -160,7 +178,10 @@ struct Layout {  // everything carved from the workspace, in order
     uint64_t mg_doubles;
     double *grid, *tab, *colA, *t_edges, *e_edges;
     int *ncol, *hash, *ehash;
-    Bank bank[2];
+    Bank bank[2], cb[2];
+    unsigned long long *sort_key[2];
+    unsigned int *sort_idx[2], *sort_hist, *comb_copies, *comb_offs;
+    double *comb_w, *td_speed, *td_cum_nu, *td_cumchi_d, *td_decay;
     FisRec fis;
     QCount *qc;
     double *flux, *flux_acc[2], *flux_acc2[2], *flux_cycle, *scal;
@@ -185,7 +206,8 @@ static int flux_copies_for(uint64_t n_tally)
 
 static uint64_t n_tally_of(const mcdc_materials *mat, const mcdc_tally_spec *t)
 {
-    return mat ? (uint64_t)t->n_bins * mat->G : (uint64_t)t->n_bins * t->n_t * t->n_e;
+    if (mat) return mat->kinetics ? (uint64_t)t->n_bins * t->n_t * mat->G : (uint64_t)t->n_bins * mat->G;
+    return (uint64_t)t->n_bins * t->n_t * t->n_e;
 }
 
 static int hash_params(const double *grid, int n, int &shift, int &lo, int &n_hash)
@@ -230,13 +252,28 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     L.tr_g = C.take<Trace>(1);
     L.ap_pos = C.take<double>(MAX_AXIS_PLANES); L.ap_sid = C.take<int>(MAX_AXIS_PLANES);
     L.lat_info = C.take<int4>(nlat); L.lat_rmask = C.take<unsigned int>(nlat);
+    {
+        uint64_t n2 = g->n_lat2 > 0 ? g->n_lat2 : 0, ne2 = n2 ? g->lat2_off[n2] : 0;
+        L.l2_nx = C.take<int>(n2); L.l2_ny = C.take<int>(n2); L.l2_off = C.take<int>(n2 + 1);
+        L.l2_px = C.take<double>(n2); L.l2_py = C.take<double>(n2);
+        L.l2_univ = C.take<int>(ne2); L.l2_bin = C.take<int>(ne2);
+        L.umid = C.take<int>(g->n_univ);
+    }
     bool ce = x != nullptr;
+    const bool td = !ce && m->kinetics != nullptr, timed = ce || td;
     if (!ce) {
         uint64_t mg = (uint64_t)m->n_mat * m->G;
         // one contiguous blob (staged in shared memory by the kernels): six [n_mat][G] tables, cumS, src_cum
         L.mg_doubles = 6 * mg + mg * m->G + m->G;
         L.mg_blob = C.take<double>(L.mg_doubles);
         L.grid = L.tab = L.colA = L.t_edges = L.e_edges = nullptr; L.ncol = L.hash = L.ehash = nullptr;
+        L.td_speed = L.td_cum_nu = L.td_cumchi_d = L.td_decay = nullptr;
+        if (td) {
+            uint64_t J = m->kinetics->n_dgroup;
+            L.td_speed = C.take<double>(m->G); L.td_cum_nu = C.take<double>(mg * (J + 1));
+            L.td_cumchi_d = C.take<double>((uint64_t)m->n_mat * J * m->G + 1); L.td_decay = C.take<double>((uint64_t)m->n_mat * J + 1);
+            L.t_edges = C.take<double>(t->n_t + 1);
+        }
     } else {
         int sh, lo, nh;
         hash_params(x->grid, x->n_grid, sh, lo, nh);
@@ -250,17 +287,27 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         L.mg_blob = nullptr;
         L.mg_doubles = 0;
     }
-    for (int b = 0; b < 2; b++) {
-        Bank &B = L.bank[b];
+    for (int b = 0; b < 4; b++) {  // the two particle banks; for time-dependent problems also the two census banks
+        Bank &B = b < 2 ? L.bank[b] : L.cb[b - 2];
+        if (b >= 2 && !timed) { memset(&B, 0, sizeof B); continue; }
         B.x = C.take<double>(cap); B.y = C.take<double>(cap); B.z = C.take<double>(cap);
         B.ux = C.take<double>(cap); B.uy = C.take<double>(cap); B.uz = C.take<double>(cap);
         B.w = C.take<double>(cap);
-        B.E = ce ? C.take<double>(cap) : nullptr; B.t = ce ? C.take<double>(cap) : nullptr;
+        B.E = ce ? C.take<double>(cap) : nullptr; B.t = timed ? C.take<double>(cap) : nullptr;
         B.cell = C.take<int>(cap); B.elem = C.take<int>(cap); B.gl = C.take<int>(cap);
-        B.tbin = ce ? C.take<int>(cap) : nullptr;
+        B.tbin = timed ? C.take<int>(cap) : nullptr;
         B.ev = C.take<uint32_t>(cap);
         B.ctr = C.take<uint32_t>(cap); B.slot = C.take<uint32_t>(cap);
-        B.id = ce ? C.take<uint64_t>(cap) : nullptr;
+        B.id = timed ? C.take<uint64_t>(cap) : nullptr;
+    }
+    if (timed) {
+        for (int b = 0; b < 2; b++) { L.sort_key[b] = C.take<unsigned long long>(cap); L.sort_idx[b] = C.take<unsigned int>(cap); }
+        L.sort_hist = C.take<unsigned int>(256 * (cap / RS_TILE + 1) + 4);
+        L.comb_copies = C.take<unsigned int>(cap + 4); L.comb_offs = C.take<unsigned int>(cap + 4);
+        L.comb_w = C.take<double>(cap);
+    } else {
+        L.sort_key[0] = L.sort_key[1] = nullptr; L.sort_idx[0] = L.sort_idx[1] = nullptr;
+        L.sort_hist = L.comb_copies = L.comb_offs = nullptr; L.comb_w = nullptr;
     }
     {
         FisRec &F = L.fis;
@@ -314,7 +361,11 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
         if (g->cell_fill_type[c] == 1) {
             n_lat_cells++;
             if (c >= g->univ_cell_off[1]) return fail(MCDC_EGEOM, "the lattice-filled cell must belong to the root universe");
-        } else if (g->cell_fill[c] < 0 || g->cell_fill[c] >= n_mat) return fail(MCDC_EINVAL, "cell %d material %d out of range", c, g->cell_fill[c]);
+        } else if (g->cell_fill_type[c] == 2) {
+            if (g->n_lat2 < 1 || g->cell_fill[c] < 0 || g->cell_fill[c] >= g->n_lat2) return fail(MCDC_EGEOM, "cell %d names second-level lattice %d", c, g->cell_fill[c]);
+            if (c < g->univ_cell_off[1]) return fail(MCDC_EGEOM, "a second-level lattice must fill a cell of a lattice element's universe, not of the root");
+        } else if (g->cell_fill_type[c] != 0) return fail(MCDC_EGEOM, "cell %d: fill type %d", c, g->cell_fill_type[c]);
+        else if (g->cell_fill[c] < 0 || g->cell_fill[c] >= n_mat) return fail(MCDC_EINVAL, "cell %d material %d out of range", c, g->cell_fill[c]);
         if (t->cell_bin[c] < 0 || t->cell_bin[c] >= t->n_bins) return fail(MCDC_EINVAL, "cell_bin out of range");
     }
     for (int sidx = 0; sidx < g->n_surf; sidx++) {
@@ -325,6 +376,7 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
         if (n_lat_cells != 1) return fail(MCDC_EGEOM, "exactly one lattice-filled cell is supported");
         if (g->lat_nx < 1 || g->lat_ny < 1 || !(g->lat_px > 0) || !(g->lat_py > 0)) return fail(MCDC_EGEOM, "lattice shape");
         if ((unsigned long long)g->lat_nx * g->lat_nx * g->lat_ny >= 0x100000000ull) return fail(MCDC_EGEOM, "lattice too large (nx*nx*ny must be < 2^32)");
+        if ((long long)g->lat_nx * g->lat_ny > (1 << 20)) return fail(MCDC_EGEOM, "lattice too large (at most 2^20 elements)");
         if (!t->lat_bin) return fail(MCDC_EINVAL, "lat_bin missing");
         int max_lat_bin = 0;
         for (int e = 0; e < g->lat_nx * g->lat_ny; e++) {
@@ -336,6 +388,44 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
         for (int c = g->univ_cell_off[1]; c < g->n_cell; c++)
             if (t->cell_bin[c] + max_lat_bin >= t->n_bins) return fail(MCDC_EINVAL, "cell_bin[%d] + max lat_bin reaches past n_bins", c);
     } else if (n_lat_cells) return fail(MCDC_EGEOM, "lattice-filled cell without a lattice");
+    if (g->n_lat2 < 0) return fail(MCDC_EGEOM, "n_lat2");
+    if (g->n_lat2 > 0) {  // second-level lattices (R37)
+        if (!g->has_lattice) return fail(MCDC_EGEOM, "second-level lattices need a first-level lattice");
+        if (!g->lat2_nx || !g->lat2_ny || !g->lat2_px || !g->lat2_py || !g->lat2_off || !g->lat2_univ || !t->lat2_bin)
+            return fail(MCDC_EINVAL, "second-level lattice arrays missing");
+        if (g->lat2_off[0] != 0) return fail(MCDC_EINVAL, "lat2_off[0] must be 0");
+        // universes that lattice elements of either level use; which of them hold a second-level lattice
+        std::vector<char> has2(g->n_univ, 0);
+        for (int u = 1; u < g->n_univ; u++) {
+            int n2 = 0;
+            for (int c = g->univ_cell_off[u]; c < g->univ_cell_off[u + 1]; c++) n2 += g->cell_fill_type[c] == 2;
+            if (n2 > 1) return fail(MCDC_EGEOM, "universe %d has more than one cell filled by a second-level lattice", u);
+            has2[u] = n2 == 1;
+        }
+        // largest cell_bin per universe; largest (lat2_bin + cell_bin) per second-level lattice
+        std::vector<int> ubin(g->n_univ, 0), l2max(g->n_lat2, 0);
+        for (int u = 1; u < g->n_univ; u++)
+            for (int c = g->univ_cell_off[u]; c < g->univ_cell_off[u + 1]; c++) ubin[u] = std::max(ubin[u], t->cell_bin[c]);
+        for (int k = 0; k < g->n_lat2; k++) {
+            if (g->lat2_nx[k] < 1 || g->lat2_ny[k] < 1 || !(g->lat2_px[k] > 0) || !(g->lat2_py[k] > 0)) return fail(MCDC_EGEOM, "second-level lattice %d: shape", k);
+            if ((long long)g->lat2_nx[k] * g->lat2_ny[k] > 2047) return fail(MCDC_EGEOM, "second-level lattice %d has more than 2047 elements", k);
+            if (g->lat2_off[k + 1] - g->lat2_off[k] != g->lat2_nx[k] * g->lat2_ny[k]) return fail(MCDC_EINVAL, "lat2_off[%d]", k + 1);
+            for (int e = g->lat2_off[k]; e < g->lat2_off[k + 1]; e++) {
+                int u = g->lat2_univ[e];
+                if (u < 1 || u >= g->n_univ) return fail(MCDC_EGEOM, "second-level lattice %d names universe %d", k, u);
+                if (has2[u]) return fail(MCDC_EGEOM, "second-level lattice %d: universe %d holds a lattice itself (two levels at most)", k, u);
+                if (t->lat2_bin[e] < 0 || t->lat2_bin[e] >= (1 << 19)) return fail(MCDC_EINVAL, "lat2_bin out of range (0 .. 2^19 - 1)");
+                l2max[k] = std::max(l2max[k], t->lat2_bin[e] + ubin[u]);
+            }
+        }
+        // inside second-level lattice k of first-level element e the bin is lat_bin[e] + lat2_bin + cell_bin
+        for (int e = 0; e < g->lat_nx * g->lat_ny; e++) {
+            int u = g->lat_univ[e];
+            for (int c = g->univ_cell_off[u]; c < g->univ_cell_off[u + 1]; c++)
+                if (g->cell_fill_type[c] == 2 && t->lat_bin[e] + l2max[g->cell_fill[c]] >= t->n_bins)
+                    return fail(MCDC_EINVAL, "lat_bin[%d] + lat2_bin + cell_bin reaches past n_bins", e);
+        }
+    }
     for (int k = 0; k < 3; k++)
         if (!(s->hi[k] >= s->lo[k])) return fail(MCDC_EINVAL, "source box: hi < lo on axis %d", k);
     if (m) {
@@ -351,6 +441,18 @@ static int validate(const mcdc_geometry *g, const mcdc_materials *m, const mcdc_
             if (ss + m->sig_f[i] > m->sig_t[i] * (1.0 + 1e-12)) return fail(MCDC_EINVAL, "Sigma_s + Sigma_f > Sigma_t (material/group %d)", i);
         }
         if (!s->group_pdf) return fail(MCDC_EINVAL, "source group pdf missing");
+        if (m->kinetics) {  // time-dependent multi-group (R38-R40)
+            const mcdc_kinetics *kn = m->kinetics;
+            if (!kn->speed || kn->n_dgroup < 0 || kn->n_dgroup > 64) return fail(MCDC_EINVAL, "kinetics: speed / n_dgroup");
+            if (kn->n_dgroup > 0 && (!kn->nu_d || !kn->decay || !kn->chi_d)) return fail(MCDC_EINVAL, "kinetics: delayed-neutron arrays missing");
+            for (int gg = 0; gg < m->G; gg++) if (!(kn->speed[gg] > 0.0)) return fail(MCDC_EINVAL, "kinetics: speed must be > 0");
+            for (int i = 0; i < m->n_mat * kn->n_dgroup; i++) if (!(kn->decay[i] > 0.0)) return fail(MCDC_EINVAL, "kinetics: decay constants must be > 0");
+            for (int i = 0; i < m->n_mat * kn->n_dgroup * m->G; i++) if (!(kn->nu_d[i] >= 0.0) || !(kn->chi_d[i] >= 0.0)) return fail(MCDC_EINVAL, "kinetics: negative yield / spectrum");
+            if (kn->census_target < 0) return fail(MCDC_EINVAL, "kinetics: census_target");
+            if (t->n_t < 1 || !t->t_edges) return fail(MCDC_EINVAL, "time-dependent problem without time edges");
+            for (int i = 0; i < t->n_t; i++) if (!(t->t_edges[i + 1] > t->t_edges[i])) return fail(MCDC_EINVAL, "t_edges");
+            if (!(s->t >= t->t_edges[0]) || !(s->t < t->t_edges[t->n_t])) return fail(MCDC_EINVAL, "source time outside the time edges");
+        }
     } else {
         if (x->n_grid < 2 || x->n_nuc < 1) return fail(MCDC_EINVAL, "CE grid");
         for (int i = 1; i < x->n_grid; i++)
@@ -441,6 +543,9 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     int nref = g->cell_surf_off[g->n_cell];
     int nlat = g->has_lattice ? g->lat_nx * g->lat_ny : 0;
     Geo &G = c.geo;
+    G.n_lat2 = g->n_lat2;
+    G.l2_nx = L.l2_nx; G.l2_ny = L.l2_ny; G.l2_off = L.l2_off; G.l2_px = L.l2_px; G.l2_py = L.l2_py;
+    G.l2_univ = L.l2_univ; G.l2_bin = L.l2_bin; G.umid = L.umid;
     G.n_surf = g->n_surf; G.n_cell = g->n_cell; G.n_univ = g->n_univ; G.has_lat = g->has_lattice;
     G.lat_nx = g->has_lattice ? g->lat_nx : 1; G.lat_ny = g->has_lattice ? g->lat_ny : 1;
     G.lat_x0 = g->lat_x0; G.lat_y0 = g->lat_y0; G.lat_px = g->lat_px; G.lat_py = g->lat_py;
@@ -452,11 +557,15 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     G.lat_info = L.lat_info; G.cell_info = L.cell_info; G.lat_rmask = L.lat_rmask; G.ufast = L.ufast;
     G.ap_pos = L.ap_pos; G.ap_sid = L.ap_sid;
     // host staging must outlive the async copies: keep vectors until the sync at the end
-    std::vector<double> h_mg, h_tab, h_colA, h_ap_pos;
+    std::vector<double> h_mg, h_tab, h_colA, h_ap_pos, h_cum_nu, h_cumchi_d;
     std::vector<int> h_ncol, h_hash, h_ehash, h_cfill(g->cell_fill, g->cell_fill + g->n_cell), h_ap_sid;
     std::vector<int4> h_ufast, h_latinfo(nlat), h_cellinfo(g->n_cell);
     std::vector<unsigned int> h_rmask(nlat);
     for (int cc = 0; cc < g->n_cell; cc++) if (g->cell_fill_type[cc] == 1) h_cfill[cc] = 0;
+    std::vector<int> h_umid(g->n_univ, -1);
+    for (int u = 1; u < g->n_univ; u++)
+        for (int cc = g->univ_cell_off[u]; cc < g->univ_cell_off[u + 1]; cc++)
+            if (g->cell_fill_type[cc] == 2) h_umid[u] = cc;
     cudaError_t e = cudaSuccess;
 #define UP(dst, src, n) do { if (e == cudaSuccess) e = up(dst, src, (uint64_t)(n), st); } while (0)
     UP(L.surf_type, g->surf_type, g->n_surf); UP(L.surf_bc, g->surf_bc, g->n_surf);
@@ -464,6 +573,13 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     UP(L.cso, g->cell_surf_off, g->n_cell + 1); UP(L.csi, g->cell_surf_id, nref); UP(L.css, g->cell_surf_sense, nref);
     UP(L.cft, g->cell_fill_type, g->n_cell); UP(L.cfill, h_cfill.data(), g->n_cell); UP(L.cbin, t->cell_bin, g->n_cell);
     UP(L.uco, g->univ_cell_off, g->n_univ + 1);
+    UP(L.umid, h_umid.data(), g->n_univ);
+    if (g->n_lat2 > 0) {
+        int ne2 = g->lat2_off[g->n_lat2];
+        UP(L.l2_nx, g->lat2_nx, g->n_lat2); UP(L.l2_ny, g->lat2_ny, g->n_lat2); UP(L.l2_off, g->lat2_off, g->n_lat2 + 1);
+        UP(L.l2_px, g->lat2_px, g->n_lat2); UP(L.l2_py, g->lat2_py, g->n_lat2);
+        UP(L.l2_univ, g->lat2_univ, ne2); UP(L.l2_bin, t->lat2_bin, ne2);
+    }
     classify_universes(g, h_ufast);
     UP(L.ufast, h_ufast.data(), g->n_univ);
     // every axis plane of the problem gets an index the boundary codes can name (the first MAX_AXIS_PLANES of them)
@@ -583,6 +699,31 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
         UP(L.mg_blob, h_mg.data(), h_mg.size());
         c.mg_stage = L.mg_doubles * 8 <= MG_STAGE_MAX_BYTES ? (int)L.mg_doubles : 0;
         c.n_tally = t->n_bins * Gn;
+        if (m->kinetics) {  // time-dependent multi-group: cumulative yields / delayed spectra, plain left-to-right sums
+            const mcdc_kinetics *kn = m->kinetics;
+            const int J = kn->n_dgroup;
+            h_cum_nu.assign(mg * (J + 1), 0.0);
+            h_cumchi_d.assign((size_t)nm * J * Gn + 1, 0.0);
+            for (int mm = 0; mm < nm; mm++) {
+                for (int j = 0; j < J; j++) {
+                    double cc = 0.0;
+                    for (int gg = 0; gg < Gn; gg++) { cc += kn->chi_d[((size_t)mm * J + j) * Gn + gg]; h_cumchi_d[((size_t)mm * J + j) * Gn + gg] = cc; }
+                }
+                for (int gg = 0; gg < Gn; gg++) {
+                    double cn = m->nu[mm * Gn + gg];
+                    h_cum_nu[((size_t)mm * Gn + gg) * (J + 1)] = cn;
+                    for (int j = 0; j < J; j++) { cn += kn->nu_d[((size_t)mm * J + j) * Gn + gg]; h_cum_nu[((size_t)mm * Gn + gg) * (J + 1) + 1 + j] = cn; }
+                }
+            }
+            UP(L.td_speed, kn->speed, Gn); UP(L.td_cum_nu, h_cum_nu.data(), h_cum_nu.size());
+            UP(L.td_cumchi_d, h_cumchi_d.data(), (size_t)nm * J * Gn); UP(L.td_decay, kn->decay, (size_t)nm * J);
+            UP(L.t_edges, t->t_edges, t->n_t + 1);
+            c.td.on = 1; c.td.J = J; c.td.speed = L.td_speed; c.td.cum_nu = L.td_cum_nu; c.td.cumchi_d = L.td_cumchi_d; c.td.decay = L.td_decay;
+            c.ce.n_t = t->n_t; c.ce.t_edges = L.t_edges;
+            c.n_tally = t->n_bins * t->n_t * Gn;
+            if (dev->schedule != 0 || dev->persist_threshold < 0) { delete p; return fail(MCDC_EINVAL, "time-dependent multi-group runs use the default schedule (persistent kernel) only"); }
+            if ((uint64_t)kn->census_target > cap) { delete p; return fail(MCDC_EINVAL, "census_target exceeds the bank capacity"); }
+        }
     } else {
         int ng = x->n_grid, nm = x->n_mat;
         h_tab.assign((size_t)nm * ng * CE_ROW, 0.0); h_colA.assign((size_t)nm * CE_ROW, 1.0); h_ncol.assign(nm, 0);
@@ -650,7 +791,17 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
         c.n_tally = t->n_bins * t->n_t * t->n_e;
     }
     c.n_bins = t->n_bins;
-    for (int b = 0; b < 2; b++) c.bank[b] = L.bank[b];
+    for (int b = 0; b < 2; b++) { c.bank[b] = L.bank[b]; p->cb[b] = L.cb[b]; p->sort_key[b] = L.sort_key[b]; p->sort_idx[b] = L.sort_idx[b]; }
+    p->sort_hist = L.sort_hist; p->comb_copies = L.comb_copies; p->comb_offs = L.comb_offs; p->comb_w = L.comb_w;
+    p->td = m && m->kinetics; p->timed = x || p->td;
+    p->census_target = p->td ? (long long)m->kinetics->census_target : 0;
+    p->first_interval = 0;
+    if (p->timed) {
+        while (p->first_interval + 1 < t->n_t && s->t >= t->t_edges[p->first_interval + 1]) p->first_interval++;
+        if (p->td) p->persist = 0x7fffffff;  // one persistent launch per census interval
+    }
+    p->cb_cur = 0; p->census_n = 0;
+    c.cbank = L.cb[0]; c.census_stop = 0;
     c.fis = L.fis;
     c.work = L.work;
     c.cap = (unsigned int)cap;
@@ -668,7 +819,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     c.flux_copy_mask = p->flux_copies - 1;
     p->part = L.part; p->sites = L.sites;
     p->trace_base = L.trace; p->trace_count = L.trace_count;
-    p->tally_private = c.n_tally <= PRIVATE_TALLY_MAX;
+    p->tally_private = c.n_tally <= PRIVATE_TALLY_MAX && !p->td && g->n_lat2 == 0;  // those variants exist with the global tally only
     if (p->tally_private && (size_t)c.mg_stage * 8 + (size_t)c.n_tally * BS * 8 > 48 * 1024)
         c.mg_stage = 0;  // 48 KB default dynamic shared memory limit
     c.flux_aggregate = c.n_tally <= AGGREGATE_TALLY_MAX ? 1 : 0;
@@ -734,11 +885,11 @@ static unsigned int grid_for(uint64_t n)
 
 // the persistent kernel: at most the blocks that are resident at once (its idle warps wait for other warps' pushes,
 // so every block of the grid must be running)
-template <bool CE, bool PRIV, bool W> static unsigned int grid_persist(mcdc_problem *p, uint64_t n, size_t smem)
+template <bool CE, bool PRIV, bool W, int X> static unsigned int grid_persist(mcdc_problem *p, uint64_t n, size_t smem)
 {
     if (p->persist_blocks_per_sm == 0) {
         int nb = 0, sms = 148;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_persist<CE, PRIV, W>, BS, smem) != cudaSuccess || nb < 1) nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_persist<CE, PRIV, W, X>, BS, smem) != cudaSuccess || nb < 1) nb = 1;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
         p->persist_blocks_per_sm = nb;
         p->n_sm = sms;
@@ -794,7 +945,7 @@ static int device_error_code(mcdc_problem *p, int e)
     return 0;
 }
 
-template <bool CE, bool PRIV, bool W> static int transport_t(mcdc_problem *p, uint64_t M)
+template <bool CE, bool PRIV, bool W, int X> static int transport_t(mcdc_problem *p, uint64_t M)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
@@ -808,16 +959,16 @@ template <bool CE, bool PRIV, bool W> static int transport_t(mcdc_problem *p, ui
     while (upper > 0) {
         if (s > 4000000u) return fail(MCDC_ELOST, "sweep guard exceeded");
         if (p->schedule != 1 && p->persist > 0 && upper <= (uint64_t)p->persist) {
-            CUDA_OK(cudaMemsetAsync(c.work, 0, 32, st));
+            CUDA_OK(cudaMemsetAsync(c.work, 0, 16, st));  // head, pushed, ended, born; work[4] (census count) is kept
             if (CE) CUDA_OK(cudaMemsetAsync(c.bank[(s + 1) & 1].ev, 0, sizeof(uint32_t) * (size_t)p->cap, st));
-            { ProfScope ps(p, MCDC_PROF_PERSIST); k_persist<CE, PRIV, W><<<grid_persist<CE, PRIV, W>(p, upper, smem), BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_PERSIST); k_persist<CE, PRIV, W, X><<<grid_persist<CE, PRIV, W, X>(p, upper, smem), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
             p->work.host_counters[13]++;
             break;
         }
         unsigned int gr = grid_for(upper);
         if (p->schedule != 1) {
-            { ProfScope ps(p, MCDC_PROF_SWEEP); k_sweep<CE, PRIV, W><<<gr, BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_SWEEP); k_sweep<CE, PRIV, W, X><<<gr, BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
             if (p->schedule == 2) {
                 { ProfScope ps(p, MCDC_PROF_SCATTER); k_scatter<CE><<<gr, BS, smem_mg, st>>>(c, s); }
@@ -825,7 +976,7 @@ template <bool CE, bool PRIV, bool W> static int transport_t(mcdc_problem *p, ui
                 p->n_launches += 2;
             }
         } else {
-            { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV, W><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
+            { ProfScope ps(p, MCDC_PROF_SEGMENT); k_segment<CE, PRIV, W, X><<<grid_for(M), BS, smem, st>>>(c, s, n0); }
             p->n_launches++;
         }
         p->work.host_counters[13]++;
@@ -852,14 +1003,37 @@ template <bool CE, bool PRIV, bool W> static int transport_t(mcdc_problem *p, ui
     return 0;
 }
 
+// time-dependent multi-group: persistent kernel only (the host never launches anything else for it), weighted, global
+// tally; the sweep / monolithic branches of transport_t are dead code for it
+template <int X> static int transport_td(mcdc_problem *p, uint64_t M)
+{
+    Ctx &c = p->ctx;
+    cudaStream_t st = p->stream;
+    const size_t smem = (size_t)c.mg_stage * sizeof(double);
+    CUDA_OK(cudaMemsetAsync(c.qc, 0, sizeof(QCount) * RING, st));
+    CUDA_OK(cudaMemsetAsync(c.work, 0, 16, st));  // head, pushed, ended, born; work[4] (census count) is kept
+    CUDA_OK(cudaMemsetAsync(c.bank[1].ev, 0, sizeof(uint32_t) * (size_t)p->cap, st));
+    { ProfScope ps(p, MCDC_PROF_PERSIST); k_persist<false, false, true, X><<<grid_persist<false, false, true, X>(p, M, smem), BS, smem, st>>>(c, 0u, (unsigned int)M); }
+    p->n_launches++;
+    p->work.host_counters[13]++;
+    CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
 static int transport(mcdc_problem *p, uint64_t M)
 {
-    if (p->ctx.implicit) {  // weighted kernels (implicit capture, R36)
-        if (p->mode == 0) return p->tally_private ? transport_t<false, true, true>(p, M) : transport_t<false, false, true>(p, M);
-        return p->tally_private ? transport_t<true, true, true>(p, M) : transport_t<true, false, true>(p, M);
+    const bool W = p->ctx.implicit != 0, priv = p->tally_private;
+    if (p->td) return p->ctx.geo.n_lat2 ? transport_td<X_TD | X_L2>(p, M) : transport_td<X_TD>(p, M);
+    if (p->ctx.geo.n_lat2) {  // second-level lattices (R37): generic-geometry variants, global tally
+        if (p->mode == 0) return W ? transport_t<false, false, true, X_L2>(p, M) : transport_t<false, false, false, X_L2>(p, M);
+        return W ? transport_t<true, false, true, X_L2>(p, M) : transport_t<true, false, false, X_L2>(p, M);
     }
-    if (p->mode == 0) return p->tally_private ? transport_t<false, true, false>(p, M) : transport_t<false, false, false>(p, M);
-    return p->tally_private ? transport_t<true, true, false>(p, M) : transport_t<true, false, false>(p, M);
+    if (W) {  // weighted kernels (implicit capture, R36)
+        if (p->mode == 0) return priv ? transport_t<false, true, true, 0>(p, M) : transport_t<false, false, true, 0>(p, M);
+        return priv ? transport_t<true, true, true, 0>(p, M) : transport_t<true, false, true, 0>(p, M);
+    }
+    if (p->mode == 0) return priv ? transport_t<false, true, false, 0>(p, M) : transport_t<false, false, false, 0>(p, M);
+    return priv ? transport_t<true, true, false, 0>(p, M) : transport_t<true, false, false, 0>(p, M);
 }
 
 // Weight balance of the transport just finished (the scalars and counters are in pinned memory): source weight,
@@ -872,7 +1046,7 @@ static void add_balance(mcdc_problem *p, double source_weight, const uint64_t *b
     const unsigned long long *cn = p->pin->counters;
     w.balance[0] += source_weight;
     w.balance[2] += sc[1];
-    if (p->ctx.implicit) {
+    if (p->ctx.implicit || p->td) {  // the weighted kernels ran
         w.balance[1] += sc[2]; w.balance[3] += sc[3]; w.balance[4] += sc[4]; w.balance[5] += sc[5];
     } else {
         w.balance[1] += p->ctx.w0 * (double)((cn[2] - before[2]) + (cn[3] - before[3]));
@@ -981,9 +1155,182 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     return 0;
 }
 
+// ------------------------------------------------------------------ fixed source by census intervals (R40)
+// one draw of stream (seed, id, domain, cycle) on the host: the comb's offset (same Philox4x32-10 as the device's)
+static double host_draw(uint64_t seed, uint64_t id, uint32_t domain, uint32_t cycle, uint32_t index)
+{
+    uint32_t c0 = (uint32_t)id, c1 = (uint32_t)(id >> 32), c2 = (domain << 24) | cycle, c3 = index >> 1;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; r++) {
+        uint64_t p0 = 0xD2511F53ull * c0, p1 = 0xCD9E8D57ull * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    uint64_t u = (index & 1u) ? (((uint64_t)c3 << 32) | c2) : (((uint64_t)c1 << 32) | c0);
+    return ((double)(u >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+// The census bank becomes the source bank of interval k: its particles are keyed by id (those of later intervals get
+// the largest key), radix-sorted, the first M -- the particles of interval k in id order -- moved to bank[0], through
+// the comb if population control is on, and the rest kept in the other census bank.
+template <bool CE> static int census_to_source_t(mcdc_problem *p, int k, uint64_t seed, uint64_t *M_out)
+{
+    Ctx &c = p->ctx;
+    cudaStream_t st = p->stream;
+    RunStats &w = p->work;
+    const unsigned int n = (unsigned int)p->census_n;
+    *M_out = 0;
+    if (n == 0) {
+        w.census_counts.push_back(0); w.census_counts.push_back(0);
+        w.census_weights.push_back(0.0); w.census_weights.push_back(0.0);
+        return 0;
+    }
+    const Bank &S = p->cb[p->cb_cur], &KEEP = p->cb[1 - p->cb_cur];
+    const unsigned int nb = (n + BS - 1) / BS, nbt = (n + RS_TILE - 1) / RS_TILE;
+    CUDA_OK(cudaMemsetAsync(c.work + 5, 0, 4, st));
+    k_census_keys<<<nb, BS, 0, st>>>(S, n, k, p->sort_key[0], p->sort_idx[0], c.work + 5);
+    int a = 0;
+    for (int pass = 0; pass < 8; pass++, a ^= 1) {
+        k_rs_hist<<<nbt, BS, 0, st>>>(p->sort_key[a], n, 8 * pass, p->sort_hist);
+        k_scan_top<<<1, 1024, 0, st>>>(p->sort_hist, 256u * nbt);
+        k_rs_scatter<<<nbt, BS, 0, st>>>(p->sort_key[a], p->sort_idx[a], p->sort_key[1 - a], p->sort_idx[1 - a], n, 8 * pass, p->sort_hist);
+    }
+    p->n_launches += 25;
+    CUDA_OK(cudaMemcpyAsync(&p->pin->census[1], c.work + 5, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaStreamSynchronize(st));
+    const unsigned int M = p->pin->census[1];
+    const unsigned int *idx = p->sort_idx[0];
+    // total weight of the interval's particles (left-to-right sums in id order; the comb's running sums)
+    double W = (double)M;
+    const bool weighted = c.implicit || p->td;
+    if (M > 0 && weighted) {
+        k_comb_weights<<<(M + BS - 1) / BS, BS, 0, st>>>(S, idx, M, p->comb_w);
+        k_dscan<<<1, 1024, 0, st>>>(p->comb_w, M);
+        CUDA_OK(cudaMemcpyAsync(&p->pin->comb_w, p->comb_w + (M - 1), 8, cudaMemcpyDeviceToHost, st));
+        CUDA_OK(cudaStreamSynchronize(st));
+        W = p->pin->comb_w;
+        p->n_launches += 2;
+    }
+    uint64_t M_run = M;
+    double W_run = W;
+    const bool comb = p->census_target > 0 && M > 0 && weighted;
+    if (comb) {
+        const unsigned int T = (unsigned int)p->census_target;
+        const double xi = host_draw(seed, (uint64_t)k, 3u, 0u, 0u);  // the comb's own stream: domain 3, id = interval
+        k_comb_copies<<<(M + BS - 1) / BS, BS, 0, st>>>(p->comb_w, M, T, xi, p->comb_copies);
+        CUDA_OK(cudaMemcpyAsync(p->comb_offs, p->comb_copies, sizeof(unsigned int) * M, cudaMemcpyDeviceToDevice, st));
+        k_scan_top<<<1, 1024, 0, st>>>(p->comb_offs, M);
+        k_comb_write<CE><<<(M + BS - 1) / BS, BS, 0, st>>>(S, idx, p->comb_copies, p->comb_offs, p->comb_w, M, T, seed, k, c.bank[0]);
+        p->n_launches += 3;
+        M_run = T;
+        W_run = W / (double)T * (double)T;
+    }
+    k_census_move<CE><<<nb, BS, 0, st>>>(S, idx, M, n, c.bank[0], KEEP, comb ? 0 : 1);
+    p->n_launches++;
+    // the kept particles are the new census bank; the interval's launch appends to it
+    p->cb_cur = 1 - p->cb_cur;
+    c.cbank = p->cb[p->cb_cur];
+    p->census_n = n - M;
+    p->pin->census[2] = n - M;
+    CUDA_OK(cudaMemcpyAsync(c.work + 4, &p->pin->census[2], 4, cudaMemcpyHostToDevice, st));
+    CUDA_OK(cudaGetLastError());
+    w.census_counts.push_back(M); w.census_counts.push_back(M_run);
+    w.census_weights.push_back(W); w.census_weights.push_back(W_run);
+    *M_out = M_run;
+    return 0;
+}
+
+// one census interval of a fixed-source run (time edge k -> k + 1)
+static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
+{
+    Ctx &c = p->ctx;
+    cudaStream_t st = p->stream;
+    const int n_t = c.ce.n_t;
+    if (N < 1 || capacity_for(N) > p->cap) return fail(MCDC_EINVAL, "n_particles exceeds the capacity this problem was created for");
+    if (N > 60000000ull) return fail(MCDC_EINVAL, "at most 6e7 source particles per fixed-source run (32-bit secondary counters)");
+    if (p->schedule == 1) return fail(MCDC_EINVAL, "census intervals need the persistent kernel (schedule 0 or 2)");
+    if (k < p->first_interval || k >= n_t) return fail(MCDC_EINVAL, "census interval %d outside [%d, %d)", k, p->first_interval, n_t);
+    if (k == p->first_interval) {
+        int rc = begin_run(p);
+        if (rc) return rc;
+        CUDA_OK(cudaMemsetAsync(c.work, 0, 32, st));
+        CUDA_OK(cudaMemsetAsync(c.scal, 0, 64, st));
+        p->cb_cur = 0; c.cbank = p->cb[0]; p->census_n = 0;
+    } else if (p->work.next_interval != k) return fail(MCDC_EINVAL, "census intervals must be run in order: expected %d, got %d", p->work.next_interval, k);
+    RunStats &w = p->work;
+    c.seed = seed; c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
+    c.max_secondaries = 64ull * (N + (uint64_t)p->census_target * (uint64_t)n_t) + 4096;  // R25a
+    c.census_stop = k + 1 < n_t ? 1 : 0;
+    CUDA_OK(cudaEventRecord(p->t0, st));
+    uint64_t M = 0;
+    if (k == p->first_interval) {
+        const unsigned int nbk = (unsigned int)((N + BS - 1) / BS);
+        if (p->mode == 1) k_source<true><<<nbk, BS, 0, st>>>(c, (unsigned int)N);
+        else k_source<false, true><<<nbk, BS, 0, st>>>(c, (unsigned int)N);
+        p->n_launches++;
+        M = N;
+        w.census_counts.push_back(N); w.census_counts.push_back(N);
+        w.census_weights.push_back((double)N); w.census_weights.push_back((double)N);
+        w.host_counters[0] = N;
+    } else {
+        int rc = p->mode == 1 ? census_to_source_t<true>(p, k, seed, &M) : census_to_source_t<false>(p, k, seed, &M);
+        if (rc) return abandon(p, rc);
+    }
+    if (M > 0) {
+        const int keep = p->persist;
+        p->persist = 0x7fffffff;  // the census lives in the persistent kernel
+        int rc = transport(p, M);
+        p->persist = keep;
+        if (rc) return abandon(p, rc);
+    }
+    CUDA_OK(cudaEventRecord(p->t1, st));
+    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[w.set], p->flux_acc2[w.set],
+                                                          c.n_tally, 1.0 / (double)N, 1);
+    p->n_launches++;
+    CUDA_OK(cudaMemcpyAsync(&p->pin->census[0], c.work + 4, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaMemcpyAsync(p->pin->counters, c.counters, sizeof p->pin->counters, cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaMemcpyAsync(&p->pin->err, c.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaStreamSynchronize(st));
+    CUDA_OK(cudaGetLastError());
+    profile_collect(p);
+    int rc = device_error_code(p, p->pin->err);
+    if (rc) return abandon(p, rc);
+    p->census_n = p->pin->census[0];
+    if (p->census_n > p->cap) return abandon(p, fail(MCDC_EBANK, "census bank overflow (capacity %llu)", (unsigned long long)p->cap));
+    float ms = 0.f;
+    CUDA_OK(cudaEventElapsedTime(&ms, p->t0, p->t1));
+    p->ms_transport += ms;
+    // results so far (the scalars and counters run over all intervals of the run)
+    const double k_c = p->pin->scal[0] / (double)N, leak = p->pin->scal[1] / (double)N;
+    w.k_cycle.assign(1, k_c);
+    w.k_acc = k_c; w.k_acc2 = k_c * k_c; w.leak_acc = leak; w.leak_acc2 = leak * leak; w.n_active = 1;
+    w.host_counters[12] = std::max<uint64_t>(w.host_counters[12], std::max<uint64_t>(p->census_n, M));
+    for (int i = 0; i < 6; i++) w.balance[i] = 0.0;
+    {
+        const uint64_t zero[MCDC_N_COUNTERS] = {0};
+        // weight started: source particles (1 each) + children (continuous energy: 1 each; multi-group: the parent's, scal[6])
+        const double started = (double)N + (p->td ? p->pin->scal[6] : (double)p->pin->counters[15]);
+        add_balance(p, started, zero);
+    }
+    w.next_interval = k + 1;
+    p->bank_count = 0;
+    p->last_N = N;
+    publish(p);
+    return 0;
+}
+
 extern "C" int mcdc_run_cycle(mcdc_problem *p, uint64_t N, uint32_t cycle, int32_t active, uint64_t seed, double *k_cycle)
 {
-    if (!p || p->mode != 0) return fail(MCDC_EINVAL, "mcdc_run_cycle needs a multi-group problem");
+    if (!p) return fail(MCDC_EINVAL, "null");
+    if (p->timed) {  // fixed-source problem: one census interval
+        int rc = interval_internal(p, N, (int)cycle, seed);
+        if (rc) return rc;
+        if (k_cycle) *k_cycle = p->work.k_cycle.back();
+        return 0;
+    }
+    if (p->mode != 0) return fail(MCDC_EINVAL, "mcdc_run_cycle needs a multi-group problem");
     if (cycle == 0) { int rc = begin_run(p); if (rc) return rc; }
     int rc = cycle_internal(p, N, cycle, active, seed, cycle == 0, nullptr);
     if (rc) return rc;
@@ -994,7 +1341,7 @@ extern "C" int mcdc_run_cycle(mcdc_problem *p, uint64_t N, uint32_t cycle, int32
 
 extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t N, int32_t n_inactive, int32_t n_active, uint64_t seed)
 {
-    if (!p || p->mode != 0) return fail(MCDC_EINVAL, "mcdc_run_eigenvalue needs a multi-group problem");
+    if (!p || p->mode != 0 || p->td) return fail(MCDC_EINVAL, "mcdc_run_eigenvalue needs a multi-group eigenvalue problem");
     if (n_inactive < 0 || n_active < 0) return fail(MCDC_EINVAL, "cycle counts");
     int rc = begin_run(p);
     if (rc) return rc;
@@ -1010,7 +1357,7 @@ extern "C" int mcdc_run_cycle_host(mcdc_problem *p, uint64_t N, uint32_t cycle, 
                                    const mcdc_site *sites_in, uint64_t n_in, mcdc_site *sites_out, uint64_t max_out,
                                    uint64_t *n_out, double *flux_cycle, double *k_cycle, double *leak_cycle)
 {
-    if (!p || p->mode != 0) return fail(MCDC_EINVAL, "mcdc_run_cycle_host needs a multi-group problem");
+    if (!p || p->mode != 0 || p->td) return fail(MCDC_EINVAL, "mcdc_run_cycle_host needs a multi-group eigenvalue problem");
     static_assert(sizeof(Site) == sizeof(mcdc_site), "site layout");
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
@@ -1043,7 +1390,14 @@ extern "C" int mcdc_run_cycle_host(mcdc_problem *p, uint64_t N, uint32_t cycle, 
 
 extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
 {
-    if (!p || p->mode != 1) return fail(MCDC_EINVAL, "mcdc_run_fixed_source needs a continuous-energy problem");
+    if (!p || !p->timed) return fail(MCDC_EINVAL, "mcdc_run_fixed_source needs a continuous-energy or a time-dependent multi-group problem");
+    if (p->td) {  // census interval by census interval (population control happens between them, R40)
+        for (int k = p->first_interval; k < p->ctx.ce.n_t; k++) {
+            int rc = interval_internal(p, N, k, seed);
+            if (rc) return rc;
+        }
+        return 0;
+    }
     if (N < 1 || capacity_for(N) > p->cap) return fail(MCDC_EINVAL, "n_particles exceeds the capacity this problem was created for");
     if (N > 60000000ull) return fail(MCDC_EINVAL, "at most 6e7 source particles per fixed-source run (32-bit secondary counters)");
     Ctx &c = p->ctx;
@@ -1051,6 +1405,7 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
     int rc = begin_run(p);
     if (rc) return rc;
     c.seed = seed; c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
+    c.census_stop = 0;  // one launch to the last time edge: a census is a synchronisation point only (R24)
     c.max_secondaries = 64 * N + 4096;  // R25a: the prompt chain must die out
     CUDA_OK(cudaMemsetAsync(c.scal, 0, 64, st));
     CUDA_OK(cudaEventRecord(p->t0, st));
@@ -1109,6 +1464,16 @@ extern "C" int mcdc_set_physics(mcdc_problem *p, const mcdc_physics *ph)
     c.kT = ph->kT;
     c.implicit = ph->implicit_capture ? 1 : 0;
     c.w_roulette = ph->w_roulette; c.w_survive = ph->w_survive;
+    return 0;
+}
+
+extern "C" int mcdc_get_census(const mcdc_problem *p, uint64_t *counts, double *weights, int32_t max, int32_t *n)
+{
+    if (!p || !counts || !weights || !n) return fail(MCDC_EINVAL, "null");
+    const RunStats &r = p->pub;
+    int m = (int)std::min<size_t>(r.census_counts.size() / 2, (size_t)std::max(max, 0));
+    for (int i = 0; i < 2 * m; i++) { counts[i] = r.census_counts[i]; weights[i] = r.census_weights[i]; }
+    *n = m;
     return 0;
 }
 

@@ -66,6 +66,16 @@ CASES = {
     "mirror_sphere": lambda: inputs.curved_mirror("sphere", n_particles=3000, n_inactive=1, n_active=2),
     "mirror_cyl_z": lambda: inputs.curved_mirror("cyl_z", n_particles=3000, n_inactive=1, n_active=2),
     "mirror_cyl_x": lambda: inputs.curved_mirror("cyl_x", n_particles=3000, n_inactive=1, n_active=2),
+    # two-level lattices (R37): assemblies of pin lattices, 2-D and finite height, a homogeneous reflector assembly, an
+    # assembly universe with a moderator gap around its pin lattice (surfaces of the cell the inner lattice fills)
+    "C4_2l": lambda: inputs.config4(n_particles=4000, n_inactive=1, n_active=2, n_asm=2, n_pin=3, n_refl=3, two_level=True),
+    "C4_2l_3d": lambda: inputs.config4(n_particles=3000, n_inactive=1, n_active=2, n_asm=1, n_pin=4, n_refl=4, two_level=True,
+                                      height=6.0),
+    "C4_2l_homog": lambda: inputs.config4(n_particles=3000, n_inactive=1, n_active=2, n_asm=2, n_pin=3, n_refl=3, two_level=True,
+                                         reflector_lattice=False),
+    "C4_2l_17": lambda: inputs.config4(n_particles=5000, n_inactive=1, n_active=2, two_level=True),
+    "asm_gap": lambda: inputs.assembly_gap(2, 3),
+    "asm_gap_wide": lambda: inputs.assembly_gap(3, 2, gap=0.6),
     "slab": lambda: inputs.slab_beam(n_particles=5000),
     "sphere": lambda: inputs.sphere_absorber(n_particles=5000),
 }
@@ -96,7 +106,7 @@ def test_mg_parity(gpu, orc, name, schedule, persist):
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d", "lat1x6", "lat3x5", "mirror_sphere",
-                                  "mirror_cyl_x"])
+                                  "mirror_cyl_x", "C4_2l", "C4_2l_3d", "C4_2l_homog", "asm_gap", "asm_gap_wide"])
 @pytest.mark.parametrize("schedule,persist", [(0, -1), (0, 0), (1, 0), (2, -1), (0, 100)])
 def test_mg_traces_identical(gpu, orc, name, schedule, persist):
     """100 particles x 2 cycles: identical per-particle event sequences (SURVEY.md 8d parity protocol 1)."""
@@ -186,7 +196,7 @@ def test_geometry_unit_parity(gpu, orc, height):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5"])
+@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5", "C4_2l", "C4_2l_3d", "asm_gap", "C4_2l_17"])
 def test_geometry_unit_parity_plain_cells(gpu, orc, name):
     """Cells outside a lattice (box, pin cell: straight-line path; mixed surfaces: generic loops) and a small lattice:
     locate + nearest boundary of random points, every device path against the oracle."""
@@ -282,6 +292,39 @@ def test_segment_guard(gpu, orc):
         g.run()
     assert e.value.code == -4
     g.close()
+
+
+def test_two_level_equals_flat_on_gpu(gpu):
+    """The same quarter core as one flat lattice (straight-line geometry path) and as a lattice of lattices (generic
+    path): identical event counters and fission bank, k per cycle and per-pin flux to rounding."""
+    kw = dict(n_particles=20000, n_inactive=1, n_active=2)
+    gf = gpu.Problem(inputs.config4(**kw))
+    g2 = gpu.Problem(inputs.config4(two_level=True, **kw))
+    rf, r2 = gf.run(), g2.run()
+    assert np.allclose(rf["k_cycle"], r2["k_cycle"], rtol=1e-11)
+    assert (rf["counters"][:12] == r2["counters"][:12]).all()
+    assert np.allclose(rf["flux_mean"], r2["flux_mean"], rtol=1e-9, atol=1e-13 * rf["flux_mean"].max())
+    bf, b2 = gf.bank(), g2.bank()
+    assert len(bf) == len(b2) and (bf["g"] == b2["g"]).all() and np.allclose(bf["x"], b2["x"], rtol=0, atol=1e-10)
+    gf.close()
+    g2.close()
+
+
+def test_two_level_validation(gpu):
+    P = inputs.assembly_gap(2, 3)
+    for key, val in (("lat2_off", np.array([0, 8], np.int32)), ("lat2_univ", np.full(9, 3, np.int32)),
+                     ("lat2_bin", np.full(9, 10_000, np.int32)), ("lat2_nx", np.array([0], np.int32))):
+        bad = dict(P)
+        bad[key] = val
+        with pytest.raises(gpu.McdcError) as e:
+            gpu.Problem(bad)
+        assert e.value.code in (-1, -2), key
+    bad = dict(P)
+    bad["cell_fill"] = P["cell_fill"].copy()
+    bad["cell_fill"][P["cell_fill_type"] == 2] = 1  # names a second-level lattice that does not exist
+    with pytest.raises(gpu.McdcError) as e:
+        gpu.Problem(bad)
+    assert e.value.code == -2
 
 
 def test_validation_errors(gpu):

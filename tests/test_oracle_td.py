@@ -108,6 +108,8 @@ def test_td_population_control_is_unbiased_and_conserves_weight(orc):
         for before, after, w_before, w_after in cen[1:]:
             assert after == target and before > 0
             assert w_after == pytest.approx(w_before, rel=1e-12)
+        b = o.balance()  # tracks replaced by the comb are neither lost nor counted twice
+        assert b["absorbed"] + b["leaked"] + b["cutoff"] + b["roulette_loss"] - b["roulette_gain"] == pytest.approx(b["source"], rel=1e-10)
 
 
 def test_td_time_edges_are_census_points(orc):
