@@ -146,7 +146,8 @@ def job_value(units_per_rank: float, world: int, seconds_max: float) -> float:
 WORKLOADS = {"C1": ("C1: 1-group infinite medium (reflecting unit cube)", 10_000),
              "C2": ("C2: 7-group infinite medium (reflecting unit cube)", 100_000),
              "C3": ("C3: 2-D pin cell, 7 groups", 1_000_000),
-             "C4": ("C4: 2-D quarter core, 7 groups, 2x2 17x17-pin assemblies + reflector, k-eigenvalue cycle", 10_000_000)}
+             "C4": ("C4: 2-D quarter core, 7 groups, 2x2 17x17-pin assemblies + reflector, k-eigenvalue cycle", 10_000_000),
+             "C4_2L": ("C4 as a two-level lattice (assemblies of pin lattices; generic geometry path)", 10_000_000)}
 
 
 def workload(args):
@@ -154,7 +155,8 @@ def workload(args):
     BASELINE.json configurations with the same code path (documentation runs, not the headline)."""
     from paper_2501_05440_b200 import inputs
     N = args.particles if args.particles else WORKLOADS[args.config][1]
-    fn = {"C1": inputs.config1, "C2": inputs.config2, "C3": inputs.config3, "C4": inputs.config4}[args.config]
+    fn = {"C1": inputs.config1, "C2": inputs.config2, "C3": inputs.config3, "C4": inputs.config4,
+          "C4_2L": lambda **kw: inputs.config4(two_level=True, **kw)}[args.config]
     return fn(n_particles=N, n_inactive=args.warmup, n_active=args.steps), N
 
 

@@ -473,6 +473,9 @@ __global__ void __launch_bounds__(BS) k_surface(Ctx c, unsigned int s)
 #ifndef MCDC_PERSIST_MINBLOCKS
 #define MCDC_PERSIST_MINBLOCKS 3
 #endif
+#ifndef MCDC_PERSIST_MINBLOCKS_CE
+#define MCDC_PERSIST_MINBLOCKS_CE 3  // resident blocks per SM the continuous-energy variant is compiled for
+#endif
 #ifndef MCDC_REFILL
 #define MCDC_REFILL 4  // dead lanes without a ticket at which a warp goes back to the queue
 #endif
@@ -539,7 +542,8 @@ __device__ __forceinline__ bool make_child_td(const Ctx &c, Rng &rng, int mat, i
 }
 
 template <bool CE, bool PRIVATE, bool W, int X>
-__global__ void __launch_bounds__(BS, MCDC_PERSIST_MINBLOCKS * 256 / BS) k_persist(Ctx c, unsigned int s, unsigned int n0)
+__global__ void __launch_bounds__(BS, (CE ? MCDC_PERSIST_MINBLOCKS_CE : MCDC_PERSIST_MINBLOCKS) * 256 / BS)
+k_persist(Ctx c, unsigned int s, unsigned int n0)
 {
     constexpr bool TD = (X & X_TD) != 0;
     constexpr bool GROW = CE || TD;  // fissions put secondaries into the running population: the work queue grows

@@ -137,3 +137,55 @@ def test_c5_full(gpu, orc):
     kg = r["counters"][11] / r["counters"][0]
     ko = ro["counters"][11] / ro["counters"][0]
     assert abs(kg - ko) < 0.02
+
+
+def test_c4_two_level_full_equals_flat(gpu, orc):
+    """C4 at 10^7 particles per cycle described as a lattice of assemblies of 17 x 17 pin lattices (R37): the same
+    random numbers meet the same geometry, so counters and the fission bank size equal the flat run's, k and the per-pin
+    flux agree to rounding; 150 sampled histories equal the oracle's event by event."""
+    N = 10_000_000
+    gf = gpu.Problem(inputs.config4())
+    kf = [gf.run_cycle(N, c, 1, 1) for c in range(2)]
+    rf = gf.results()
+    nf = gf.dims().bank_count
+    gf.close()
+    P2 = inputs.config4(two_level=True)
+    g2 = gpu.Problem(P2)
+    g2.set_trace(77_000, 150, 2048)
+    k2 = [g2.run_cycle(N, c, 1, 1) for c in range(2)]
+    r2 = g2.results()
+    assert g2.dims().bank_count == nf
+    assert np.allclose(kf, k2, rtol=1e-10)
+    assert (rf["counters"][:12] == r2["counters"][:12]).all()
+    assert np.allclose(rf["flux_mean"], r2["flux_mean"], rtol=1e-8, atol=1e-12 * rf["flux_mean"].max())
+    invariants(r2)
+    tg = g2.trace()
+    tg = tg[tg["cycle"] == 0]
+    o = orc.Oracle(P2)
+    o.set_trace(77_000, 150, 1_000_000)
+    o.run(n_particles=77_150, n_inactive=0, n_active=1)
+    compare_traces(tg, o.trace())
+    g2.close()
+
+
+def test_td_full_equals_kinetics(gpu):
+    """Time-dependent multi-group at 10^6 source particles with the comb on (census_target 5 x 10^5): the flux in every
+    time bin and group equals the closed-form kinetics integral of the infinite medium (tests/test_oracle_td.py) within
+    5 sigma, sigma from 8 seeds at 10^5; population and weight at every census as the comb prescribes."""
+    from tests.test_oracle_td import kinetics_flux
+    P = inputs.td_infinite(n_particles=1_000_000, G=2, census_target=500_000)
+    ref = kinetics_flux(P)
+    g = gpu.Problem(P)
+    r = g.run()
+    f = r["flux_mean"].reshape(8, 2)
+    cen = g.census()
+    assert len(cen) == 8 and cen[0][1] == 1_000_000 and all(c[1] == 500_000 for c in cen[1:])
+    assert all(abs(c[3] - c[2]) <= 1e-9 * c[2] for c in cen)
+    g.close()
+    Ps = inputs.td_infinite(n_particles=100_000, G=2, census_target=50_000)
+    gs = gpu.Problem(Ps)
+    runs = np.array([gs.run(seed=s)["flux_mean"].reshape(8, 2) for s in range(10, 18)])
+    gs.close()
+    sig = runs.std(0, ddof=1)
+    assert (np.abs(runs.mean(0) - ref) < 5 * sig / math.sqrt(8) + 1e-4 * ref).all()
+    assert (np.abs(f - ref) < 5 * sig / math.sqrt(10) + 1e-4 * ref).all(), (f, ref, sig)
