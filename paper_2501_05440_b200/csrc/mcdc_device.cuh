@@ -48,6 +48,7 @@ struct Geo {
     // first-level element that holds a second-level lattice is never LAT_FAST (generic geometry path).
     int n_lat2;
     const int *l2_nx, *l2_ny, *l2_off, *l2_univ, *l2_bin, *umid;
+    const int4 *l2_info;
     const double *l2_px, *l2_py;
 };
 constexpr int INNER_SHIFT = 20;
@@ -55,6 +56,12 @@ constexpr int HIT_BITS = 12;  // hit codes (surfaces, lattice walls) are below P
 __device__ __forceinline__ int outer_of(const Geo &, int elem) { return elem & ((1 << INNER_SHIFT) - 1); }
 __device__ __forceinline__ int inner_of(const Geo &, int elem) { return (elem >> INNER_SHIFT) - 1; }
 constexpr int LAT_FAST = 1 << 30, CELL_FAST = 1 << 30, CELL_NO_NEIGHBOUR = (1 << 30) - 1;
+// LAT_FAST2 (lat_info[e].x): the element's universe is ONE cell without surfaces filled by second-level lattice k
+// (k in the high 16 bits of lat_info[e].w) and the enclosing cell's surfaces fit the boundary-code pattern: elements
+// of that lattice whose own universe is simple (l2_info[..].x & LAT_FAST) take the two-level straight-line path.
+// l2_info[l2_off[k] + i]: x = universe | LAT_FAST, y = tally-bin offset, z = codes for -x,+x,-y,+y: 1 = second-level
+// wall (an event), 3 = the lattice's rim (the first-level element's code for that direction applies).
+constexpr int LAT_FAST2 = 1 << 29, UNIV_MASK = (1 << 29) - 1;
 
 struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi running chi sums.  One contiguous
     int G, n_mat, blob_doubles;  // blob: the transport kernels copy it to shared memory when it fits
@@ -393,7 +400,7 @@ __device__ __forceinline__ void local_xy(const Geo &G, int elem, double x, doubl
     yl = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
 }
 
-__device__ __forceinline__ int elem_universe(const Geo &G, int elem) { return __ldg(&G.lat_info[elem].x) & (LAT_FAST - 1); }
+__device__ __forceinline__ int elem_universe(const Geo &G, int elem) { return __ldg(&G.lat_info[elem].x) & UNIV_MASK; }
 
 // second-level lattice k: lower-left corner in its universe's coordinates (centred on the origin, R37)
 __device__ __forceinline__ double l2_x0(const Geo &G, int k) { return -0.5 * (__ldg(G.l2_nx + k) * __ldg(G.l2_px + k)); }
@@ -734,6 +741,87 @@ __device__ __forceinline__ double nearest_fast(const Geo &G, int codes_xy, int c
     return best;
 }
 
+// Straight-line path inside a second-level lattice (R37; see LAT_FAST2): per axis ONE candidate -- the second-level
+// wall ahead, or at the lattice's rim what the first-level element's code names (first-level wall or an axis plane of
+// the enclosing cell) -- plus the pin universe's z-cylinder.  Same formulas, coordinates (global -> first-level element
+// -> second-level element, two subtractions) and candidate order as nearest2: the enclosing cell's planes, the
+// cylinder, second-level walls, first-level walls.
+__device__ __forceinline__ double nearest_fast2(const Geo &G, const int4 li, const int4 l2i, int cyl, double x, double y, double z,
+                                                double ux, double uy, double uz, int elem, int last, int &hit)
+{
+    const double INF = __longlong_as_double(0x7ff0000000000000LL);
+    const int outer = outer_of(G, elem), inner = inner_of(G, elem), k = li.w >> 16;
+    int ix, iy;
+    elem_xy(G, outer, ix, iy);
+    const int nx2 = __ldg(G.l2_nx + k);
+    const int jy = inner / nx2, jx = inner - jy * nx2;
+    const double px2 = __ldg(G.l2_px + k), py2 = __ldg(G.l2_py + k);
+    const double x02 = l2_x0(G, k), y02 = l2_y0(G, k);
+    const double xo = x - (G.lat_x0 + (ix + 0.5) * G.lat_px), yo = y - (G.lat_y0 + (iy + 0.5) * G.lat_py);
+    const double xl = xo - (x02 + (jx + 0.5) * px2), yl = yo - (y02 + (jy + 0.5) * py2);
+    const double inv_ux = 1.0 / ux, inv_uy = 1.0 / uy;
+    const bool xp = ux > 0.0, yp = uy > 0.0, zp = uz > 0.0;
+    // kind per axis: 0 nothing, 1 axis plane of the enclosing cell, 2 second-level wall, 3 first-level wall
+    int kx = 2, ky = 2, hx = G.n_surf + 4 + (xp ? 1 : 0), hy = G.n_surf + 6 + (yp ? 1 : 0);
+    double dx = (x02 + (jx + (xp ? 1 : 0)) * px2 - xo) * inv_ux, dy = (y02 + (jy + (yp ? 1 : 0)) * py2 - yo) * inv_uy;
+    if (((l2i.z >> (xp ? 8 : 0)) & 255) == 3) {
+        const int co = (li.z >> (xp ? 8 : 0)) & 255;
+        kx = co == 0 ? 0 : (co == 1 ? 3 : 1);
+        double pw = G.lat_x0 + (ix + (xp ? 1 : 0)) * G.lat_px;
+        hx = G.n_surf + (xp ? 1 : 0);
+        if (co >= 2) { pw = __ldg(G.ap_pos + co - 2); hx = __ldg(G.ap_sid + co - 2); }
+        dx = (pw - x) * inv_ux;
+    }
+    if (((l2i.z >> (yp ? 24 : 16)) & 255) == 3) {
+        const int co = (li.z >> (yp ? 24 : 16)) & 255;
+        ky = co == 0 ? 0 : (co == 1 ? 3 : 1);
+        double pw = G.lat_y0 + (iy + (yp ? 1 : 0)) * G.lat_py;
+        hy = G.n_surf + 2 + (yp ? 1 : 0);
+        if (co >= 2) { pw = __ldg(G.ap_pos + co - 2); hy = __ldg(G.ap_sid + co - 2); }
+        dy = (pw - y) * inv_uy;
+    }
+    if (kx == 0 || ux == 0.0 || hx == last || !(dx > 0.0)) dx = INF;
+    if (ky == 0 || uy == 0.0 || hy == last || !(dy > 0.0)) dy = INF;
+    const int cz = (li.w >> (zp ? 8 : 0)) & 255;
+    double dz = INF;
+    int hz = -1;
+    if (cz >= 2) {
+        hz = __ldg(G.ap_sid + cz - 2);
+        if (uz != 0.0 && hz != last) { dz = (__ldg(G.ap_pos + cz - 2) - z) / uz; if (!(dz > 0.0)) dz = INF; }
+    }
+    double dc = INF;
+    if (cyl >= 0) {
+        const double *q = G.surf_param + 4 * cyl;
+        const double da = xl - __ldg(q), db = yl - __ldg(q + 1), r = __ldg(q + 2);
+        const double a = ux * ux + uy * uy, kk = da * ux + db * uy;
+        double num = -1.0;
+        if (cyl == last) { if (kk < 0.0) num = -2.0 * kk; }
+        else {
+            const double cc = da * da + db * db - r * r;
+            const double disc = kk * kk - a * cc;
+            if (disc >= 0.0) {
+                const double sq = sqrt(disc);
+                num = cc < 0.0 ? sq - kk : -kk - sq;
+            }
+        }
+        if (a != 0.0 && num > 0.0) {
+            dc = num / a;
+            if (!(dc > 0.0)) dc = INF;
+        }
+    }
+    double best = INF;
+    hit = -1;
+    if (kx == 1 && dx < best) { best = dx; hit = hx; }
+    if (ky == 1 && dy < best) { best = dy; hit = hy; }
+    if (dz < best) { best = dz; hit = hz; }
+    if (dc < best) { best = dc; hit = cyl; }
+    if (kx == 2 && dx < best) { best = dx; hit = hx; }
+    if (ky == 2 && dy < best) { best = dy; hit = hy; }
+    if (kx == 3 && dx < best) { best = dx; hit = hx; }
+    if (ky == 3 && dy < best) { best = dy; hit = hy; }
+    return best;
+}
+
 __device__ __forceinline__ bool surface_in_cell(const Geo &G, int c, int s)
 {
     int k1 = __ldg(G.cso + c + 1);
@@ -869,7 +957,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     if (p.elem >= 0) {
         li = __ldg(G.lat_info + (L2 ? outer_of(G, p.elem) : p.elem));
         bin += li.y;
-        cyl = __ldg(&G.ufast[li.x & (LAT_FAST - 1)].y);
+        cyl = __ldg(&G.ufast[li.x & UNIV_MASK].y);
     } else {
         li = __ldg(G.cell_info + p.cell);
         cyl = li.y;
@@ -904,7 +992,13 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     double d_coll = -log(rng.next(c)) / sig_t;
     int hit;
     double d_surf;
-    if (li.x & LAT_FAST) d_surf = nearest_fast(G, li.z, li.w, cyl, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.elem, p.last, hit);
+    int4 l2i = make_int4(0, 0, 0, 0);
+    if (L2 && p.elem >= (1 << INNER_SHIFT) && (li.x & LAT_FAST2))  // second-level element of a simple assembly (R37)
+        l2i = __ldg(G.l2_info + __ldg(G.l2_off + (li.w >> 16)) + inner_of(G, p.elem));
+    if (L2 && (l2i.x & LAT_FAST)) {
+        bin += l2i.y;
+        d_surf = nearest_fast2(G, li, l2i, __ldg(&G.ufast[l2i.x & UNIV_MASK].y), p.x, p.y, p.z, p.ux, p.uy, p.uz, p.elem, p.last, hit);
+    } else if (li.x & LAT_FAST) d_surf = nearest_fast(G, li.z, li.w, cyl, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.elem, p.last, hit);
     else {
         unsigned int root_mask = p.elem >= 0 ? __ldg(G.lat_rmask + (L2 ? outer_of(G, p.elem) : p.elem)) : 0xffffffffu;
         if (L2) {
@@ -1270,7 +1364,7 @@ __device__ __forceinline__ int do_surface_fast(const Geo &G, Particle &p, int hi
         int e2 = p.elem + (w == 0 ? -1 : w == 1 ? 1 : w == 2 ? -G.lat_nx : G.lat_nx);
         const int4 l2 = __ldg(G.lat_info + e2);
         if (!(l2.x & LAT_FAST)) return 0;
-        const int4 uf = __ldg(G.ufast + (l2.x & (LAT_FAST - 1)));
+        const int4 uf = __ldg(G.ufast + (l2.x & UNIV_MASK));
         p.elem = e2;
         p.last = -1;
         int cell = uf.z;
@@ -1305,6 +1399,70 @@ __device__ __forceinline__ int do_surface_fast(const Geo &G, Particle &p, int hi
     return 0;
 }
 
+// Surface event from a second-level element on the two-level straight-line path (see nearest_fast2): second-level wall
+// into a simple element of the same lattice, first-level wall into a LAT_FAST2 element (the second-level index by floor,
+// clamped, as in descend), the pin's z-cylinder, a reflecting axis plane.  0: none of these (generic path), 1 done.
+__device__ __forceinline__ int do_surface_fast2(const Geo &G, Particle &p, int hit, const int4 li, const int4 l2i)
+{
+    const int outer = outer_of(G, p.elem), inner = inner_of(G, p.elem);
+    if (hit >= G.n_surf) {
+        int e2 = outer, k = li.w >> 16, inner2;
+        double xo, yo;
+        if (hit >= G.n_surf + 4) {
+            const int w = hit - G.n_surf - 4, nx2 = __ldg(G.l2_nx + k);
+            inner2 = inner + (w == 0 ? -1 : w == 1 ? 1 : w == 2 ? -nx2 : nx2);
+            local_xy(G, outer, p.x, p.y, xo, yo);
+        } else {
+            const int w = hit - G.n_surf;
+            e2 = outer + (w == 0 ? -1 : w == 1 ? 1 : w == 2 ? -G.lat_nx : G.lat_nx);
+            const int4 li2 = __ldg(G.lat_info + e2);
+            if (!(li2.x & LAT_FAST2)) return 0;
+            k = li2.w >> 16;
+            local_xy(G, e2, p.x, p.y, xo, yo);
+            const int nx2 = __ldg(G.l2_nx + k), ny2 = __ldg(G.l2_ny + k);
+            int jx = (int)floor((xo - l2_x0(G, k)) / __ldg(G.l2_px + k));
+            int jy = (int)floor((yo - l2_y0(G, k)) / __ldg(G.l2_py + k));
+            jx = jx < 0 ? 0 : (jx > nx2 - 1 ? nx2 - 1 : jx);
+            jy = jy < 0 ? 0 : (jy > ny2 - 1 ? ny2 - 1 : jy);
+            inner2 = jy * nx2 + jx;
+        }
+        const int4 l2n = __ldg(G.l2_info + __ldg(G.l2_off + k) + inner2);
+        if (!(l2n.x & LAT_FAST)) return 0;
+        const int4 uf = __ldg(G.ufast + (l2n.x & UNIV_MASK));
+        int cell = uf.z;
+        if (uf.y >= 0) {
+            double xl, yl;
+            inner_xy(G, k, inner2, xo, yo, xl, yl);
+            const double *q = G.surf_param + 4 * uf.y;
+            const double da = xl - __ldg(q), db = yl - __ldg(q + 1), r = __ldg(q + 2);
+            cell = (da * da + db * db - r * r > 0.0) ? uf.w : uf.z;
+        }
+        p.elem = e2 | ((inner2 + 1) << INNER_SHIFT);
+        p.cell = cell;
+        p.last = -1;
+        return 1;
+    }
+    const int4 uf = __ldg(G.ufast + (l2i.x & UNIV_MASK));
+    if (hit == uf.y) {
+        if (__ldg(G.surf_bc + hit) != 0) return 0;
+        double xl, yl;
+        innermost_xy(G, p.elem, p.x, p.y, xl, yl);
+        const double *q = G.surf_param + 4 * hit;
+        const double nx = xl - __ldg(q), ny = yl - __ldg(q + 1);
+        p.last = hit;
+        p.cell = (p.ux * nx + p.uy * ny > 0.0) ? uf.w : uf.z;  // the side being entered (R11)
+        return 1;
+    }
+    if (__ldg(G.surf_bc + hit) == 1) {
+        const int t = __ldg(G.surf_type + hit);
+        if (t > 2) return 0;
+        if (t == 0) p.ux = -p.ux; else if (t == 1) p.uy = -p.uy; else p.uz = -p.uz;
+        p.last = hit;
+        return 1;
+    }
+    return 0;
+}
+
 template <bool L2 = true>
 __device__ __forceinline__ bool location_is_fast(const Geo &G, int cell, int elem)
 {
@@ -1330,7 +1488,13 @@ __device__ __forceinline__ bool finish_pending(const Ctx &c, const Acc &acc, Par
     if (pend >= PEND_TIME) return true;
     if (pend >= PEND_SCATTER) { do_scatter<CE>(c, acc, p, rng, (int)(pend & 7u)); return true; }
     int r = 0;
-    if (location_is_fast<L2>(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)pend);
+    if (L2 && p.elem >= (1 << INNER_SHIFT)) {
+        const int4 li = __ldg(c.geo.lat_info + outer_of(c.geo, p.elem));
+        if (li.x & LAT_FAST2) {
+            const int4 l2i = __ldg(c.geo.l2_info + __ldg(c.geo.l2_off + (li.w >> 16)) + inner_of(c.geo, p.elem));
+            if (l2i.x & LAT_FAST) r = do_surface_fast2(c.geo, p, (int)pend, li, l2i);
+        }
+    } else if (location_is_fast<L2>(c.geo, p.cell, p.elem)) r = do_surface_fast(c.geo, p, (int)pend);
     if (r == 0) r = (L2 ? do_surface2(*acc.geo, p, (int)pend) : do_surface(*acc.geo, p, (int)pend)) ? 1 : -1;
     return r > 0;
 }

@@ -900,8 +900,12 @@ __global__ void k_test_geometry(Ctx c, const double *x, const double *u, unsigne
     double d = -1.0;
     if (ok) {
         const int4 li = elem >= 0 ? __ldg(G.lat_info + outer_of(G, elem)) : __ldg(G.cell_info + cell);
-        const int cyl = elem >= 0 ? __ldg(&G.ufast[li.x & (LAT_FAST - 1)].y) : li.y;
-        if (path == 0 && (li.x & LAT_FAST)) d = nearest_fast(G, li.z, li.w, cyl, px, py, pz, ux, uy, uz, elem, -1, hit);
+        const int cyl = elem >= 0 ? __ldg(&G.ufast[li.x & UNIV_MASK].y) : li.y;
+        int4 l2i = make_int4(0, 0, 0, 0);
+        if (path == 0 && elem >= (1 << INNER_SHIFT) && (li.x & LAT_FAST2))
+            l2i = __ldg(G.l2_info + __ldg(G.l2_off + (li.w >> 16)) + inner_of(G, elem));
+        if (l2i.x & LAT_FAST) d = nearest_fast2(G, li, l2i, __ldg(&G.ufast[l2i.x & UNIV_MASK].y), px, py, pz, ux, uy, uz, elem, -1, hit);
+        else if (path == 0 && (li.x & LAT_FAST)) d = nearest_fast(G, li.z, li.w, cyl, px, py, pz, ux, uy, uz, elem, -1, hit);
         else {
             unsigned int mask = (elem >= 0 && path != 2) ? __ldg(G.lat_rmask + outer_of(G, elem)) : 0xffffffffu;
             d = G.n_lat2 ? nearest2(s_geo, px, py, pz, ux, uy, uz, cell, elem, -1, hit, mask) : nearest(s_geo, px, py, pz, ux, uy, uz, cell, elem, -1, hit, mask);

@@ -168,7 +168,7 @@ struct Carver {
 
 struct Layout {  // everything carved from the workspace, in order
     int *surf_type, *surf_bc, *cso, *csi, *css, *cft, *cfill, *cbin, *uco, *ap_sid;
-    int4 *lat_info, *ufast, *cell_info;
+    int4 *lat_info, *ufast, *cell_info, *l2_info;
     int *l2_nx, *l2_ny, *l2_off, *l2_univ, *l2_bin, *umid;
     double *l2_px, *l2_py;
     Trace *tr_g;
@@ -256,7 +256,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
         uint64_t n2 = g->n_lat2 > 0 ? g->n_lat2 : 0, ne2 = n2 ? g->lat2_off[n2] : 0;
         L.l2_nx = C.take<int>(n2); L.l2_ny = C.take<int>(n2); L.l2_off = C.take<int>(n2 + 1);
         L.l2_px = C.take<double>(n2); L.l2_py = C.take<double>(n2);
-        L.l2_univ = C.take<int>(ne2); L.l2_bin = C.take<int>(ne2);
+        L.l2_univ = C.take<int>(ne2); L.l2_bin = C.take<int>(ne2); L.l2_info = C.take<int4>(ne2);
         L.umid = C.take<int>(g->n_univ);
     }
     bool ce = x != nullptr;
@@ -545,7 +545,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     Geo &G = c.geo;
     G.n_lat2 = g->n_lat2;
     G.l2_nx = L.l2_nx; G.l2_ny = L.l2_ny; G.l2_off = L.l2_off; G.l2_px = L.l2_px; G.l2_py = L.l2_py;
-    G.l2_univ = L.l2_univ; G.l2_bin = L.l2_bin; G.umid = L.umid;
+    G.l2_univ = L.l2_univ; G.l2_bin = L.l2_bin; G.umid = L.umid; G.l2_info = L.l2_info;
     G.n_surf = g->n_surf; G.n_cell = g->n_cell; G.n_univ = g->n_univ; G.has_lat = g->has_lattice;
     G.lat_nx = g->has_lattice ? g->lat_nx : 1; G.lat_ny = g->has_lattice ? g->lat_ny : 1;
     G.lat_x0 = g->lat_x0; G.lat_y0 = g->lat_y0; G.lat_px = g->lat_px; G.lat_py = g->lat_py;
@@ -559,7 +559,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
     // host staging must outlive the async copies: keep vectors until the sync at the end
     std::vector<double> h_mg, h_tab, h_colA, h_ap_pos, h_cum_nu, h_cumchi_d;
     std::vector<int> h_ncol, h_hash, h_ehash, h_cfill(g->cell_fill, g->cell_fill + g->n_cell), h_ap_sid;
-    std::vector<int4> h_ufast, h_latinfo(nlat), h_cellinfo(g->n_cell);
+    std::vector<int4> h_ufast, h_latinfo(nlat), h_cellinfo(g->n_cell), h_l2info;
     std::vector<unsigned int> h_rmask(nlat);
     for (int cc = 0; cc < g->n_cell; cc++) if (g->cell_fill_type[cc] == 1) h_cfill[cc] = 0;
     std::vector<int> h_umid(g->n_univ, -1);
@@ -660,12 +660,30 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
                 }
                 int e_ = iy * g->lat_nx + ix;
                 int u = g->lat_univ[e_];
+                // two-level straight-line path: the universe is one cell without surfaces that lattice k2 fills
+                int k2 = -1;
+                if (fast && g->n_lat2 > 0 && g->univ_cell_off[u + 1] - g->univ_cell_off[u] == 1) {
+                    int cc = g->univ_cell_off[u];
+                    if (g->cell_fill_type[cc] == 2 && g->cell_surf_off[cc + 1] == g->cell_surf_off[cc] && g->cell_fill[cc] < 65536) k2 = g->cell_fill[cc];
+                }
                 if (!h_ufast[u].x) fast = false;
                 h_rmask[e_] = mask;
-                h_latinfo[e_] = make_int4(u | (fast ? LAT_FAST : 0), t->lat_bin[e_],
-                                          code[0] | (code[1] << 8) | (code[2] << 16) | (code[3] << 24), code[4] | (code[5] << 8));
+                h_latinfo[e_] = make_int4(u | (fast ? LAT_FAST : 0) | (k2 >= 0 ? LAT_FAST2 : 0), t->lat_bin[e_],
+                                          code[0] | (code[1] << 8) | (code[2] << 16) | (code[3] << 24),
+                                          code[4] | (code[5] << 8) | ((k2 >= 0 ? k2 : 0) << 16));
             }
         UP(L.lat_info, h_latinfo.data(), nlat); UP(L.lat_rmask, h_rmask.data(), nlat);
+    }
+    if (g->n_lat2 > 0) {  // per second-level element: universe (| LAT_FAST if simple), bin offset, wall / rim codes
+        h_l2info.resize(g->lat2_off[g->n_lat2]);
+        for (int k = 0; k < g->n_lat2; k++)
+            for (int jy = 0; jy < g->lat2_ny[k]; jy++)
+                for (int jx = 0; jx < g->lat2_nx[k]; jx++) {
+                    int i = g->lat2_off[k] + jy * g->lat2_nx[k] + jx, u = g->lat2_univ[i];
+                    int cd[4] = {jx > 0 ? 1 : 3, jx + 1 < g->lat2_nx[k] ? 1 : 3, jy > 0 ? 1 : 3, jy + 1 < g->lat2_ny[k] ? 1 : 3};
+                    h_l2info[i] = make_int4(u | (h_ufast[u].x ? LAT_FAST : 0), t->lat2_bin[i], cd[0] | (cd[1] << 8) | (cd[2] << 16) | (cd[3] << 24), 0);
+                }
+        UP(L.l2_info, h_l2info.data(), h_l2info.size());
     }
 
     // ---- cross sections: derived tables built here, in plain left-to-right float64 sums
