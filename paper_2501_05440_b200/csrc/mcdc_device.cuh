@@ -150,6 +150,8 @@ struct Ctx {
     Trace tr;
     const Trace *tr_g;   // copy of tr in global memory for the out-of-line trace_event (see Acc::geo)
     unsigned long long seed;
+    uint32_t rk[20];     // the ten Philox round keys of the seed (rk[2r], rk[2r+1]): launch constants read straight from the
+                         // kernel-parameter bank by the XORs of the rounds (no key-bump additions in the draw path)
     unsigned int cycle;
     double w0, k_prev;
     // options set by mcdc_set_physics: free-gas thermal scattering below 400 kT (R35; kT in eV, 0 = target at rest),
@@ -179,6 +181,31 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
+#ifndef MCDC_NEXT_PRE
+#define MCDC_NEXT_PRE 1
+#endif
+#ifndef MCDC_NEXT3
+#define MCDC_NEXT3 1
+#endif
+#ifndef MCDC_GROUP_COUNT
+#define MCDC_GROUP_COUNT 1
+#endif
+// the same with the round keys precomputed (Ctx::rk)
+__device__ __forceinline__ void philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20],
+                                                 uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3)
+{
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ rk[2 * r];
+        c1 = l1;
+        c2 = h0 ^ c3 ^ rk[2 * r + 1];
+        c3 = l0;
+    }
+    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+
 // Stream (seed, id, domain 0, cycle): counter = (id_lo, id_hi, cycle, draw/2); one block yields the draws 2b
 // (words 1:0) and 2b+1 (words 3:2); xi = ((u >> 11) + 0.5) 2^-53.  The block is kept in registers so that two
 // consecutive draws cost one Philox evaluation; seed and cycle are launch constants read from the Ctx at use.
@@ -199,8 +226,7 @@ struct Rng {
         uint32_t b = ctr >> 1;
         if (b != blk) {
             uint32_t o0, o1, o2, o3;
-            philox4x32_10((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b, (uint32_t)c.seed, (uint32_t)(c.seed >> 32), o0, o1,
-                          o2, o3);
+            philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b, c.rk, o0, o1, o2, o3);
             u0 = ((uint64_t)o1 << 32) | o0;
             u1 = ((uint64_t)o3 << 32) | o2;
             blk = b;
@@ -208,6 +234,82 @@ struct Rng {
         uint64_t u = (ctr & 1u) ? u1 : u0;
         ctr++;
         return ((double)(u >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+    }
+    // The first draw of a segment (distance to collision), leaving the block of the draw AFTER it in the cache: a lane
+    // at an even draw index evaluates its block (both draws in it), a lane at an odd index takes its cached word and
+    // evaluates the NEXT block -- one evaluation site reached by every lane of the warp together, and the reaction draw
+    // (or the next segment's first draw) finds its block cached whatever the parity.
+    __device__ __forceinline__ double next_pre(const Ctx &c)
+    {
+        const uint32_t b = ctr >> 1;
+        const bool odd = (ctr & 1u) != 0u;
+        uint32_t o0, o1, o2, o3;
+        if (odd && b != blk) {  // no cached block to take the odd word from (a particle just loaded): rare
+            philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b, c.rk, o0, o1, o2, o3);
+            u1 = ((uint64_t)o3 << 32) | o2;
+            blk = b;
+        }
+        const uint64_t old1 = u1;
+        if (odd || b != blk) {
+            const uint32_t bb = odd ? b + 1u : b;
+            philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, bb, c.rk, o0, o1, o2, o3);
+            u0 = ((uint64_t)o1 << 32) | o0;
+            u1 = ((uint64_t)o3 << 32) | o2;
+            blk = bb;
+        }
+        const uint64_t u = odd ? old1 : u0;
+        ctr++;
+        return ((double)(u >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+    }
+    // The next TWO draws at once (a continuous-energy elastic scatter: mu_cm, azimuth): one evaluation site for every
+    // lane -- an even draw index evaluates its own block (both draws), an odd one takes its cached word and evaluates
+    // the next block for the second draw.
+    __device__ __forceinline__ void next2(const Ctx &c, double &x0, double &x1)
+    {
+        const uint32_t b = ctr >> 1;
+        const bool odd = (ctr & 1u) != 0u;
+        uint32_t o0, o1, o2, o3;
+        if (odd && b != blk) {
+            philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b, c.rk, o0, o1, o2, o3);
+            u1 = ((uint64_t)o3 << 32) | o2;
+            blk = b;
+        }
+        const uint64_t old1 = u1;
+        if (odd || b != blk) {
+            const uint32_t bb = odd ? b + 1u : b;
+            philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, bb, c.rk, o0, o1, o2, o3);
+            u0 = ((uint64_t)o1 << 32) | o0;
+            u1 = ((uint64_t)o3 << 32) | o2;
+            blk = bb;
+        }
+        const uint64_t a0 = odd ? old1 : u0, a1 = odd ? u0 : u1;
+        ctr += 2u;
+        const double sc = 1.0 / 9007199254740992.0;
+        x0 = ((double)(a0 >> 11) + 0.5) * sc;
+        x1 = ((double)(a1 >> 11) + 0.5) * sc;
+    }
+    // The next THREE draws at once (a multi-group scatter: group, mu, phi).  They span the blocks b = ctr / 2 and b + 1
+    // whatever the parity: block b + 1 is evaluated by every lane together, block b only by the lanes that do not hold
+    // it -- two evaluations per warp where three separate next() calls make three (each reached by half the lanes).
+    __device__ __forceinline__ void next3(const Ctx &c, double &x0, double &x1, double &x2)
+    {
+        const uint32_t b = ctr >> 1;
+        uint32_t o0, o1, o2, o3;
+        if (b != blk) {
+            philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b, c.rk, o0, o1, o2, o3);
+            u0 = ((uint64_t)o1 << 32) | o0;
+            u1 = ((uint64_t)o3 << 32) | o2;
+        }
+        philox4x32_10_rk((uint32_t)id, (uint32_t)(id >> 32), c.cycle, b + 1u, c.rk, o0, o1, o2, o3);
+        const uint64_t v0 = ((uint64_t)o1 << 32) | o0, v1 = ((uint64_t)o3 << 32) | o2;
+        const bool odd = (ctr & 1u) != 0u;
+        const uint64_t a0 = odd ? u1 : u0, a1 = odd ? v0 : u1, a2 = odd ? v1 : v0;
+        u0 = v0; u1 = v1; blk = b + 1u;
+        ctr += 3u;
+        const double sc = 1.0 / 9007199254740992.0;
+        x0 = ((double)(a0 >> 11) + 0.5) * sc;
+        x1 = ((double)(a1 >> 11) + 0.5) * sc;
+        x2 = ((double)(a2 >> 11) + 0.5) * sc;
     }
 };
 
@@ -989,7 +1091,11 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     }
 
     // candidate distances: collision (one draw every segment), boundary, time edge (R12)
+#if MCDC_NEXT_PRE
+    double d_coll = -log(rng.next_pre(c)) / sig_t;
+#else
     double d_coll = -log(rng.next(c)) / sig_t;
+#endif
     int hit;
     double d_surf;
     int4 l2i = make_int4(0, 0, 0, 0);
@@ -1186,12 +1292,28 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const Acc &acc, Particl
     if (!CE) {
         const int G = c.mg.G;
         double sig_s = mgv(acc, c.mg.o_sig_s + mat * G + p.g);
+#if MCDC_NEXT3
+        double xg, a, b;
+        rng.next3(c, xg, a, b);
+        double vv = xg * sig_s;
+#else
         double vv = rng.next(c) * sig_s;
+#endif
         const int row = c.mg.o_cumS + (mat * G + p.g) * G;
+#if MCDC_GROUP_COUNT
+        // first i with cumS[i] > vv (else G - 1) = how many of the first G - 1 running sums are <= vv (they never
+        // decrease: S >= 0 is validated): a fixed trip count, the same for every lane
+        int i = 0;
+        for (int j = 0; j < G - 1; j++) i += !(mgv(acc, row + j) > vv) ? 1 : 0;
+        p.g = i;
+#else
         int i = 0;
         while (i < G - 1 && !(mgv(acc, row + i) > vv)) i++;
         p.g = i;
+#endif
+#if !MCDC_NEXT3
         double a = rng.next(c), b = rng.next(c);
+#endif
         iso_dir(a, b, p.ux, p.uy, p.uz);
     } else {
         double A = __ldg(c.ce.colA + mat * CE_ROW + col);
@@ -1202,13 +1324,15 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const Acc &acc, Particl
             rng.init(rng.id, ctr);
             En = o[0]; p.ux = o[1]; p.uy = o[2]; p.uz = o[3];
         } else {
-            double mu_cm = 2.0 * rng.next(c) - 1.0;
+            double xi_mu, xi_phi;
+            rng.next2(c, xi_mu, xi_phi);
+            double mu_cm = 2.0 * xi_mu - 1.0;
             double den = A * A + 2.0 * A * mu_cm + 1.0;
             double mu = 0.0;
             if (den > 0.0) mu = (1.0 + A * mu_cm) / sqrt(den);
             En = p.E * den / ((A + 1.0) * (A + 1.0));
             double sp, cp;
-            sincospi(2.0 * rng.next(c), &sp, &cp);
+            sincospi(2.0 * xi_phi, &sp, &cp);
             double ox, oy, oz;
             rotate_dir(p.ux, p.uy, p.uz, mu, sp, cp, ox, oy, oz);
             p.ux = ox; p.uy = oy; p.uz = oz;

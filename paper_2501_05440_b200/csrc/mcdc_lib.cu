@@ -32,6 +32,14 @@ static int fail(int code, const char *fmt, ...)
         if (e_ != cudaSuccess) return fail(MCDC_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));   \
     } while (0)
 
+// seed of the run and its ten Philox round keys (Ctx::rk)
+static void set_seed(Ctx &c, uint64_t seed)
+{
+    c.seed = seed;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; r++) { c.rk[2 * r] = k0; c.rk[2 * r + 1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+}
+
 static const int LAG = 3;                 // sweeps the host may run ahead of the queue-count read-back
 // live particles at or below which the persistent kernel takes over from the event sweeps.  Measured on B200
 // (profiles/r02_schedules.md, ms per C4 cycle): 1.5e6 -> 36.1, 4e6 -> 33.7, 6e6 -> 32.3, 9e6 -> 30.5, always -> 29.2:
@@ -1123,7 +1131,7 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     if (cycle >= (1u << 24)) return fail(MCDC_EINVAL, "cycle index too large for the RNG counter layout");
     uint64_t M = sample ? N : p->bank_count;
     if (M == 0) return fail(MCDC_EBANK, "empty source bank");
-    c.seed = seed; c.cycle = cycle;
+    set_seed(c, seed); c.cycle = cycle;
     c.w0 = sample ? 1.0 : (double)N / (double)M;  // source renormalisation (R6)
     c.k_prev = p->k_prev;
     c.max_secondaries = ~0ull;
@@ -1277,7 +1285,7 @@ static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
         p->cb_cur = 0; c.cbank = p->cb[0]; p->census_n = 0;
     } else if (p->work.next_interval != k) return fail(MCDC_EINVAL, "census intervals must be run in order: expected %d, got %d", p->work.next_interval, k);
     RunStats &w = p->work;
-    c.seed = seed; c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
+    set_seed(c, seed); c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
     c.max_secondaries = 64ull * (N + (uint64_t)p->census_target * (uint64_t)n_t) + 4096;  // R25a
     c.census_stop = k + 1 < n_t ? 1 : 0;
     CUDA_OK(cudaEventRecord(p->t0, st));
@@ -1422,7 +1430,7 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
     cudaStream_t st = p->stream;
     int rc = begin_run(p);
     if (rc) return rc;
-    c.seed = seed; c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
+    set_seed(c, seed); c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
     c.census_stop = 0;  // one launch to the last time edge: a census is a synchronisation point only (R24)
     c.max_secondaries = 64 * N + 4096;  // R25a: the prompt chain must die out
     CUDA_OK(cudaMemsetAsync(c.scal, 0, 64, st));
