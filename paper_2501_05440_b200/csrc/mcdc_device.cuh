@@ -67,6 +67,8 @@ struct MGTab {  // [n_mat][G] each; cumS [n_mat][G][G] running row sums; cumchi 
     int G, n_mat, blob_doubles;  // blob: the transport kernels copy it to shared memory when it fits
     const double *blob;
     int o_sig_t, o_sig_s, o_sig_f, o_nu, o_nusf, o_cumS, o_cumchi, o_src_cum;  // offsets (doubles) into the blob
+    int half;     // largest power of two <= G - 1 (0 for one group): first step of the group-transfer bisection
+    int o_inv_t;  // 1 / Sigma_t: the distance to collision is -ln(xi) * (1 / Sigma_t), one multiply instead of a division
 };
 
 struct CETab {
@@ -181,6 +183,9 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     o0 = c0; o1 = c1; o2 = c2; o3 = c3;
 }
 
+#ifndef MCDC_INV_SIGT
+#define MCDC_INV_SIGT 1
+#endif
 #ifndef MCDC_NEXT_PRE
 #define MCDC_NEXT_PRE 1
 #endif
@@ -188,7 +193,7 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 #define MCDC_NEXT3 1
 #endif
 #ifndef MCDC_GROUP_COUNT
-#define MCDC_GROUP_COUNT 1
+#define MCDC_GROUP_COUNT 2
 #endif
 // the same with the round keys precomputed (Ctx::rk)
 __device__ __forceinline__ void philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20],
@@ -1091,7 +1096,9 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     }
 
     // candidate distances: collision (one draw every segment), boundary, time edge (R12)
-#if MCDC_NEXT_PRE
+#if MCDC_NEXT_PRE && MCDC_INV_SIGT
+    double d_coll = CE ? -log(rng.next_pre(c)) / sig_t : -log(rng.next_pre(c)) * mgv(acc, c.mg.o_inv_t + mat * c.mg.G + p.g);
+#elif MCDC_NEXT_PRE
     double d_coll = -log(rng.next_pre(c)) / sig_t;
 #else
     double d_coll = -log(rng.next(c)) / sig_t;
@@ -1300,9 +1307,16 @@ __device__ __forceinline__ void do_scatter(const Ctx &c, const Acc &acc, Particl
         double vv = rng.next(c) * sig_s;
 #endif
         const int row = c.mg.o_cumS + (mat * G + p.g) * G;
-#if MCDC_GROUP_COUNT
+#if MCDC_GROUP_COUNT == 2
         // first i with cumS[i] > vv (else G - 1) = how many of the first G - 1 running sums are <= vv (they never
-        // decrease: S >= 0 is validated): a fixed trip count, the same for every lane
+        // decrease: S >= 0 is validated), found by bisection with a fixed trip count, the same for every lane
+        int i = 0;
+        for (int h = c.mg.half; h > 0; h >>= 1) {
+            const int j = i + h;
+            if (j <= G - 1 && !(mgv(acc, row + j - 1) > vv)) i = j;
+        }
+        p.g = i;
+#elif MCDC_GROUP_COUNT
         int i = 0;
         for (int j = 0; j < G - 1; j++) i += !(mgv(acc, row + j) > vv) ? 1 : 0;
         p.g = i;

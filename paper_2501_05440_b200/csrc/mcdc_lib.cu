@@ -272,7 +272,7 @@ static void carve(Layout &L, void *ws, const mcdc_geometry *g, const mcdc_materi
     if (!ce) {
         uint64_t mg = (uint64_t)m->n_mat * m->G;
         // one contiguous blob (staged in shared memory by the kernels): six [n_mat][G] tables, cumS, src_cum
-        L.mg_doubles = 6 * mg + mg * m->G + m->G;
+        L.mg_doubles = 7 * mg + mg * m->G + m->G;
         L.mg_blob = C.take<double>(L.mg_doubles);
         L.grid = L.tab = L.colA = L.t_edges = L.e_edges = nullptr; L.ncol = L.hash = L.ehash = nullptr;
         L.td_speed = L.td_cum_nu = L.td_cumchi_d = L.td_decay = nullptr;
@@ -702,6 +702,9 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
         T.G = Gn; T.n_mat = nm; T.blob = L.mg_blob; T.blob_doubles = (int)L.mg_doubles;
         T.o_sig_t = 0; T.o_sig_s = (int)mg; T.o_sig_f = (int)(2 * mg); T.o_nu = (int)(3 * mg); T.o_nusf = (int)(4 * mg);
         T.o_cumchi = (int)(5 * mg); T.o_cumS = (int)(6 * mg); T.o_src_cum = (int)(6 * mg + mg * Gn);
+        T.o_inv_t = (int)(6 * mg + mg * Gn + Gn);
+        T.half = 0;
+        while (2 * std::max(T.half, 1) <= Gn - 1 || (T.half == 0 && Gn - 1 >= 1)) T.half = T.half ? 2 * T.half : 1;
         h_mg.assign(L.mg_doubles, 0.0);
         for (int mm = 0; mm < nm; mm++) {
             double cc = 0.0;
@@ -717,6 +720,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
                 cc += m->chi[i];
                 h_mg[T.o_cumchi + i] = cc;
                 h_mg[T.o_nusf + i] = m->nu[i] * m->sig_f[i];
+                h_mg[T.o_inv_t + i] = 1.0 / m->sig_t[i];
             }
         }
         double cs = 0.0;
