@@ -393,6 +393,42 @@ def assembly_gap(n_asm=2, n_pin=3, n_particles=4000, n_inactive=1, n_active=2, s
     return P
 
 
+def two_level_rect(nxo=2, nyo=3, nxi=3, nyi=2, n_particles=4000, n_inactive=1, n_active=2, seed=53, G=3, pitch=1.26, r=0.54):
+    """Non-square lattices at both levels (index-transposition check): nxo x nyo assemblies, each one cell filled by one
+    of two nxi x nyi pin lattices (different pin maps); rectangular pins of pitch (pitch, 0.9 pitch).  x = 0, y = 0
+    reflect, the far faces are vacuum.  One tally bin per pin."""
+    g = _Geom()
+    px, py = float(pitch), float(0.9 * pitch)
+    ax, ay = nxi * px, nyi * py
+    x0 = g.surf(PLANE_X, [0.0], REFLECT)
+    x1 = g.surf(PLANE_X, [nxo * ax], VACUUM)
+    y0 = g.surf(PLANE_Y, [0.0], REFLECT)
+    y1 = g.surf(PLANE_Y, [nyo * ay], VACUUM)
+    cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
+    g.cell(0, [(x0, +1), (x1, -1), (y0, +1), (y1, -1)], 0, lattice=True)
+    g.cell(1, [(cy, -1)], 0)
+    g.cell(1, [(cy, +1)], 1)
+    g.cell(2, [], 1)
+    g.cell(3, [], 0, lattice2=True)
+    g.cell(4, [], 1, lattice2=True)
+    npi = nxi * nyi
+    inner = []
+    for kind in (0, 1):
+        un = np.array([[1 if (ix + 2 * iy + kind) % 3 else 2 for ix in range(nxi)] for iy in range(nyi)], np.int32)
+        inner.append(dict(nx=nxi, ny=nyi, px=px, py=py, univ=un, bin=np.arange(npi, dtype=np.int32).reshape(nyi, nxi)))
+    univ = np.array([[3 + (ix + iy) % 2 for ix in range(nxo)] for iy in range(nyo)], np.int32)
+    bins = (np.arange(nxo * nyo, dtype=np.int32) * npi).reshape(nyo, nxo)
+    lat = dict(x0=0.0, y0=0.0, px=float(ax), py=float(ay), nx=nxo, ny=nyo, univ=univ, bin=bins)
+    P = g.finish(lat=lat, n_bins=nxo * nyo * npi, lat2=inner)
+    rng = np.random.default_rng(7)
+    mats = [mg_fuel(rng, G, 1.5), mg_moderator(rng, G)]
+    P.update(_mg_pack(mats))
+    P.update(_src([0, 0, 0], [nxo * ax, nyo * ay, 0], G=G, pdf=mats[0]["chi"]))
+    P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
+    P["name"] = "two_level_rect"
+    return P
+
+
 def geom_rect_lattice(nx, ny, pitch=1.26, r=0.54, x_hi=VACUUM, y_hi=REFLECT):
     """nx x ny pin lattice filling the box [0, nx p] x [0, ny p] (parity geometry for non-square and one-column /
     one-row lattices): universes 1 = fuel pin (material 0 in a cylinder, 1 outside), 2 = moderator only, in a

@@ -74,6 +74,8 @@ CASES = {
     "C4_2l_homog": lambda: inputs.config4(n_particles=3000, n_inactive=1, n_active=2, n_asm=2, n_pin=3, n_refl=3, two_level=True,
                                          reflector_lattice=False),
     "C4_2l_17": lambda: inputs.config4(n_particles=5000, n_inactive=1, n_active=2, two_level=True),
+    "rect_2l": lambda: inputs.two_level_rect(2, 3, 3, 2),
+    "rect_2l_1col": lambda: inputs.two_level_rect(1, 2, 1, 4),
     "asm_gap": lambda: inputs.assembly_gap(2, 3),
     "asm_gap_wide": lambda: inputs.assembly_gap(3, 2, gap=0.6),
     "slab": lambda: inputs.slab_beam(n_particles=5000),
@@ -106,7 +108,7 @@ def test_mg_parity(gpu, orc, name, schedule, persist):
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d", "lat1x6", "lat3x5", "mirror_sphere",
-                                  "mirror_cyl_x", "C4_2l", "C4_2l_3d", "C4_2l_homog", "asm_gap", "asm_gap_wide"])
+                                  "mirror_cyl_x", "C4_2l", "C4_2l_3d", "C4_2l_homog", "asm_gap", "asm_gap_wide", "rect_2l", "rect_2l_1col"])
 @pytest.mark.parametrize("schedule,persist", [(0, -1), (0, 0), (1, 0), (2, -1), (0, 100)])
 def test_mg_traces_identical(gpu, orc, name, schedule, persist):
     """100 particles x 2 cycles: identical per-particle event sequences (SURVEY.md 8d parity protocol 1)."""
@@ -196,7 +198,7 @@ def test_geometry_unit_parity(gpu, orc, height):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5", "C4_2l", "C4_2l_3d", "asm_gap", "C4_2l_17"])
+@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5", "C4_2l", "C4_2l_3d", "asm_gap", "C4_2l_17", "rect_2l"])
 def test_geometry_unit_parity_plain_cells(gpu, orc, name):
     """Cells outside a lattice (box, pin cell: straight-line path; mixed surfaces: generic loops) and a small lattice:
     locate + nearest boundary of random points, every device path against the oracle."""

@@ -53,13 +53,14 @@ def test_two_level_equals_flat_lattice(orc, n_asm, n_pin, n_refl, height):
     assert (lat["surf"] >= ns + 4).sum() > 200 and (lat["surf"] < ns + 4).sum() > 20  # walls of both levels were crossed
 
 
-@pytest.mark.parametrize("case", ["core2l", "core2l_3d", "gap", "gap_wide", "core2l_homog_reflector"])
+@pytest.mark.parametrize("case", ["core2l", "core2l_3d", "gap", "gap_wide", "core2l_homog_reflector", "rect", "rect_1col"])
 def test_trace_two_level_vs_brute_force(orc, case):
     """Two-level lattices event by event (packed element, local cell, wall codes of both levels, surfaces of the cell
     the inner lattice fills) against brute force over all grid lines and all pins."""
     P = dict(core2l=lambda: inputs.config4(n_particles=50, n_asm=1, n_pin=3, n_refl=3, two_level=True),
              core2l_3d=lambda: inputs.config4(n_particles=40, n_asm=2, n_pin=2, n_refl=2, two_level=True, height=5.0),
              gap=lambda: inputs.assembly_gap(2, 3), gap_wide=lambda: inputs.assembly_gap(3, 2, gap=0.6),
+             rect=lambda: inputs.two_level_rect(2, 3, 3, 2), rect_1col=lambda: inputs.two_level_rect(1, 2, 1, 4),
              core2l_homog_reflector=lambda: inputs.config4(n_particles=50, n_asm=1, n_pin=3, n_refl=3, two_level=True,
                                                            reflector_lattice=False))[case]()
     tr = _compare(orc, P, 50, 50)
