@@ -39,7 +39,8 @@ struct Geo {
     const int *cso, *csi, *css, *cft, *cfill, *cbin, *uco;
     const int4 *lat_info, *cell_info;
     const unsigned int *lat_rmask;
-    const int4 *ufast;      // per universe: x = 1 if it is one cell, or two cells split by one CYL_Z; y = that
+    const int4 *ufast;      // per universe: x bit 0 = it is one cell, or two cells split by one CYL_Z (bit 1: which lies
+                            // strictly inside every lattice element that can hold the universe); y = that
                             // cylinder (or -1); z = cell inside it (or the only cell); w = cell outside it
     const double *ap_pos;   // [n_ap] position of axis plane j
     const int *ap_sid;      // [n_ap] its surface id
@@ -57,7 +58,8 @@ __device__ __forceinline__ int outer_of(const Geo &, int elem) { return elem & (
 __device__ __forceinline__ int inner_of(const Geo &, int elem) { return (elem >> INNER_SHIFT) - 1; }
 constexpr int LAT_FAST = 1 << 30, CELL_FAST = 1 << 30, CELL_NO_NEIGHBOUR = (1 << 30) - 1;
 // LAT_FAST2 (lat_info[e].x): the element's universe is ONE cell without surfaces filled by second-level lattice k
-// (k in the high 16 bits of lat_info[e].w) and the enclosing cell's surfaces fit the boundary-code pattern: elements
+// (k in the high 16 bits of lat_info[e].w; for the other elements those bits hold the universe's z-cylinder + 1)
+// and the enclosing cell's surfaces fit the boundary-code pattern: elements
 // of that lattice whose own universe is simple (l2_info[..].x & LAT_FAST) take the two-level straight-line path.
 // l2_info[l2_off[k] + i]: x = universe | LAT_FAST, y = tally-bin offset, z = codes for -x,+x,-y,+y: 1 = second-level
 // wall (an event), 3 = the lattice's rim (the first-level element's code for that direction applies).
@@ -1064,7 +1066,7 @@ __device__ __forceinline__ int advance(const Ctx &c, Particle &p, Rng &rng, int 
     if (p.elem >= 0) {
         li = __ldg(G.lat_info + (L2 ? outer_of(G, p.elem) : p.elem));
         bin += li.y;
-        cyl = __ldg(&G.ufast[li.x & UNIV_MASK].y);
+        cyl = (li.w >> 16) - 1;  // the pin universe's z-cylinder rides in the element's table entry (LAT_FAST elements)
     } else {
         li = __ldg(G.cell_info + p.cell);
         cyl = li.y;
@@ -1506,7 +1508,8 @@ __device__ __forceinline__ int do_surface_fast(const Geo &G, Particle &p, int hi
         p.elem = e2;
         p.last = -1;
         int cell = uf.z;
-        if (uf.y >= 0) {
+        if (uf.x & 2) cell = uf.w;  // the cylinder lies strictly inside the element: a particle on a wall is outside it
+        else if (uf.y >= 0) {
             double xl, yl;
             local_xy(G, e2, p.x, p.y, xl, yl);
             const double *q = G.surf_param + 4 * uf.y;
@@ -1568,7 +1571,8 @@ __device__ __forceinline__ int do_surface_fast2(const Geo &G, Particle &p, int h
         if (!(l2n.x & LAT_FAST)) return 0;
         const int4 uf = __ldg(G.ufast + (l2n.x & UNIV_MASK));
         int cell = uf.z;
-        if (uf.y >= 0) {
+        if (uf.x & 2) cell = uf.w;  // the cylinder lies strictly inside the element: a particle on a wall is outside it
+        else if (uf.y >= 0) {
             double xl, yl;
             inner_xy(G, k, inner2, xo, yo, xl, yl);
             const double *q = G.surf_param + 4 * uf.y;

@@ -542,7 +542,10 @@ __device__ __forceinline__ bool make_child_td(const Ctx &c, Rng &rng, int mat, i
 }
 
 template <bool CE, bool PRIVATE, bool W, int X>
-__global__ void __launch_bounds__(BS, (CE ? MCDC_PERSIST_MINBLOCKS_CE : MCDC_PERSIST_MINBLOCKS) * 256 / BS)
+#ifndef MCDC_PERSIST_BLOCKS_RAW
+#define MCDC_PERSIST_BLOCKS_RAW ((CE ? MCDC_PERSIST_MINBLOCKS_CE : MCDC_PERSIST_MINBLOCKS) * 256 / BS)
+#endif
+__global__ void __launch_bounds__(BS, MCDC_PERSIST_BLOCKS_RAW)
 k_persist(Ctx c, unsigned int s, unsigned int n0)
 {
     constexpr bool TD = (X & X_TD) != 0;

@@ -589,6 +589,18 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
         UP(L.l2_univ, g->lat2_univ, ne2); UP(L.l2_bin, t->lat2_bin, ne2);
     }
     classify_universes(g, h_ufast);
+    {   // bit 1: the universe's cylinder lies strictly inside the smallest lattice element of the problem (with a margin far
+        // above rounding), so a particle that enters the element through a wall is outside the cylinder
+        double hx = 1e300, hy = 1e300;
+        if (g->has_lattice) { hx = 0.5 * g->lat_px; hy = 0.5 * g->lat_py; }
+        for (int k = 0; k < g->n_lat2; k++) { hx = std::min(hx, 0.5 * g->lat2_px[k]); hy = std::min(hy, 0.5 * g->lat2_py[k]); }
+        for (int u = 1; u < g->n_univ; u++) {
+            int cyl = h_ufast[u].y;
+            if (!h_ufast[u].x || cyl < 0) continue;
+            const double *q = g->surf_param + 4 * cyl;
+            if (std::fabs(q[0]) + q[2] < hx * (1.0 - 1e-6) && std::fabs(q[1]) + q[2] < hy * (1.0 - 1e-6)) h_ufast[u].x |= 2;
+        }
+    }
     UP(L.ufast, h_ufast.data(), g->n_univ);
     // every axis plane of the problem gets an index the boundary codes can name (the first MAX_AXIS_PLANES of them)
     std::vector<int> ap_of(g->n_surf, -1);
@@ -678,7 +690,7 @@ extern "C" int mcdc_create(const mcdc_geometry *g, const mcdc_materials *m, cons
                 h_rmask[e_] = mask;
                 h_latinfo[e_] = make_int4(u | (fast ? LAT_FAST : 0) | (k2 >= 0 ? LAT_FAST2 : 0), t->lat_bin[e_],
                                           code[0] | (code[1] << 8) | (code[2] << 16) | (code[3] << 24),
-                                          code[4] | (code[5] << 8) | ((k2 >= 0 ? k2 : 0) << 16));
+                                          code[4] | (code[5] << 8) | ((k2 >= 0 ? k2 : h_ufast[u].y + 1) << 16));
             }
         UP(L.lat_info, h_latinfo.data(), nlat); UP(L.lat_rmask, h_rmask.data(), nlat);
     }
