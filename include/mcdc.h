@@ -6,7 +6,7 @@
  * replicable random number generation"; PAPER.md:51 one "segment" = one event; PAPER.md:55 dual
  * particle banks; PAPER.md:57 per-event kernels; PAPER.md:124 inactive/active cycles
  * time-dependent fixed source).  The paper prints no formulas; every step follows the readings
- * R1..R31 of DESIGN.md section 3 (= SURVEY.md 8c).
+ * R1..R40 of DESIGN.md section 3 (R1..R31 = SURVEY.md 8c).
  *
  * Conventions for every call
  *   - plain C: pointers + sizes only.  All INPUT pointers are HOST pointers; the library copies what
