@@ -1098,7 +1098,8 @@ static void add_balance(mcdc_problem *p, double source_weight, const uint64_t *b
 
 // children of the M parents' fission records -> bank[0]; returns their number.  Also brings the cycle's scalars,
 // the device counters and the error flag to the host (one synchronisation).
-static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
+// wait = false: everything is queued and the caller synchronises (one wait per cycle), then reads p->pin->total
+static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total, bool wait = true)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
@@ -1116,6 +1117,7 @@ static int emit_children(mcdc_problem *p, uint64_t M, uint64_t *total)
     CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->counters, c.counters, sizeof p->pin->counters, cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(&p->pin->err, c.err, sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (!wait) return 0;
     CUDA_OK(cudaStreamSynchronize(st));
     CUDA_OK(cudaGetLastError());
     profile_collect(p);
@@ -1165,18 +1167,22 @@ static int cycle_internal(mcdc_problem *p, uint64_t N, uint32_t cycle, int activ
     for (int i = 0; i < MCDC_N_COUNTERS; i++) before[i] = cycle == 0 ? 0 : p->pin->counters[i];
     int rc = transport(p, M);
     if (rc) return abandon(p, rc);
+    // the fission bank, the read-backs and the cycle's tally statistics are queued together: ONE wait per cycle (a
+    // cycle that turns out to have failed has then added to the work accumulators, which the next run clears)
     uint64_t total = 0;
-    rc = emit_children(p, M, &total);
+    rc = emit_children(p, M, &total, false);
     if (rc) return abandon(p, rc);
-    rc = device_error_code(p, p->pin->err);
-    if (rc) return abandon(p, rc);
-    add_balance(p, c.w0 * (double)M, before);
     CUDA_OK(cudaEventRecord(p->t1, st));
     k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[p->work.set],
                                                           p->flux_acc2[p->work.set], c.n_tally, 1.0 / (double)N, active);
     if (flux_cycle_host) CUDA_OK(cudaMemcpyAsync(flux_cycle_host, p->flux_cycle, sizeof(double) * c.n_tally, cudaMemcpyDeviceToHost, st));
     p->n_launches++;
-    CUDA_OK(cudaStreamSynchronize(st));
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return abandon(p, fail(MCDC_ECUDA, "cycle: %s", cudaGetErrorString(cudaGetLastError())));
+    profile_collect(p);
+    total = p->pin->total;
+    rc = device_error_code(p, p->pin->err);
+    if (rc) return abandon(p, rc);
+    add_balance(p, c.w0 * (double)M, before);
     float ms = 0.f;
     CUDA_OK(cudaEventElapsedTime(&ms, p->t0, p->t1));
     p->ms_transport += ms;
