@@ -719,6 +719,32 @@ def config5(n_particles=1_000_000, seed=1, n_grid=50_000, jitter=False, absorber
     return P
 
 
+def ce_lattice(kind="two_level", n_particles=2000, seed=1, n_grid=6000):
+    """The C5 nuclide data and time / energy bins in a lattice geometry with vacuum faces (continuous-energy kernels with
+    lattice and second-level lattice geometry): kind 'two_level' = two_level_rect(2, 2, 3, 2), 'gap' = geom_assembly_gap,
+    'flat' = geom_rect_lattice(4, 3).  Material 0 fuel, 1 moderator as in C5; one spatial bin per pin."""
+    if kind == "two_level":
+        G = two_level_rect(2, 2, 3, 2)
+        side = (2 * 3 * 1.26, 2 * 2 * 0.9 * 1.26)
+    elif kind == "gap":
+        G = assembly_gap(2, 3)
+        side = (2 * (3 * 1.26 + 0.4),) * 2
+    else:
+        G = rect_lattice(4, 3)
+        side = (4 * 1.26, 3 * 1.26)
+    geo_keys = ("surf_type", "surf_param", "surf_bc", "cell_surf_off", "cell_surf_id", "cell_surf_sense", "cell_fill_type",
+                "cell_fill", "cell_bin", "univ_cell_off", "lat", "n_bins", "lat2_nx", "lat2_ny", "lat2_px", "lat2_py",
+                "lat2_off", "lat2_univ", "lat2_bin")
+    P = {k: G[k] for k in geo_keys if k in G}
+    C = config5(n_particles=n_particles, seed=seed, n_grid=n_grid)
+    for k, v in C.items():
+        if k not in geo_keys:
+            P[k] = v
+    P.update(_src([0, 0, 0], [side[0], side[1], 0], E=2.0e6, t=0.0))
+    P["name"] = "ce_" + kind
+    return P
+
+
 # --------------------------------------------------------------------------- pin problems (closed forms)
 def slab_beam(L=2.0, sig_t=1.3, n_particles=100_000, seed=7):
     """Pure absorber slab, mono-directional normal beam born on x=0+: leakage = exp(-Sigma_t L)."""

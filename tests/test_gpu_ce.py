@@ -32,6 +32,10 @@ CE_CASES = {
     "ce_fission": lambda: _fis(),
     "ce_mix": lambda: inputs.ce_two_nuclide_mix(n_particles=3000, n_grid=3000),
     "ce_clock": lambda: inputs.ce_scatter_clock(n_particles=3000, n_grid=3000),
+    # continuous energy in lattices (one level, two levels incl. non-square, an assembly with a gap around its pins)
+    "ce_flat_lattice": lambda: inputs.ce_lattice("flat", n_particles=1500),
+    "ce_two_level": lambda: inputs.ce_lattice("two_level", n_particles=1500),
+    "ce_gap": lambda: inputs.ce_lattice("gap", n_particles=1500),
     "ce_clamp": lambda: inputs.ce_single_scatterer(A=1.0, n_particles=4000, E0=2.0e-5, sig_el=0.9, sig_c=0.1),
 }
 
@@ -116,5 +120,24 @@ def test_ce_source_traces_with_secondaries_in_flight(gpu, orc):
     o.set_trace(300, 100, 2_000_000)
     rc, ro = o.run()
     compare_traces(g.trace(), o.trace())
+    compare_ce(r, ro)
+    g.close()
+
+
+@pytest.mark.parametrize("kind", ["flat", "two_level", "gap"])
+@pytest.mark.parametrize("schedule,persist", [(0, 0), (0, -1), (1, 0)])
+def test_ce_lattice_traces(gpu, orc, kind, schedule, persist):
+    """Continuous energy inside one- and two-level lattices: event sequences of source particles 0..199 (lattice walls
+    of both levels, packed element locations, time and energy) equal the oracle's."""
+    P = inputs.ce_lattice(kind, n_particles=600)
+    g = gpu.Problem(P, schedule=schedule, persist_threshold=persist, search=1)
+    g.set_trace(0, 200, 1024)
+    r = g.run()
+    o = orc.Oracle(P)
+    o.set_trace(0, 200, 1_000_000)
+    rc, ro = o.run()
+    tg = g.trace()
+    assert (tg["ev"] == 7).sum() > 50
+    compare_traces(tg, o.trace())
     compare_ce(r, ro)
     g.close()
