@@ -633,12 +633,16 @@ def td_infinite(n_particles=20_000, seed=47, G=1, J=1, t_end=4.0e-3, n_t=8, cens
         P = geom_box([0, 0, 0], [1, 1, 1], REFLECT)
         lo, hi = [0, 0, 0], [1, 1, 1]
     else:
-        P = geom_pincell()
+        if geom == "lattice2":  # a two-level lattice with vacuum faces (fuel 0 / moderator 1 as in the pin cell)
+            P = _geometry_of(two_level_rect(2, 2, 3, 2))
+            lo, hi = [0, 0, 0], [2 * 3 * 1.26, 2 * 2 * 0.9 * 1.26, 0]
+        else:
+            P = geom_pincell()
+            lo, hi = [-0.63, -0.63, 0], [0.63, 0.63, 0]
         mod = dict(sig_t=sig_t * 1.3, S=S * 1.5, sig_f=sig_f * 0.0, nu=nu_p, chi=chi, sig_c=sig_t * 1.3 - (S * 1.5).sum(1))
         mats = [mat, mod]
         td = dict(speed=speed, J=J, nu_d=np.stack([nu_d, nu_d * 0.0]), decay=np.stack([decay, decay]),
                   chi_d=np.stack([chi_d, chi_d]), census_target=int(census_target))
-        lo, hi = [-0.63, -0.63, 0], [0.63, 0.63, 0]
     P.update(_mg_pack(mats))
     P.update(_src(lo, hi, G=G, pdf=chi))
     P["td"] = td
@@ -719,6 +723,16 @@ def config5(n_particles=1_000_000, seed=1, n_grid=50_000, jitter=False, absorber
     return P
 
 
+GEO_KEYS = ("surf_type", "surf_param", "surf_bc", "cell_surf_off", "cell_surf_id", "cell_surf_sense", "cell_fill_type",
+            "cell_fill", "cell_bin", "univ_cell_off", "lat", "n_bins", "lat2_nx", "lat2_ny", "lat2_px", "lat2_py",
+            "lat2_off", "lat2_univ", "lat2_bin")
+
+
+def _geometry_of(G):
+    """the geometry and spatial-tally part of a problem dict"""
+    return {k: G[k] for k in GEO_KEYS if k in G}
+
+
 def ce_lattice(kind="two_level", n_particles=2000, seed=1, n_grid=6000):
     """The C5 nuclide data and time / energy bins in a lattice geometry with vacuum faces (continuous-energy kernels with
     lattice and second-level lattice geometry): kind 'two_level' = two_level_rect(2, 2, 3, 2), 'gap' = geom_assembly_gap,
@@ -732,13 +746,10 @@ def ce_lattice(kind="two_level", n_particles=2000, seed=1, n_grid=6000):
     else:
         G = rect_lattice(4, 3)
         side = (4 * 1.26, 3 * 1.26)
-    geo_keys = ("surf_type", "surf_param", "surf_bc", "cell_surf_off", "cell_surf_id", "cell_surf_sense", "cell_fill_type",
-                "cell_fill", "cell_bin", "univ_cell_off", "lat", "n_bins", "lat2_nx", "lat2_ny", "lat2_px", "lat2_py",
-                "lat2_off", "lat2_univ", "lat2_bin")
-    P = {k: G[k] for k in geo_keys if k in G}
+    P = _geometry_of(G)
     C = config5(n_particles=n_particles, seed=seed, n_grid=n_grid)
     for k, v in C.items():
-        if k not in geo_keys:
+        if k not in GEO_KEYS:
             P[k] = v
     P.update(_src([0, 0, 0], [side[0], side[1], 0], E=2.0e6, t=0.0))
     P["name"] = "ce_" + kind

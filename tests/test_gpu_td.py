@@ -33,6 +33,7 @@ TD_CASES = {
     "pin_G2_comb": lambda: inputs.td_infinite(n_particles=3000, G=2, geom="pin", census_target=2500),
     "pin_G1_implicit_comb": lambda: _with(inputs.td_infinite(n_particles=2500, G=1, geom="pin", census_target=2500),
                                           implicit_capture=1),
+    "lattice2_G2_comb": lambda: inputs.td_infinite(n_particles=3000, G=2, geom="lattice2", census_target=2000, t_end=4.0e-4),
     "cube_G2_two_bins": lambda: inputs.td_infinite(n_particles=3000, G=2, n_t=2),
     "cube_G2_fine": lambda: inputs.td_infinite(n_particles=2000, G=2, t_end=8.0e-5, n_t=16),  # time bins << a lifetime
     "cube_G1_late_source": lambda: _with(inputs.td_infinite(n_particles=2000, G=1, census_target=1000), src_t=1.2e-3),
@@ -62,7 +63,7 @@ def test_td_parity(gpu, orc, name):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["cube_G2", "pin_G2", "pin_G1_implicit_comb", "cube_G2_fine"])
+@pytest.mark.parametrize("name", ["cube_G2", "pin_G2", "pin_G1_implicit_comb", "cube_G2_fine", "lattice2_G2_comb"])
 def test_td_traces(gpu, orc, name):
     """Event sequences of source particles 0..99 (up to the first comb, which re-keys the tracks): time, time-edge
     events, group transfers, the census interruptions."""
