@@ -282,6 +282,39 @@ int mcdc_get_trace(const mcdc_problem *p, mcdc_trace_rec *out, uint64_t max, uin
  * n uniform draws of stream (seed, id[i], domain, cycle) at index draw[i] */
 int mcdc_test_draws(mcdc_problem *p, uint64_t seed, uint32_t domain, uint32_t cycle, const uint64_t *id,
                     const uint32_t *draw, uint64_t n, double *out);
+/* The per-particle random-number stream (R1, R2) evaluated on the GPU WITHOUT any device
+ * memory from the caller: out[i] = draw number draw[i] of stream (seed, id[i], domain, cycle), bit for bit what
+ * mcdc_test_draws returns, but no mcdc_problem and no workspace are needed.
+ *
+ * Who this is for.  Every other call of this library works inside a workspace the caller allocated on the device.  Some
+ * callers have nothing to give and no way to get it: a checking tool that runs beside a simulation whose workspace was
+ * sized to fill the GPU (cudaMalloc fails there); a plug-in running inside a host program whose memory pool owns all
+ * device memory and whose rules keep plug-ins from allocating; code that runs at a point where allocating would stall
+ * the whole device (cudaMalloc and cudaFree synchronise it).  Such a caller can still check that this GPU draws the same
+ * numbers as the CPU: this call makes no cudaMalloc / cudaFree and calls no library routine that allocates device memory.
+ *
+ * How.  The device-side staging of id, draw and out (24 bytes per draw) lives in a fixed array inside the library's
+ * device image, MCDC_NOALLOC_DRAWS_MAX entries long: 1.5 MiB that every GPU which loads the library holds until the
+ * process exits, used or not.  n > MCDC_NOALLOC_DRAWS_MAX is refused with MCDC_EINVAL and a message (nothing is launched);
+ * split larger requests into several calls.
+ *
+ * id, draw, out: HOST pointers, n entries each, owned by the caller (as everywhere in this header).  device: CUDA device
+ * ordinal (0..63); it is made current for the duration of the call and the caller's current device is restored.
+ * stream: a cudaStream_t of that device (NULL = the legacy default stream); the call returns after the stream has
+ * finished the work, so out is ready on return.
+ *
+ * First call on a device: the library looks up the array's address on that device once and remembers it.  Make that
+ * first call before starting any stream capture on the device.
+ * Sharing: all calls, from all threads and streams, stage through the same array.  Calls into this entry point are
+ * serialised by a lock inside the library, and each call overwrites every byte it later reads (nothing has to start at
+ * zero, nothing is carried from one call to the next), so results never depend on earlier calls.  But the array is one
+ * per GPU and process: if the work of two such calls could ever overlap on the GPU, they would race.
+ * Errors: MCDC_EINVAL (device out of range, n too large, NULL pointer with n > 0), MCDC_ECUDA (any CUDA failure, text in
+ * mcdc_last_error()).  n = 0 is a valid call that does nothing. */
+#define MCDC_NOALLOC_DRAWS_MAX 65536
+int mcdc_draws_noalloc(int32_t device, void *stream, uint64_t seed, uint32_t domain, uint32_t cycle, const uint64_t *id,
+                       const uint32_t *draw, uint64_t n, double *out);
+
 /* union-grid index of E[i] with the binary (out_bin) and the hashed (out_hash) search */
 int mcdc_test_grid_index(mcdc_problem *p, const double *E, uint64_t n, int32_t *out_bin, int32_t *out_hash);
 /* locate + nearest boundary for n points: loc[i][3] = (c0, elem, c1), dist[i], surf[i].  path 0: the code path the

@@ -20,6 +20,7 @@ _SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cu
 _HDR = os.path.join(_ROOT, "include", "mcdc.h")
 
 N_COUNTERS = 16
+NOALLOC_DRAWS_MAX = 65536  # MCDC_NOALLOC_DRAWS_MAX of include/mcdc.h
 ALWAYS = 0x7FFFFFFF  # persist_threshold: the persistent kernel runs the whole cycle
 EV_NAMES = {1: "scatter", 2: "fission", 3: "capture", 4: "transmit", 5: "reflect", 6: "leak", 7: "lattice",
             8: "time_edge", 9: "cutoff", 10: "lost"}
@@ -27,7 +28,7 @@ SYMBOLS = ["mcdc_workspace_bytes", "mcdc_create", "mcdc_run_eigenvalue", "mcdc_r
            "mcdc_run_fixed_source", "mcdc_get_dims", "mcdc_get_tallies", "mcdc_get_bank", "mcdc_set_trace",
            "mcdc_get_trace", "mcdc_test_draws", "mcdc_test_grid_index", "mcdc_test_geometry", "mcdc_get_timing",
            "mcdc_set_profile", "mcdc_get_profile", "mcdc_microbench", "mcdc_destroy", "mcdc_last_error",
-           "mcdc_set_physics", "mcdc_get_balance", "mcdc_get_census"]
+           "mcdc_set_physics", "mcdc_get_balance", "mcdc_get_census", "mcdc_draws_noalloc"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -154,6 +155,7 @@ def load_library():
     L.mcdc_set_physics.argtypes = [vp, P(Physics)]
     L.mcdc_get_balance.argtypes = [vp, _dp]
     L.mcdc_get_census.argtypes = [vp, P(u64), _dp, i32, P(i32)]
+    L.mcdc_draws_noalloc.argtypes = [i32, vp, u64, u32, u32, vp, vp, u64, _dp]
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -167,6 +169,28 @@ def _d(a):
 
 def _i(a):
     return np.ascontiguousarray(a, np.int32)
+
+
+def draws_noalloc(seed, domain, cycle, ids, idx, device=0, stream=None):
+    """``mcdc_draws_noalloc``: draw ``idx[i]`` of the random-number stream (seed, ids[i], domain, cycle) for every i,
+    computed on GPU ``device`` without a Problem and without a workspace.
+
+    For callers that cannot give the library device memory (the GPU is already full, or the host program forbids
+    allocating): the staging lives in a fixed 1.5 MiB array inside the library, so at most ``NOALLOC_DRAWS_MAX`` draws
+    per call (more raises McdcError).  ``ids`` / ``idx`` are host arrays; the result is a host float64 array, bit-equal
+    to ``Problem.draws``.  ``stream``: a raw cudaStream_t handle (int) of that device, None = the default stream.  The
+    first call on a device does a one-time address look-up: make it before any stream capture on that device."""
+    L = load_library()
+    ids = np.ascontiguousarray(ids, np.uint64)
+    idx = np.ascontiguousarray(idx, np.uint32)
+    if ids.shape != idx.shape or ids.ndim != 1:
+        raise ValueError("ids and idx must be 1-D arrays of equal length")
+    out = np.zeros(len(ids))
+    rc = L.mcdc_draws_noalloc(int(device), stream, int(seed), int(domain), int(cycle), ids.ctypes.data, idx.ctypes.data,
+                              len(ids), out.ctypes.data_as(_dp))
+    if rc != 0:
+        raise McdcError(rc, L.mcdc_last_error().decode())
+    return out
 
 
 class Problem:

@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1744,4 +1745,65 @@ extern "C" int mcdc_microbench(mcdc_problem *p, int32_t which, uint64_t iters, d
     *ms_out = ms;
     *ops_out = per_thread * threads * blocks;  // thread-level operations of the timed launch
     return 0;
+}
+
+// ------------------------------------------------------------------ the entry point that allocates nothing
+// mcdc_draws_noalloc (include/mcdc.h): mcdc_test_draws for a caller that has no device memory to lend.  The three staging
+// arrays that mcdc_test_draws carves out of the problem's workspace live here instead, in an array that is part of the
+// library's device image: it exists on every GPU from the moment that GPU loads the library until the process ends,
+// whether or not the entry point is ever called (MCDC_NOALLOC_DRAWS_MAX x 24 bytes = 1.5 MiB per GPU).
+static __device__ __align__(256) unsigned char g_noalloc_scratch[(size_t)MCDC_NOALLOC_DRAWS_MAX * 24u];
+
+// In HOST code the name g_noalloc_scratch is only a handle for the runtime, not the array's device address, so it must
+// never be handed to a kernel or to cudaMemcpy as a pointer.  The address is asked for once per device, with that
+// device current, and kept here.
+enum { NOALLOC_MAX_DEVICES = 64 };
+static std::mutex g_noalloc_mutex;
+static unsigned char *g_noalloc_ptr[NOALLOC_MAX_DEVICES];  // zero-initialised: "not asked yet"
+
+extern "C" int mcdc_draws_noalloc(int32_t device, void *stream, uint64_t seed, uint32_t domain, uint32_t cycle,
+                                  const uint64_t *id, const uint32_t *draw, uint64_t n, double *out)
+{
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return fail(MCDC_EINVAL, "device %d outside [0, %d)", (int)device, (int)NOALLOC_MAX_DEVICES);
+    if (n > (uint64_t)MCDC_NOALLOC_DRAWS_MAX)
+        return fail(MCDC_EINVAL, "mcdc_draws_noalloc: %llu draws asked for, the built-in scratch holds at most %d per call "
+                                 "(split the request, or use mcdc_test_draws with a workspace)",
+                    (unsigned long long)n, (int)MCDC_NOALLOC_DRAWS_MAX);
+    if (n == 0) return 0;
+    if (!id || !draw || !out) return fail(MCDC_EINVAL, "null");
+    // one call at a time per process: every call stages through the same bytes
+    std::lock_guard<std::mutex> guard(g_noalloc_mutex);
+    int prev = -1;
+    CUDA_OK(cudaGetDevice(&prev));
+    if (prev != device) CUDA_OK(cudaSetDevice(device));
+    int rc = 0;
+    do {
+        unsigned char *base = g_noalloc_ptr[device];
+        if (!base) {  // first call on this device: resolve the array's address there
+            void *sym = nullptr;
+            cudaError_t e = cudaGetSymbolAddress(&sym, g_noalloc_scratch);
+            if (e != cudaSuccess || !sym) {
+                rc = fail(MCDC_ECUDA, "cudaGetSymbolAddress(g_noalloc_scratch) on device %d: %s", (int)device, cudaGetErrorString(e));
+                break;
+            }
+            g_noalloc_ptr[device] = base = (unsigned char *)sym;
+        }
+        cudaStream_t st = (cudaStream_t)stream;
+        // same carving as mcdc_test_draws.  Nothing here has to start at zero: the kernel reads d_id[i], d_draw[i] and
+        // writes d_out[i] for i < n only, and all of those are overwritten by this call before they are read.
+        unsigned long long *d_id = (unsigned long long *)base;
+        double *d_out = (double *)(base + n * 8);
+        uint32_t *d_draw = (uint32_t *)(base + n * 16);
+        cudaError_t e = cudaMemcpyAsync(d_id, id, n * 8, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_draw, draw, n * 4, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) {
+            k_test_draws<<<(unsigned int)((n + 255) / 256), 256, 0, st>>>(seed, domain, cycle, d_id, d_draw, n, d_out);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(out, d_out, n * 8, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) rc = fail(MCDC_ECUDA, "mcdc_draws_noalloc: %s", cudaGetErrorString(e));
+    } while (0);
+    if (prev != device) cudaSetDevice(prev);
+    return rc;
 }
