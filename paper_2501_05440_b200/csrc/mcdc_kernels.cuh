@@ -314,6 +314,16 @@ __device__ __forceinline__ bool count_secondaries(const Ctx &c, unsigned int n)
     return true;
 }
 
+// the same limit looked at BEFORE children are made (time-dependent multi-group: only the children that are really born
+// are counted afterwards, so the count cannot be taken up front as the continuous-energy branch does).  The read is not
+// atomic with the later count: lanes that fission at the same moment can overshoot the limit by their own children, which
+// a runaway guard tolerates.
+__device__ __forceinline__ bool secondaries_allowed(const Ctx &c, unsigned int n)
+{
+    if (*(volatile unsigned long long *)(c.counters + 15) + n > c.max_secondaries) { atomicExch(c.err, -3); return false; }
+    return true;
+}
+
 __device__ __forceinline__ void mark_lost(const Ctx &c)
 {
     atomicExch(c.err, -2);
@@ -503,9 +513,14 @@ __device__ __forceinline__ bool ring_put(const Ctx &c, const Bank &O, const unsi
     // it -- more than `cap` secondaries wait: bank overflow
     if (*(volatile uint32_t *)(O.ev + i) != free_) {
         if (*(volatile const unsigned int *)head + c.cap <= n_in + a) atomicExch(c.err, -3);
+        // A ticket for the previous lap's entry has been issued; its holder takes the entry on its next loop trip.  The
+        // wait is short when the holder is a lane of another warp.  It cannot end when the holder is a lane of THIS warp
+        // (it is parked at the loop top until this lane gets there), which takes `cap` pushes within one loop trip, i.e.
+        // a ring about as small as the number of resident lanes: the bounded wait (tens of milliseconds) then reports
+        // the bank as too small (MCDC_EBANK), which it is.  DESIGN.md section 5 lists this limit.
         unsigned int spins = 0;
         while (*(volatile uint32_t *)(O.ev + i) != free_ && *(volatile int *)c.err == 0)
-            if (++spins > (1u << 22)) atomicExch(c.err, -3);
+            if (++spins > (1u << 16)) atomicExch(c.err, -3);
         if (*(volatile int *)c.err != 0) return false;
     }
     O.x[i] = p.x; O.y[i] = p.y; O.z[i] = p.z; O.ux[i] = p.ux; O.uy[i] = p.uy; O.uz[i] = p.uz;
@@ -588,6 +603,11 @@ k_persist(Ctx c, unsigned int s, unsigned int n0)
                 backlog = __shfl_sync(FULL, backlog, 0);
                 n_take = min((unsigned int)nw, backlog);
             }
+        }
+        if (GROW && n_take) {  // the run is being stopped (bank overflow, lost particle): hand out no more work
+            int e = 0;
+            if (lane == 0) e = *(volatile int *)c.err;
+            if (__shfl_sync(FULL, e, 0)) n_take = 0;
         }
         const bool take = n_take > 0;
         if (take) {
@@ -679,7 +699,7 @@ k_persist(Ctx c, unsigned int s, unsigned int n0)
                 n_end++;
                 if (!GROW) record_fission<CE>(c, p, rng.ctr, slot, aux);
                 else if (TD) {
-                    if (aux > 0) {
+                    if (aux > 0 && secondaries_allowed(c, (unsigned int)aux)) {
                         // every child is counted as born first; one that is never born, or that waits for a later
                         // interval, is counted as ended at once (the termination test stays ended == n_in + born)
                         atomicAdd(born, (unsigned int)aux);

@@ -915,6 +915,11 @@ extern "C" void mcdc_destroy(mcdc_problem *p)
 
 extern "C" const char *mcdc_last_error(void) { return g_err.c_str(); }
 
+#ifndef MCDC_BUILD_ID
+#define MCDC_BUILD_ID "unknown"
+#endif
+extern "C" const char *mcdc_build_id(void) { return MCDC_BUILD_ID; }
+
 // ------------------------------------------------------------------ drivers
 #ifndef MCDC_GRID_PER_SM
 #define MCDC_GRID_PER_SM 16ull  // measured (ms per C4 cycle): 4 -> 42.9, 8 -> 41.5, 16 -> 40.9, 64 -> 42.3, 1024 -> 45.1
@@ -1136,6 +1141,7 @@ static int abandon(mcdc_problem *p, int rc)
     cudaMemsetAsync(p->ctx.fis.n, 0, sizeof(int) * (size_t)p->cap, p->stream);
     cudaStreamSynchronize(p->stream);
     p->dirty = true;
+    p->work.next_interval = -1;  // fixed source: the next call has to name the first interval again
     g_err = keep;
     return rc;
 }
@@ -1291,7 +1297,9 @@ template <bool CE> static int census_to_source_t(mcdc_problem *p, int k, uint64_
 }
 
 // one census interval of a fixed-source run (time edge k -> k + 1)
-static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
+// publish_now = false: the caller runs several intervals as ONE call and publishes after the last (a failure part-way
+// then leaves the previous call's results readable)
+static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed, bool publish_now = true)
 {
     Ctx &c = p->ctx;
     cudaStream_t st = p->stream;
@@ -1306,7 +1314,8 @@ static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
         CUDA_OK(cudaMemsetAsync(c.work, 0, 32, st));
         CUDA_OK(cudaMemsetAsync(c.scal, 0, 64, st));
         p->cb_cur = 0; c.cbank = p->cb[0]; p->census_n = 0;
-    } else if (p->work.next_interval != k) return fail(MCDC_EINVAL, "census intervals must be run in order: expected %d, got %d", p->work.next_interval, k);
+    } else if (p->work.next_interval < 0) return fail(MCDC_EINVAL, "no fixed-source run is under way (none started, or the last interval failed): start again from interval %d", p->first_interval);
+    else if (p->work.next_interval != k) return fail(MCDC_EINVAL, "census intervals must be run in order: expected %d, got %d", p->work.next_interval, k);
     RunStats &w = p->work;
     set_seed(c, seed); c.cycle = 0; c.w0 = 1.0; c.k_prev = 1.0;
     c.max_secondaries = 64ull * (N + (uint64_t)p->census_target * (uint64_t)n_t) + 4096;  // R25a
@@ -1334,9 +1343,6 @@ static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
         if (rc) return abandon(p, rc);
     }
     CUDA_OK(cudaEventRecord(p->t1, st));
-    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[w.set], p->flux_acc2[w.set],
-                                                          c.n_tally, 1.0 / (double)N, 1);
-    p->n_launches++;
     CUDA_OK(cudaMemcpyAsync(&p->pin->census[0], c.work + 4, 4, cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->scal, c.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_OK(cudaMemcpyAsync(p->pin->counters, c.counters, sizeof p->pin->counters, cudaMemcpyDeviceToHost, st));
@@ -1344,10 +1350,16 @@ static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
     CUDA_OK(cudaStreamSynchronize(st));
     CUDA_OK(cudaGetLastError());
     profile_collect(p);
+    // the error flag is read BEFORE this interval's flux is folded into the run's accumulators: after an earlier
+    // interval was published they are the published set, and a failed interval must not reach them
     int rc = device_error_code(p, p->pin->err);
     if (rc) return abandon(p, rc);
     p->census_n = p->pin->census[0];
     if (p->census_n > p->cap) return abandon(p, fail(MCDC_EBANK, "census bank overflow (capacity %llu)", (unsigned long long)p->cap));
+    k_accumulate<<<(c.n_tally + BS - 1) / BS, BS, 0, st>>>(c.flux, p->flux_copies, p->flux_cycle, p->flux_acc[w.set], p->flux_acc2[w.set],
+                                                          c.n_tally, 1.0 / (double)N, 1);
+    p->n_launches++;
+    CUDA_OK(cudaGetLastError());
     float ms = 0.f;
     CUDA_OK(cudaEventElapsedTime(&ms, p->t0, p->t1));
     p->ms_transport += ms;
@@ -1366,7 +1378,7 @@ static int interval_internal(mcdc_problem *p, uint64_t N, int k, uint64_t seed)
     w.next_interval = k + 1;
     p->bank_count = 0;
     p->last_N = N;
-    publish(p);
+    if (publish_now) publish(p);
     return 0;
 }
 
@@ -1442,7 +1454,7 @@ extern "C" int mcdc_run_fixed_source(mcdc_problem *p, uint64_t N, uint64_t seed)
     if (!p || !p->timed) return fail(MCDC_EINVAL, "mcdc_run_fixed_source needs a continuous-energy or a time-dependent multi-group problem");
     if (p->td) {  // census interval by census interval (population control happens between them, R40)
         for (int k = p->first_interval; k < p->ctx.ce.n_t; k++) {
-            int rc = interval_internal(p, N, k, seed);
+            int rc = interval_internal(p, N, k, seed, k + 1 == p->ctx.ce.n_t);  // one call: published once, at the end
             if (rc) return rc;
         }
         return 0;

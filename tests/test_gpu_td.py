@@ -143,3 +143,49 @@ def test_td_validation(gpu):
     with pytest.raises(gpu.McdcError):
         g.L.mcdc_run_eigenvalue(g.h, 500, 1, 1, 1) and g._check(-1)
     g.close()
+
+
+def _supercritical_td(n=500):
+    """The G = 1 kinetics medium with its prompt yield raised to k_prompt = 1.47: the population grows about tenfold per
+    census interval, so a run of a few intervals ends in the runaway guard (R25a) -- in a LATER interval than the first."""
+    P = inputs.td_infinite(n_particles=n, G=1, t_end=8.0e-4, n_t=8)
+    P["mg_nu"] = P["mg_nu"] * 1.6
+    return P
+
+
+def test_td_failed_interval_leaves_the_last_successful_results(gpu):
+    """mcdc.h: a failed run call leaves the results of the last successful call readable.  Interval by interval, the
+    flux of the failed interval must not reach the published accumulators; mcdc_run_fixed_source publishes once, at the
+    end, so a failure part-way leaves the previous call's results; after a failure the run has to start again."""
+    P = _supercritical_td()
+    N, seed, nt = P["run"]["n_particles"], P["run"]["seed"], len(P["t_edges"]) - 1
+    g = gpu.Problem(P, max_particles=200000)
+    good, failed_at = None, None
+    for k in range(nt):
+        try:
+            g.run_cycle(N, k, 1, seed)
+        except gpu.McdcError as e:
+            assert e.code == -3  # MCDC_EBANK: the secondaries limit, raised on the device
+            failed_at = k
+            break
+        good = g.results()
+        cen = g.census()
+    assert failed_at is not None and failed_at >= 1, failed_at
+    after = g.results()
+    assert (after["flux_mean"] == good["flux_mean"]).all() and (after["counters"] == good["counters"]).all()
+    assert after["k_mean"] == good["k_mean"] and g.census() == cen
+    with pytest.raises(gpu.McdcError) as e:
+        g.run_cycle(N, failed_at, 1, seed)  # the run is over: the failed interval cannot be tried again
+    assert e.value.code == -1 and "start again" in str(e.value)
+    # a new run from the first interval works, and reproduces the first run's intervals
+    for k in range(failed_at):
+        g.run_cycle(N, k, 1, seed)
+    again = g.results()
+    assert np.allclose(again["flux_mean"], good["flux_mean"], rtol=1e-12, atol=0) and (again["counters"] == good["counters"]).all()
+    # the same run as ONE call fails as a whole and publishes nothing of it
+    with pytest.raises(gpu.McdcError) as e:
+        g.run()
+    assert e.value.code == -3
+    kept = g.results()
+    assert (kept["flux_mean"] == again["flux_mean"]).all() and (kept["counters"] == again["counters"]).all()
+    g.close()
