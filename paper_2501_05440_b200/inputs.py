@@ -233,7 +233,23 @@ def tube_positions():
     return [(8 + i, 8 + j) for i in (-6, -3, 0, 3, 6) for j in (-6, -3, 0, 3, 6)]
 
 
-def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_reflect=False, height=None):
+def _pin_universes(g, cy, zf):
+    """Universes 1..6 (pins: material u - 1 inside the cylinder, moderator 6 outside) and 7 (moderator only).  zf = the
+    z plane that ends the fuel (axial reflector above it: "fully 3D"), or None: with it every pin universe
+    has three cells -- fuel (inside the cylinder AND below zf), moderator beside it (outside the cylinder, below zf) and
+    the moderator of the axial reflector (above zf, the whole element)."""
+    for u in range(1, 7):
+        if zf is None:
+            g.cell(u, [(cy, -1)], u - 1)
+            g.cell(u, [(cy, +1)], 6)
+        else:
+            g.cell(u, [(cy, -1), (zf, -1)], u - 1)
+            g.cell(u, [(cy, +1), (zf, -1)], 6)
+            g.cell(u, [(zf, +1)], 6)
+    g.cell(7, [], 6)
+
+
+def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_reflect=False, height=None, axial_reflector=None):
     """C4: one (n_asm*n_pin+n_refl)^2 lattice; elements [0,n_asm*n_pin)^2
     are fuelled assemblies, the rest moderator 'reflector' elements.  x=0,y=0 REFLECT,
     outer faces VACUUM.  Materials: 0,1,2 fuel variants; 3,4 alternate fuel; 5 tube fill; 6 moderator.
@@ -249,15 +265,16 @@ def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_refl
     y1 = g.surf(PLANE_Y, [side], outer)
     cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
     root = [(x0, +1), (x1, -1), (y0, +1), (y1, -1)]
+    zf = None
     if height is not None:  # finite height: reflecting mid-plane at z = 0, vacuum top at z = height
         z0 = g.surf(PLANE_Z, [0.0], REFLECT)
         z1 = g.surf(PLANE_Z, [float(height)], outer)
         root += [(z0, +1), (z1, -1)]
+        if axial_reflector:  # the top `axial_reflector` cm of every pin are moderator
+            assert 0.0 < axial_reflector < height
+            zf = g.surf(PLANE_Z, [float(height - axial_reflector)], TRANSMIT)
     g.cell(0, root, 0, lattice=True)
-    for u in range(1, 7):
-        g.cell(u, [(cy, -1)], u - 1)
-        g.cell(u, [(cy, +1)], 6)
-    g.cell(7, [], 6)
+    _pin_universes(g, cy, zf)
     univ = np.full((n, n), 7, np.int32)
     bins = np.full((n, n), nfuel * nfuel, np.int32)
     tubes = set(tube_positions()) if n_pin == 17 else set()
@@ -279,7 +296,7 @@ def geom_quarter_core(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl=17, all_refl
 
 
 def geom_quarter_core_2l(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl_asm=1, all_reflect=False, height=None,
-                         reflector_lattice=True):
+                         reflector_lattice=True, axial_reflector=None):
     """The quarter core of geom_quarter_core as a TWO-LEVEL lattice (the paper's multi-group benchmark
     is a core of assemblies of pins): a first-level (n_asm + n_refl_asm)^2 lattice of assemblies of pitch n_pin * pitch;
     every assembly universe is one cell without surfaces filled by a second-level n_pin x n_pin pin lattice.  Same pin
@@ -298,15 +315,16 @@ def geom_quarter_core_2l(pitch=1.26, r=0.54, n_asm=2, n_pin=17, n_refl_asm=1, al
     y1 = g.surf(PLANE_Y, [side], outer)
     cy = g.surf(CYL_Z, [0.0, 0.0, r], TRANSMIT)
     root = [(x0, +1), (x1, -1), (y0, +1), (y1, -1)]
+    zf = None
     if height is not None:
         z0 = g.surf(PLANE_Z, [0.0], REFLECT)
         z1 = g.surf(PLANE_Z, [float(height)], outer)
         root += [(z0, +1), (z1, -1)]
+        if axial_reflector:
+            assert 0.0 < axial_reflector < height
+            zf = g.surf(PLANE_Z, [float(height - axial_reflector)], TRANSMIT)
     g.cell(0, root, 0, lattice=True)
-    for u in range(1, 7):
-        g.cell(u, [(cy, -1)], u - 1)
-        g.cell(u, [(cy, +1)], 6)
-    g.cell(7, [], 6)
+    _pin_universes(g, cy, zf)
     g.cell(8, [], 0, lattice2=True)
     g.cell(9, [], 1, lattice2=True)
     if reflector_lattice:
@@ -580,11 +598,12 @@ def config3(n_particles=1_000_000, n_inactive=20, n_active=80, seed=1, same_mate
 
 
 def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform=False,
-            n_asm=2, n_pin=17, n_refl=17, G=7, height=None, two_level=False, reflector_lattice=True):
+            n_asm=2, n_pin=17, n_refl=17, G=7, height=None, two_level=False, reflector_lattice=True, axial_reflector=None):
     """C4: 2-D quarter core stand-in for the paper's C5G7 workload: 7 synthetic
     materials from seed 4.  uniform=True: all materials identical + all faces reflecting (pin).
     two_level=True: the same core described as a lattice of assemblies of pin lattices (n_refl must be a
-    multiple of n_pin)."""
+    multiple of n_pin).  height: the fully 3-D core (reflecting mid-plane z = 0, vacuum top); axial_reflector: the top
+    so many cm of every pin are moderator (the source then lies in the fuelled part)."""
     rng = np.random.default_rng(4)
     mats = [mg_fuel(rng, G, kt) for kt in (1.05, 1.15, 1.25)]
     mats += [mg_fuel(rng, G, kt, thermal_boost=1.5) for kt in (1.10, 1.20)]
@@ -594,12 +613,14 @@ def config4(n_particles=10_000_000, n_inactive=20, n_active=100, seed=1, uniform
     if two_level:
         assert n_refl % n_pin == 0
         P = geom_quarter_core_2l(n_asm=n_asm, n_pin=n_pin, n_refl_asm=n_refl // n_pin, all_reflect=uniform, height=height,
-                                 reflector_lattice=reflector_lattice)
+                                 reflector_lattice=reflector_lattice, axial_reflector=axial_reflector)
     else:
-        P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform, height=height)
+        P = geom_quarter_core(n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, all_reflect=uniform, height=height,
+                              axial_reflector=axial_reflector)
     P.update(_mg_pack(mats))
     side = n_asm * n_pin * 1.26
-    P.update(_src([0, 0, 0], [side, side, 0.9 * height if height else 0], G=G, pdf=mats[0]["chi"]))
+    z_src = 0.9 * ((height - axial_reflector) if axial_reflector else height) if height else 0
+    P.update(_src([0, 0, 0], [side, side, z_src], G=G, pdf=mats[0]["chi"]))
     P["run"] = dict(kind="eigen", n_particles=n_particles, n_inactive=n_inactive, n_active=n_active, seed=seed)
     P["name"] = "C4"
     return P

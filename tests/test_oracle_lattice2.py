@@ -18,13 +18,15 @@ def _flat_elem(packed, n_outer, n_pin):
     return (ay * n_pin + py) * (n_outer * n_pin) + ax * n_pin + px
 
 
-@pytest.mark.parametrize("n_asm,n_pin,n_refl,height", [(2, 3, 3, None), (1, 4, 4, 6.0), (2, 5, 5, None)])
-def test_two_level_equals_flat_lattice(orc, n_asm, n_pin, n_refl, height):
+@pytest.mark.parametrize("n_asm,n_pin,n_refl,height,axial", [(2, 3, 3, None, None), (1, 4, 4, 6.0, None), (2, 5, 5, None, None),
+                                                              (1, 3, 3, 6.0, 2.0)])
+def test_two_level_equals_flat_lattice(orc, n_asm, n_pin, n_refl, height, axial):
     """A core of (n_asm + 1)^2 assemblies of n_pin^2 pins, flat (one lattice) and two-level: identical k per cycle,
     event counters and fission bank; per-pin flux to rounding; and the traced histories agree event by event once the
     two-level locations and wall codes are mapped to the flat ones (second-level wall n_surf+4+w and first-level wall
     n_surf+w are both flat wall n_surf+w)."""
-    kw = dict(n_particles=1500, n_inactive=1, n_active=2, n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, height=height)
+    kw = dict(n_particles=1500, n_inactive=1, n_active=2, n_asm=n_asm, n_pin=n_pin, n_refl=n_refl, height=height,
+              axial_reflector=axial)
     Pf, P2 = inputs.config4(**kw), inputs.config4(two_level=True, **kw)
     assert "lat2_nx" in P2 and "lat2_nx" not in Pf
     of, o2 = orc.Oracle(Pf), orc.Oracle(P2)
@@ -53,12 +55,14 @@ def test_two_level_equals_flat_lattice(orc, n_asm, n_pin, n_refl, height):
     assert (lat["surf"] >= ns + 4).sum() > 200 and (lat["surf"] < ns + 4).sum() > 20  # walls of both levels were crossed
 
 
-@pytest.mark.parametrize("case", ["core2l", "core2l_3d", "gap", "gap_wide", "core2l_homog_reflector", "rect", "rect_1col"])
+@pytest.mark.parametrize("case", ["core2l", "core2l_3d", "core2l_3d_axial", "gap", "gap_wide", "core2l_homog_reflector", "rect", "rect_1col"])
 def test_trace_two_level_vs_brute_force(orc, case):
     """Two-level lattices event by event (packed element, local cell, wall codes of both levels, surfaces of the cell
     the inner lattice fills) against brute force over all grid lines and all pins."""
     P = dict(core2l=lambda: inputs.config4(n_particles=50, n_asm=1, n_pin=3, n_refl=3, two_level=True),
              core2l_3d=lambda: inputs.config4(n_particles=40, n_asm=2, n_pin=2, n_refl=2, two_level=True, height=5.0),
+             core2l_3d_axial=lambda: inputs.config4(n_particles=40, n_asm=2, n_pin=2, n_refl=2, two_level=True, height=5.0,
+                                                    axial_reflector=1.5),
              gap=lambda: inputs.assembly_gap(2, 3), gap_wide=lambda: inputs.assembly_gap(3, 2, gap=0.6),
              rect=lambda: inputs.two_level_rect(2, 3, 3, 2), rect_1col=lambda: inputs.two_level_rect(1, 2, 1, 4),
              core2l_homog_reflector=lambda: inputs.config4(n_particles=50, n_asm=1, n_pin=3, n_refl=3, two_level=True,

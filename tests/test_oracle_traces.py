@@ -57,17 +57,22 @@ def test_trace_curved_mirrors_vs_brute_force(orc, kind):
     assert ((tr["ev"] == 5) & (tr["surf"] == curved)).sum() >= 100
 
 
-@pytest.mark.parametrize("case", ["C4small", "C4_3d", "lat1x6", "lat5x1", "lat3x5", "C4edge"])
+@pytest.mark.parametrize("case", ["C4small", "C4_3d", "C4_3d_axial", "lat1x6", "lat5x1", "lat3x5", "C4edge"])
 def test_trace_lattice_vs_brute_force(orc, case):
     """One-level lattices, event by event (incl. element and local cell of every event): the oracle's neighbour /
     wall-ahead logic (R14) against brute force over every grid line and every pin of the lattice."""
     P = dict(C4small=lambda: inputs.config4(n_particles=60, n_asm=1, n_pin=3, n_refl=1),
              C4_3d=lambda: inputs.config4(n_particles=60, n_asm=1, n_pin=4, n_refl=1, height=6.0),
+             C4_3d_axial=lambda: inputs.config4(n_particles=60, n_asm=1, n_pin=4, n_refl=1, height=6.0, axial_reflector=2.0),
              lat1x6=lambda: inputs.rect_lattice(1, 6), lat5x1=lambda: inputs.rect_lattice(5, 1),
              lat3x5=lambda: inputs.rect_lattice(3, 5),
              C4edge=lambda: inputs.config4(n_particles=40, n_asm=2, n_pin=5, n_refl=2))[case]()
     tr = _compare(orc, P, 60, 60)
     assert (tr["ev"] == 7).sum() >= 50  # lattice-wall events
+    if case == "C4_3d_axial":  # the plane between fuel and axial reflector (the last surface) was crossed from all three
+        zf = len(P["surf_type"]) - 1          # cells of a pin universe: fuel, the moderator beside it, the reflector above
+        hit = tr[(tr["ev"] == 4) & (tr["surf"] == zf)]
+        assert len(hit) >= 20 and len(set(int(c) for c in hit["c1"])) >= 3
 
 
 def _compare_ce(orc, P, n_src):

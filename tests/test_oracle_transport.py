@@ -328,6 +328,52 @@ def test_quarter_core_finite_height_leakage(orc):
     assert r["counters"][EV["lattice"]] == 0
 
 
+@pytest.mark.parametrize("two_level", [False, True])
+@pytest.mark.parametrize("start", ["fuel", "moderator"])
+def test_axial_reflector_beam_leakage(orc, two_level, start):
+    """Fully 3-D core with an axial reflector: every pin universe has a z plane that
+    ends the fuel (fuel below it inside the cylinder, moderator beside and above).  Pure absorbers with different cross
+    sections in fuel and moderator, a beam along +z from the mid-plane: started inside a fuel cylinder it leaks through
+    the top with probability exp(-Sigma_fuel h_fuel - Sigma_mod h_refl), started beside it with exp(-Sigma_mod height);
+    a survivor of the fuelled part crosses the new plane exactly once (transmit events); no lattice wall, no cylinder."""
+    hgt, h_r, s_fuel, s_mod, N = 3.0, 1.0, 0.5, 0.2, 40000
+    P = inputs.config4(n_particles=N, n_inactive=0, n_active=1, n_asm=1, n_pin=2, n_refl=2, G=1, height=hgt,
+                       axial_reflector=h_r, two_level=two_level)
+    P["mg_sig_t"][:5] = s_fuel; P["mg_sig_t"][5:] = s_mod
+    P["mg_sig_c"][:] = P["mg_sig_t"]
+    for k in ("mg_sig_f", "mg_nu", "mg_S"):
+        P[k][:] = 0.0
+    P["mg_chi"][:] = 1.0
+    if start == "fuel":   # a square well inside the cylinder of pin (0, 0) (centre 0.63, 0.63; r = 0.54)
+        P["src_lo"][:] = [0.33, 0.33, 1e-9]; P["src_hi"][:] = [0.93, 0.93, 1e-9]
+        p_plane = math.exp(-s_fuel * (hgt - h_r))
+        p = p_plane * math.exp(-s_mod * h_r)
+    else:                 # the corner of the same element, outside the cylinder
+        P["src_lo"][:] = [0.02, 0.02, 1e-9]; P["src_hi"][:] = [0.12, 0.12, 1e-9]
+        p_plane = math.exp(-s_mod * (hgt - h_r))
+        p = math.exp(-s_mod * hgt)
+    P["src_iso"] = 0
+    P["src_dir"][:] = [0.0, 0.0, 1.0]
+    rc, r = orc.Oracle(P).run()
+    assert rc == 0
+    assert abs(r["leak_mean"] - p) < 3.5 * math.sqrt(p * (1 - p) / N)
+    c = r["counters"]
+    assert abs(c[EV["transmit"]] / N - p_plane) < 3.5 * math.sqrt(p_plane * (1 - p_plane) / N)
+    assert c[EV["lattice"]] == 0 and c[EV["reflect"]] == 0 and c[EV["lost"]] == 0
+    assert c[EV["capture"]] + c[EV["leak"]] == N
+
+
+def test_axial_reflector_returns_neutrons(orc):
+    """A core of fuelled height 4 with 2 cm of axial reflector on top against the bare core of the same fuelled height,
+    same seed: the reflector scatters neutrons back, so k is higher and fewer histories leak (the ordering any transport
+    code must reproduce; a reflector cell filled with the wrong material or never entered would not)."""
+    kw = dict(n_particles=20000, n_inactive=2, n_active=6, n_asm=1, n_pin=3, n_refl=1)
+    rc, refl = orc.Oracle(inputs.config4(height=6.0, axial_reflector=2.0, **kw)).run()
+    rc, bare = orc.Oracle(inputs.config4(height=4.0, **kw)).run()
+    assert refl["k_mean"] > bare["k_mean"] + 3 * math.hypot(refl["k_sdev"], bare["k_sdev"])
+    assert refl["leak_mean"] < bare["leak_mean"] - 3 * math.hypot(refl["leak_sdev"], bare["leak_sdev"])
+
+
 def test_all_core_variant_equals_serial_run(orc):
     """orc_run_eigenvalue_mt (bench.py's all-core cpu_baseline) splits the source particles in contiguous id ranges:
     identical integer counters and bank, tallies equal to summation order; one thread = the serial run bit for bit."""
