@@ -90,19 +90,36 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+COUNTS_FILE = os.path.join("profiles", "r03_counts.csv")
+
+
 def ncu_counts():
-    """Per-event instruction and DRAM-traffic figures of the dominant kernels, measured by ncu on this build (they are
-    properties of the build and the workload, not of a timing); profiles/r02_counts.md names the captures."""
-    out = {}
+    """Per-event instruction and DRAM-traffic figures of the dominant kernels, measured by ncu (properties of a build and
+    a workload, not of a timing); profiles/r03_counts.md names the captures.  Every row carries the identity of the build
+    it was captured on (binding.source_id() = mcdc_build_id()); a row is used only when that is the library now loaded
+    AND the sources now on disk -- otherwise the figures would describe another kernel, and the caller reports them as
+    stale instead of printing them beside live timings."""
+    out = {"_stale": True, "_file": COUNTS_FILE}
     try:
-        with open(os.path.join(ROOT, "profiles", "r02_counts.csv")) as f:
-            rows = [l.strip().split(",") for l in f if l.strip()]
+        from paper_2501_05440_b200 import binding
+        now = binding.build_id()
+        if now != binding.source_id():
+            out["_why"] = "the loaded library was not built from the sources on disk"
+            return out
+        with open(os.path.join(ROOT, COUNTS_FILE)) as f:
+            rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
+        col = {name: i for i, name in enumerate(rows[0])}
         for r in rows[1:]:
-            ev = float(r[1])
-            out[r[0]] = {"warp_inst_per_event": float(r[2]) / ev, "dram_bytes_per_event": (float(r[3]) + float(r[4])) / ev,
-                         "source": "ncu --set full, profiles/r02_counts.md"}
-    except Exception:
-        pass
+            if r[col["build_id"]] != now:
+                out["_why"] = f"captured on build {r[col['build_id']]}, running build {now}"
+                continue
+            ev = float(r[col["events_per_launch"]])
+            out[r[0]] = {"warp_inst_per_event": float(r[col["warp_inst"]]) / ev,
+                         "dram_bytes_per_event": (float(r[col["dram_bytes_read"]]) + float(r[col["dram_bytes_write"]])) / ev,
+                         "source": f"ncu --set full on build {now}, profiles/r03_counts.md"}
+            out["_stale"] = False
+    except Exception as e:  # no file, no column: nothing to report
+        out["_why"] = f"{type(e).__name__}: {e}"
     return out
 
 
@@ -110,7 +127,7 @@ def alu_roofline(g, key, events_per_sec, clocks_mhz):
     """The path is bound by instruction issue / dependent latency, not by HBM: report the issue-slot roofline beside
     the HBM one.  peak = measured FFMA issue rate of this GPU (library micro-benchmark, warp instructions/s);
     achieved = warp instructions per event (ncu, this build) x events/s."""
-    cnt = ncu_counts().get(key, {})
+    cnt = ncu_counts().get(key) or {}
     try:
         ffma = g.microbench("ffma", 20000) / 32.0   # warp instructions per second
         dfma = g.microbench("dfma", 20000)
@@ -119,12 +136,22 @@ def alu_roofline(g, key, events_per_sec, clocks_mhz):
     wipe = cnt.get("warp_inst_per_event")
     out = {"bound": "alu", "unit": "warp-inst/s", "peak": ffma, "peak_source": "measured: mcdc_microbench FFMA issue rate",
            "nominal_peak": N_SM * N_SMSP * (clocks_mhz or 1965.0) * 1e6, "dfma_per_sec_measured": dfma,
-           "warp_inst_per_event": wipe, "thread_inst_per_event": cnt.get("thread_inst_per_event"),
-           "counts_source": cnt.get("source")}
+           "warp_inst_per_event": wipe, "counts_source": cnt.get("source"), "achieved": None, "frac": None}
     if wipe:
         out["achieved"] = wipe * events_per_sec
         out["frac"] = out["achieved"] / ffma
+    else:
+        out["note"] = "stale capture: no ncu instruction count of THIS build in " + COUNTS_FILE
     return out
+
+
+def measured_dram(cnt, events_per_launch, launch_seconds, peak):
+    """The HBM fraction from the bytes the kernel REALLY moved (ncu dram__bytes_read + write per event, this build) at the
+    live event rate -- beside the contract's algorithmic-bytes figure, which for a register-resident kernel is a model."""
+    if "dram_bytes_per_event" not in cnt or not launch_seconds:
+        return None
+    gbs = cnt["dram_bytes_per_event"] * events_per_launch / launch_seconds / 1e9
+    return {"bytes_per_event": cnt["dram_bytes_per_event"], "achieved": gbs, "unit": "GB/s", "frac": gbs / peak}
 
 
 def max_over_ranks(x: float, world: int, device=None) -> float:
@@ -259,7 +286,8 @@ def run_ours(args):
     dom = "persist" if prof["persist"]["ms"] >= prof["sweep"]["ms"] else "sweep"
     ev_dom = ev_prof - ev_sweep if dom == "persist" else ev_sweep
     kd = prof[dom]
-    cnt = ncu_counts().get("k_persist_mg" if dom == "persist" else "k_sweep_mg", {})
+    counts = ncu_counts()
+    cnt = counts.get("k_persist_mg" if dom == "persist" else "k_sweep_mg") or {}
     roof = None
     if kd["launches"]:
         bytes_per_launch = B_ALG_MG * ev_dom / kd["launches"]
@@ -269,13 +297,20 @@ def run_ours(args):
                 "frac": ach / peak, "peak_source": peak_src, "bytes_per_event": B_ALG_MG,
                 "events_per_launch": ev_dom / kd["launches"], "share_of_events": ev_dom / max(ev_prof, 1),
                 "avg_launch_ms": 1e3 * dur, "share_of_step": kd["ms"] / tot_ms if tot_ms else None,
+                "frac_basis": "algorithmic bytes per event (SURVEY.md 8d model: state read + written every event); "
+                              "the bytes really moved are in measured_dram, the bound that binds is roofline.alu",
+                "binding_bound": "alu (instruction issue)",
                 "traffic": (cnt["dram_bytes_per_event"] * ev_dom / kd["launches"]) if "dram_bytes_per_event" in cnt else None,
                 "traffic_source": cnt.get("source"),
+                "measured_dram": measured_dram(cnt, ev_dom / kd["launches"], dur, peak),
                 "whole_event": {"bytes_per_event": B_ALG_MG, "achieved": ev_per_s / world * B_ALG_MG / 1e9,
                                 "frac": ev_per_s / world * B_ALG_MG / 1e9 / peak},
                 "kernel_ms": {k: round(v["ms"] / n_prof, 3) for k, v in prof.items() if v["launches"]},
                 "note": "the persistent kernel keeps particle state in registers: the algorithmic bytes of SURVEY.md 8d "
                         "(state read + written every event) are mostly never moved; DRAM traffic is far below them"}
+        if "dram_bytes_per_event" not in cnt:
+            roof["traffic_stale"] = True
+            roof["traffic_stale_why"] = counts.get("_why")
         roof["alu"] = alu_roofline(g, "k_persist_mg" if dom == "persist" else "k_sweep_mg", ev_per_s / world,
                                    (clocks or {}).get("sm_mhz"))
 
@@ -311,7 +346,7 @@ def run_ours(args):
                    "l2": "particle bank (>1.2 GB) larger than L2" if N >= 2_000_000 else "bank fits in L2 (small configuration)", "schedule": ("persistent asynchronous kernel: one launch per cycle, warps refill dead lanes from a ticket queue (library default)"
                                 if args.persist == 0 and args.schedule == 0 else f"schedule {args.schedule}, persist_threshold {args.persist}"),
                    "k_mean": res["k_mean"]},
-        "events_per_sec": ev_per_s, "events_per_history": events / max(tracks, 1),
+        "events_per_sec": ev_per_s, "events_per_history": events / max(tracks, 1), "events_timed": events,
         "roofline": roof, "e2e": e2e, "gpu_launches": int(nl1 - nl0), "clocks": clocks,
     }
 
@@ -375,7 +410,8 @@ def bench_ce(binding, inputs, args, peak):
     dom = "persist" if prof["persist"]["ms"] >= prof["sweep"]["ms"] else "sweep"
     kd = prof[dom]
     ev_dom = ev - ev_sweep if dom == "persist" else ev_sweep
-    cnt = ncu_counts().get("k_persist_ce" if dom == "persist" else "k_sweep_ce", {})
+    counts = ncu_counts()
+    cnt = counts.get("k_persist_ce" if dom == "persist" else "k_sweep_ce") or {}
     ach = B_ALG_CE * ev_dom / (kd["ms"] * 1e-3) / 1e9 if kd["ms"] else None
     ev_per_s = ev / (best * 1e-3)
     roof = {"bound": "hbm", "kernel": f"k_{dom}<CE>", "achieved": ach, "peak": peak, "unit": "GB/s",
@@ -383,12 +419,19 @@ def bench_ce(binding, inputs, args, peak):
             "events_per_launch": ev_dom / max(kd["launches"], 1), "avg_launch_ms": kd["ms"] / max(kd["launches"], 1),
             "traffic": (cnt["dram_bytes_per_event"] * ev_dom / max(kd["launches"], 1)) if "dram_bytes_per_event" in cnt else None,
             "traffic_source": cnt.get("source"),
+            "frac_basis": "algorithmic bytes per event (SURVEY.md 8d model); bytes really moved: measured_dram",
+            "binding_bound": "latency / instruction issue (roofline.alu)",
+            "target_frac": 0.40, "meets_target": bool(ach and ach / peak >= 0.40),
+            "measured_dram": measured_dram(cnt, ev_dom / max(kd["launches"], 1), kd["ms"] * 1e-3 / max(kd["launches"], 1), peak),
             "whole_event": {"bytes_per_event": B_ALG_CE, "frac": ev_per_s * B_ALG_CE / 1e9 / peak}}
+    if "dram_bytes_per_event" not in cnt:
+        roof["traffic_stale"] = True
+        roof["traffic_stale_why"] = counts.get("_why")
     roof["alu"] = alu_roofline(g, "k_persist_ce" if dom == "persist" else "k_sweep_ce", ev_per_s, None)
     g.close()
     return {"workload": "C5: continuous-energy time-dependent pin cell", "source_particles": args.ce_particles,
             "histories_per_sec": args.ce_particles / (best * 1e-3), "tracks": int(r["counters"][0]),
-            "events_per_sec": ev_per_s, "ms": best, "roofline": roof,
+            "events_per_sec": ev_per_s, "events": ev, "ms": best, "roofline": roof,
             "kernel_ms": {k: round(v["ms"], 3) for k, v in prof.items() if v["launches"]}}
 
 

@@ -278,13 +278,9 @@ int mcdc_set_trace(mcdc_problem *p, uint64_t first_id, uint32_t n_ids, uint32_t 
 /* copies at most max records (ordered by cycle, id, seq); *n = records available */
 int mcdc_get_trace(const mcdc_problem *p, mcdc_trace_rec *out, uint64_t max, uint64_t *n);
 
-/* unit-level entry points (device kernels behind them; used by the parity tests):
- * n uniform draws of stream (seed, id[i], domain, cycle) at index draw[i] */
-int mcdc_test_draws(mcdc_problem *p, uint64_t seed, uint32_t domain, uint32_t cycle, const uint64_t *id,
-                    const uint32_t *draw, uint64_t n, double *out);
 /* The per-particle random-number stream (R1, R2) evaluated on the GPU WITHOUT any device
  * memory from the caller: out[i] = draw number draw[i] of stream (seed, id[i], domain, cycle), bit for bit what
- * mcdc_test_draws returns, but no mcdc_problem and no workspace are needed.
+ * mcdc_test_draws (include/mcdc_test.h) returns, but no mcdc_problem and no workspace are needed.
  *
  * Who this is for.  Every other call of this library works inside a workspace the caller allocated on the device.  Some
  * callers have nothing to give and no way to get it: a checking tool that runs beside a simulation whose workspace was
@@ -315,15 +311,6 @@ int mcdc_test_draws(mcdc_problem *p, uint64_t seed, uint32_t domain, uint32_t cy
 int mcdc_draws_noalloc(int32_t device, void *stream, uint64_t seed, uint32_t domain, uint32_t cycle, const uint64_t *id,
                        const uint32_t *draw, uint64_t n, double *out);
 
-/* union-grid index of E[i] with the binary (out_bin) and the hashed (out_hash) search */
-int mcdc_test_grid_index(mcdc_problem *p, const double *E, uint64_t n, int32_t *out_bin, int32_t *out_hash);
-/* locate + nearest boundary for n points: loc[i][3] = (c0, elem, c1), dist[i], surf[i].  path 0: the code path the
- * transport kernels take from that point (straight-line inside simple lattice elements, else the generic loops over
- * the enclosing cell's surfaces that create() could not rule out); 1: generic loops with that pruned list; 2: generic
- * loops over every surface (no pruning).  All three must agree. */
-int mcdc_test_geometry(mcdc_problem *p, const double *x, const double *u, uint64_t n, int32_t path, int32_t *loc,
-                       double *dist, int32_t *surf);
-
 /* device time (ms, CUDA events on the library's stream) of the transport part of the last run call, and the
  * number of kernels it launched */
 int mcdc_get_timing(const mcdc_problem *p, double *ms_transport, uint64_t *n_launches);
@@ -337,13 +324,10 @@ enum { MCDC_PROF_SWEEP = 0, MCDC_PROF_SCATTER, MCDC_PROF_SURFACE, MCDC_PROF_PERS
 int mcdc_set_profile(mcdc_problem *p, int32_t on);
 int mcdc_get_profile(const mcdc_problem *p, double *ms, uint64_t *launches, uint64_t *sweep_events);
 
-/* Arithmetic micro-benchmarks of this GPU (the ALU roofline's denominators): runs `iters` loop trips of
- * independent register-only chains of one operation on 148 x 8 blocks of 256 threads; returns the device time of the
- * launch and the thread-level operations it performed (FFMA / DFMA: fused multiply-adds; LOG, DIV, SQRT, SINCOSPI, RCP:
- * float64 library calls; PHILOX: Philox4x32-10 blocks = two draws each). */
-enum { MCDC_MB_FFMA = 0, MCDC_MB_DFMA, MCDC_MB_LOG, MCDC_MB_DIV, MCDC_MB_SQRT, MCDC_MB_SINCOSPI, MCDC_MB_RCP, MCDC_MB_PHILOX,
-       MCDC_MB_COUNT };
-int mcdc_microbench(mcdc_problem *p, int32_t which, uint64_t iters, double *ms, double *ops);
+/* identity of the sources this library was compiled from: the first 16 hex digits of a sha256 over csrc/ and this header,
+ * put in by the build (binding.build); "unknown" for a hand build without -DMCDC_BUILD_ID.  Measurement files that
+ * describe a build (profiles/r03_counts.csv) carry the same string; static storage, never NULL. */
+const char *mcdc_build_id(void);
 
 void mcdc_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);

@@ -58,8 +58,20 @@ SITE_DTYPE = np.dtype([("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("ux", "<f8"), 
                        ("g", "<i4"), ("pad", "<i4")], align=True)
 
 
+_SO_SAN = os.path.join(_HERE, "libmcdc_oracle_san.so")
+
+
 def build(force: bool = False) -> str:
-    """Compile the oracle (gcc -O2).  Building the checker is not using it."""
+    """Compile the oracle (gcc -O2).  Building the checker is not using it.
+
+    MCDC_ORACLE_SANITIZE=1 in the environment builds and loads an AddressSanitizer + UndefinedBehaviorSanitizer
+    instrumented copy instead (profiles/r03_oracle_sanitizers.md gives the command and its result)."""
+    if os.environ.get("MCDC_ORACLE_SANITIZE") == "1":
+        if force or not os.path.exists(_SO_SAN) or any(os.path.getmtime(s) > os.path.getmtime(_SO_SAN) for s in _SRC):
+            subprocess.check_call(["gcc", "-O1", "-g", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-fno-omit-frame-pointer",
+                                   "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                                   "-o", _SO_SAN, _SRC[0], "-lm"])
+        return _SO_SAN
     if force or not os.path.exists(_SO) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC):
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", _SO, _SRC[0], "-lm"])
     return _SO

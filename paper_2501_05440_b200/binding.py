@@ -17,7 +17,7 @@ _ROOT = os.path.dirname(_HERE)
 _SO = os.path.join(_HERE, "libmcdc_b200.so")
 _SRC = [os.path.join(_HERE, "csrc", f) for f in ("mcdc_lib.cu", "mcdc_kernels.cuh", "mcdc_device.cuh", "mcdc_census.cuh",
                                                    "mcdc_microbench.cuh")]
-_HDR = os.path.join(_ROOT, "include", "mcdc.h")
+_HDRS = [os.path.join(_ROOT, "include", f) for f in ("mcdc.h", "mcdc_test.h")]
 
 N_COUNTERS = 16
 NOALLOC_DRAWS_MAX = 65536  # MCDC_NOALLOC_DRAWS_MAX of include/mcdc.h
@@ -28,7 +28,7 @@ SYMBOLS = ["mcdc_workspace_bytes", "mcdc_create", "mcdc_run_eigenvalue", "mcdc_r
            "mcdc_run_fixed_source", "mcdc_get_dims", "mcdc_get_tallies", "mcdc_get_bank", "mcdc_set_trace",
            "mcdc_get_trace", "mcdc_test_draws", "mcdc_test_grid_index", "mcdc_test_geometry", "mcdc_get_timing",
            "mcdc_set_profile", "mcdc_get_profile", "mcdc_microbench", "mcdc_destroy", "mcdc_last_error",
-           "mcdc_set_physics", "mcdc_get_balance", "mcdc_get_census", "mcdc_draws_noalloc"]
+           "mcdc_set_physics", "mcdc_get_balance", "mcdc_get_census", "mcdc_draws_noalloc", "mcdc_build_id"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -108,13 +108,31 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC"]
 
 
+def source_id() -> str:
+    """Identity of the CUDA sources as they are on disk: sha256 over csrc/* and include/*.h, 16 hex digits.  build()
+    compiles it into the library (mcdc_build_id), so a measurement file can name the build it was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(_SRC + _HDRS):
+        h.update(os.path.basename(f).encode() + b"\0")
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile the CUDA library for sm_100a with nvcc (in-tree, next to this file)."""
-    deps = _SRC + [_HDR]
+    deps = _SRC + _HDRS
     if force or not os.path.exists(_SO) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in deps):
-        cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", _SO, _SRC[0]]
+        cmd = (["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
+               + [f'-DMCDC_BUILD_ID="{source_id()}"', "-o", _SO, _SRC[0]])
         subprocess.check_call(cmd)
     return _SO
+
+
+def build_id() -> str:
+    """source_id() of the sources the LOADED library was compiled from ("unknown" if built by hand without it)."""
+    return load_library().mcdc_build_id().decode()
 
 
 _lib = None
@@ -159,6 +177,7 @@ def load_library():
     L.mcdc_destroy.argtypes = [vp]
     L.mcdc_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
+    L.mcdc_build_id.restype = C.c_char_p
     _lib = L
     return L
 

@@ -1,6 +1,7 @@
 // mcdc_lib.cu -- host side of the C-ABI (include/mcdc.h): input validation and derived tables, workspace
 // carving, the sweep / cycle drivers and result read-back.  All device work is in mcdc_kernels.cuh.
 #include "../../include/mcdc.h"
+#include "../../include/mcdc_test.h"
 #include "mcdc_kernels.cuh"
 #include "mcdc_census.cuh"
 #include "mcdc_microbench.cuh"

@@ -1,4 +1,5 @@
-"""The C-ABI library loads and exports every symbol include/mcdc.h declares (no compute call, no GPU)."""
+"""The C-ABI library loads and exports every symbol include/*.h declares (mcdc.h: the product boundary; mcdc_test.h: the
+unit-level and micro-benchmark entry points) -- no compute call, no GPU."""
 import ctypes
 import os
 import re
@@ -9,7 +10,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "mcdc.h")).read()
+    src = "".join(open(os.path.join(ROOT, "include", f)).read() for f in sorted(os.listdir(os.path.join(ROOT, "include")))
+                  if f.endswith(".h"))
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(mcdc_[a-z_0-9]+)\s*\(", src)))
 
@@ -22,6 +24,12 @@ def test_library_exports_every_declared_symbol():
     for s in syms:
         assert hasattr(L, s), s
     assert sorted(binding.SYMBOLS) == syms
+
+
+def test_product_header_has_no_test_entry_points():
+    src = open(os.path.join(ROOT, "include", "mcdc.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    assert not re.findall(r"\bmcdc_(test_[a-z_]+|microbench)\s*\(", src)
 
 
 def test_binding_struct_sizes_match_header():

@@ -83,7 +83,60 @@ def test_c4_full_sampled_traces(gpu, orc, first):
     o.set_trace(first, 150, 1_000_000)
     o.run(n_particles=first + 150, n_inactive=0, n_active=1)
     compare_traces(tg, o.trace())
-    assert 1.0 < k0 < 2.0
+    # k of cycle 0 (a mean over source histories, which depend on (seed, id) only) against the oracle's cycle-0 k at 10^5
+    # histories: within 4 sigma of a 10^5 run, sigma measured from eight GPU seeds at that size
+    rc, ro = orc.Oracle(P).run(n_particles=100_000, n_inactive=0, n_active=1)
+    gs = gpu.Problem(inputs.config4(n_particles=100_000))
+    sig = np.std([gs.run_cycle(100_000, 0, 1, seed) for seed in range(2, 10)], ddof=1)
+    gs.close()
+    assert 0.0 < sig < 0.02 and abs(k0 - ro["k_cycle"][0]) < 4 * sig * math.sqrt(1.01)
+    g.close()
+
+
+REFILL_LANES = 444 * 256  # resident lanes of k_persist (3 blocks of 256 on each of 148 SMs): more particles than this
+                          # and lanes are refilled from the ticket queue while their neighbours are mid-history
+
+
+@pytest.mark.parametrize("name", ["C4", "C3", "C4_2l", "C4_implicit", "C3_implicit"])
+def test_mg_parity_refill_regime(gpu, orc, name):
+    """Element-by-element tally parity in the regime the benchmark runs in (finding 1): 3 x 10^5 particles
+    per cycle is 2.6 x the resident lanes of the persistent kernel, so every lane ends a history, takes a new ticket and
+    re-initialises its state and random-number stream next to running neighbours, and (global tally flavour) all 64
+    replicated tally copies are written.  Default schedule, 1 inactive + 2 active cycles; k per cycle, every flux bin and
+    the leakage within 1e-9 of the serial oracle, counters equal, the fission bank site by site."""
+    N = 300_000
+    kw = dict(n_particles=N, n_inactive=1, n_active=2)
+    P = {"C4": lambda: inputs.config4(**kw), "C3": lambda: inputs.config3(**kw),
+         "C4_2l": lambda: inputs.config4(two_level=True, **kw),
+         "C4_implicit": lambda: inputs.config4(**kw), "C3_implicit": lambda: inputs.config3(**kw)}[name]()
+    if name.endswith("implicit"):
+        P["implicit_capture"] = 1
+    g = gpu.Problem(P)
+    r = g.run()
+    o = orc.Oracle(P)
+    rc, ro = o.run()
+    assert rc == 0
+    compare_results(r, ro)
+    invariants(r) if not name.endswith("implicit") else None
+    # lanes were refilled: the persistent kernel took every history of every cycle from its queue, far more than it has lanes
+    assert r["counters"][13] == 3                      # one persistent launch per cycle
+    assert r["counters"][14] == r["counters"][0] > 3 * 2 * REFILL_LANES
+    # The fission bank, site by site (same order by construction: sorted by parent, child).  Group exact; directions are
+    # fresh isotropic samples: 1e-12.  Positions carry the history's rounding differences (FMA contraction, libm),
+    # amplified where a distance is ill-conditioned -- a flight almost parallel to z in these 2-D geometries
+    # (d = (p - x) / u_x: a last-bit difference in the numerator is divided by sin(polar angle); z, which no surface
+    # bounds, takes all of it) or a near-tangent cylinder crossing (divided by the chord's half-length).  Over ~5e7
+    # events per run such events do occur (DESIGN.md 3.2; measured on B200: 99.9 % of the sites within 1e-11, worst
+    # x / y 2.5e-10, worst z 3.0e-9), so: at most 0.5 % of the sites beyond 1e-11, none beyond 1e-9 (x, y) / 1e-8 (z).
+    bg, bo = g.bank(), o.bank()
+    assert len(bg) == len(bo) and len(bo) > REFILL_LANES
+    assert (bg["g"] == bo["g"]).all()
+    for f in ("ux", "uy", "uz"):
+        assert np.abs(bg[f] - bo[f]).max() < 1e-12, f
+    for f, worst in (("x", 1e-9), ("y", 1e-9), ("z", 1e-8)):
+        d = np.abs(bg[f] - bo[f]) - 1e-9 * np.abs(bo[f])
+        assert d.max() < worst, (f, d.max())
+        assert (d > 1e-11).mean() < 5e-3, (f, int((d > 1e-11).sum()))
     g.close()
 
 
@@ -96,7 +149,12 @@ def test_c4_full_k_and_flux(gpu, orc):
     invariants(r)
     Po = inputs.config4(n_particles=100_000, n_inactive=3, n_active=6)  # same cycles: the source is still converging
     rc, ro = orc.Oracle(Po).run()
-    assert abs(r["k_mean"] - ro["k_mean"]) < 3 * math.hypot(r["k_sdev"], ro["k_sdev"]) + 2e-3
+    # Two runs of different size: the GPU's 10^7 and the oracle's 10^5 particles per cycle.  The difference of their k
+    # means has the statistical spread (3 combined sigma of the mean over 6 active cycles) plus the well-known 1/N
+    # bias of power iteration with a finite population (source renormalisation, R6), which at N = 10^5 is of order
+    # 1/N x (a few hundred) ~ 1e-3 for a loosely coupled core like C4.  The exact-parity check of the same kernels is
+    # test_mg_parity_refill_regime; this one only guards the statistics at full size.
+    assert abs(r["k_mean"] - ro["k_mean"]) < 3 * math.hypot(r["k_sdev"], ro["k_sdev"]) + 1e-3
     fg, fo = r["flux_mean"].reshape(-1, 7), ro["flux_mean"].reshape(-1, 7)
     tg, to = fg.sum(), fo.sum()
     assert abs(tg - to) / to < 0.01

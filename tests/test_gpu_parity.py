@@ -47,9 +47,11 @@ def compare_traces(tg, to, atol=1e-11):
 
 def float_atol(name):
     """Absolute tolerance on positions.  Specular reflection off a CURVED wall amplifies the last-bit differences
-    between the two implementations (FMA contraction, libm) along near-tangent multi-bounce paths: measured worst
-    case 1.2e-9 cm after dozens of bounces; tallies and k still agree to 1e-9 relative."""
-    return 1e-7 if name.startswith("mirror") else 1e-11
+    between the two implementations (FMA contraction, libm) along near-tangent multi-bounce paths (a
+    direction error e becomes up to ~(1 + 2 L / (r cos theta)) e at a bounce with chord L, radius r and incidence theta;
+    dozens of bounces of an ulp-level 1e-16 reach 1e-9): measured worst case 1.2e-9 cm.  The bound is ten times the
+    measured worst case (VERDICT r2 finding 2: it was 1e-7 before); tallies and k still agree to 1e-9 relative."""
+    return 1e-8 if name.startswith("mirror") else 1e-11
 
 
 CASES = {
