@@ -174,7 +174,12 @@ WORKLOADS = {"C1": ("C1: 1-group infinite medium (reflecting unit cube)", 10_000
              "C2": ("C2: 7-group infinite medium (reflecting unit cube)", 100_000),
              "C3": ("C3: 2-D pin cell, 7 groups", 1_000_000),
              "C4": ("C4: 2-D quarter core, 7 groups, 2x2 17x17-pin assemblies + reflector, k-eigenvalue cycle", 10_000_000),
-             "C4_2L": ("C4 as a two-level lattice (assemblies of pin lattices; generic geometry path)", 10_000_000)}
+             "C4_2L": ("C4 as a two-level lattice (assemblies of pin lattices; generic geometry path)", 10_000_000),
+             # row f1 ("fully 3D"): finite height 64.26 cm (the core's half height = its side; reflecting
+             # mid-plane, vacuum top), with and without 21.42 cm of axial reflector above the fuel
+             "C4_3D": ("C4 fully 3-D: finite height (reflecting mid-plane, vacuum top)", 10_000_000),
+             "C4_3D_AX": ("C4 fully 3-D with an axial reflector (a z plane inside every pin universe)", 10_000_000),
+             "C4_2L_3D_AX": ("C4 fully 3-D with an axial reflector, as a two-level lattice", 10_000_000)}
 
 
 def workload(args):
@@ -183,7 +188,10 @@ def workload(args):
     from paper_2501_05440_b200 import inputs
     N = args.particles if args.particles else WORKLOADS[args.config][1]
     fn = {"C1": inputs.config1, "C2": inputs.config2, "C3": inputs.config3, "C4": inputs.config4,
-          "C4_2L": lambda **kw: inputs.config4(two_level=True, **kw)}[args.config]
+          "C4_2L": lambda **kw: inputs.config4(two_level=True, **kw),
+          "C4_3D": lambda **kw: inputs.config4(height=64.26, **kw),
+          "C4_3D_AX": lambda **kw: inputs.config4(height=64.26, axial_reflector=21.42, **kw),
+          "C4_2L_3D_AX": lambda **kw: inputs.config4(height=64.26, axial_reflector=21.42, two_level=True, **kw)}[args.config]
     return fn(n_particles=N, n_inactive=args.warmup, n_active=args.steps), N
 
 

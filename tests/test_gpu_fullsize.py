@@ -97,7 +97,7 @@ REFILL_LANES = 444 * 256  # resident lanes of k_persist (3 blocks of 256 on each
                           # and lanes are refilled from the ticket queue while their neighbours are mid-history
 
 
-@pytest.mark.parametrize("name", ["C4", "C3", "C4_2l", "C4_implicit", "C3_implicit"])
+@pytest.mark.parametrize("name", ["C4", "C3", "C4_2l", "C4_implicit", "C3_implicit", "C4_3d_axial"])
 def test_mg_parity_refill_regime(gpu, orc, name):
     """Element-by-element tally parity in the regime the benchmark runs in (finding 1): 3 x 10^5 particles
     per cycle is 2.6 x the resident lanes of the persistent kernel, so every lane ends a history, takes a new ticket and
@@ -108,7 +108,8 @@ def test_mg_parity_refill_regime(gpu, orc, name):
     kw = dict(n_particles=N, n_inactive=1, n_active=2)
     P = {"C4": lambda: inputs.config4(**kw), "C3": lambda: inputs.config3(**kw),
          "C4_2l": lambda: inputs.config4(two_level=True, **kw),
-         "C4_implicit": lambda: inputs.config4(**kw), "C3_implicit": lambda: inputs.config3(**kw)}[name]()
+         "C4_implicit": lambda: inputs.config4(**kw), "C3_implicit": lambda: inputs.config3(**kw),
+         "C4_3d_axial": lambda: inputs.config4(height=64.26, axial_reflector=21.42, **kw)}[name]()
     if name.endswith("implicit"):
         P["implicit_capture"] = 1
     g = gpu.Problem(P)

@@ -62,6 +62,11 @@ CASES = {
     "C4small": lambda: inputs.config4(n_particles=3001, n_inactive=1, n_active=2, n_asm=1, n_pin=3, n_refl=1),
     "mixed": lambda: inputs.mixed_surfaces(n_particles=4000),
     "C4_3d": lambda: inputs.config4(n_particles=4000, n_inactive=1, n_active=2, n_asm=1, n_pin=4, n_refl=1, height=6.0),
+    # fully 3-D cores with an axial reflector (row f1): a z plane inside every pin universe (fuel below, moderator above)
+    "C4_3d_axial": lambda: inputs.config4(n_particles=4000, n_inactive=1, n_active=2, n_asm=1, n_pin=4, n_refl=1, height=6.0,
+                                         axial_reflector=2.0),
+    "C4_2l_3d_axial": lambda: inputs.config4(n_particles=3000, n_inactive=1, n_active=2, n_asm=1, n_pin=4, n_refl=4, two_level=True,
+                                            height=6.0, axial_reflector=2.0),
     "lat1x6": lambda: inputs.rect_lattice(1, 6),
     "lat5x1": lambda: inputs.rect_lattice(5, 1),
     "lat3x5": lambda: inputs.rect_lattice(3, 5),
@@ -109,7 +114,7 @@ def test_mg_parity(gpu, orc, name, schedule, persist):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d", "lat1x6", "lat3x5", "mirror_sphere",
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C4small", "mixed", "C4_3d", "C4_3d_axial", "C4_2l_3d_axial", "lat1x6", "lat3x5", "mirror_sphere",
                                   "mirror_cyl_x", "C4_2l", "C4_2l_3d", "C4_2l_homog", "asm_gap", "asm_gap_wide", "rect_2l", "rect_2l_1col"])
 @pytest.mark.parametrize("schedule,persist", [(0, -1), (0, 0), (1, 0), (2, -1), (0, 100)])
 def test_mg_traces_identical(gpu, orc, name, schedule, persist):
@@ -174,9 +179,9 @@ def test_rng_bit_exact(gpu, orc):
     g.close()
 
 
-@pytest.mark.parametrize("height", [None, 3.0])
-def test_geometry_unit_parity(gpu, orc, height):
-    P = inputs.config4(n_particles=1000, height=height)
+@pytest.mark.parametrize("height,axial", [(None, None), (3.0, None), (3.0, 1.0)])
+def test_geometry_unit_parity(gpu, orc, height, axial):
+    P = inputs.config4(n_particles=1000, height=height, axial_reflector=axial)
     g = gpu.Problem(P, max_particles=20000)
     o = orc.Oracle(P)
     rng = np.random.default_rng(5)
@@ -200,7 +205,8 @@ def test_geometry_unit_parity(gpu, orc, height):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5", "C4_2l", "C4_2l_3d", "asm_gap", "C4_2l_17", "rect_2l"])
+@pytest.mark.parametrize("name", ["C1", "C3", "mixed", "mirror_cyl_z", "lat3x5", "C4_2l", "C4_2l_3d", "C4_3d_axial", "C4_2l_3d_axial",
+                                  "asm_gap", "C4_2l_17", "rect_2l"])
 def test_geometry_unit_parity_plain_cells(gpu, orc, name):
     """Cells outside a lattice (box, pin cell: straight-line path; mixed surfaces: generic loops) and a small lattice:
     locate + nearest boundary of random points, every device path against the oracle."""
